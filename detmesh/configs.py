@@ -33,7 +33,7 @@ class Workload:
 
 
 def philox_u01_host(key0: int, key1: int, ctr, n: int) -> np.ndarray:
-    """n uniforms ((w>>8)+0.5)*2^-24 from Philox4x32-10 words, counter (c0, c1, block, c3), block = 0,1,...
+    """n uniforms ((w>>9)+0.5)*2^-23 from Philox4x32-10 words, counter (c0, c1, block, c3), block = 0,1,...
     Input-generator use only (BASELINE.json configs[2] intensities)."""
     M0, M1, W0, W1 = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85
     out = []
@@ -49,7 +49,7 @@ def philox_u01_host(key0: int, key1: int, ctr, n: int) -> np.ndarray:
         out.extend(c)
         blk += 1
     w = np.array(out[:n], dtype=np.uint64)
-    return ((w >> np.uint64(8)).astype(np.float64) + 0.5) * 2.0 ** -24
+    return ((w >> np.uint64(9)).astype(np.float64) + 0.5) * 2.0 ** -23
 
 
 def _surface(name, segments, n_theta, mat_in, mat_out, band_counts=None):

@@ -84,13 +84,15 @@ void orc_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
 
 typedef struct { uint64_t seed, history; uint32_t stream, draw; } orc_rng;
 
-/* draw k of a stream = word (k mod 4) of block k/4; u = ((w >> 8) + 0.5) * 2^-24 in (0,1) */
+/* draw k of a stream = word (k mod 4) of block k/4; u = ((w >> 9) + 0.5) * 2^-23 in (0,1).
+ * 23 bits, not the 24 of SURVEY.md O3: (k + 0.5) with k < 2^23 has 24 significant bits and is exact in
+ * float32 as well as in double, so the float32 CUDA path sees identical uniforms (reading R3). */
 static double rng_next(orc_rng *g) {
     uint32_t ctr[4] = {(uint32_t)g->history, (uint32_t)(g->history >> 32), g->draw >> 2, g->stream};
     uint32_t key[2] = {(uint32_t)g->seed, (uint32_t)(g->seed >> 32)};
     uint32_t w[4];
     philox4x32_10(ctr, key, w);
-    double u = ((double)(w[g->draw & 3u] >> 8) + 0.5) * (1.0 / 16777216.0);
+    double u = ((double)(w[g->draw & 3u] >> 9) + 0.5) * (1.0 / 8388608.0);
     g->draw++;
     return u;
 }

@@ -1,0 +1,121 @@
+// gadep_common.cuh -- shared device-side types of the CUDA path (sm_100a).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <math.h>
+
+#define GD_HD __host__ __device__ __forceinline__
+#define GD_D __device__ __forceinline__
+
+#define GD_MEC2 0.51099895f
+#define GD_TWO_MEC2 1.0219979f
+#define GD_TBACK 1.0e-4f            // negative-t acceptance window [mm] (reading Q5)
+#define GD_MAT_KILL (-1)
+#define GD_MAX_LINES 64
+#define GD_MAX_MAT 16
+#define GD_STACK 96                 // LBVH depth bound: 63 Morton bits + index tie-break bits
+
+#define GD_F_ESCAPED 1u
+#define GD_F_PEAK 2u
+#define GD_F_LEAK 4u
+#define GD_F_NONSCORING 8u
+
+// ---------------------------------------------------------------- BVH layout
+// Binary BVH, children's boxes stored in the parent (one 64-byte node = 4 x 16 B loads):
+//   n0xy = (c0.lo.x, c0.hi.x, c0.lo.y, c0.hi.y)   n1xy = same for child 1
+//   nz   = (c0.lo.z, c0.hi.z, c1.lo.z, c1.hi.z)   link = (child0, child1, -, -)
+// child >= 0: inner node index; child < 0: leaf, ~child = index into the leaf-ordered triangle array.
+struct __align__(16) GdNode {
+    float4 n0xy, n1xy, nz;
+    int4 link;
+};
+
+// Leaf-ordered triangle: 48 bytes.  v0.w = caller's triangle index (bits), v1.w = side materials
+// (inside & 0xFFFF) | (outside << 16), v2.w = surface index (bits).
+struct __align__(16) GdTri {
+    float4 v0, v1, v2;
+};
+
+struct GdBvh {
+    const GdNode *nodes;
+    const GdTri *tris;
+    int n_tri;
+    int root_is_leaf;   // n_tri == 1
+};
+
+struct GdCounters {    // device-side totals, 64-bit
+    unsigned long long n_histories, n_queries, n_box_tests, n_tri_tests, n_crossings, n_pe, n_compton, n_coherent,
+        n_pair, n_escaped, n_leak, n_cutoff;
+};
+
+struct GdLocalCounters {  // per-thread, 32-bit
+    unsigned n_queries, n_box_tests, n_tri_tests, n_crossings, n_pe, n_compton, n_coherent, n_pair, n_escaped, n_leak,
+        n_cutoff;
+};
+
+struct GdSource {
+    int kind;
+    float pos[3], dir[3];
+    float cyl_r, cyl_z0, cyl_z1, ex_r, ex_z0, ex_z1;
+    int n_lines;
+    float line_mev[GD_MAX_LINES];
+    float line_cum[GD_MAX_LINES];   // running sums of the intensities, float32 left to right
+    int line_bin[GD_MAX_LINES];     // spectrum bin of the line energy (host, double)
+};
+
+struct GdMaterials {
+    int n_mat, n_grid;
+    float ln_e0, inv_dln, e_cut;
+    const float *table;             // device [n_mat][4][n_grid]: ln(mu) for channels 0..2 (-1e30 = zero), mu for 3
+    unsigned scoring_mask;          // bit m set = material m scores
+    int world_material;
+};
+
+struct GdVec3 {
+    float x, y, z;
+};
+GD_HD GdVec3 gd_make(float x, float y, float z) { GdVec3 v = {x, y, z}; return v; }
+GD_HD float gd_get(const GdVec3 &v, int k) { return k == 0 ? v.x : (k == 1 ? v.y : v.z); }
+
+// ---------------------------------------------------------------- Philox4x32-10 (Salmon et al., SC'11)
+GD_HD void gd_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                            uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+#ifdef __CUDA_ARCH__
+        uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+#else
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t h0 = (uint32_t)(p0 >> 32), l0 = (uint32_t)p0, h1 = (uint32_t)(p1 >> 32), l1 = (uint32_t)p1;
+#endif
+        uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
+        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Counter-based stream: key = seed, counter = (history_lo, history_hi, draw/4, stream); draw k = word k%4.
+struct GdRng {
+    uint32_t k0, k1, h0, h1, stream, draw;
+    uint32_t w[4];
+    uint32_t block;   // block index held in w, 0xFFFFFFFF = none
+};
+GD_HD void gd_rng_init(GdRng &g, unsigned long long seed, unsigned long long history, uint32_t stream, uint32_t draw) {
+    g.k0 = (uint32_t)seed; g.k1 = (uint32_t)(seed >> 32);
+    g.h0 = (uint32_t)history; g.h1 = (uint32_t)(history >> 32);
+    g.stream = stream; g.draw = draw; g.block = 0xFFFFFFFFu;
+}
+// u = ((w >> 9) + 0.5) * 2^-23 in (0,1): k + 0.5 with k < 2^23 is exact in float32
+GD_HD float gd_rng_next(GdRng &g) {
+    uint32_t b = g.draw >> 2;
+    if (b != g.block) {
+        gd_philox4x32_10(g.h0, g.h1, b, g.stream, g.k0, g.k1, g.w);
+        g.block = b;
+    }
+    uint32_t k = g.draw & 3u;
+    uint32_t w = k == 0 ? g.w[0] : (k == 1 ? g.w[1] : (k == 2 ? g.w[2] : g.w[3]));
+    g.draw++;
+    return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f);
+}

@@ -25,12 +25,12 @@ def test_philox_known_answer_vectors():
 
 
 def test_philox_stream_layout_against_independent_python_implementation():
-    # counter = (history_lo, history_hi, draw/4, stream), key = (seed_lo, seed_hi); u = ((w>>8)+0.5) 2^-24
+    # counter = (history_lo, history_hi, draw/4, stream), key = (seed_lo, seed_hi); u = ((w>>9)+0.5) 2^-23
     for seed, hist, stream in [(1, 0, 0), (7, 123456789012, 2), (2 ** 40 + 3, 2 ** 33 + 5, 1)]:
         ref = dm.philox_u01_host(seed & 0xFFFFFFFF, seed >> 32, (hist & 0xFFFFFFFF, hist >> 32, 0, stream), 12)
         got = [orc.u01(seed, hist, stream, k) for k in range(12)]
         assert np.array_equal(ref, np.array(got))
-        assert all(0.0 < u < 1.0 and np.float32(u) == u for u in got)   # exactly representable in float32
+        assert all(0.0 < u < 1.0 and float(np.float32(u)) == float(u) for u in got)   # exactly representable in float32
 
 
 # ------------------------------------------------------------------ O1 / O2 tables
