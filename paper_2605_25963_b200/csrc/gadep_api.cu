@@ -1,0 +1,569 @@
+// gadep_api.cu -- host side of libgadep.so: the C ABI of include/gadep.h.  Argument marshalling, validation,
+// device buffers and kernel launches only; every step of the hot path runs in the kernels.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <new>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include <curand_kernel.h>
+
+#include "../../include/gadep.h"
+#include "gadep_build_kernels.cuh"
+#include "gadep_transport_kernels.cuh"
+
+struct gadep_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    int n_sm = 148;
+    // materials
+    bool have_mat = false;
+    int n_mat = 0, n_grid = 0;
+    double e_min = 0, e_max = 0;
+    float *d_table = nullptr;
+    unsigned scoring_mask = 0;
+    // mesh
+    bool have_mesh = false, have_bvh = false;
+    int n_vert = 0, n_tri = 0, n_surf = 0, world = 0;
+    float *d_verts = nullptr;
+    int *d_tris = nullptr, *d_tri_mats = nullptr, *d_tri_surf = nullptr;
+    GdNode *d_nodes = nullptr;
+    GdTri *d_leaf_tris = nullptr;
+    int bvh_depth = 0;
+    // source
+    bool have_src = false;
+    GdSource src;
+    GdSource *d_src = nullptr;
+    // tallies
+    unsigned long long *d_tally = nullptr;   // [cap_bins + 1][emitted 64][peak 64]
+    int cap_bins = 0;
+    GdCounters *d_counters = nullptr;
+    int n_bins = 0;
+    float spec_e_max = 0;
+    bool results_stale = false, have_results = false;
+    std::vector<unsigned long long> h_spectrum;
+    unsigned long long h_emitted[GADEP_MAX_LINES], h_peak[GADEP_MAX_LINES];
+    GdCounters h_counters;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, evb0 = nullptr, evb1 = nullptr;
+    bool run_timed = false;
+    float last_run_ms = 0, last_build_ms = 0;
+    int last_run_launches = 0, last_build_launches = 0;
+};
+
+static int gd_fail(gadep_ctx *c, int code, const char *fmt, ...) {
+    if (c) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof(buf), fmt, ap);
+        va_end(ap);
+        c->err = buf;
+    }
+    return code;
+}
+
+#define GD_CUDA(c, call)                                                                                  \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess)                                                                            \
+            return gd_fail((c), GADEP_E_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+static bool gd_is_device_ptr(const void *p) {
+    if (!p) return false;
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
+    if (!out) return GADEP_E_NULL;
+    *out = nullptr;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0 || device < 0 || device >= n_dev) {
+        cudaGetLastError();
+        return GADEP_E_CUDA;   // no CPU fallback
+    }
+    gadep_ctx *c = new (std::nothrow) gadep_ctx();
+    if (!c) return GADEP_E_NOMEM;
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    memset(&c->src, 0, sizeof(c->src));
+    memset(&c->h_counters, 0, sizeof(c->h_counters));
+    memset(c->h_emitted, 0, sizeof(c->h_emitted));
+    memset(c->h_peak, 0, sizeof(c->h_peak));
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_counters, sizeof(GdCounters));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_src, sizeof(GdSource));
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->evb0);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->evb1);
+    if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
+    *out = c;
+    return GADEP_OK;
+}
+
+static void gd_free_mesh(gadep_ctx *c) {
+    cudaFree(c->d_verts); cudaFree(c->d_tris); cudaFree(c->d_tri_mats); cudaFree(c->d_tri_surf);
+    cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris);
+    c->d_verts = nullptr; c->d_tris = c->d_tri_mats = c->d_tri_surf = nullptr;
+    c->d_nodes = nullptr; c->d_leaf_tris = nullptr;
+    c->have_mesh = c->have_bvh = false;
+}
+
+extern "C" void gadep_destroy(gadep_ctx *c) {
+    if (!c) return;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    gd_free_mesh(c);
+    cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->evb0) cudaEventDestroy(c->evb0);
+    if (c->evb1) cudaEventDestroy(c->evb1);
+    delete c;
+}
+
+extern "C" const char *gadep_last_error(const gadep_ctx *c) { return c ? c->err.c_str() : "null context"; }
+
+extern "C" int gadep_set_materials(gadep_ctx *c, int n_mat, int n_grid, double e_min, double e_max, const float *mu,
+                                   const unsigned char *is_scoring) {
+    if (!c) return GADEP_E_NULL;
+    if (!mu || !is_scoring) return gd_fail(c, GADEP_E_NULL, "mu / is_scoring is null");
+    if (n_mat <= 0 || n_mat > GADEP_MAX_MATERIALS || n_grid < 2 || n_grid > 1024 || !(e_min > 0) || !(e_max > e_min))
+        return gd_fail(c, GADEP_E_ARG, "bad material table shape or energy range");
+    size_t n = (size_t)n_mat * 4 * n_grid;
+    std::vector<float> tab(n);
+    for (int m = 0; m < n_mat; ++m)
+        for (int ch = 0; ch < 4; ++ch)
+            for (int g = 0; g < n_grid; ++g) {
+                size_t i = ((size_t)m * 4 + ch) * n_grid + g;
+                float v = mu[i];
+                if (!std::isfinite(v) || v < 0) return gd_fail(c, GADEP_E_ARG, "mu[%d][%d][%d] negative or non-finite", m, ch, g);
+                tab[i] = ch < 3 ? (v > 0 ? (float)std::log((double)v) : -1.0e30f) : v;
+            }
+    GD_CUDA(c, cudaSetDevice(c->device));
+    cudaFree(c->d_table); c->d_table = nullptr;
+    GD_CUDA(c, cudaMalloc(&c->d_table, n * sizeof(float)));
+    GD_CUDA(c, cudaMemcpyAsync(c->d_table, tab.data(), n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->n_mat = n_mat; c->n_grid = n_grid; c->e_min = e_min; c->e_max = e_max;
+    c->scoring_mask = 0;
+    for (int m = 0; m < n_mat; ++m) if (is_scoring[m]) c->scoring_mask |= 1u << m;
+    c->have_mat = true;
+    return GADEP_OK;
+}
+
+extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, const int *triangles,
+                               const int *tri_surface, int n_tri, const int *surf_inside, const int *surf_outside,
+                               int n_surf, int world_material) {
+    if (!c) return GADEP_E_NULL;
+    if (!vertices || !triangles || !tri_surface || !surf_inside || !surf_outside) return gd_fail(c, GADEP_E_NULL, "null mesh array");
+    if (n_vert <= 0 || n_tri <= 0 || n_surf <= 0) return gd_fail(c, GADEP_E_ARG, "empty mesh");
+    int mat_hi = c->have_mat ? c->n_mat : GADEP_MAX_MATERIALS;
+    if (world_material < 0 || world_material >= mat_hi) return gd_fail(c, GADEP_E_INDEX, "world material %d out of range", world_material);
+    for (int s = 0; s < n_surf; ++s) {
+        if (surf_inside[s] < GADEP_MAT_KILL || surf_inside[s] >= mat_hi || surf_outside[s] < GADEP_MAT_KILL || surf_outside[s] >= mat_hi)
+            return gd_fail(c, GADEP_E_INDEX, "surface %d: material id out of range", s);
+    }
+    for (size_t i = 0; i < (size_t)n_vert * 3; ++i)
+        if (!std::isfinite(vertices[i])) return gd_fail(c, GADEP_E_NONFINITE, "vertex %zu is not finite", i / 3);
+    std::vector<int> mats(n_tri);
+    std::vector<std::vector<unsigned long long>> edges(n_surf);
+    for (int t = 0; t < n_tri; ++t) {
+        int s = tri_surface[t];
+        if (s < 0 || s >= n_surf) return gd_fail(c, GADEP_E_INDEX, "triangle %d: surface %d out of range", t, s);
+        int v[3] = {triangles[3 * t], triangles[3 * t + 1], triangles[3 * t + 2]};
+        for (int k = 0; k < 3; ++k)
+            if (v[k] < 0 || v[k] >= n_vert) return gd_fail(c, GADEP_E_INDEX, "triangle %d: vertex %d out of range", t, v[k]);
+        const float *a = vertices + 3 * (size_t)v[0], *b = vertices + 3 * (size_t)v[1], *q = vertices + 3 * (size_t)v[2];
+        double e1[3] = {(double)b[0] - a[0], (double)b[1] - a[1], (double)b[2] - a[2]};
+        double e2[3] = {(double)q[0] - a[0], (double)q[1] - a[1], (double)q[2] - a[2]};
+        double nx = e1[1] * e2[2] - e1[2] * e2[1], ny = e1[2] * e2[0] - e1[0] * e2[2], nz = e1[0] * e2[1] - e1[1] * e2[0];
+        if (v[0] == v[1] || v[1] == v[2] || v[0] == v[2] || nx * nx + ny * ny + nz * nz == 0.0)
+            return gd_fail(c, GADEP_E_DEGENERATE, "triangle %d has zero area", t);
+        mats[t] = (surf_inside[s] & 0xFFFF) | (int)((unsigned)(surf_outside[s] & 0xFFFF) << 16);
+        for (int k = 0; k < 3; ++k)
+            edges[s].push_back(((unsigned long long)(unsigned)v[k] << 32) | (unsigned)v[(k + 1) % 3]);
+    }
+    // closed + consistently oriented: every directed edge once, its reverse once (PAPER.md:193 needs closed geometry)
+    for (int s = 0; s < n_surf; ++s) {
+        std::vector<unsigned long long> &e = edges[s];
+        std::sort(e.begin(), e.end());
+        for (size_t i = 1; i < e.size(); ++i)
+            if (e[i] == e[i - 1]) return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %d: directed edge used twice (non-manifold or inconsistent winding)", s);
+        for (size_t i = 0; i < e.size(); ++i) {
+            unsigned long long rev = (e[i] << 32) | (e[i] >> 32);
+            if (!std::binary_search(e.begin(), e.end(), rev)) return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %d is not closed (open edge)", s);
+        }
+    }
+    GD_CUDA(c, cudaSetDevice(c->device));
+    gd_free_mesh(c);
+    GD_CUDA(c, cudaMalloc(&c->d_verts, sizeof(float) * 3 * (size_t)n_vert));
+    GD_CUDA(c, cudaMalloc(&c->d_tris, sizeof(int) * 3 * (size_t)n_tri));
+    GD_CUDA(c, cudaMalloc(&c->d_tri_mats, sizeof(int) * (size_t)n_tri));
+    GD_CUDA(c, cudaMalloc(&c->d_tri_surf, sizeof(int) * (size_t)n_tri));
+    GD_CUDA(c, cudaMemcpyAsync(c->d_verts, vertices, sizeof(float) * 3 * (size_t)n_vert, cudaMemcpyHostToDevice, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(c->d_tris, triangles, sizeof(int) * 3 * (size_t)n_tri, cudaMemcpyHostToDevice, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(c->d_tri_mats, mats.data(), sizeof(int) * (size_t)n_tri, cudaMemcpyHostToDevice, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(c->d_tri_surf, tri_surface, sizeof(int) * (size_t)n_tri, cudaMemcpyHostToDevice, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->n_vert = n_vert; c->n_tri = n_tri; c->n_surf = n_surf; c->world = world_material;
+    c->have_mesh = true;
+    return GADEP_OK;
+}
+
+// ---------------------------------------------------------------- BVH build
+extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
+    if (!c) return GADEP_E_NULL;
+    if (flags != 0) return gd_fail(c, GADEP_E_ARG, "unknown build flags %d", flags);
+    if (!c->have_mesh) return gd_fail(c, GADEP_E_ORDER, "gadep_build_bvh before gadep_load_mesh");
+    GD_CUDA(c, cudaSetDevice(c->device));
+    const int n = c->n_tri;
+    cudaStream_t st = c->stream;
+    cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris);
+    c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->have_bvh = false;
+    const int n_tiles = (n + GD_SORT_TILE - 1) / GD_SORT_TILE;
+    // one scratch arena: tri_lo, tri_hi, node_lo, node_hi (float4) | keys x2 | vals x2 | hist | tree ints | scene, depth
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+    size_t o_tlo = take(sizeof(float4) * n), o_thi = take(sizeof(float4) * n);
+    size_t o_nlo = take(sizeof(float4) * n), o_nhi = take(sizeof(float4) * n);
+    size_t o_k0 = take(8 * (size_t)n), o_k1 = take(8 * (size_t)n);
+    size_t o_v0 = take(4 * (size_t)n), o_v1 = take(4 * (size_t)n);
+    size_t o_hist = take(4 * (size_t)256 * n_tiles);
+    size_t o_cl = take(4 * (size_t)n), o_cr = take(4 * (size_t)n), o_pi = take(4 * (size_t)n), o_pl = take(4 * (size_t)n);
+    size_t o_vis = take(4 * (size_t)n), o_scene = take(4 * 8);
+    unsigned char *arena = nullptr;
+    GD_CUDA(c, cudaMalloc(&arena, off));
+    int rc = GADEP_OK;
+    int depth = 0, launches = 0;
+    cudaError_t e = cudaSuccess;
+    do {
+        if ((e = cudaMalloc(&c->d_nodes, sizeof(GdNode) * (size_t)std::max(n - 1, 1))) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_leaf_tris, sizeof(GdTri) * (size_t)n)) != cudaSuccess) break;
+        float4 *tri_lo = (float4 *)(arena + o_tlo), *tri_hi = (float4 *)(arena + o_thi);
+        float4 *node_lo = (float4 *)(arena + o_nlo), *node_hi = (float4 *)(arena + o_nhi);
+        unsigned long long *keys[2] = {(unsigned long long *)(arena + o_k0), (unsigned long long *)(arena + o_k1)};
+        unsigned *vals[2] = {(unsigned *)(arena + o_v0), (unsigned *)(arena + o_v1)};
+        unsigned *hist = (unsigned *)(arena + o_hist);
+        int *child_l = (int *)(arena + o_cl), *child_r = (int *)(arena + o_cr);
+        int *parent_int = (int *)(arena + o_pi), *parent_leaf = (int *)(arena + o_pl);
+        int *visits = (int *)(arena + o_vis), *scene = (int *)(arena + o_scene);
+        const int tb = 256, nb = (n + tb - 1) / tb;
+        cudaEventRecord(c->evb0, st);
+        gd_k_init_scene<<<1, 32, 0, st>>>(scene);
+        gd_k_tri_bounds<<<nb, tb, 0, st>>>(c->d_verts, c->d_tris, n, tri_lo, tri_hi, scene);
+        gd_k_morton<<<nb, tb, 0, st>>>(tri_lo, tri_hi, n, scene, keys[0], vals[0]);
+        launches += 3;
+        int cur = 0;
+        for (int shift = 0; shift < 64; shift += 8) {
+            gd_k_sort_hist<<<n_tiles, GD_SORT_THREADS, 0, st>>>(keys[cur], n, shift, hist, n_tiles);
+            gd_k_scan<<<1, 1024, 0, st>>>(hist, 256 * n_tiles);
+            gd_k_sort_scatter<<<n_tiles, GD_SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n,
+                                                                   shift, hist, n_tiles);
+            cur ^= 1;
+            launches += 3;
+        }
+        gd_k_leaf_tris<<<nb, tb, 0, st>>>(c->d_verts, c->d_tris, c->d_tri_mats, c->d_tri_surf, vals[cur], n, c->d_leaf_tris);
+        launches += 1;
+        if (n > 1) {
+            cudaMemsetAsync(visits, 0, 4 * (size_t)n, st);
+            cudaMemsetAsync(parent_leaf, 0xFF, 4 * (size_t)n, st);
+            gd_k_karras<<<nb, tb, 0, st>>>(keys[cur], n, child_l, child_r, parent_int, parent_leaf);
+            gd_k_refit<<<nb, tb, 0, st>>>(n, child_l, child_r, parent_int, parent_leaf, tri_lo, tri_hi, vals[cur], node_lo,
+                                          node_hi, visits, c->d_nodes, scene + 6);
+            launches += 2;
+        }
+        cudaEventRecord(c->evb1, st);
+        if ((e = cudaGetLastError()) != cudaSuccess) break;
+        if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
+        if (n > 1 && (e = cudaMemcpy(&depth, scene + 6, sizeof(int), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
+        cudaEventElapsedTime(&c->last_build_ms, c->evb0, c->evb1);
+    } while (0);
+    cudaFree(arena);
+    if (e != cudaSuccess) rc = gd_fail(c, GADEP_E_CUDA, "BVH build failed: %s", cudaGetErrorString(e));
+    else if (depth >= GD_STACK) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
+    if (rc != GADEP_OK) return rc;
+    c->bvh_depth = depth;
+    c->last_build_launches = launches;
+    c->have_bvh = true;
+    return GADEP_OK;
+}
+
+static GdBvh gd_bvh_view(const gadep_ctx *c) {
+    GdBvh b;
+    b.nodes = c->d_nodes; b.tris = c->d_leaf_tris; b.n_tri = c->n_tri; b.root_is_leaf = c->n_tri == 1;
+    return b;
+}
+
+// ---------------------------------------------------------------- source
+extern "C" int gadep_set_source(gadep_ctx *c, const gadep_source *s) {
+    if (!c) return GADEP_E_NULL;
+    if (!s || !s->line_mev || !s->line_intensity) return gd_fail(c, GADEP_E_NULL, "null source");
+    if (!c->have_mat) return gd_fail(c, GADEP_E_ORDER, "gadep_set_source before gadep_set_materials");
+    if (s->kind < 0 || s->kind > 2) return gd_fail(c, GADEP_E_ARG, "unknown source kind %d", s->kind);
+    if (s->n_lines <= 0 || s->n_lines > GADEP_MAX_LINES) return gd_fail(c, GADEP_E_ARG, "n_lines %d out of range", s->n_lines);
+    GdSource g;
+    memset(&g, 0, sizeof(g));
+    g.kind = s->kind;
+    for (int k = 0; k < 3; ++k) { g.pos[k] = s->pos[k]; g.dir[k] = s->dir[k]; }
+    g.cyl_r = s->cyl_r; g.cyl_z0 = s->cyl_z0; g.cyl_z1 = s->cyl_z1;
+    g.ex_r = s->ex_r; g.ex_z0 = s->ex_z0; g.ex_z1 = s->ex_z1;
+    g.n_lines = s->n_lines;
+    if (s->kind == GADEP_SRC_VOLUME && !(s->cyl_r > 0 && s->cyl_z1 > s->cyl_z0)) return gd_fail(c, GADEP_E_ARG, "empty source cylinder");
+    if (s->kind == GADEP_SRC_BEAM) {
+        double n2 = (double)s->dir[0] * s->dir[0] + (double)s->dir[1] * s->dir[1] + (double)s->dir[2] * s->dir[2];
+        if (!(std::fabs(n2 - 1.0) < 1e-3)) return gd_fail(c, GADEP_E_ARG, "beam direction is not a unit vector");
+    }
+    float cum = 0.0f;
+    for (int l = 0; l < s->n_lines; ++l) {
+        float e = s->line_mev[l], w = s->line_intensity[l];
+        if (!(w >= 0) || !std::isfinite(w)) return gd_fail(c, GADEP_E_ARG, "line %d: negative intensity", l);
+        if (!((double)e >= c->e_min * (1 - 1e-6) && (double)e <= c->e_max * (1 + 1e-6)))
+            return gd_fail(c, GADEP_E_ARG, "line %d: energy %g outside the table range", l, (double)e);
+        cum += w;
+        g.line_mev[l] = e; g.line_cum[l] = cum;
+    }
+    if (!(cum > 0)) return gd_fail(c, GADEP_E_ARG, "all line intensities are zero");
+    c->src = g;
+    c->have_src = true;
+    return GADEP_OK;
+}
+
+// ---------------------------------------------------------------- run
+static int gd_ensure_tally(gadep_ctx *c, int n_bins) {
+    if (c->d_tally && c->cap_bins >= n_bins) return GADEP_OK;
+    cudaFree(c->d_tally); c->d_tally = nullptr;
+    GD_CUDA(c, cudaMalloc(&c->d_tally, sizeof(unsigned long long) * ((size_t)n_bins + 1 + 2 * GADEP_MAX_LINES)));
+    c->cap_bins = n_bins;
+    return GADEP_OK;
+}
+
+static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned long long n, unsigned long long seed,
+                               int n_bins, float e_max, bool accumulate, float *d_edep, unsigned *d_flags) {
+    if (!c->have_mat || !c->have_mesh || !c->have_bvh || !c->have_src)
+        return gd_fail(c, GADEP_E_ORDER, "run needs materials, mesh, BVH and source");
+    if (n_bins <= 0 || n_bins > (1 << 20) || !(e_max > 0)) return gd_fail(c, GADEP_E_ARG, "bad spectrum shape");
+    GD_CUDA(c, cudaSetDevice(c->device));
+    bool same_shape = c->d_tally && c->n_bins == n_bins && c->spec_e_max == e_max;
+    int rc = gd_ensure_tally(c, n_bins);
+    if (rc) return rc;
+    cudaStream_t st = c->stream;
+    size_t tally_bytes = sizeof(unsigned long long) * ((size_t)n_bins + 1 + 2 * GADEP_MAX_LINES);
+    if (!(accumulate && same_shape)) {
+        GD_CUDA(c, cudaMemsetAsync(c->d_tally, 0, tally_bytes, st));
+        GD_CUDA(c, cudaMemsetAsync(c->d_counters, 0, sizeof(GdCounters), st));
+    }
+    c->n_bins = n_bins; c->spec_e_max = e_max;
+    double de = (double)e_max / n_bins;
+    for (int l = 0; l < c->src.n_lines; ++l) {
+        double b = std::floor((double)c->src.line_mev[l] / de);
+        c->src.line_bin[l] = b >= n_bins ? n_bins : (int)b;
+    }
+    GD_CUDA(c, cudaMemcpyAsync(c->d_src, &c->src, sizeof(GdSource), cudaMemcpyHostToDevice, st));
+    GdMaterials M;
+    M.n_mat = c->n_mat; M.n_grid = c->n_grid;
+    M.ln_e0 = (float)std::log(c->e_min);
+    M.inv_dln = (float)((c->n_grid - 1) / (std::log(c->e_max) - std::log(c->e_min)));
+    M.e_cut = (float)c->e_min;
+    M.table = c->d_table; M.scoring_mask = c->scoring_mask; M.world_material = c->world;
+    GdTally T;
+    T.spectrum = c->d_tally; T.emitted = c->d_tally + n_bins + 1; T.peak = T.emitted + GADEP_MAX_LINES;
+    T.counters = c->d_counters; T.n_bins = n_bins; T.inv_de = (float)((double)n_bins / (double)e_max);
+    size_t smem = sizeof(float) * (size_t)c->n_mat * 4 * c->n_grid + sizeof(unsigned) * ((size_t)n_bins + 1);
+    if (smem > 200 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum (%zu B) do not fit in shared memory", smem);
+    GD_CUDA(c, cudaFuncSetAttribute(gd_k_transport, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 1;
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gd_k_transport, GD_RUN_THREADS, smem));
+    if (per_sm < 1) per_sm = 1;
+    unsigned long long want = (n + GD_RUN_THREADS - 1) / GD_RUN_THREADS;
+    int grid = (int)std::min<unsigned long long>((unsigned long long)c->n_sm * per_sm, std::max<unsigned long long>(want, 1));
+    GD_CUDA(c, cudaEventRecord(c->ev0, st));
+    c->last_run_launches = 0;
+    if (n > 0) {
+        gd_k_transport<<<grid, GD_RUN_THREADS, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+        c->last_run_launches = 1;
+    }
+    GD_CUDA(c, cudaEventRecord(c->ev1, st));
+    GD_CUDA(c, cudaGetLastError());
+    c->results_stale = true; c->have_results = true; c->run_timed = true;
+    return GADEP_OK;
+}
+
+static int gd_fetch_results(gadep_ctx *c) {
+    if (!c->have_results) return gd_fail(c, GADEP_E_ORDER, "no run yet");
+    if (!c->results_stale) return GADEP_OK;
+    GD_CUDA(c, cudaSetDevice(c->device));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->d_tally && c->n_bins > 0) {
+        c->h_spectrum.resize((size_t)c->n_bins + 1);
+        GD_CUDA(c, cudaMemcpy(c->h_spectrum.data(), c->d_tally, sizeof(unsigned long long) * ((size_t)c->n_bins + 1), cudaMemcpyDeviceToHost));
+        GD_CUDA(c, cudaMemcpy(c->h_emitted, c->d_tally + c->n_bins + 1, sizeof(c->h_emitted), cudaMemcpyDeviceToHost));
+        GD_CUDA(c, cudaMemcpy(c->h_peak, c->d_tally + c->n_bins + 1 + GADEP_MAX_LINES, sizeof(c->h_peak), cudaMemcpyDeviceToHost));
+    }
+    GD_CUDA(c, cudaMemcpy(&c->h_counters, c->d_counters, sizeof(GdCounters), cudaMemcpyDeviceToHost));
+    if (c->run_timed) { cudaEventElapsedTime(&c->last_run_ms, c->ev0, c->ev1); c->run_timed = false; }
+    c->results_stale = false;
+    return GADEP_OK;
+}
+
+extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned long long seed, const gadep_run_opts *opts,
+                         unsigned long long *spectrum) {
+    if (!c) return GADEP_E_NULL;
+    if (!opts) return gd_fail(c, GADEP_E_NULL, "null run options");
+    bool dev_out = gd_is_device_ptr(spectrum);
+    if ((opts->flags & GADEP_RUN_ASYNC) && spectrum && !dev_out)
+        return gd_fail(c, GADEP_E_ARG, "GADEP_RUN_ASYNC needs a device spectrum pointer");
+    int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
+                                 (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
+    if (rc) return rc;
+    size_t bytes = sizeof(unsigned long long) * ((size_t)opts->n_bins + 1);
+    if (spectrum && dev_out) GD_CUDA(c, cudaMemcpyAsync(spectrum, c->d_tally, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    if (opts->flags & GADEP_RUN_ASYNC) return GADEP_OK;
+    rc = gd_fetch_results(c);
+    if (rc) return rc;
+    if (spectrum && !dev_out) memcpy(spectrum, c->h_spectrum.data(), bytes);
+    return GADEP_OK;
+}
+
+extern "C" int gadep_fepe(const gadep_ctx *cc, int line, int mode, double *fepe, double *std_err) {
+    gadep_ctx *c = const_cast<gadep_ctx *>(cc);
+    if (!c) return GADEP_E_NULL;
+    if (!fepe) return gd_fail(c, GADEP_E_NULL, "null output");
+    int rc = gd_fetch_results(c);
+    if (rc) return rc;
+    if (line < 0 || line >= c->src.n_lines) return gd_fail(c, GADEP_E_ARG, "line %d out of range", line);
+    double em = (double)c->h_emitted[line];
+    double p = 0.0;
+    if (em > 0) {
+        if (mode == 0) p = (double)c->h_peak[line] / em;
+        else if (mode == 1) {
+            int b = c->src.line_bin[line];
+            if (b < 1 || b >= c->n_bins - 1) return gd_fail(c, GADEP_E_ARG, "line %d lies outside the spectrum", line);
+            p = ((double)c->h_spectrum[b] - 0.5 * ((double)c->h_spectrum[b - 1] + (double)c->h_spectrum[b + 1])) / em;
+        } else return gd_fail(c, GADEP_E_ARG, "unknown mode %d", mode);
+    }
+    *fepe = p;
+    if (std_err) *std_err = em > 0 ? std::sqrt(std::max(p * (1.0 - p), 0.0) / em) : 0.0;
+    return GADEP_OK;
+}
+
+// ---------------------------------------------------------------- hooks
+extern "C" int gadep_trace_rays(gadep_ctx *c, const float *org, const float *dir, long long n_rays, int filter_material,
+                                float t_min, int *tri_out, float *t_out) {
+    if (!c) return GADEP_E_NULL;
+    if (!org || !dir || !tri_out || !t_out) return gd_fail(c, GADEP_E_NULL, "null ray array");
+    if (!c->have_bvh) return gd_fail(c, GADEP_E_ORDER, "gadep_trace_rays before gadep_build_bvh");
+    if (n_rays < 0) return gd_fail(c, GADEP_E_ARG, "negative ray count");
+    if (n_rays == 0) return GADEP_OK;
+    GD_CUDA(c, cudaSetDevice(c->device));
+    bool dev = gd_is_device_ptr(org);
+    if (dev != gd_is_device_ptr(dir) || dev != gd_is_device_ptr(tri_out) || dev != gd_is_device_ptr(t_out))
+        return gd_fail(c, GADEP_E_ARG, "ray arrays must live in one memory space");
+    cudaStream_t st = c->stream;
+    const float *d_org = org, *d_dir = dir;
+    int *d_tri = tri_out;
+    float *d_t = t_out;
+    float *stage = nullptr;
+    size_t nb3 = sizeof(float) * 3 * (size_t)n_rays, nb1 = sizeof(float) * (size_t)n_rays;
+    if (!dev) {
+        GD_CUDA(c, cudaMalloc(&stage, 2 * nb3 + 2 * nb1));
+        d_org = stage; d_dir = stage + 3 * n_rays; d_tri = (int *)(stage + 6 * n_rays); d_t = stage + 7 * n_rays;
+        cudaMemcpyAsync(stage, org, nb3, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(stage + 3 * n_rays, dir, nb3, cudaMemcpyHostToDevice, st);
+    }
+    cudaMemsetAsync(c->d_counters, 0, sizeof(GdCounters), st);
+    int grid = (int)std::min<long long>((n_rays + 255) / 256, (long long)c->n_sm * 8);
+    cudaEventRecord(c->ev0, st);
+    gd_k_trace<<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t, c->d_counters);
+    cudaEventRecord(c->ev1, st);
+    c->last_run_launches = 1;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && !dev) {
+        cudaMemcpyAsync(tri_out, d_tri, nb1, cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(t_out, d_t, nb1, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaMemcpy(&c->h_counters, c->d_counters, sizeof(GdCounters), cudaMemcpyDeviceToHost);
+    cudaFree(stage);
+    if (e != cudaSuccess) return gd_fail(c, GADEP_E_CUDA, "trace failed: %s", cudaGetErrorString(e));
+    cudaEventElapsedTime(&c->last_run_ms, c->ev0, c->ev1);
+    c->run_timed = false;
+    return GADEP_OK;
+}
+
+extern "C" int gadep_run_histories(gadep_ctx *c, unsigned long long first, long long n, unsigned long long seed,
+                                   float *edep_out, unsigned *flags_out) {
+    if (!c) return GADEP_E_NULL;
+    if (n < 0) return gd_fail(c, GADEP_E_ARG, "negative history count");
+    GD_CUDA(c, cudaSetDevice(c->device));
+    bool dev_e = gd_is_device_ptr(edep_out), dev_f = gd_is_device_ptr(flags_out);
+    float *d_e = edep_out;
+    unsigned *d_f = flags_out;
+    float *stage_e = nullptr;
+    unsigned *stage_f = nullptr;
+    if (edep_out && !dev_e && n > 0) { GD_CUDA(c, cudaMalloc(&stage_e, sizeof(float) * (size_t)n)); d_e = stage_e; }
+    if (flags_out && !dev_f && n > 0) { GD_CUDA(c, cudaMalloc(&stage_f, sizeof(unsigned) * (size_t)n)); d_f = stage_f; }
+    int n_bins = c->n_bins > 0 ? c->n_bins : 4096;
+    float e_max = c->spec_e_max > 0 ? c->spec_e_max : 2.0f;
+    int rc = gd_launch_transport(c, first, (unsigned long long)n, seed, n_bins, e_max, false, d_e, d_f);
+    if (rc == GADEP_OK) rc = gd_fetch_results(c);
+    if (rc == GADEP_OK && stage_e) cudaMemcpy(edep_out, stage_e, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost);
+    if (rc == GADEP_OK && stage_f) cudaMemcpy(flags_out, stage_f, sizeof(unsigned) * (size_t)n, cudaMemcpyDeviceToHost);
+    cudaFree(stage_e); cudaFree(stage_f);
+    return rc;
+}
+
+extern "C" int gadep_get_counters(const gadep_ctx *cc, gadep_counters *out) {
+    gadep_ctx *c = const_cast<gadep_ctx *>(cc);
+    if (!c) return GADEP_E_NULL;
+    if (!out) return gd_fail(c, GADEP_E_NULL, "null output");
+    if (c->have_results && c->results_stale) { int rc = gd_fetch_results(c); if (rc) return rc; }
+    memset(out, 0, sizeof(*out));
+    const GdCounters &h = c->h_counters;
+    out->n_histories = h.n_histories; out->n_queries = h.n_queries; out->n_box_tests = h.n_box_tests;
+    out->n_tri_tests = h.n_tri_tests; out->n_crossings = h.n_crossings; out->n_pe = h.n_pe; out->n_compton = h.n_compton;
+    out->n_coherent = h.n_coherent; out->n_pair = h.n_pair; out->n_escaped = h.n_escaped; out->n_leak = h.n_leak;
+    out->n_cutoff = h.n_cutoff;
+    memcpy(out->emitted, c->h_emitted, sizeof(out->emitted));
+    memcpy(out->peak, c->h_peak, sizeof(out->peak));
+    out->n_lines = c->src.n_lines;
+    out->n_bvh_nodes = c->have_bvh ? std::max(c->n_tri - 1, 0) : 0;
+    out->bvh_max_depth = c->bvh_depth;
+    out->last_run_ms = c->last_run_ms; out->last_build_ms = c->last_build_ms;
+    out->last_run_launches = c->last_run_launches; out->last_build_launches = c->last_build_launches;
+    return GADEP_OK;
+}
+
+__global__ void gd_k_philox(uint4 ctr, uint2 key, int which, unsigned *out) {
+    if (which == 0) {
+        uint32_t w[4];
+        gd_philox4x32_10(ctr.x, ctr.y, ctr.z, ctr.w, key.x, key.y, w);
+        out[0] = w[0]; out[1] = w[1]; out[2] = w[2]; out[3] = w[3];
+    } else {
+        uint4 r = curand_Philox4x32_10(ctr, key);
+        out[0] = r.x; out[1] = r.y; out[2] = r.z; out[3] = r.w;
+    }
+}
+
+extern "C" int gadep_philox_raw(gadep_ctx *c, const unsigned *ctr4, const unsigned *key2, int which, unsigned *out4) {
+    if (!c) return GADEP_E_NULL;
+    if (!ctr4 || !key2 || !out4) return gd_fail(c, GADEP_E_NULL, "null array");
+    GD_CUDA(c, cudaSetDevice(c->device));
+    unsigned *d = nullptr;
+    GD_CUDA(c, cudaMalloc(&d, 16));
+    gd_k_philox<<<1, 1, 0, c->stream>>>(make_uint4(ctr4[0], ctr4[1], ctr4[2], ctr4[3]), make_uint2(key2[0], key2[1]), which, d);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e == cudaSuccess) e = cudaMemcpy(out4, d, 16, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return gd_fail(c, GADEP_E_CUDA, "philox kernel failed: %s", cudaGetErrorString(e));
+    return GADEP_OK;
+}

@@ -1,0 +1,96 @@
+// gadep_transport_kernels.cuh -- ray-cast hook and the history-per-thread transport kernel (v0).
+// source, localisation, free flight, BVH nearest hit, boundary crossing,
+// interactions, tally into a per-block shared-memory spectrum, flush to 64-bit global tallies.
+#pragma once
+#include "gadep_physics.cuh"
+
+#define GD_RUN_THREADS 256
+
+struct GdTally {                       // device-global, 64-bit
+    unsigned long long *spectrum;      // [n_bins + 1]
+    unsigned long long *emitted;       // [GD_MAX_LINES]
+    unsigned long long *peak;          // [GD_MAX_LINES]
+    GdCounters *counters;
+    int n_bins;
+    float inv_de;                      // n_bins / e_max
+};
+
+GD_D void gd_flush_counters(const GdLocalCounters &c, GdCounters *g, unsigned n_hist) {
+    unsigned v[12] = {n_hist, c.n_queries, c.n_box_tests, c.n_tri_tests, c.n_crossings, c.n_pe, c.n_compton,
+                      c.n_coherent, c.n_pair, c.n_escaped, c.n_leak, c.n_cutoff};
+    unsigned long long *dst = (unsigned long long *)g;
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        unsigned long long x = v[k];
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) x += __shfl_down_sync(0xFFFFFFFFu, x, o);
+        if ((threadIdx.x & 31) == 0 && x) atomicAdd(&dst[k], x);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+gd_k_trace(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ dir, long long n, int filter_mat,
+           float t_min, int *__restrict__ tri_out, float *__restrict__ t_out, GdCounters *counters) {
+    GdLocalCounters cnt = {};
+    unsigned nq = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        GdRay ray;
+        gd_ray_setup(ray, gd_make(org[3 * i], org[3 * i + 1], org[3 * i + 2]),
+                     gd_make(dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]));
+        GdHit hit;
+        gd_nearest_hit(bvh, ray, t_min, GD_INF, filter_mat, hit, cnt.n_box_tests, cnt.n_tri_tests);
+        tri_out[i] = hit.leaf < 0 ? -1 : hit.orig;
+        t_out[i] = hit.leaf < 0 ? GD_INF : hit.t;
+        nq++;
+    }
+    cnt.n_queries = nq;
+    gd_flush_counters(cnt, counters, 0);
+}
+
+// dynamic shared memory: [table floats][spectrum u32 (n_bins+1)]
+__global__ void __launch_bounds__(GD_RUN_THREADS)
+gd_k_transport(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
+               unsigned long long n_hist, unsigned long long seed, GdTally tally, float *__restrict__ edep_out,
+               unsigned *__restrict__ flags_out) {
+    extern __shared__ __align__(16) unsigned char gd_smem[];
+    __shared__ GdSource s_src;
+    __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];
+    const int n_tab = M.n_mat * 4 * M.n_grid;
+    float *s_tab = (float *)gd_smem;
+    unsigned *s_spec = (unsigned *)(s_tab + n_tab);
+    for (int i = threadIdx.x; i < n_tab; i += blockDim.x) s_tab[i] = M.table[i];
+    for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) s_spec[i] = 0;
+    for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i];
+    if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }
+    __syncthreads();
+
+    GdLocalCounters cnt = {};
+    unsigned n_done = 0;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long h = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; h < n_hist; h += stride) {
+        GdHistory r;
+        gd_run_history(bvh, M, s_tab, s_src, seed, first + h, r, cnt);
+        n_done++;
+        atomicAdd(&s_emitted[r.line], 1u);
+        if (r.flags & GD_F_PEAK) {
+            atomicAdd(&s_peak[r.line], 1u);
+            atomicAdd(&s_spec[min(s_src.line_bin[r.line], tally.n_bins)], 1u);
+        } else if (r.edep > 0.0f) {
+            float b = floorf(r.edep * tally.inv_de);
+            int bin = b >= (float)tally.n_bins ? tally.n_bins : (int)b;
+            atomicAdd(&s_spec[bin], 1u);
+        }
+        if (edep_out) edep_out[h] = r.edep;
+        if (flags_out) flags_out[h] = r.flags;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) {
+        unsigned v = s_spec[i];
+        if (v) atomicAdd(&tally.spectrum[i], (unsigned long long)v);
+    }
+    if (threadIdx.x < GD_MAX_LINES) {
+        if (s_emitted[threadIdx.x]) atomicAdd(&tally.emitted[threadIdx.x], (unsigned long long)s_emitted[threadIdx.x]);
+        if (s_peak[threadIdx.x]) atomicAdd(&tally.peak[threadIdx.x], (unsigned long long)s_peak[threadIdx.x]);
+    }
+    gd_flush_counters(cnt, tally.counters, n_done);
+}
