@@ -104,6 +104,8 @@ int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
 
 #define GADEP_RUN_ASYNC 1          /* do not synchronise the stream; spectrum must then be a DEVICE pointer     */
 #define GADEP_RUN_ACCUMULATE 2     /* add to the context's tallies instead of starting from zero                */
+#define GADEP_RUN_HISTORY_PER_THREAD 4  /* measurement: the plain one-history-per-thread kernel instead of the   */
+                                   /* persistent-lane kernel (same results, bit for bit)                        */
 typedef struct {
     int n_bins;                    /* spectrum bins over [0, e_max_mev); one extra overflow slot follows        */
     float e_max_mev;

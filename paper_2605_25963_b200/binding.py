@@ -16,7 +16,7 @@ F_ESCAPED, F_PEAK, F_LEAK, F_NONSCORING = 1, 2, 4, 8
 FILTER_NONE = -2
 MAT_KILL = -1
 MAX_LINES = 64
-RUN_ASYNC, RUN_ACCUMULATE = 1, 2
+RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD = 1, 2, 4
 
 EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_set_materials", "gadep_load_mesh",
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",

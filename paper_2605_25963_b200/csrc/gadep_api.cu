@@ -43,6 +43,8 @@ struct gadep_ctx {
     unsigned long long *d_tally = nullptr;   // [cap_bins + 1][emitted 64][peak 64]
     int cap_bins = 0;
     GdCounters *d_counters = nullptr;
+    unsigned long long *d_next = nullptr;     // history counter of the refill kernel
+    int kernel_variant = 1;                   // 1 = persistent lanes with refill, 0 = history per thread
     int n_bins = 0;
     float spec_e_max = 0;
     bool results_stale = false, have_results = false;
@@ -101,6 +103,7 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_counters, sizeof(GdCounters));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_src, sizeof(GdSource));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_next, sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb0);
@@ -123,7 +126,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters);
+    cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     if (c->evb0) cudaEventDestroy(c->evb0);
@@ -380,16 +383,27 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     T.counters = c->d_counters; T.n_bins = n_bins; T.inv_de = (float)((double)n_bins / (double)e_max);
     size_t smem = sizeof(float) * (size_t)c->n_mat * 4 * c->n_grid + sizeof(unsigned) * ((size_t)n_bins + 1);
     if (smem > 200 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum (%zu B) do not fit in shared memory", smem);
-    GD_CUDA(c, cudaFuncSetAttribute(gd_k_transport, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const bool refill = c->kernel_variant == 1;
+    const void *kern = refill ? (const void *)gd_k_transport_refill : (const void *)gd_k_transport;
+    GD_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1;
-    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gd_k_transport, GD_RUN_THREADS, smem));
+    if (refill) GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gd_k_transport_refill, GD_RUN_THREADS, smem));
+    else GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gd_k_transport, GD_RUN_THREADS, smem));
     if (per_sm < 1) per_sm = 1;
     unsigned long long want = (n + GD_RUN_THREADS - 1) / GD_RUN_THREADS;
     int grid = (int)std::min<unsigned long long>((unsigned long long)c->n_sm * per_sm, std::max<unsigned long long>(want, 1));
     GD_CUDA(c, cudaEventRecord(c->ev0, st));
     c->last_run_launches = 0;
     if (n > 0) {
-        gd_k_transport<<<grid, GD_RUN_THREADS, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+        if (refill) {
+            unsigned long long warps = (unsigned long long)grid * (GD_RUN_THREADS / 32);
+            unsigned chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / (warps * 16)));
+            GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
+            gd_k_transport_refill<<<grid, GD_RUN_THREADS, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
+                                                                     d_flags, c->d_next, chunk);
+        } else {
+            gd_k_transport<<<grid, GD_RUN_THREADS, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+        }
         c->last_run_launches = 1;
     }
     GD_CUDA(c, cudaEventRecord(c->ev1, st));
@@ -422,6 +436,7 @@ extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned 
     bool dev_out = gd_is_device_ptr(spectrum);
     if ((opts->flags & GADEP_RUN_ASYNC) && spectrum && !dev_out)
         return gd_fail(c, GADEP_E_ARG, "GADEP_RUN_ASYNC needs a device spectrum pointer");
+    c->kernel_variant = (opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : 1;
     int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
                                  (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
     if (rc) return rc;

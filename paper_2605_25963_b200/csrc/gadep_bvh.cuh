@@ -156,8 +156,17 @@ GD_HD float gd_as_float(int i) {
 #endif
 }
 
-GD_HD void gd_test_leaf(const GdBvh &bvh, const GdRay &ray, int leaf, int filter_mat, float t_min, GdHit &hit,
-                        unsigned &n_tri_tests) {
+// Facets already crossed on the current straight flight segment and still inside the negative-t window: a line meets
+// a planar facet at most once, so they can never be the next boundary (without this, two facets of a corner cut
+// thinner than the window would be re-accepted behind the photon for ever).
+struct GdExclude {
+    int a, b, c;
+};
+GD_HD GdExclude gd_no_exclude() { GdExclude x = {-1, -1, -1}; return x; }
+
+GD_HD void gd_test_leaf(const GdBvh &bvh, const GdRay &ray, int leaf, int filter_mat, float t_min, const GdExclude &ex,
+                        GdHit &hit, unsigned &n_tri_tests) {
+    if (leaf == ex.a || leaf == ex.b || leaf == ex.c) return;
     const GdTri &tr = bvh.tris[leaf];
     float4 p0 = tr.v0, p1 = tr.v1, p2 = tr.v2;
     float t, det;
@@ -177,10 +186,10 @@ GD_HD void gd_test_leaf(const GdBvh &bvh, const GdRay &ray, int leaf, int filter
 }
 
 // Nearest facet with t in (t_min, t_max].  On return hit.leaf < 0 if none.
-GD_HD void gd_nearest_hit(const GdBvh &bvh, const GdRay &ray, float t_min, float t_max, int filter_mat, GdHit &hit,
-                          unsigned &n_box_tests, unsigned &n_tri_tests) {
+GD_HD void gd_nearest_hit(const GdBvh &bvh, const GdRay &ray, float t_min, float t_max, int filter_mat,
+                          const GdExclude &ex, GdHit &hit, unsigned &n_box_tests, unsigned &n_tri_tests) {
     hit.t = t_max; hit.leaf = -1; hit.orig = 0x7FFFFFFF; hit.leaving = 0; hit.mats = 0;
-    if (bvh.root_is_leaf) { gd_test_leaf(bvh, ray, 0, filter_mat, t_min, hit, n_tri_tests); return; }
+    if (bvh.root_is_leaf) { gd_test_leaf(bvh, ray, 0, filter_mat, t_min, ex, hit, n_tri_tests); return; }
     int stack[GD_STACK];
     int sp = 0;
     int node = 0;
@@ -219,7 +228,7 @@ GD_HD void gd_nearest_hit(const GdBvh &bvh, const GdRay &ray, float t_min, float
             }
         }
         // leaf
-        gd_test_leaf(bvh, ray, ~node, filter_mat, t_min, hit, n_tri_tests);
+        gd_test_leaf(bvh, ray, ~node, filter_mat, t_min, ex, hit, n_tri_tests);
         if (sp == 0) return;
         node = stack[--sp];
     }

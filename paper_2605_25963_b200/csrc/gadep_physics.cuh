@@ -102,127 +102,176 @@ GD_HD void gd_deposit(const GdMaterials &M, int m, float e, float &dep, unsigned
     else flags |= GD_F_NONSCORING;
 }
 
-// One history: O4 source, O5 start material, O7 flight loop, O8-O12 interactions, O14 flags.
-GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *tab, const GdSource &S,
-                          unsigned long long seed, unsigned long long history, GdHistory &out, GdLocalCounters &cnt) {
+// ---------------------------------------------------------------- lane state machine
+// One lane carries one history at a time; every step of a live lane issues exactly one nearest-hit query
+// (mode LOCATE: O5 start material; mode FLIGHT: O7.3), so a warp's lanes stay together in the traversal.
+#define GD_MODE_NEED 0
+#define GD_MODE_LOCATE 1
+#define GD_MODE_FLIGHT 2
+#define GD_MODE_DONE 3
+
+struct GdLane {
+    GdVec3 pos, dir;
+    float e, tau, mu[4], mu_tot, sdist;
+    int m, need_mu, mode;
     GdRng g;
-    gd_rng_init(g, seed, history, 0, 0);
-    // ---- O4 source
+    unsigned long long history;
+    float dep;
+    unsigned flags, n_events;
+    int line, pending, p_m;
+    GdVec3 p_pos, p_axis;
+    GdExclude ex;          // facets crossed on this flight segment within the last GD_TBACK of path
+    int n_stall;           // consecutive crossings without progress (safety net)
+};
+
+// O4: source sampling on stream 0; leaves the lane in mode LOCATE
+GD_HD void gd_lane_start(GdLane &L, const GdSource &S, unsigned long long seed, unsigned long long history) {
+    L.history = history;
+    gd_rng_init(L.g, seed, history, 0, 0);
     int nl = S.n_lines;
-    float ul = gd_rng_next(g) * S.line_cum[nl - 1];
+    float ul = gd_rng_next(L.g) * S.line_cum[nl - 1];
     int line = nl - 1;
     for (int l = 0; l < nl; ++l) if (ul < S.line_cum[l]) { line = l; break; }
-    GdVec3 pos, dir;
-    float e = S.line_mev[line];
+    L.line = line;
+    L.e = S.line_mev[line];
     if (S.kind == 1) {
         for (;;) {
-            float u1 = gd_rng_next(g), u2 = gd_rng_next(g), u3 = gd_rng_next(g);
+            float u1 = gd_rng_next(L.g), u2 = gd_rng_next(L.g), u3 = gd_rng_next(L.g);
             float r = S.cyl_r * sqrtf(u1);
             float z = S.cyl_z0 + (S.cyl_z1 - S.cyl_z0) * u3;
             if (S.ex_r > 0.0f && r < S.ex_r && z >= S.ex_z0 && z <= S.ex_z1) continue;
             float s, c;
             gd_sincos_2pi(u2, s, c);
-            pos = gd_make(r * c, r * s, z);
+            L.pos = gd_make(r * c, r * s, z);
             break;
         }
     } else {
-        pos = gd_make(S.pos[0], S.pos[1], S.pos[2]);
+        L.pos = gd_make(S.pos[0], S.pos[1], S.pos[2]);
     }
-    if (S.kind == 2) dir = gd_make(S.dir[0], S.dir[1], S.dir[2]);
-    else dir = gd_sample_isotropic(g);
+    if (S.kind == 2) L.dir = gd_make(S.dir[0], S.dir[1], S.dir[2]);
+    else L.dir = gd_sample_isotropic(L.g);
+    L.dep = 0.0f; L.flags = 0; L.n_events = 0; L.pending = 0;
+    L.m = 0; L.need_mu = 1; L.mu_tot = 0.0f; L.tau = 0.0f; L.sdist = 0.0f;
+    L.ex = gd_no_exclude(); L.n_stall = 0;
+    L.mode = GD_MODE_LOCATE;
+}
 
-    GdRay ray;
-    GdHit hit;
-    // ---- O5 start material: nearest facet ahead, no filter
-    int m;
-    {
-        gd_ray_setup(ray, pos, dir);
-        cnt.n_queries++;
-        gd_nearest_hit(bvh, ray, 0.0f, GD_INF, -2, hit, cnt.n_box_tests, cnt.n_tri_tests);
-        m = hit.leaf < 0 ? M.world_material : (hit.leaving ? gd_mat_inside(hit.mats) : gd_mat_outside(hit.mats));
+// parameters of the lane's next query
+GD_HD void gd_lane_query(GdLane &L, const GdMaterials &M, const float *tab, float &t_min, float &t_max, int &filter) {
+    if (L.mode == GD_MODE_LOCATE) { t_min = 0.0f; t_max = GD_INF; filter = -2; return; }
+    if (L.need_mu) { L.mu_tot = gd_mu_lookup(M, tab, L.m, L.e, L.mu); L.need_mu = 0; }     // O2
+    L.sdist = L.mu_tot > 0.0f ? L.tau / L.mu_tot : GD_INF;                                  // O7.2
+    t_min = -GD_TBACK; t_max = L.sdist; filter = L.m;                                       // O7.3
+}
+
+// the current photon ended: start the next annihilation photon if one waits; returns true when the history is over
+GD_HD bool gd_lane_next_photon(GdLane &L, unsigned long long seed) {
+    if (L.pending == 0) return true;
+    L.pos = L.p_pos; L.m = L.p_m; L.e = GD_MEC2; L.need_mu = 1;
+    unsigned stream;
+    if (L.pending == 2) { L.dir = L.p_axis; stream = 1; }
+    else { L.dir = gd_make(-L.p_axis.x, -L.p_axis.y, -L.p_axis.z); stream = 2; }
+    L.pending--;
+    gd_rng_init(L.g, seed, L.history, stream, 0);
+    L.tau = -logf(gd_rng_next(L.g));                                                        // O7.1
+    L.ex = gd_no_exclude(); L.n_stall = 0;
+    return false;
+}
+
+// consume the query result; returns true when the history is finished (out is then valid)
+GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const GdSource &S, unsigned long long seed, const GdHit &hit,
+                        GdHistory &out, GdLocalCounters &cnt) {
+    bool photon_done = false;
+    if (L.mode == GD_MODE_LOCATE) {                                                         // O5
+        L.m = hit.leaf < 0 ? M.world_material : (hit.leaving ? gd_mat_inside(hit.mats) : gd_mat_outside(hit.mats));
+        L.tau = -logf(gd_rng_next(L.g));                                                    // O7.1
+        L.need_mu = 1;
+        L.mode = GD_MODE_FLIGHT;
+        return false;
     }
-
-    float dep = 0.0f;
-    unsigned flags = 0, n_events = 0;
-    int pending = 0;              // 2: annihilation photons A and B wait; 1: B waits
-    GdVec3 p_pos = pos, p_axis = dir;
-    int p_m = m;
-    unsigned draw0 = g.draw;
-    unsigned stream = 0;
-
-    for (;;) {                    // photons of this history: primary, then A (stream 1), then B (stream 2)
-        gd_rng_init(g, seed, history, stream, draw0);
-        float tau = -logf(gd_rng_next(g));                       // O7.1
-        float mu[4], mu_tot = 0.0f;
-        bool need_mu = true;
-        for (;;) {                // flight loop
-            if (need_mu) { mu_tot = (m >= 0) ? gd_mu_lookup(M, tab, m, e, mu) : 0.0f; need_mu = false; }
-            float sdist = mu_tot > 0.0f ? tau / mu_tot : GD_INF;     // O7.2
-            gd_ray_setup(ray, pos, dir);
-            cnt.n_queries++;
-            gd_nearest_hit(bvh, ray, -GD_TBACK, sdist, m, hit, cnt.n_box_tests, cnt.n_tri_tests);   // O7.3
-            if (hit.leaf >= 0) {                                    // O7.6 boundary first
-                float t = fmaxf(hit.t, 0.0f);
-                pos.x += t * dir.x; pos.y += t * dir.y; pos.z += t * dir.z;
-                tau -= mu_tot * t;
-                m = hit.leaving ? gd_mat_outside(hit.mats) : gd_mat_inside(hit.mats);
-                cnt.n_crossings++;
-                need_mu = true;
-                if (m == GD_MAT_KILL) { flags |= GD_F_ESCAPED; cnt.n_escaped++; break; }
-                continue;
-            }
-            if (!(sdist < GD_INF)) {                                // O7.5 nothing ahead, no interaction
-                flags |= GD_F_ESCAPED; cnt.n_escaped++;
-                if (m != M.world_material) { flags |= GD_F_LEAK; cnt.n_leak++; }
-                break;
-            }
-            // ---- O7.4 / O8 interaction at pos + s d
-            pos.x += sdist * dir.x; pos.y += sdist * dir.y; pos.z += sdist * dir.z;
-            n_events++;
-            if (e < M.e_cut) { gd_deposit(M, m, e, dep, flags); cnt.n_cutoff++; break; }
-            float us = gd_rng_next(g) * mu_tot;
+    if (hit.leaf >= 0) {                                                                    // O7.6 boundary first
+        float t = fmaxf(hit.t, 0.0f);
+        L.pos.x += t * L.dir.x; L.pos.y += t * L.dir.y; L.pos.z += t * L.dir.z;
+        L.tau -= L.mu_tot * t;
+        L.m = hit.leaving ? gd_mat_outside(hit.mats) : gd_mat_inside(hit.mats);
+        cnt.n_crossings++;
+        L.need_mu = 1;
+        if (t > GD_TBACK) { L.ex = gd_no_exclude(); L.n_stall = 0; }      // earlier facets left the window
+        L.ex.c = L.ex.b; L.ex.b = L.ex.a; L.ex.a = hit.leaf;
+        if (L.m == GD_MAT_KILL) { L.flags |= GD_F_ESCAPED; cnt.n_escaped++; photon_done = true; }
+        else if (++L.n_stall > 32) {       // > 32 facets inside 0.1 um: degenerate mesh; stop instead of spinning
+            L.flags |= GD_F_ESCAPED | GD_F_LEAK; cnt.n_escaped++; cnt.n_leak++; photon_done = true;
+        }
+    } else if (!(L.sdist < GD_INF)) {                                                       // O7.5
+        L.flags |= GD_F_ESCAPED; cnt.n_escaped++;
+        if (L.m != M.world_material) { L.flags |= GD_F_LEAK; cnt.n_leak++; }
+        photon_done = true;
+    } else {                                                                                // O7.4 / O8 interaction
+        L.pos.x += L.sdist * L.dir.x; L.pos.y += L.sdist * L.dir.y; L.pos.z += L.sdist * L.dir.z;
+        L.n_events++;
+        L.ex = gd_no_exclude(); L.n_stall = 0;                            // new flight segment
+        if (L.e < M.e_cut) { gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_cutoff++; photon_done = true; }
+        else {
+            float us = gd_rng_next(L.g) * L.mu_tot;
             int ch = -1;
             float acc = 0.0f;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) { acc += mu[c]; if (ch < 0 && us < acc) ch = c; }
-            if (ch < 0) ch = mu[3] > 0.0f ? 3 : (mu[2] > 0.0f ? 2 : (mu[1] > 0.0f ? 1 : 0));
-            if (ch == 0) {                                          // O9 photoelectric
-                gd_deposit(M, m, e, dep, flags); cnt.n_pe++;
-                break;
-            } else if (ch == 1) {                                   // O10 Compton
+            for (int c = 0; c < 4; ++c) { acc += L.mu[c]; if (ch < 0 && us < acc) ch = c; }
+            if (ch < 0) ch = L.mu[3] > 0.0f ? 3 : (L.mu[2] > 0.0f ? 2 : (L.mu[1] > 0.0f ? 1 : 0));
+            if (ch == 0) {                                                                  // O9 photoelectric
+                gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_pe++;
+                photon_done = true;
+            } else if (ch == 1) {                                                           // O10 Compton
                 float cost;
-                float eps = gd_sample_compton(g, e, cost);
-                float uphi = gd_rng_next(g);
-                float e_new = eps * e;
-                gd_deposit(M, m, e - e_new, dep, flags);
-                dir = gd_rotate(dir, cost, uphi);
-                e = e_new;
+                float eps = gd_sample_compton(L.g, L.e, cost);
+                float uphi = gd_rng_next(L.g);
+                float e_new = eps * L.e;
+                gd_deposit(M, L.m, L.e - e_new, L.dep, L.flags);
+                L.dir = gd_rotate(L.dir, cost, uphi);
+                L.e = e_new;
                 cnt.n_compton++;
-                need_mu = true;
-                if (e < M.e_cut) { gd_deposit(M, m, e, dep, flags); cnt.n_cutoff++; break; }
-            } else if (ch == 2) {                                   // O11 coherent: E, m, mu unchanged
-                float cost = gd_sample_thomson(g);
-                float uphi = gd_rng_next(g);
-                dir = gd_rotate(dir, cost, uphi);
+                L.need_mu = 1;
+                if (L.e < M.e_cut) { gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_cutoff++; photon_done = true; }
+            } else if (ch == 2) {                                                           // O11 coherent
+                float cost = gd_sample_thomson(L.g);
+                float uphi = gd_rng_next(L.g);
+                L.dir = gd_rotate(L.dir, cost, uphi);
                 cnt.n_coherent++;
-            } else {                                                // O12 pair
-                gd_deposit(M, m, e - GD_TWO_MEC2, dep, flags);
-                p_axis = gd_sample_isotropic(g);
-                p_pos = pos; p_m = m; pending = 2;
+            } else {                                                                        // O12 pair
+                gd_deposit(M, L.m, L.e - GD_TWO_MEC2, L.dep, L.flags);
+                L.p_axis = gd_sample_isotropic(L.g);
+                L.p_pos = L.pos; L.p_m = L.m; L.pending = 2;
                 cnt.n_pair++;
-                break;
+                photon_done = true;
             }
-            tau = -logf(gd_rng_next(g));                            // O7.1 after every interaction
+            if (!photon_done) L.tau = -logf(gd_rng_next(L.g));                              // O7.1
         }
-        if (pending == 0) break;
-        pos = p_pos; m = p_m; e = GD_MEC2; draw0 = 0;
-        if (pending == 2) { dir = p_axis; stream = 1; }
-        else { dir = gd_make(-p_axis.x, -p_axis.y, -p_axis.z); stream = 2; }
-        pending--;
     }
+    if (!photon_done) return false;
+    if (!gd_lane_next_photon(L, seed)) return false;
     // ---- O14
-    if (!(flags & (GD_F_ESCAPED | GD_F_NONSCORING))) { flags |= GD_F_PEAK; dep = S.line_mev[line]; }
-    flags |= ((unsigned)line & 0xFFu) << 8;
-    flags |= (n_events > 0xFFFFu ? 0xFFFFu : n_events) << 16;
-    out.edep = dep; out.flags = flags; out.line = line;
+    if (!(L.flags & (GD_F_ESCAPED | GD_F_NONSCORING))) { L.flags |= GD_F_PEAK; L.dep = S.line_mev[L.line]; }
+    L.flags |= ((unsigned)L.line & 0xFFu) << 8;
+    L.flags |= (L.n_events > 0xFFFFu ? 0xFFFFu : L.n_events) << 16;
+    out.edep = L.dep; out.flags = L.flags; out.line = L.line;
+    L.mode = GD_MODE_NEED;
+    return true;
+}
+
+// One whole history on one lane (history-per-thread kernel, host emulation)
+GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *tab, const GdSource &S,
+                          unsigned long long seed, unsigned long long history, GdHistory &out, GdLocalCounters &cnt) {
+    GdLane L;
+    gd_lane_start(L, S, seed, history);
+    GdRay ray;
+    GdHit hit;
+    for (;;) {
+        float t_min, t_max;
+        int filter;
+        gd_lane_query(L, M, tab, t_min, t_max, filter);
+        gd_ray_setup(ray, L.pos, L.dir);
+        cnt.n_queries++;
+        gd_nearest_hit(bvh, ray, t_min, t_max, filter, L.ex, hit, cnt.n_box_tests, cnt.n_tri_tests);
+        if (gd_lane_post(L, M, S, seed, hit, out, cnt)) return;
+    }
 }
