@@ -35,6 +35,7 @@ struct gadep_ctx {
     GdNode *d_nodes = nullptr;
     GdTri *d_leaf_tris = nullptr;
     int bvh_depth = 0;
+    int n_ref = 0;                 // leaves of the BVH: facet references after splitting
     // source
     bool have_src = false;
     GdSource src;
@@ -229,12 +230,33 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     if (flags != 0) return gd_fail(c, GADEP_E_ARG, "unknown build flags %d", flags);
     if (!c->have_mesh) return gd_fail(c, GADEP_E_ORDER, "gadep_build_bvh before gadep_load_mesh");
     GD_CUDA(c, cudaSetDevice(c->device));
-    const int n = c->n_tri;
+    const int n_tri = c->n_tri;
     cudaStream_t st = c->stream;
     cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris);
     c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->have_bvh = false;
+    const int tb = 256, nbt = (n_tri + tb - 1) / tb;
+    int launches = 0;
+    // ---- phase A: how many references (reference splitting) -> one 4-byte read-back sizes the arena
+    unsigned *counts = nullptr;
+    int *scene = nullptr;
+    GD_CUDA(c, cudaMalloc(&counts, 4 * (size_t)n_tri));
+    if (cudaMalloc(&scene, 4 * 16) != cudaSuccess) { cudaFree(counts); return gd_fail(c, GADEP_E_CUDA, "cudaMalloc failed"); }
+    cudaEventRecord(c->evb0, st);
+    gd_k_init_scene<<<1, 32, 0, st>>>(scene);
+    gd_k_ref_count<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts);
+    gd_k_scan<<<1, 1024, 0, st>>>(counts, n_tri, (unsigned *)(scene + 8));
+    launches += 3;
+    unsigned n_ref_u = 0;
+    cudaError_t e = cudaMemcpyAsync(&n_ref_u, scene + 8, 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess || n_ref_u < (unsigned)n_tri || n_ref_u > (unsigned)n_tri * GD_MAX_SPLITS) {
+        cudaFree(counts); cudaFree(scene);
+        return gd_fail(c, GADEP_E_CUDA, "BVH build (reference count) failed: %s", cudaGetErrorString(e));
+    }
+    const int n = (int)n_ref_u;
+    const int nb = (n + tb - 1) / tb;
     const int n_tiles = (n + GD_SORT_TILE - 1) / GD_SORT_TILE;
-    // one scratch arena: tri_lo, tri_hi, node_lo, node_hi (float4) | keys x2 | vals x2 | hist | tree ints | scene, depth
+    // ---- phase B: one scratch arena
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
     size_t o_tlo = take(sizeof(float4) * n), o_thi = take(sizeof(float4) * n);
@@ -243,45 +265,42 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     size_t o_v0 = take(4 * (size_t)n), o_v1 = take(4 * (size_t)n);
     size_t o_hist = take(4 * (size_t)256 * n_tiles);
     size_t o_cl = take(4 * (size_t)n), o_cr = take(4 * (size_t)n), o_pi = take(4 * (size_t)n), o_pl = take(4 * (size_t)n);
-    size_t o_vis = take(4 * (size_t)n), o_scene = take(4 * 8);
+    size_t o_vis = take(4 * (size_t)n), o_rt = take(4 * (size_t)n);
     unsigned char *arena = nullptr;
-    GD_CUDA(c, cudaMalloc(&arena, off));
+    if (cudaMalloc(&arena, off) != cudaSuccess) { cudaFree(counts); cudaFree(scene); return gd_fail(c, GADEP_E_NOMEM, "BVH scratch (%zu B)", off); }
     int rc = GADEP_OK;
-    int depth = 0, launches = 0;
-    cudaError_t e = cudaSuccess;
+    int depth = 0;
     do {
         if ((e = cudaMalloc(&c->d_nodes, sizeof(GdNode) * (size_t)std::max(n - 1, 1))) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_leaf_tris, sizeof(GdTri) * (size_t)n)) != cudaSuccess) break;
-        float4 *tri_lo = (float4 *)(arena + o_tlo), *tri_hi = (float4 *)(arena + o_thi);
+        float4 *ref_lo = (float4 *)(arena + o_tlo), *ref_hi = (float4 *)(arena + o_thi);
         float4 *node_lo = (float4 *)(arena + o_nlo), *node_hi = (float4 *)(arena + o_nhi);
         unsigned long long *keys[2] = {(unsigned long long *)(arena + o_k0), (unsigned long long *)(arena + o_k1)};
         unsigned *vals[2] = {(unsigned *)(arena + o_v0), (unsigned *)(arena + o_v1)};
         unsigned *hist = (unsigned *)(arena + o_hist);
         int *child_l = (int *)(arena + o_cl), *child_r = (int *)(arena + o_cr);
         int *parent_int = (int *)(arena + o_pi), *parent_leaf = (int *)(arena + o_pl);
-        int *visits = (int *)(arena + o_vis), *scene = (int *)(arena + o_scene);
-        const int tb = 256, nb = (n + tb - 1) / tb;
-        cudaEventRecord(c->evb0, st);
-        gd_k_init_scene<<<1, 32, 0, st>>>(scene);
-        gd_k_tri_bounds<<<nb, tb, 0, st>>>(c->d_verts, c->d_tris, n, tri_lo, tri_hi, scene);
-        gd_k_morton<<<nb, tb, 0, st>>>(tri_lo, tri_hi, n, scene, keys[0], vals[0]);
-        launches += 3;
+        int *visits = (int *)(arena + o_vis), *ref_tri = (int *)(arena + o_rt);
+        gd_k_make_refs<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts, ref_lo, ref_hi, ref_tri, scene);
+        gd_k_morton<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, scene, keys[0], vals[0]);
+        launches += 2;
         int cur = 0;
         for (int shift = 0; shift < 64; shift += 8) {
             gd_k_sort_hist<<<n_tiles, GD_SORT_THREADS, 0, st>>>(keys[cur], n, shift, hist, n_tiles);
-            gd_k_scan<<<1, 1024, 0, st>>>(hist, 256 * n_tiles);
+            gd_k_scan<<<1, 1024, 0, st>>>(hist, 256 * n_tiles, nullptr);
             gd_k_sort_scatter<<<n_tiles, GD_SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n,
                                                                    shift, hist, n_tiles);
             cur ^= 1;
             launches += 3;
         }
-        gd_k_leaf_tris<<<nb, tb, 0, st>>>(c->d_verts, c->d_tris, c->d_tri_mats, c->d_tri_surf, vals[cur], n, c->d_leaf_tris);
+        gd_k_leaf_tris<<<nb, tb, 0, st>>>(c->d_verts, c->d_tris, c->d_tri_mats, c->d_tri_surf, ref_tri, vals[cur], n,
+                                          c->d_leaf_tris);
         launches += 1;
         if (n > 1) {
             cudaMemsetAsync(visits, 0, 4 * (size_t)n, st);
             cudaMemsetAsync(parent_leaf, 0xFF, 4 * (size_t)n, st);
             gd_k_karras<<<nb, tb, 0, st>>>(keys[cur], n, child_l, child_r, parent_int, parent_leaf);
-            gd_k_refit<<<nb, tb, 0, st>>>(n, child_l, child_r, parent_int, parent_leaf, tri_lo, tri_hi, vals[cur], node_lo,
+            gd_k_refit<<<nb, tb, 0, st>>>(n, child_l, child_r, parent_int, parent_leaf, ref_lo, ref_hi, vals[cur], node_lo,
                                           node_hi, visits, c->d_nodes, scene + 6);
             launches += 2;
         }
@@ -291,11 +310,12 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         if (n > 1 && (e = cudaMemcpy(&depth, scene + 6, sizeof(int), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
         cudaEventElapsedTime(&c->last_build_ms, c->evb0, c->evb1);
     } while (0);
-    cudaFree(arena);
+    cudaFree(arena); cudaFree(counts); cudaFree(scene);
     if (e != cudaSuccess) rc = gd_fail(c, GADEP_E_CUDA, "BVH build failed: %s", cudaGetErrorString(e));
     else if (depth >= GD_STACK) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
     if (rc != GADEP_OK) return rc;
     c->bvh_depth = depth;
+    c->n_ref = n;
     c->last_build_launches = launches;
     c->have_bvh = true;
     return GADEP_OK;
@@ -303,7 +323,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
 
 static GdBvh gd_bvh_view(const gadep_ctx *c) {
     GdBvh b;
-    b.nodes = c->d_nodes; b.tris = c->d_leaf_tris; b.n_tri = c->n_tri; b.root_is_leaf = c->n_tri == 1;
+    b.nodes = c->d_nodes; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
     return b;
 }
 
@@ -551,7 +571,7 @@ extern "C" int gadep_get_counters(const gadep_ctx *cc, gadep_counters *out) {
     memcpy(out->emitted, c->h_emitted, sizeof(out->emitted));
     memcpy(out->peak, c->h_peak, sizeof(out->peak));
     out->n_lines = c->src.n_lines;
-    out->n_bvh_nodes = c->have_bvh ? std::max(c->n_tri - 1, 0) : 0;
+    out->n_bvh_nodes = c->have_bvh ? std::max(c->n_ref - 1, 0) : 0;
     out->bvh_max_depth = c->bvh_depth;
     out->last_run_ms = c->last_run_ms; out->last_build_ms = c->last_build_ms;
     out->last_run_launches = c->last_run_launches; out->last_build_launches = c->last_build_launches;

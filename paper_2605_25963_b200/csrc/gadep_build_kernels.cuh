@@ -17,33 +17,77 @@ __global__ void gd_k_init_scene(int *scene) {
     else if (threadIdx.x < 6) scene[threadIdx.x] = (int)0x80000000;
 }
 
-// per facet: AABB (lo, hi as float4 pairs) and centroid bounds of the scene
-__global__ void gd_k_tri_bounds(const float *__restrict__ verts, const int *__restrict__ tris, int n_tri,
-                                float4 *__restrict__ tri_lo, float4 *__restrict__ tri_hi, int *scene) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    float cx = 0, cy = 0, cz = 0;
-    bool ok = i < n_tri;
-    if (ok) {
-        int a = tris[3 * i], b = tris[3 * i + 1], c = tris[3 * i + 2];
-        float ax = verts[3 * a], ay = verts[3 * a + 1], az = verts[3 * a + 2];
-        float bx = verts[3 * b], by = verts[3 * b + 1], bz = verts[3 * b + 2];
-        float qx = verts[3 * c], qy = verts[3 * c + 1], qz = verts[3 * c + 2];
-        float lx = fminf(ax, fminf(bx, qx)), ly = fminf(ay, fminf(by, qy)), lz = fminf(az, fminf(bz, qz));
-        float hx = fmaxf(ax, fmaxf(bx, qx)), hy = fmaxf(ay, fmaxf(by, qy)), hz = fmaxf(az, fmaxf(bz, qz));
-        cx = 0.5f * (lx + hx); cy = 0.5f * (ly + hy); cz = 0.5f * (lz + hz);
-        tri_lo[i] = make_float4(lx, ly, lz, cx);
-        tri_hi[i] = make_float4(hx, hy, hz, cy);
+#define GD_MAX_SPLITS 16
+
+GD_D void gd_load_tri(const float *__restrict__ verts, const int *__restrict__ tris, int i, float p[3][3], float lo[3],
+                      float hi[3]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        int v = tris[3 * i + c];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) p[c][a] = verts[3 * v + a];
     }
-    int lo[3] = {ok ? gd_f2o(cx) : 0x7FFFFFFF, ok ? gd_f2o(cy) : 0x7FFFFFFF, ok ? gd_f2o(cz) : 0x7FFFFFFF};
-    int hi[3] = {ok ? gd_f2o(cx) : (int)0x80000000, ok ? gd_f2o(cy) : (int)0x80000000, ok ? gd_f2o(cz) : (int)0x80000000};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        lo[a] = fminf(p[0][a], fminf(p[1][a], p[2][a]));
+        hi[a] = fmaxf(p[0][a], fmaxf(p[1][a], p[2][a]));
+    }
+}
+
+// number of references each facet contributes (reference splitting of loose AABBs, gd_split_count)
+__global__ void gd_k_ref_count(const float *__restrict__ verts, const int *__restrict__ tris, int n_tri,
+                               unsigned *__restrict__ counts) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_tri) return;
+    float p[3][3], lo[3], hi[3];
+    gd_load_tri(verts, tris, i, p, lo, hi);
+    int axis;
+    counts[i] = (unsigned)gd_split_count(p, lo, hi, GD_MAX_SPLITS, axis);
+}
+
+// per reference: AABB (lo.w = centroid x, hi.w = centroid y), facet index; scene bounds of the centroids
+__global__ void gd_k_make_refs(const float *__restrict__ verts, const int *__restrict__ tris, int n_tri,
+                               const unsigned *__restrict__ offsets, float4 *__restrict__ ref_lo,
+                               float4 *__restrict__ ref_hi, int *__restrict__ ref_tri, int *scene) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int slo[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF};
+    int shi[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
+    if (i < n_tri) {
+        float p[3][3], lo[3], hi[3];
+        gd_load_tri(verts, tris, i, p, lo, hi);
+        int axis;
+        int k = gd_split_count(p, lo, hi, GD_MAX_SPLITS, axis);
+        unsigned base = offsets[i];
+        float ext = hi[axis] - lo[axis];
+        for (int j = 0; j < k; ++j) {
+            float rl[3] = {lo[0], lo[1], lo[2]}, rh[3] = {hi[0], hi[1], hi[2]};
+            if (k > 1) {
+                float a0 = lo[axis] + ext * (float)j / (float)k;
+                float b0 = (j == k - 1) ? hi[axis] : lo[axis] + ext * (float)(j + 1) / (float)k;
+                float cl[3], ch[3];
+                gd_clip_tri_box(p, axis, a0, b0, cl, ch);
+                if (cl[0] <= ch[0] && cl[1] <= ch[1] && cl[2] <= ch[2]) {      // else keep the whole facet box (safe)
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) { rl[a] = fmaxf(cl[a], lo[a]); rh[a] = fminf(ch[a], hi[a]); }
+                }
+            }
+            float cx = 0.5f * (rl[0] + rh[0]), cy = 0.5f * (rl[1] + rh[1]), cz = 0.5f * (rl[2] + rh[2]);
+            ref_lo[base + j] = make_float4(rl[0], rl[1], rl[2], cx);
+            ref_hi[base + j] = make_float4(rh[0], rh[1], rh[2], cy);
+            ref_tri[base + j] = i;
+            int ox = gd_f2o(cx), oy = gd_f2o(cy), oz = gd_f2o(cz);
+            slo[0] = min(slo[0], ox); slo[1] = min(slo[1], oy); slo[2] = min(slo[2], oz);
+            shi[0] = max(shi[0], ox); shi[1] = max(shi[1], oy); shi[2] = max(shi[2], oz);
+        }
+    }
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        lo[k] = __reduce_min_sync(0xFFFFFFFFu, lo[k]);
-        hi[k] = __reduce_max_sync(0xFFFFFFFFu, hi[k]);
+        slo[k] = __reduce_min_sync(0xFFFFFFFFu, slo[k]);
+        shi[k] = __reduce_max_sync(0xFFFFFFFFu, shi[k]);
     }
     if ((threadIdx.x & 31) == 0) {
 #pragma unroll
-        for (int k = 0; k < 3; ++k) { atomicMin(&scene[k], lo[k]); atomicMax(&scene[3 + k], hi[k]); }
+        for (int k = 0; k < 3; ++k) { atomicMin(&scene[k], slo[k]); atomicMax(&scene[3 + k], shi[k]); }
     }
 }
 
@@ -81,7 +125,7 @@ __global__ void gd_k_sort_hist(const unsigned long long *__restrict__ keys, int 
 }
 
 // exclusive scan of `count` unsigneds in place, single block of 1024 threads
-__global__ void gd_k_scan(unsigned *data, int count) {
+__global__ void gd_k_scan(unsigned *data, int count, unsigned *total) {
     __shared__ unsigned s_w[32];
     __shared__ unsigned s_carry;
     if (threadIdx.x == 0) s_carry = 0;
@@ -108,6 +152,7 @@ __global__ void gd_k_scan(unsigned *data, int count) {
         if (threadIdx.x == 1023) s_carry = excl + v;
         __syncthreads();
     }
+    if (total && threadIdx.x == 0) *total = s_carry;
 }
 
 // stable scatter: tile order, chunk order, lane order preserved
@@ -167,10 +212,11 @@ __global__ void gd_k_karras(const unsigned long long *__restrict__ keys, int n, 
 // leaf-ordered triangle records
 __global__ void gd_k_leaf_tris(const float *__restrict__ verts, const int *__restrict__ tris,
                                const int *__restrict__ tri_mats, const int *__restrict__ tri_surf,
-                               const unsigned *__restrict__ order, int n, GdTri *__restrict__ out) {
+                               const int *__restrict__ ref_tri, const unsigned *__restrict__ order, int n,
+                               GdTri *__restrict__ out) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    int o = (int)order[i];
+    int o = ref_tri[order[i]];
     int a = tris[3 * o], b = tris[3 * o + 1], c = tris[3 * o + 2];
     GdTri t;
     t.v0 = make_float4(verts[3 * a], verts[3 * a + 1], verts[3 * a + 2], __int_as_float(o));

@@ -166,9 +166,10 @@ GD_HD GdExclude gd_no_exclude() { GdExclude x = {-1, -1, -1}; return x; }
 
 GD_HD void gd_test_leaf(const GdBvh &bvh, const GdRay &ray, int leaf, int filter_mat, float t_min, const GdExclude &ex,
                         GdHit &hit, unsigned &n_tri_tests) {
-    if (leaf == ex.a || leaf == ex.b || leaf == ex.c) return;
     const GdTri &tr = bvh.tris[leaf];
     float4 p0 = tr.v0, p1 = tr.v1, p2 = tr.v2;
+    const int facet = gd_as_int(p0.w);                       // caller's facet index (a facet may own several leaves)
+    if (facet == ex.a || facet == ex.b || facet == ex.c) return;
     float t, det;
     n_tri_tests++;
     if (!gd_ray_tri(ray, p0, p1, p2, t, det)) return;
@@ -179,23 +180,38 @@ GD_HD void gd_test_leaf(const GdBvh &bvh, const GdRay &ray, int leaf, int filter
         int from = leaving ? gd_mat_inside(mats) : gd_mat_outside(mats);
         if (from != filter_mat) return;
     }
-    int orig = gd_as_int(p0.w);
+    int orig = facet;
     if (t < hit.t || hit.leaf < 0 || orig < hit.orig) {
         hit.t = t; hit.leaf = leaf; hit.orig = orig; hit.leaving = leaving; hit.mats = mats;
     }
 }
 
+#ifdef __CUDA_ARCH__
+#define GD_WARP_ALL(p) __all_sync(0xFFFFFFFFu, (p))
+#else
+#define GD_WARP_ALL(p) (p)
+#endif
+
 // Nearest facet with t in (t_min, t_max].  On return hit.leaf < 0 if none.
+// WARP-SYNCHRONOUS: all 32 lanes of a warp must call it together (lanes without a ray pass active = false).  The
+// vote at the end of every outer iteration re-converges the warp once per leaf visit; without it the lanes of a
+// warp drift apart inside the two nested loops and the kernel runs at ~3.6 of 32 lanes (profiles/r01_*).
+// SYNC = false: plain per-lane loop (history-per-thread kernel, host emulation).
+template <bool SYNC>
 GD_HD void gd_nearest_hit(const GdBvh &bvh, const GdRay &ray, float t_min, float t_max, int filter_mat,
-                          const GdExclude &ex, GdHit &hit, unsigned &n_box_tests, unsigned &n_tri_tests) {
+                          const GdExclude &ex, bool active, GdHit &hit, unsigned &n_box_tests, unsigned &n_tri_tests) {
     hit.t = t_max; hit.leaf = -1; hit.orig = 0x7FFFFFFF; hit.leaving = 0; hit.mats = 0;
-    if (bvh.root_is_leaf) { gd_test_leaf(bvh, ray, 0, filter_mat, t_min, ex, hit, n_tri_tests); return; }
+    if (bvh.root_is_leaf) {
+        if (active) gd_test_leaf(bvh, ray, 0, filter_mat, t_min, ex, hit, n_tri_tests);
+        return;
+    }
     int stack[GD_STACK];
     int sp = 0;
     int node = 0;
+    bool done = !active;
     const float pad = 4.0e-7f;     // far side padded by ~3 ulp (robust slab test)
     for (;;) {
-        while (node >= 0) {
+        while (!done && node >= 0) {
             const GdNode &nd = bvh.nodes[node];
             float4 a = nd.n0xy, b = nd.n1xy, z = nd.nz;
             int4 lk = nd.link;
@@ -222,14 +238,61 @@ GD_HD void gd_nearest_hit(const GdBvh &bvh, const GdRay &ray, float t_min, float
                 node = lk.x;
             } else if (h1) {
                 node = lk.y;
+            } else if (sp == 0) {
+                done = true;
             } else {
-                if (sp == 0) return;
                 node = stack[--sp];
             }
         }
-        // leaf
-        gd_test_leaf(bvh, ray, ~node, filter_mat, t_min, ex, hit, n_tri_tests);
-        if (sp == 0) return;
-        node = stack[--sp];
+        if (!done) {     // leaf
+            gd_test_leaf(bvh, ray, ~node, filter_mat, t_min, ex, hit, n_tri_tests);
+            if (sp == 0) done = true;
+            else node = stack[--sp];
+        }
+        if (SYNC ? GD_WARP_ALL(done) : done) break;
     }
+}
+
+// ---------------------------------------------------------------- reference splitting for long thin facets
+// A cap of a revolved surface is a fan of N_theta slivers (PAPER.md:82-90 angularly equidistant sampling); the AABB
+// of a sliver covers up to a quarter of the cap, so a ray through the cap would have to test dozens of them.  The
+// builder therefore cuts a long facet into k references along its longest axis; each reference keeps the facet
+// index and gets the AABB of the facet clipped to its slab.  (Early split clipping, Ernst & Greiner 2007, restated.)
+// k = how loose the facet's AABB is: half its surface area over the facet area (2 for a tight axis-aligned fit)
+GD_HD int gd_split_count(const float p[3][3], const float lo[3], const float hi[3], int max_splits, int &axis) {
+    float e[3] = {hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]};
+    axis = e[0] > e[1] ? (e[0] > e[2] ? 0 : 2) : (e[1] > e[2] ? 1 : 2);
+    float ux = p[1][0] - p[0][0], uy = p[1][1] - p[0][1], uz = p[1][2] - p[0][2];
+    float vx = p[2][0] - p[0][0], vy = p[2][1] - p[0][1], vz = p[2][2] - p[0][2];
+    float cx = uy * vz - uz * vy, cy = uz * vx - ux * vz, cz = ux * vy - uy * vx;
+    float area = 0.5f * sqrtf(cx * cx + cy * cy + cz * cz);
+    float half_sa = e[0] * e[1] + e[1] * e[2] + e[2] * e[0];
+    if (!(area > 0.0f) || !(e[axis] > 0.0f)) return 1;
+    int k = (int)ceilf(half_sa / area * 0.25f);
+    if (k < 1) k = 1;
+    if (k > max_splits) k = max_splits;
+    return k;
+}
+
+// AABB of triangle (p0,p1,p2) clipped to the slab [a,b] on `axis`; conservative (padded by 1 ulp-ish of the slab)
+GD_HD void gd_clip_tri_box(const float p[3][3], int axis, float a, float b, float lo[3], float hi[3]) {
+    for (int k = 0; k < 3; ++k) { lo[k] = 3.0e38f; hi[k] = -3.0e38f; }
+    for (int i = 0; i < 3; ++i) {
+        const float *u = p[i], *v = p[(i + 1) % 3];
+        float ua = u[axis], va = v[axis];
+        if (ua >= a && ua <= b)
+            for (int k = 0; k < 3; ++k) { lo[k] = fminf(lo[k], u[k]); hi[k] = fmaxf(hi[k], u[k]); }
+        for (int s = 0; s < 2; ++s) {       // edge crossings with the two slab planes
+            float pl = s == 0 ? a : b;
+            if ((ua < pl && va > pl) || (ua > pl && va < pl)) {
+                float f = (pl - ua) / (va - ua);
+                for (int k = 0; k < 3; ++k) {
+                    float x = k == axis ? pl : u[k] + f * (v[k] - u[k]);
+                    float padk = 4.0e-7f * (fabsf(u[k]) + fabsf(v[k])) + 1.0e-30f;
+                    lo[k] = fminf(lo[k], x - padk); hi[k] = fmaxf(hi[k], x + padk);
+                }
+            }
+        }
+    }
+    lo[axis] = fmaxf(lo[axis], a); hi[axis] = fminf(hi[axis], b);
 }

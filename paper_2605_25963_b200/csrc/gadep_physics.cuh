@@ -197,7 +197,7 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const GdSource &S, unsi
         cnt.n_crossings++;
         L.need_mu = 1;
         if (t > GD_TBACK) { L.ex = gd_no_exclude(); L.n_stall = 0; }      // earlier facets left the window
-        L.ex.c = L.ex.b; L.ex.b = L.ex.a; L.ex.a = hit.leaf;
+        L.ex.c = L.ex.b; L.ex.b = L.ex.a; L.ex.a = hit.orig;
         if (L.m == GD_MAT_KILL) { L.flags |= GD_F_ESCAPED; cnt.n_escaped++; photon_done = true; }
         else if (++L.n_stall > 32) {       // > 32 facets inside 0.1 um: degenerate mesh; stop instead of spinning
             L.flags |= GD_F_ESCAPED | GD_F_LEAK; cnt.n_escaped++; cnt.n_leak++; photon_done = true;
@@ -271,7 +271,7 @@ GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *t
         gd_lane_query(L, M, tab, t_min, t_max, filter);
         gd_ray_setup(ray, L.pos, L.dir);
         cnt.n_queries++;
-        gd_nearest_hit(bvh, ray, t_min, t_max, filter, L.ex, hit, cnt.n_box_tests, cnt.n_tri_tests);
+        gd_nearest_hit<false>(bvh, ray, t_min, t_max, filter, L.ex, true, hit, cnt.n_box_tests, cnt.n_tri_tests);
         if (gd_lane_post(L, M, S, seed, hit, out, cnt)) return;
     }
 }

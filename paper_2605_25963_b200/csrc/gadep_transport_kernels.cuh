@@ -33,15 +33,21 @@ gd_k_trace(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ d
            float t_min, int *__restrict__ tri_out, float *__restrict__ t_out, GdCounters *counters) {
     GdLocalCounters cnt = {};
     unsigned nq = 0;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long base = (long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31); base < n; base += stride) {   // warp-uniform
+        const long long i = base + (threadIdx.x & 31);
+        const bool active = i < n;
         GdRay ray;
-        gd_ray_setup(ray, gd_make(org[3 * i], org[3 * i + 1], org[3 * i + 2]),
-                     gd_make(dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]));
+        if (active) gd_ray_setup(ray, gd_make(org[3 * i], org[3 * i + 1], org[3 * i + 2]),
+                                 gd_make(dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]));
+        else gd_ray_setup(ray, gd_make(0.f, 0.f, 0.f), gd_make(0.f, 0.f, 1.f));
         GdHit hit;
-        gd_nearest_hit(bvh, ray, t_min, GD_INF, filter_mat, gd_no_exclude(), hit, cnt.n_box_tests, cnt.n_tri_tests);
-        tri_out[i] = hit.leaf < 0 ? -1 : hit.orig;
-        t_out[i] = hit.leaf < 0 ? GD_INF : hit.t;
-        nq++;
+        gd_nearest_hit<true>(bvh, ray, t_min, GD_INF, filter_mat, gd_no_exclude(), active, hit, cnt.n_box_tests, cnt.n_tri_tests);
+        if (active) {
+            tri_out[i] = hit.leaf < 0 ? -1 : hit.orig;
+            t_out[i] = hit.leaf < 0 ? GD_INF : hit.t;
+            nq++;
+        }
     }
     cnt.n_queries = nq;
     gd_flush_counters(cnt, counters, 0);
@@ -124,6 +130,7 @@ gd_k_transport_refill(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src
     unsigned long long w_cur = 0, w_end = 0;     // warp-uniform chunk of history indices [w_cur, w_end)
     GdLane L;
     L.mode = GD_MODE_NEED;
+    L.ex = gd_no_exclude();
     for (;;) {
         // ---- refill
         unsigned need_mask = __ballot_sync(0xFFFFFFFFu, L.mode == GD_MODE_NEED);
@@ -145,16 +152,21 @@ gd_k_transport_refill(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src
             else w_cur += n_need;
         }
         if (__all_sync(0xFFFFFFFFu, L.mode == GD_MODE_DONE)) break;
-        // ---- one query per live lane
-        if (L.mode != GD_MODE_DONE) {
-            float t_min, t_max;
-            int filter;
+        // ---- one query per live lane; the traversal is warp-synchronous
+        const bool live = L.mode != GD_MODE_DONE;
+        float t_min = 0.0f, t_max = 0.0f;
+        int filter = -2;
+        GdRay ray;
+        if (live) {
             gd_lane_query(L, M, s_tab, t_min, t_max, filter);
-            GdRay ray;
             gd_ray_setup(ray, L.pos, L.dir);
-            GdHit hit;
             cnt.n_queries++;
-            gd_nearest_hit(bvh, ray, t_min, t_max, filter, L.ex, hit, cnt.n_box_tests, cnt.n_tri_tests);
+        } else {
+            gd_ray_setup(ray, gd_make(0.f, 0.f, 0.f), gd_make(0.f, 0.f, 1.f));
+        }
+        GdHit hit;
+        gd_nearest_hit<true>(bvh, ray, t_min, t_max, filter, L.ex, live, hit, cnt.n_box_tests, cnt.n_tri_tests);
+        if (live) {
             GdHistory r;
             if (gd_lane_post(L, M, s_src, seed, hit, r, cnt)) {
                 n_done++;
