@@ -105,7 +105,8 @@ int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
 #define GADEP_RUN_ASYNC 1          /* do not synchronise the stream; spectrum must then be a DEVICE pointer     */
 #define GADEP_RUN_ACCUMULATE 2     /* add to the context's tallies instead of starting from zero                */
 #define GADEP_RUN_HISTORY_PER_THREAD 4  /* measurement: the plain one-history-per-thread kernel instead of the   */
-                                   /* persistent-lane kernel (same results, bit for bit)                        */
+                                   /* warp-resident wavefront kernel (same results, bit for bit)                */
+#define GADEP_RUN_PERSISTENT_LANES 8    /* measurement: one history per lane with refill (same results)           */
 typedef struct {
     int n_bins;                    /* spectrum bins over [0, e_max_mev); one extra overflow slot follows        */
     float e_max_mev;
@@ -152,6 +153,8 @@ typedef struct {
     int n_bvh_nodes, bvh_max_depth;
     float last_run_ms, last_build_ms;      /* CUDA-event times of the last gadep_run / gadep_build_bvh kernels   */
     int last_run_launches, last_build_launches;
+    unsigned long long n_safety_queries;   /* wavefront kernel: facet-free-sphere queries issued                 */
+    unsigned long long n_skipped_queries;  /* flights whose nearest-hit query was answered by such a sphere      */
 } gadep_counters;
 /* Counters of the last gadep_run / gadep_run_histories / gadep_trace_rays (HOST output). */
 int gadep_get_counters(const gadep_ctx *ctx, gadep_counters *out);

@@ -16,7 +16,7 @@ F_ESCAPED, F_PEAK, F_LEAK, F_NONSCORING = 1, 2, 4, 8
 FILTER_NONE = -2
 MAT_KILL = -1
 MAX_LINES = 64
-RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD = 1, 2, 4
+RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES = 1, 2, 4, 8
 
 EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_set_materials", "gadep_load_mesh",
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
@@ -46,7 +46,8 @@ class GadepCounters(C.Structure):
                                              "n_cutoff")] + \
                [("emitted", C.c_ulonglong * MAX_LINES), ("peak", C.c_ulonglong * MAX_LINES), ("n_lines", C.c_int),
                 ("n_bvh_nodes", C.c_int), ("bvh_max_depth", C.c_int), ("last_run_ms", C.c_float),
-                ("last_build_ms", C.c_float), ("last_run_launches", C.c_int), ("last_build_launches", C.c_int)]
+                ("last_build_ms", C.c_float), ("last_run_launches", C.c_int), ("last_build_launches", C.c_int),
+                ("n_safety_queries", C.c_ulonglong), ("n_skipped_queries", C.c_ulonglong)]
 
     def as_dict(self):
         d = {n: int(getattr(self, n)) for n, _ in self._fields_[:12]}
@@ -54,7 +55,8 @@ class GadepCounters(C.Structure):
         d.update(emitted=[int(x) for x in self.emitted[:nl]], peak=[int(x) for x in self.peak[:nl]], n_lines=nl,
                  n_bvh_nodes=int(self.n_bvh_nodes), bvh_max_depth=int(self.bvh_max_depth),
                  last_run_ms=float(self.last_run_ms), last_build_ms=float(self.last_build_ms),
-                 last_run_launches=int(self.last_run_launches), last_build_launches=int(self.last_build_launches))
+                 last_run_launches=int(self.last_run_launches), last_build_launches=int(self.last_build_launches),
+                 n_safety_queries=int(self.n_safety_queries), n_skipped_queries=int(self.n_skipped_queries))
         return d
 
 

@@ -15,6 +15,7 @@
 #include "../../include/gadep.h"
 #include "gadep_build_kernels.cuh"
 #include "gadep_transport_kernels.cuh"
+#include "gadep_wave_kernels.cuh"
 
 struct gadep_ctx {
     int device = 0;
@@ -33,6 +34,7 @@ struct gadep_ctx {
     float *d_verts = nullptr;
     int *d_tris = nullptr, *d_tri_mats = nullptr, *d_tri_surf = nullptr;
     GdNode *d_nodes = nullptr;
+    GdNode4 *d_nodes4 = nullptr;
     GdTri *d_leaf_tris = nullptr;
     int bvh_depth = 0;
     int n_ref = 0;                 // leaves of the BVH: facet references after splitting
@@ -45,7 +47,10 @@ struct gadep_ctx {
     int cap_bins = 0;
     GdCounters *d_counters = nullptr;
     unsigned long long *d_next = nullptr;     // history counter of the refill kernel
-    int kernel_variant = 1;                   // 1 = persistent lanes with refill, 0 = history per thread
+    int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
+    float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
+    size_t pair_floats = 0;
+    GdWaveTune tune = {8, 8, 4, 4.0f, 8.0f};
     int n_bins = 0;
     float spec_e_max = 0;
     bool results_stale = false, have_results = false;
@@ -110,13 +115,19 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb1);
     if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
+    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,leaf_thresh" (measurement sweeps)
+        int a, b, d;
+        float lm = c->tune.lam_max, cm = c->tune.cap_mfp;
+        int k = sscanf(t, "%d,%d,%d,%f,%f", &a, &b, &d, &lm, &cm);
+        if (k >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && lm >= 0 && cm > 0) c->tune = {a, b, d, lm, cm};
+    }
     *out = c;
     return GADEP_OK;
 }
 
 static void gd_free_mesh(gadep_ctx *c) {
     cudaFree(c->d_verts); cudaFree(c->d_tris); cudaFree(c->d_tri_mats); cudaFree(c->d_tri_surf);
-    cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris);
+    cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris); cudaFree(c->d_nodes4); c->d_nodes4 = nullptr;
     c->d_verts = nullptr; c->d_tris = c->d_tri_mats = c->d_tri_surf = nullptr;
     c->d_nodes = nullptr; c->d_leaf_tris = nullptr;
     c->have_mesh = c->have_bvh = false;
@@ -127,7 +138,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next);
+    cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     if (c->evb0) cudaEventDestroy(c->evb0);
@@ -232,8 +243,8 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     GD_CUDA(c, cudaSetDevice(c->device));
     const int n_tri = c->n_tri;
     cudaStream_t st = c->stream;
-    cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris);
-    c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->have_bvh = false;
+    cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris); cudaFree(c->d_nodes4);
+    c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->d_nodes4 = nullptr; c->have_bvh = false;
     const int tb = 256, nbt = (n_tri + tb - 1) / tb;
     int launches = 0;
     // ---- phase A: how many references (reference splitting) -> one 4-byte read-back sizes the arena
@@ -273,6 +284,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     do {
         if ((e = cudaMalloc(&c->d_nodes, sizeof(GdNode) * (size_t)std::max(n - 1, 1))) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_leaf_tris, sizeof(GdTri) * (size_t)n)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_nodes4, sizeof(GdNode4) * (size_t)std::max(n - 1, 1))) != cudaSuccess) break;
         float4 *ref_lo = (float4 *)(arena + o_tlo), *ref_hi = (float4 *)(arena + o_thi);
         float4 *node_lo = (float4 *)(arena + o_nlo), *node_hi = (float4 *)(arena + o_nhi);
         unsigned long long *keys[2] = {(unsigned long long *)(arena + o_k0), (unsigned long long *)(arena + o_k1)};
@@ -302,7 +314,8 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
             gd_k_karras<<<nb, tb, 0, st>>>(keys[cur], n, child_l, child_r, parent_int, parent_leaf);
             gd_k_refit<<<nb, tb, 0, st>>>(n, child_l, child_r, parent_int, parent_leaf, ref_lo, ref_hi, vals[cur], node_lo,
                                           node_hi, visits, c->d_nodes, scene + 6);
-            launches += 2;
+            gd_k_collapse4<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes4);
+            launches += 3;
         }
         cudaEventRecord(c->evb1, st);
         if ((e = cudaGetLastError()) != cudaSuccess) break;
@@ -312,7 +325,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     } while (0);
     cudaFree(arena); cudaFree(counts); cudaFree(scene);
     if (e != cudaSuccess) rc = gd_fail(c, GADEP_E_CUDA, "BVH build failed: %s", cudaGetErrorString(e));
-    else if (depth >= GD_STACK) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
+    else if (depth >= GD_STACK || 3 * ((depth + 1) / 2) + 4 > GD_STACK4) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
     if (rc != GADEP_OK) return rc;
     c->bvh_depth = depth;
     c->n_ref = n;
@@ -323,7 +336,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
 
 static GdBvh gd_bvh_view(const gadep_ctx *c) {
     GdBvh b;
-    b.nodes = c->d_nodes; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
+    b.nodes = c->d_nodes; b.nodes4 = c->d_nodes4; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
     return b;
 }
 
@@ -401,28 +414,43 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     GdTally T;
     T.spectrum = c->d_tally; T.emitted = c->d_tally + n_bins + 1; T.peak = T.emitted + GADEP_MAX_LINES;
     T.counters = c->d_counters; T.n_bins = n_bins; T.inv_de = (float)((double)n_bins / (double)e_max);
+    if (n > 0xFFFFFFFFull) return gd_fail(c, GADEP_E_ARG, "more than 2^32-1 histories in one launch");
     size_t smem = sizeof(float) * (size_t)c->n_mat * 4 * c->n_grid + sizeof(unsigned) * ((size_t)n_bins + 1);
-    if (smem > 200 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum (%zu B) do not fit in shared memory", smem);
-    const bool refill = c->kernel_variant == 1;
-    const void *kern = refill ? (const void *)gd_k_transport_refill : (const void *)gd_k_transport;
+    const int variant = c->kernel_variant;
+    const int threads = variant == 2 ? GD_W_THREADS : GD_RUN_THREADS;
+    if (variant == 2) smem += sizeof(float) * (size_t)GD_W_WARPS * GD_W_NF * GD_W_SLOTS;
+    if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
+    const void *kern = variant == 2 ? (const void *)gd_k_transport_wave
+                                    : (variant == 1 ? (const void *)gd_k_transport_refill : (const void *)gd_k_transport);
     GD_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1;
-    if (refill) GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gd_k_transport_refill, GD_RUN_THREADS, smem));
-    else GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gd_k_transport, GD_RUN_THREADS, smem));
-    if (per_sm < 1) per_sm = 1;
-    unsigned long long want = (n + GD_RUN_THREADS - 1) / GD_RUN_THREADS;
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
+    if (per_sm < 1) return gd_fail(c, GADEP_E_CUDA, "transport kernel does not fit on an SM (%zu B shared memory)", smem);
+    const unsigned long long per_block = variant == 2 ? (unsigned long long)GD_W_WARPS * GD_W_SLOTS : GD_RUN_THREADS;
+    unsigned long long want = (n + per_block - 1) / per_block;
     int grid = (int)std::min<unsigned long long>((unsigned long long)c->n_sm * per_sm, std::max<unsigned long long>(want, 1));
+    if (variant == 2) {
+        size_t need = (size_t)grid * GD_W_WARPS * GD_W_SLOTS * 8;
+        if (need > c->pair_floats) {
+            cudaFree(c->d_pair); c->d_pair = nullptr; c->pair_floats = 0;
+            GD_CUDA(c, cudaMalloc(&c->d_pair, need * sizeof(float)));
+            c->pair_floats = need;
+        }
+    }
     GD_CUDA(c, cudaEventRecord(c->ev0, st));
     c->last_run_launches = 0;
     if (n > 0) {
-        if (refill) {
-            unsigned long long warps = (unsigned long long)grid * (GD_RUN_THREADS / 32);
-            unsigned chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / (warps * 16)));
-            GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
-            gd_k_transport_refill<<<grid, GD_RUN_THREADS, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
-                                                                     d_flags, c->d_next, chunk);
+        unsigned long long warps = (unsigned long long)grid * (threads / 32);
+        unsigned chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / (warps * 16)));
+        if (variant != 0) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
+        if (variant == 2) {
+            gd_k_transport_wave<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
+                                                             c->d_next, chunk, c->d_pair, c->tune);
+        } else if (variant == 1) {
+            gd_k_transport_refill<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
+                                                               d_flags, c->d_next, chunk);
         } else {
-            gd_k_transport<<<grid, GD_RUN_THREADS, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+            gd_k_transport<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
         }
         c->last_run_launches = 1;
     }
@@ -456,7 +484,7 @@ extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned 
     bool dev_out = gd_is_device_ptr(spectrum);
     if ((opts->flags & GADEP_RUN_ASYNC) && spectrum && !dev_out)
         return gd_fail(c, GADEP_E_ARG, "GADEP_RUN_ASYNC needs a device spectrum pointer");
-    c->kernel_variant = (opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : 1;
+    c->kernel_variant = (opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((opts->flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2);
     int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
                                  (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
     if (rc) return rc;
@@ -516,9 +544,14 @@ extern "C" int gadep_trace_rays(gadep_ctx *c, const float *org, const float *dir
         cudaMemcpyAsync(stage + 3 * n_rays, dir, nb3, cudaMemcpyHostToDevice, st);
     }
     cudaMemsetAsync(c->d_counters, 0, sizeof(GdCounters), st);
-    int grid = (int)std::min<long long>((n_rays + 255) / 256, (long long)c->n_sm * 8);
+    int per_sm = 1;
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gd_k_trace_wave, 256, 0));
+    int grid = (int)std::min<long long>((n_rays + 255) / 256, (long long)c->n_sm * std::max(per_sm, 1));
+    unsigned chunk = (unsigned)std::min<long long>(2048, std::max<long long>(32, n_rays / ((long long)grid * 8 * 8)));
+    cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st);
     cudaEventRecord(c->ev0, st);
-    gd_k_trace<<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t, c->d_counters);
+    gd_k_trace_wave<<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
+                                          c->d_counters, c->d_next, chunk, c->tune);
     cudaEventRecord(c->ev1, st);
     c->last_run_launches = 1;
     cudaError_t e = cudaGetLastError();
@@ -567,7 +600,7 @@ extern "C" int gadep_get_counters(const gadep_ctx *cc, gadep_counters *out) {
     out->n_histories = h.n_histories; out->n_queries = h.n_queries; out->n_box_tests = h.n_box_tests;
     out->n_tri_tests = h.n_tri_tests; out->n_crossings = h.n_crossings; out->n_pe = h.n_pe; out->n_compton = h.n_compton;
     out->n_coherent = h.n_coherent; out->n_pair = h.n_pair; out->n_escaped = h.n_escaped; out->n_leak = h.n_leak;
-    out->n_cutoff = h.n_cutoff;
+    out->n_cutoff = h.n_cutoff; out->n_safety_queries = h.n_safety; out->n_skipped_queries = h.n_skipped;
     memcpy(out->emitted, c->h_emitted, sizeof(out->emitted));
     memcpy(out->peak, c->h_peak, sizeof(out->peak));
     out->n_lines = c->src.n_lines;
@@ -602,3 +635,12 @@ extern "C" int gadep_philox_raw(gadep_ctx *c, const unsigned *ctr4, const unsign
     if (e != cudaSuccess) return gd_fail(c, GADEP_E_CUDA, "philox kernel failed: %s", cudaGetErrorString(e));
     return GADEP_OK;
 }
+
+#ifdef GD_DIAG
+extern "C" int gadep_debug_read(unsigned long long *out128, int reset) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out128, gd_diag, sizeof(unsigned long long) * 128);
+    if (reset) { unsigned long long z[128] = {}; cudaMemcpyToSymbol(gd_diag, z, sizeof(z)); }
+    return 0;
+}
+#endif

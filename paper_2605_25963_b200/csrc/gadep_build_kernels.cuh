@@ -268,3 +268,40 @@ __global__ void gd_k_refit(int n, const int *__restrict__ child_l, const int *__
         cur = parent_int[cur];
     }
 }
+
+// ---------------------------------------------------------------- 4-wide collapse
+// Node4(i) holds, for each child of binary node i, that child itself if it is a leaf and its two children otherwise
+// (2-4 entries).  Written for every binary node; the traversal only ever reaches those an even number of binary
+// levels below the root (or below a leaf-shortened path).
+__global__ void gd_k_collapse4(int n_inner, const int *__restrict__ child_l, const int *__restrict__ child_r,
+                               const float4 *__restrict__ ref_lo, const float4 *__restrict__ ref_hi,
+                               const unsigned *__restrict__ order, const float4 *__restrict__ node_lo,
+                               const float4 *__restrict__ node_hi, GdNode4 *__restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_inner) return;
+    int c[4] = {GD_NO_CHILD, GD_NO_CHILD, GD_NO_CHILD, GD_NO_CHILD};
+    int k = 0;
+    const int two[2] = {child_l[i], child_r[i]};
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        if (two[j] < 0) c[k++] = two[j];
+        else { c[k++] = child_l[two[j]]; c[k++] = child_r[two[j]]; }
+    }
+    float lo[4][3], hi[4][3];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+        if (c[j] != GD_NO_CHILD) {
+            if (c[j] < 0) { int o = (int)order[~c[j]]; a = ref_lo[o]; b = ref_hi[o]; }
+            else { a = node_lo[c[j]]; b = node_hi[c[j]]; }
+        }
+        lo[j][0] = a.x; lo[j][1] = a.y; lo[j][2] = a.z; hi[j][0] = b.x; hi[j][1] = b.y; hi[j][2] = b.z;
+    }
+    GdNode4 nd;
+    nd.lox = make_float4(lo[0][0], lo[1][0], lo[2][0], lo[3][0]); nd.hix = make_float4(hi[0][0], hi[1][0], hi[2][0], hi[3][0]);
+    nd.loy = make_float4(lo[0][1], lo[1][1], lo[2][1], lo[3][1]); nd.hiy = make_float4(hi[0][1], hi[1][1], hi[2][1], hi[3][1]);
+    nd.loz = make_float4(lo[0][2], lo[1][2], lo[2][2], lo[3][2]); nd.hiz = make_float4(hi[0][2], hi[1][2], hi[2][2], hi[3][2]);
+    nd.child = make_int4(c[0], c[1], c[2], c[3]);
+    nd.pad = make_int4(0, 0, 0, 0);
+    out[i] = nd;
+}

@@ -14,6 +14,7 @@
 #define GD_MAX_LINES 64
 #define GD_MAX_MAT 16
 #define GD_STACK 96                 // LBVH depth bound: 63 Morton bits + index tie-break bits
+#define GD_STACK4 148                // 4-wide traversal: up to 3 pushes per two binary levels
 
 #define GD_F_ESCAPED 1u
 #define GD_F_PEAK 2u
@@ -36,8 +37,19 @@ struct __align__(16) GdTri {
     float4 v0, v1, v2;
 };
 
+// 4-wide node of the wavefront kernels (128 bytes = 8 x 16 B loads): the grandchildren of a binary node, boxes in SoA
+// (component k of lox .. hiz belongs to child k).  child: >= 0 inner node index (same numbering as the binary
+// nodes), < 0 leaf (~index into the leaf-ordered triangles), GD_NO_CHILD = unused entry.
+#define GD_NO_CHILD ((int)0x80000000)
+struct __align__(16) GdNode4 {
+    float4 lox, hix, loy, hiy, loz, hiz;
+    int4 child;
+    int4 pad;
+};
+
 struct GdBvh {
     const GdNode *nodes;
+    const GdNode4 *nodes4;
     const GdTri *tris;
     int n_tri;
     int root_is_leaf;   // n_tri == 1
@@ -45,7 +57,7 @@ struct GdBvh {
 
 struct GdCounters {    // device-side totals, 64-bit
     unsigned long long n_histories, n_queries, n_box_tests, n_tri_tests, n_crossings, n_pe, n_compton, n_coherent,
-        n_pair, n_escaped, n_leak, n_cutoff;
+        n_pair, n_escaped, n_leak, n_cutoff, n_safety, n_skipped;
 };
 
 struct GdLocalCounters {  // per-thread, 32-bit

@@ -1,0 +1,260 @@
+// gadep_trav.cuh -- resumable per-lane BVH traversal for the wavefront kernels (PAPER.md:219 BVH over the facets;
+// PAPER.md:191 nearest facet along the flight direction).
+//
+// A lane owns one ray at a time; its whole traversal state sits in registers (+ a local-memory stack), so that a
+// lane can (a) take a new ray the moment its ray ends while its neighbours keep going (dynamic fetch), and (b) hold
+// an unfinished ray across a physics burst of its warp.  One call of gd_trav_step advances every busy lane of the
+// warp by at most one inner-node visit and -- when enough lanes wait at a leaf -- one ray-triangle test.
+#pragma once
+#include "gadep_bvh.cuh"
+
+#define GD_TRAV_DONE ((int)0x80000000)     // node value: traversal finished (leaf codes are ~index > GD_TRAV_DONE)
+#define GD_NO_FACET 0x7FFFFFFF
+#define GD_TINF __int_as_float(0x7F800000)
+
+struct GdTrav {
+    float ox, oy, oz;        // origin (ray-triangle test)
+    float ix, iy, iz;        // safe reciprocal direction
+    float bx, by, bz;        // origin * reciprocal direction (slab test as one FMA per plane)
+    float err;               // absolute error bound of the FMA slab distances
+    float sx, sy, sz;        // Woop shear / scale
+    int kxyz;                // kx | ky << 2 | kz << 4
+    float tmin, t;           // window (tmin, t]; t shrinks to the nearest accepted hit
+    int orig;                // caller's facet index of that hit, GD_NO_FACET = none
+    int fromto;              // (from-side material & 0xFFFF) | (to-side material << 16) of that hit
+    int filter, exa, exb, exc;
+    int node, sp;
+    int slot;                // owner's handle (photon slot / ray index), < 0 = lane idle
+};
+
+GD_D void gd_trav_idle(GdTrav &T) { T.slot = -1; T.node = GD_TRAV_DONE; T.sp = 0; }
+
+GD_D void gd_trav_begin(GdTrav &T, const GdBvh &bvh, float px, float py, float pz, float dx, float dy, float dz,
+                        float t_min, float t_max, int filter, int exa, int exb, int exc, int slot) {
+    T.ox = px; T.oy = py; T.oz = pz;
+    T.ix = gd_safe_rcp(dx); T.iy = gd_safe_rcp(dy); T.iz = gd_safe_rcp(dz);
+    T.bx = px * T.ix; T.by = py * T.iy; T.bz = pz * T.iz;
+    // |fma(lo, inv, -b) - exact| <= ulp(b) (rounding of b) + rounding of the result (covered by the far-side pad)
+    T.err = fmaxf(fmaxf(fabsf(T.bx), fabsf(T.by)), fabsf(T.bz)) * 1.1920929e-7f;
+    float ax = fabsf(dx), ay = fabsf(dy), az = fabsf(dz);
+    int kz = (ax > ay) ? (ax > az ? 0 : 2) : (ay > az ? 1 : 2);
+    int kx = kz + 1; if (kx == 3) kx = 0;
+    int ky = kx + 1; if (ky == 3) ky = 0;
+    float ddz = kz == 0 ? dx : (kz == 1 ? dy : dz);
+    if (ddz < 0.0f) { int t = kx; kx = ky; ky = t; }
+    float ddx = kx == 0 ? dx : (kx == 1 ? dy : dz), ddy = ky == 0 ? dx : (ky == 1 ? dy : dz);
+    T.sz = 1.0f / ddz; T.sx = ddx * T.sz; T.sy = ddy * T.sz;
+    T.kxyz = kx | (ky << 2) | (kz << 4);
+    T.tmin = t_min; T.t = t_max; T.orig = GD_NO_FACET; T.fromto = 0;
+    T.filter = filter; T.exa = exa; T.exb = exb; T.exc = exc;
+    T.sp = 0; T.node = bvh.root_is_leaf ? ~0 : 0;
+    T.slot = slot;
+}
+
+// Safety query (filter == GD_FILTER_SAFETY): lower bound of the distance from a point to the nearest facet, as the
+// distance to the nearest leaf box (a leaf box contains its facet part), searched up to radius sqrt(r2_cap).
+// T.t carries the squared bound; leaves are resolved in their parent, so no triangle is touched.
+#define GD_FILTER_SAFETY (-3)
+GD_D void gd_trav_begin_safety(GdTrav &T, const GdBvh &bvh, float px, float py, float pz, float r2_cap, int slot) {
+    T.ox = px; T.oy = py; T.oz = pz;
+    T.ix = T.iy = T.iz = T.bx = T.by = T.bz = T.err = T.sx = T.sy = T.sz = 0.0f;
+    T.kxyz = 0; T.tmin = 0.0f; T.t = r2_cap; T.orig = GD_NO_FACET; T.fromto = 0;
+    T.filter = GD_FILTER_SAFETY; T.exa = T.exb = T.exc = -1;
+    T.sp = 0; T.node = 0;
+    if (bvh.root_is_leaf) { T.t = 0.0f; T.node = GD_TRAV_DONE; }     // no inner node to read a box from
+    T.slot = slot;
+}
+
+GD_D float gd_box_dist2(float px, float py, float pz, float lx, float hx, float ly, float hy, float lz, float hz) {
+    float dx = fmaxf(fmaxf(lx - px, px - hx), 0.0f);
+    float dy = fmaxf(fmaxf(ly - py, py - hy), 0.0f);
+    float dz = fmaxf(fmaxf(lz - pz, pz - hz), 0.0f);
+    return fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+}
+
+GD_D void gd_trav_node_safety(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
+    const GdNode &nd = bvh.nodes[T.node];
+    const float4 a = nd.n0xy, b = nd.n1xy, z = nd.nz;
+    const int4 lk = nd.link;
+    n_box_tests += 2;
+    const float d0 = gd_box_dist2(T.ox, T.oy, T.oz, a.x, a.y, a.z, a.w, z.x, z.y);
+    const float d1 = gd_box_dist2(T.ox, T.oy, T.oz, b.x, b.y, b.z, b.w, z.z, z.w);
+    bool v0 = d0 < T.t, v1 = d1 < T.t;
+    if (v0 && lk.x < 0) { T.t = d0; v0 = false; v1 = v1 && d1 < T.t; }
+    if (v1 && lk.y < 0) { T.t = d1; v1 = false; v0 = v0 && d0 < T.t; }
+    if (v0 && v1) {
+        int near_c = lk.x, far_c = lk.y;
+        if (d1 < d0) { near_c = lk.y; far_c = lk.x; }
+        stack[T.sp++] = far_c;
+        T.node = near_c;
+    } else if (v0) {
+        T.node = lk.x;
+    } else if (v1) {
+        T.node = lk.y;
+    } else {
+        T.node = T.sp == 0 ? GD_TRAV_DONE : stack[--T.sp];
+    }
+}
+
+GD_D float gd_sel3(float x, float y, float z, int k) { return k == 0 ? x : (k == 1 ? y : z); }
+
+// same arithmetic as gd_ray_tri / gd_test_leaf (gadep_bvh.cuh), on the register-resident ray
+GD_D void gd_trav_leaf(GdTrav &T, const GdBvh &bvh, int leaf, unsigned &n_tri_tests) {
+    const GdTri &tr = bvh.tris[leaf];
+    float4 p0 = tr.v0, p1 = tr.v1, p2 = tr.v2;
+    const int facet = __float_as_int(p0.w);
+    if (facet == T.exa || facet == T.exb || facet == T.exc) return;
+    n_tri_tests++;
+    const int kx = T.kxyz & 3, ky = (T.kxyz >> 2) & 3, kz = T.kxyz >> 4;
+    float a0 = p0.x - T.ox, a1 = p0.y - T.oy, a2 = p0.z - T.oz;
+    float b0 = p1.x - T.ox, b1 = p1.y - T.oy, b2 = p1.z - T.oz;
+    float c0 = p2.x - T.ox, c1 = p2.y - T.oy, c2 = p2.z - T.oz;
+    float akz = gd_sel3(a0, a1, a2, kz), bkz = gd_sel3(b0, b1, b2, kz), ckz = gd_sel3(c0, c1, c2, kz);
+    float ax = GD_SUB(gd_sel3(a0, a1, a2, kx), GD_MUL(T.sx, akz)), ay = GD_SUB(gd_sel3(a0, a1, a2, ky), GD_MUL(T.sy, akz));
+    float bx = GD_SUB(gd_sel3(b0, b1, b2, kx), GD_MUL(T.sx, bkz)), by = GD_SUB(gd_sel3(b0, b1, b2, ky), GD_MUL(T.sy, bkz));
+    float cx = GD_SUB(gd_sel3(c0, c1, c2, kx), GD_MUL(T.sx, ckz)), cy = GD_SUB(gd_sel3(c0, c1, c2, ky), GD_MUL(T.sy, ckz));
+    float u = GD_SUB(GD_MUL(cx, by), GD_MUL(cy, bx));
+    float v = GD_SUB(GD_MUL(ax, cy), GD_MUL(ay, cx));
+    float w = GD_SUB(GD_MUL(bx, ay), GD_MUL(by, ax));
+    if (u == 0.0f || v == 0.0f || w == 0.0f) {          // on an edge in float: decide in double
+        double du = GD_DSUB(GD_DMUL((double)cx, (double)by), GD_DMUL((double)cy, (double)bx));
+        double dv = GD_DSUB(GD_DMUL((double)ax, (double)cy), GD_DMUL((double)ay, (double)cx));
+        double dw = GD_DSUB(GD_DMUL((double)bx, (double)ay), GD_DMUL((double)by, (double)ax));
+        u = (float)du; v = (float)dv; w = (float)dw;
+        if ((du < 0.0 || dv < 0.0 || dw < 0.0) && (du > 0.0 || dv > 0.0 || dw > 0.0)) return;
+    } else if ((u < 0.0f || v < 0.0f || w < 0.0f) && (u > 0.0f || v > 0.0f || w > 0.0f)) {
+        return;
+    }
+    float det = u + v + w;
+    if (det == 0.0f) return;
+    float az = T.sz * akz, bz = T.sz * bkz, cz = T.sz * ckz;
+    float tt = u * az + v * bz + w * cz;
+    float t = tt / det;
+    if (!(t > T.tmin) || t > T.t) return;
+    const int leaving = det < 0.0f;
+    const int mats = __float_as_int(p1.w);
+    const int m_in = gd_mat_inside(mats), m_out = gd_mat_outside(mats);
+    const int from = leaving ? m_in : m_out, to = leaving ? m_out : m_in;
+    if (T.filter != -2 && from != T.filter) return;
+    if (t < T.t || facet < T.orig) {
+        T.t = t; T.orig = facet; T.fromto = (from & 0xFFFF) | (int)((unsigned)(to & 0xFFFF) << 16);
+    }
+}
+
+GD_D int gd_trav_pop(GdTrav &T, const int *stack) { return T.sp == 0 ? GD_TRAV_DONE : stack[--T.sp]; }
+
+// one inner-node visit (two child boxes); far sides padded by the FMA error bound and ~3 ulp
+GD_D void gd_trav_node(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
+    const GdNode &nd = bvh.nodes[T.node];
+    const float4 a = nd.n0xy, b = nd.n1xy, z = nd.nz;
+    const int4 lk = nd.link;
+    n_box_tests += 2;
+    const float pad = 4.0e-7f;
+    float x0 = fmaf(a.x, T.ix, -T.bx), x1 = fmaf(a.y, T.ix, -T.bx);
+    float y0 = fmaf(a.z, T.iy, -T.by), y1 = fmaf(a.w, T.iy, -T.by);
+    float z0 = fmaf(z.x, T.iz, -T.bz), z1 = fmaf(z.y, T.iz, -T.bz);
+    float n0 = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), T.tmin + T.err));
+    float f0 = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fminf(fmaxf(z0, z1), T.t));
+    f0 = fmaf(fabsf(f0), pad, f0) + 2.0f * T.err;
+    x0 = fmaf(b.x, T.ix, -T.bx); x1 = fmaf(b.y, T.ix, -T.bx);
+    y0 = fmaf(b.z, T.iy, -T.by); y1 = fmaf(b.w, T.iy, -T.by);
+    z0 = fmaf(z.z, T.iz, -T.bz); z1 = fmaf(z.w, T.iz, -T.bz);
+    float n1 = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), T.tmin + T.err));
+    float f1 = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fminf(fmaxf(z0, z1), T.t));
+    f1 = fmaf(fabsf(f1), pad, f1) + 2.0f * T.err;
+    const bool h0 = n0 <= f0, h1 = n1 <= f1;
+    if (h0 && h1) {
+        int near_c = lk.x, far_c = lk.y;
+        if (n1 < n0) { near_c = lk.y; far_c = lk.x; }
+        stack[T.sp++] = far_c;
+        T.node = near_c;
+    } else if (h0) {
+        T.node = lk.x;
+    } else if (h1) {
+        T.node = lk.y;
+    } else {
+        T.node = gd_trav_pop(T, stack);
+    }
+}
+
+#define GD_CSWAP(ka, ca, kb, cb) do { if (kb < ka) { float tk = ka; ka = kb; kb = tk; int tc = ca; ca = cb; cb = tc; } } while (0)
+
+// order the four (key, child) pairs, push the valid ones farthest first, continue with the nearest
+GD_D void gd_trav_descend4(GdTrav &T, int *stack, float k0, float k1, float k2, float k3, int c0, int c1, int c2, int c3) {
+    GD_CSWAP(k0, c0, k1, c1); GD_CSWAP(k2, c2, k3, c3); GD_CSWAP(k0, c0, k2, c2); GD_CSWAP(k1, c1, k3, c3);
+    GD_CSWAP(k1, c1, k2, c2);
+    if (c3 != GD_NO_CHILD) stack[T.sp++] = c3;
+    if (c2 != GD_NO_CHILD) stack[T.sp++] = c2;
+    if (c1 != GD_NO_CHILD) stack[T.sp++] = c1;
+    T.node = c0 != GD_NO_CHILD ? c0 : gd_trav_pop(T, stack);
+}
+
+// one 4-wide node visit of a ray: FMA slab tests, far sides padded by the FMA error bound and ~3 ulp
+GD_D void gd_trav_node4(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
+    const GdNode4 &nd = bvh.nodes4[T.node];
+    const float4 lox = nd.lox, hix = nd.hix, loy = nd.loy, hiy = nd.hiy, loz = nd.loz, hiz = nd.hiz;
+    const int4 ch = nd.child;
+    n_box_tests += 4;
+    const float pad = 4.0e-7f, tlo = T.tmin + T.err, e2 = 2.0f * T.err;
+    float key[4];
+    int cc[4] = {ch.x, ch.y, ch.z, ch.w};
+    const float lx[4] = {lox.x, lox.y, lox.z, lox.w}, hx[4] = {hix.x, hix.y, hix.z, hix.w};
+    const float ly[4] = {loy.x, loy.y, loy.z, loy.w}, hy[4] = {hiy.x, hiy.y, hiy.z, hiy.w};
+    const float lz[4] = {loz.x, loz.y, loz.z, loz.w}, hz[4] = {hiz.x, hiz.y, hiz.z, hiz.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        float x0 = fmaf(lx[k], T.ix, -T.bx), x1 = fmaf(hx[k], T.ix, -T.bx);
+        float y0 = fmaf(ly[k], T.iy, -T.by), y1 = fmaf(hy[k], T.iy, -T.by);
+        float z0 = fmaf(lz[k], T.iz, -T.bz), z1 = fmaf(hz[k], T.iz, -T.bz);
+        float n = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), tlo));
+        float f = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fminf(fmaxf(z0, z1), T.t));
+        f = fmaf(fabsf(f), pad, f) + e2;
+        const bool h = n <= f && cc[k] != GD_NO_CHILD;
+        key[k] = h ? n : GD_TINF;
+        cc[k] = h ? cc[k] : GD_NO_CHILD;
+    }
+    gd_trav_descend4(T, stack, key[0], key[1], key[2], key[3], cc[0], cc[1], cc[2], cc[3]);
+}
+
+// safety query on the 4-wide nodes: leaf children update the bound in place, inner children nearer than it are visited
+GD_D void gd_trav_node4_safety(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
+    const GdNode4 &nd = bvh.nodes4[T.node];
+    const float4 lox = nd.lox, hix = nd.hix, loy = nd.loy, hiy = nd.hiy, loz = nd.loz, hiz = nd.hiz;
+    const int4 ch = nd.child;
+    n_box_tests += 4;
+    float key[4];
+    int cc[4] = {ch.x, ch.y, ch.z, ch.w};
+    key[0] = gd_box_dist2(T.ox, T.oy, T.oz, lox.x, hix.x, loy.x, hiy.x, loz.x, hiz.x);
+    key[1] = gd_box_dist2(T.ox, T.oy, T.oz, lox.y, hix.y, loy.y, hiy.y, loz.y, hiz.y);
+    key[2] = gd_box_dist2(T.ox, T.oy, T.oz, lox.z, hix.z, loy.z, hiy.z, loz.z, hiz.z);
+    key[3] = gd_box_dist2(T.ox, T.oy, T.oz, lox.w, hix.w, loy.w, hiy.w, loz.w, hiz.w);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (cc[k] < 0 && cc[k] != GD_NO_CHILD && key[k] < T.t) T.t = key[k];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const bool v = cc[k] >= 0 && key[k] < T.t;
+        key[k] = v ? key[k] : GD_TINF;
+        cc[k] = v ? cc[k] : GD_NO_CHILD;
+    }
+    gd_trav_descend4(T, stack, key[0], key[1], key[2], key[3], cc[0], cc[1], cc[2], cc[3]);
+}
+
+// Advance the warp: every busy lane makes up to `n_steps` inner-node visits (no warp vote in between: a lane that
+// reaches a leaf or the end of its ray idles for the rest of the round), then the lanes waiting at a leaf run
+// their triangle test together.  One vote-free round amortises the scheduling work of the caller (fetch, retire)
+// over several node visits and gathers several lanes for the rarer, more expensive leaf step.
+GD_D void gd_trav_step(GdTrav &T, const GdBvh &bvh, int *stack, int n_steps, unsigned &n_box_tests,
+                       unsigned &n_tri_tests) {
+#pragma unroll 1
+    for (int k = 0; k < n_steps; ++k) {
+        if (T.node >= 0) {
+            if (T.filter == GD_FILTER_SAFETY) gd_trav_node4_safety(T, bvh, stack, n_box_tests);
+            else gd_trav_node4(T, bvh, stack, n_box_tests);
+        }
+    }
+    if (T.node < 0 && T.node != GD_TRAV_DONE) {
+        gd_trav_leaf(T, bvh, ~T.node, n_tri_tests);
+        T.node = gd_trav_pop(T, stack);
+    }
+}

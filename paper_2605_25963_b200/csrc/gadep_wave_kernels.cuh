@@ -1,0 +1,426 @@
+// gadep_wave_kernels.cuh -- warp-resident wavefront transport and the ray-cast hook.
+//
+// Every warp owns GD_W_SLOTS photon slots in shared memory (SoA, GD_W_NF words per slot).  A slot is in one of
+// three places: the READY queue (its next nearest-hit query is prepared), in flight on a lane (GdTrav registers),
+// or the RESULT queue (hit known, physics pending).  The warp alternates
+//   T-burst: lanes traverse; a lane whose ray ends writes the hit to its slot, pushes it to RESULT and -- as soon as
+//            `k_fetch` lanes are idle -- takes a READY slot (dynamic fetch).  The burst ends when READY is empty and
+//            `k_exit` lanes idle; unfinished rays stay in their lanes' registers.
+//   P-burst: RESULT slots are processed 32 at a time by all lanes (boundary crossing / interaction / tally /
+//            refill from the history counter / attenuation lookup) and pushed to READY.
+// There is no block-level barrier inside the loop and no particle state in global memory (only the two pending
+// annihilation photons of a pair event, which are rare, sit in a global side buffer).  Results do not depend on any
+// of this scheduling: random streams are keyed by the history index and the tallies are integers.
+#pragma once
+#include "gadep_physics.cuh"
+#include "gadep_trav.cuh"
+#include "gadep_transport_kernels.cuh"
+
+#define GD_W_THREADS 512
+#define GD_W_WARPS (GD_W_THREADS / 32)
+#define GD_W_SLOTS 64
+#define GD_W_NF 29
+
+#ifdef GD_DIAG
+__device__ unsigned long long gd_diag[128];
+#define GD_DIAG_ADD(k, v) do { dacc[k] += (unsigned long long)(v); } while (0)
+#else
+#define GD_DIAG_ADD(k, v) do {} while (0)
+#endif
+
+struct GdWaveTune {
+    int k_fetch, k_exit, n_steps;
+    float lam_max;      // safety queries only where the mean free path is below this [mm]; 0 disables them
+    float cap_mfp;      // search radius of a safety query in mean free paths
+};
+
+// ---- slot <-> registers
+#define GD_SF(f) sl[(f) * GD_W_SLOTS + s]
+GD_D unsigned gd_pack_state(const GdLane &L) {
+    return (unsigned)(L.m + 1) | ((unsigned)L.mode << 5) | ((unsigned)L.line << 7) | ((unsigned)L.pending << 13) |
+           ((unsigned)L.n_stall << 15) | (L.g.stream << 21) | ((unsigned)L.need_mu << 23) | ((unsigned)L.cool << 24) |
+           ((unsigned)L.qkind << 27);
+}
+GD_D void gd_slot_store(float *sl, int s, const GdLane &L, unsigned long long first) {
+    GD_SF(0) = L.pos.x; GD_SF(1) = L.pos.y; GD_SF(2) = L.pos.z;
+    GD_SF(3) = L.dir.x; GD_SF(4) = L.dir.y; GD_SF(5) = L.dir.z;
+    GD_SF(6) = L.e; GD_SF(7) = L.tau;
+    GD_SF(8) = L.mu[0]; GD_SF(9) = L.mu[1]; GD_SF(10) = L.mu[2]; GD_SF(11) = L.mu[3];
+    GD_SF(12) = L.mu_tot; GD_SF(13) = L.sdist;
+    GD_SF(14) = __uint_as_float(gd_pack_state(L));
+    GD_SF(15) = __uint_as_float(L.g.draw);
+    GD_SF(16) = __uint_as_float((unsigned)(L.history - first));
+    GD_SF(17) = L.dep;
+    GD_SF(18) = __uint_as_float((L.flags & 0xFFu) | ((L.n_events > 0xFFFFu ? 0xFFFFu : L.n_events) << 16));
+    GD_SF(19) = __int_as_float(L.ex.a); GD_SF(20) = __int_as_float(L.ex.b); GD_SF(21) = __int_as_float(L.ex.c);
+    GD_SF(25) = L.sc.x; GD_SF(26) = L.sc.y; GD_SF(27) = L.sc.z; GD_SF(28) = L.sr;
+}
+GD_D void gd_slot_load(const float *sl, int s, GdLane &L, unsigned long long seed, unsigned long long first) {
+    L.pos = gd_make(GD_SF(0), GD_SF(1), GD_SF(2));
+    L.dir = gd_make(GD_SF(3), GD_SF(4), GD_SF(5));
+    L.e = GD_SF(6); L.tau = GD_SF(7);
+    L.mu[0] = GD_SF(8); L.mu[1] = GD_SF(9); L.mu[2] = GD_SF(10); L.mu[3] = GD_SF(11);
+    L.mu_tot = GD_SF(12); L.sdist = GD_SF(13);
+    const unsigned st = __float_as_uint(GD_SF(14));
+    L.m = (int)(st & 31u) - 1; L.mode = (int)((st >> 5) & 3u); L.line = (int)((st >> 7) & 63u);
+    L.pending = (int)((st >> 13) & 3u); L.n_stall = (int)((st >> 15) & 63u); L.need_mu = (int)((st >> 23) & 1u);
+    L.history = first + (unsigned long long)__float_as_uint(GD_SF(16));
+    gd_rng_init(L.g, seed, L.history, (st >> 21) & 3u, __float_as_uint(GD_SF(15)));
+    L.dep = GD_SF(17);
+    const unsigned fe = __float_as_uint(GD_SF(18));
+    L.flags = fe & 0xFFu; L.n_events = fe >> 16;
+    L.ex.a = __float_as_int(GD_SF(19)); L.ex.b = __float_as_int(GD_SF(20)); L.ex.c = __float_as_int(GD_SF(21));
+    L.cool = (int)((st >> 24) & 7u); L.qkind = (int)((st >> 27) & 1u);
+    L.sc = gd_make(GD_SF(25), GD_SF(26), GD_SF(27)); L.sr = GD_SF(28);
+}
+
+// What the slot does next (mode FLIGHT, sdist known).  Purely a scheduling decision: a skipped query is one whose
+// answer is known to be "no facet within (-GD_TBACK, sdist]" because a facet-free sphere covers the whole flight.
+#define GD_PLAN_RAY 0
+#define GD_PLAN_SAFETY 1
+#define GD_PLAN_SKIP 2
+GD_D int gd_wave_plan(GdLane &L, const GdWaveTune &tune, float &r2_cap) {
+    if (L.mode != GD_MODE_FLIGHT || !(L.sdist < GD_INF) || !(tune.lam_max > 0.0f)) return GD_PLAN_RAY;
+    float d = 0.0f;
+    if (L.sr > 0.0f) {
+        const float dx = L.pos.x - L.sc.x, dy = L.pos.y - L.sc.y, dz = L.pos.z - L.sc.z;
+        d = sqrtf(dx * dx + dy * dy + dz * dz);
+        if (d * 1.0001f + L.sdist * 1.0001f + 4.0f * GD_TBACK < L.sr) return GD_PLAN_SKIP;
+    }
+    // a safety query only right after an interaction (never on a surface), in an optically thick medium, and not
+    // while an earlier sphere still covers the neighbourhood or an earlier query came back too small to pay off
+    const float lam = 1.0f / L.mu_tot;
+    if (L.ex.a >= 0 || !(lam < tune.lam_max)) return GD_PLAN_RAY;
+    if (L.sr > 0.0f && d < 0.5f * L.sr) return GD_PLAN_RAY;
+    if (L.cool > 0) { L.cool--; return GD_PLAN_RAY; }
+    const float r = tune.cap_mfp * lam;
+    r2_cap = r * r;
+    return GD_PLAN_SAFETY;
+}
+
+GD_D void gd_tally_history(const GdHistory &r, const GdSource &S, const GdTally &tally, unsigned *s_spec,
+                           unsigned *s_emitted, unsigned *s_peak) {
+    atomicAdd(&s_emitted[r.line], 1u);
+    if (r.flags & GD_F_PEAK) {
+        atomicAdd(&s_peak[r.line], 1u);
+        atomicAdd(&s_spec[min(S.line_bin[r.line], tally.n_bins)], 1u);
+    } else if (r.edep > 0.0f) {
+        float b = floorf(r.edep * tally.inv_de);
+        int bin = b >= (float)tally.n_bins ? tally.n_bins : (int)b;
+        atomicAdd(&s_spec[bin], 1u);
+    }
+}
+
+// dynamic shared memory: [table floats][spectrum u32 (n_bins+1)][slots: warps x GD_W_NF x GD_W_SLOTS floats]
+// pair_buf: global, 8 floats per slot of every warp of the grid
+__global__ void __launch_bounds__(GD_W_THREADS, 1)
+gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
+                    unsigned long long n_hist, unsigned long long seed, GdTally tally, float *__restrict__ edep_out,
+                    unsigned *__restrict__ flags_out, unsigned long long *next_history, unsigned chunk,
+                    float *__restrict__ pair_buf, GdWaveTune tune) {
+    extern __shared__ __align__(16) unsigned char gd_smem[];
+    __shared__ GdSource s_src;
+    __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];
+    __shared__ unsigned s_cnt[14];
+    __shared__ unsigned char s_qready[GD_W_WARPS][GD_W_SLOTS], s_qres[GD_W_WARPS][GD_W_SLOTS];
+    const int n_tab = M.n_mat * 4 * M.n_grid;
+    float *s_tab = (float *)gd_smem;
+    unsigned *s_spec = (unsigned *)(s_tab + n_tab);
+    float *s_slots = (float *)(s_spec + tally.n_bins + 1);
+    for (int i = threadIdx.x; i < n_tab; i += blockDim.x) s_tab[i] = M.table[i];
+    for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) s_spec[i] = 0;
+    for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i];
+    if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }
+    if (threadIdx.x < 14) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    float *sl = s_slots + (size_t)warp * GD_W_NF * GD_W_SLOTS;
+    unsigned char *q_ready = s_qready[warp], *q_res = s_qres[warp];
+    float *pair = pair_buf + ((size_t)blockIdx.x * GD_W_WARPS + warp) * GD_W_SLOTS * 8;
+    int stack[GD_STACK4];
+    GdTrav T;
+    gd_trav_idle(T);
+    unsigned n_box = 0, n_tri = 0, n_query = 0, n_done = 0;
+    unsigned long long w_cur = 0, w_end = 0;     // warp-uniform chunk of history indices [w_cur, w_end)
+    // every slot starts in RESULT with mode NEED: the first P-bursts start the first histories
+    for (int s = lane; s < GD_W_SLOTS; s += 32) {
+        GD_SF(14) = __uint_as_float((unsigned)GD_MODE_NEED << 5);
+        q_res[s] = (unsigned char)s;
+    }
+    int n_res = GD_W_SLOTS, n_ready = 0;
+#ifdef GD_DIAG
+    unsigned d_steps = 0;
+    unsigned long long dacc[20] = {};
+#endif
+    __syncwarp();
+
+    for (;;) {
+        // ================================================================ P-burst
+#ifdef GD_DIAG
+        long long d_t0 = clock64();
+#endif
+        // full batches first; a partial batch only when the warp would otherwise starve
+        bool did_full = false;
+        while (n_res >= 32 || (n_res > 0 && n_ready == 0 && !did_full)) {
+            const int take = n_res < 32 ? n_res : 32;
+            did_full = take == 32;
+            GD_DIAG_ADD(8, 1); GD_DIAG_ADD(9, take);
+            bool act = (int)lane < take;           // this lane still works on slot s in this batch
+            const int s = act ? (int)q_res[n_res - 1 - (int)lane] : 0;
+            n_res -= take;
+            GdLane L;
+            L.mode = GD_MODE_DONE;
+            GdHit hit;
+            hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
+            bool safety_result = false;
+            if (act) {
+                gd_slot_load(sl, s, L, seed, first);
+                if (L.pending) {
+                    const float *p = pair + s * 8;
+                    L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
+                }
+                // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the
+                // to-side id as "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
+                hit.t = GD_SF(22);
+                hit.orig = __float_as_int(GD_SF(23));
+                hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
+                hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
+                safety_result = L.qkind == 1;
+            }
+            // A lane whose next flight is covered by its facet-free sphere knows the answer of the query ("no facet")
+            // and goes round again in registers -- but only while its warp has nothing else to do (tail of a run,
+            // long scattering chains), so that the other lanes are not kept waiting.
+            for (int it = 0;; ++it) {
+                GdLocalCounters cnt = {};
+                if (act && L.mode != GD_MODE_NEED) {
+                    if (safety_result) {
+                        // facet-free sphere around the current point (a lower bound, rounded down)
+                        const float r = sqrtf(hit.t);
+                        L.sc = L.pos; L.sr = fmaxf(r * 0.9999f - 1.0e-5f, 0.0f);
+                        L.cool = L.sr * L.mu_tot < 2.0f ? 3 : 0;      // under two mean free paths: back off
+                        L.qkind = 0;
+                    } else {
+                        const int was_pending = L.pending;
+                        GdHistory r;
+                        if (gd_lane_post(L, M, s_src, seed, hit, r, cnt)) {
+                            n_done++;
+                            gd_tally_history(r, s_src, tally, s_spec, s_emitted, s_peak);
+                            const unsigned long long hrel = L.history - first;
+                            if (edep_out) edep_out[hrel] = r.edep;
+                            if (flags_out) flags_out[hrel] = r.flags;
+                        } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
+                            float *p = pair + s * 8;
+                            p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
+                            p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
+                        }
+                        if (cnt.n_crossings) atomicAdd(&s_cnt[4], 1u);
+                        if (cnt.n_pe) atomicAdd(&s_cnt[5], 1u);
+                        if (cnt.n_compton) atomicAdd(&s_cnt[6], 1u);
+                        if (cnt.n_coherent) atomicAdd(&s_cnt[7], 1u);
+                        if (cnt.n_pair) atomicAdd(&s_cnt[8], 1u);
+                        if (cnt.n_escaped) atomicAdd(&s_cnt[9], cnt.n_escaped);
+                        if (cnt.n_leak) atomicAdd(&s_cnt[10], cnt.n_leak);
+                        if (cnt.n_cutoff) atomicAdd(&s_cnt[11], cnt.n_cutoff);
+                    }
+                }
+                safety_result = false;
+                // ---- refill finished slots from the history counter (warp-level chunks)
+                const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, act && L.mode == GD_MODE_NEED);
+                if (need_mask) {
+                    const unsigned n_need = __popc(need_mask);
+                    unsigned long long new_base = 0;
+                    const bool refill = w_cur + n_need > w_end;
+                    if (refill) {
+                        if (lane == 0) new_base = atomicAdd(next_history, (unsigned long long)chunk);
+                        new_base = __shfl_sync(0xFFFFFFFFu, new_base, 0);
+                    }
+                    if (act && L.mode == GD_MODE_NEED) {
+                        unsigned long long h = w_cur + __popc(need_mask & lt_mask);
+                        if (h >= w_end) h = new_base + (h - w_end);
+                        if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
+                        else L.mode = GD_MODE_DONE;
+                    }
+                    if (refill) { w_cur = new_base + (w_cur + n_need - w_end); w_end = new_base + chunk; }
+                    else w_cur += n_need;
+                }
+                // ---- prepare the next query: READY (ray / safety query), or the known answer "no facet"
+                const bool live = act && L.mode != GD_MODE_DONE;
+                int plan = GD_PLAN_RAY;
+                float r2_cap = 0.0f;
+                if (live) {
+                    float t_min, t_max;
+                    int filter;
+                    gd_lane_query(L, M, s_tab, t_min, t_max, filter);
+                    plan = gd_wave_plan(L, tune, r2_cap);
+                    L.qkind = plan == GD_PLAN_SAFETY ? 1 : 0;
+                }
+                const bool skip = live && plan == GD_PLAN_SKIP;
+                const unsigned ready_mask = __ballot_sync(0xFFFFFFFFu, live && !skip);
+                const unsigned skip_mask = __ballot_sync(0xFFFFFFFFu, skip);
+                const bool spin = skip_mask != 0u && ready_mask == 0u && n_ready == 0 && n_res == 0 && it < 16;
+                if (live && !(skip && spin)) {
+                    gd_slot_store(sl, s, L, first);
+                    if (plan == GD_PLAN_SAFETY) { GD_SF(22) = r2_cap; atomicAdd(&s_cnt[12], 1u); }
+                    else if (skip) { GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
+                    if (skip) q_res[n_res + __popc(skip_mask & lt_mask)] = (unsigned char)s;
+                    else q_ready[n_ready + __popc(ready_mask & lt_mask)] = (unsigned char)s;
+                }
+                if (skip) atomicAdd(&s_cnt[13], 1u);
+                n_ready += __popc(ready_mask);
+                if (!spin) { n_res += __popc(skip_mask); break; }
+                act = skip;
+                hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET;
+            }
+            __syncwarp();
+        }
+#ifdef GD_DIAG
+        long long d_t1 = clock64(); GD_DIAG_ADD(16, d_t1 - d_t0);
+#endif
+        const unsigned busy_mask = __ballot_sync(0xFFFFFFFFu, T.slot >= 0);
+        if (n_ready == 0 && busy_mask == 0u) {
+            if (n_res == 0) break;                           // every slot is dead
+            continue;
+        }
+        // ================================================================ T-burst
+        for (;;) {
+            const unsigned idle_mask = __ballot_sync(0xFFFFFFFFu, T.slot < 0);
+            const int n_idle = __popc(idle_mask);
+            if (n_idle) {
+                if (n_ready > 0) {
+                    if (n_idle >= tune.k_fetch || n_idle == 32) {
+                        const int rank = __popc(idle_mask & lt_mask);
+                        if (T.slot < 0 && rank < n_ready) {
+                            const int s = (int)q_ready[n_ready - 1 - rank];
+                            const unsigned st = __float_as_uint(GD_SF(14));
+                            if ((st >> 27) & 1u) {
+                                gd_trav_begin_safety(T, bvh, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(22), s);
+                            } else {
+                                const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
+                                gd_trav_begin(T, bvh, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
+                                              loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
+                                              __float_as_int(GD_SF(19)), __float_as_int(GD_SF(20)), __float_as_int(GD_SF(21)), s);
+                                n_query++;
+                            }
+                        }
+                        GD_DIAG_ADD(4, 1); GD_DIAG_ADD(5, n_idle < n_ready ? n_idle : n_ready);
+                        n_ready -= n_idle < n_ready ? n_idle : n_ready;
+                    }
+                } else if ((n_res > 0 && (n_res >= 32 || n_idle >= tune.k_exit)) || n_idle == 32) {
+                    break;
+                }
+            }
+#ifdef GD_DIAG
+            {
+                unsigned a_node = __ballot_sync(0xFFFFFFFFu, T.node >= 0);
+                unsigned a_leaf = __ballot_sync(0xFFFFFFFFu, T.node < 0 && T.node != GD_TRAV_DONE);
+                GD_DIAG_ADD(0, 1); GD_DIAG_ADD(1, __popc(a_node)); GD_DIAG_ADD(2, __popc(a_leaf)); GD_DIAG_ADD(3, n_idle);
+                if (n_ready > 0) GD_DIAG_ADD(10, 1); else GD_DIAG_ADD(11, 1);
+                if (T.slot >= 0) d_steps++;
+            }
+#endif
+            gd_trav_step(T, bvh, stack, tune.n_steps, n_box, n_tri);
+            const bool fin = T.slot >= 0 && T.node == GD_TRAV_DONE;
+            const unsigned fin_mask = __ballot_sync(0xFFFFFFFFu, fin);
+#ifdef GD_DIAG
+            if (fin) d_steps = 0;
+#endif
+            if (fin_mask) {
+                if (fin) {
+                    const int s = T.slot;
+                    GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
+                    q_res[n_res + __popc(fin_mask & lt_mask)] = (unsigned char)s;
+                    T.slot = -1;
+                }
+                n_res += __popc(fin_mask);
+                __syncwarp();
+            }
+        }
+#ifdef GD_DIAG
+        GD_DIAG_ADD(17, clock64() - d_t1);
+#endif
+    }
+#ifdef GD_DIAG
+    if (lane == 0) for (int k = 0; k < 20; ++k) atomicAdd(&gd_diag[k], dacc[k]);
+#endif
+    // ---- flush: per-lane 32-bit work counters straight to the 64-bit global totals
+    {
+        unsigned v[4] = {n_done, n_query, n_box, n_tri};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            unsigned long long x = v[k];
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) x += __shfl_down_sync(0xFFFFFFFFu, x, o);
+            if (lane == 0 && x) atomicAdd(&((unsigned long long *)tally.counters)[k], x);
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) {
+        unsigned v = s_spec[i];
+        if (v) atomicAdd(&tally.spectrum[i], (unsigned long long)v);
+    }
+    if (threadIdx.x < GD_MAX_LINES) {
+        if (s_emitted[threadIdx.x]) atomicAdd(&tally.emitted[threadIdx.x], (unsigned long long)s_emitted[threadIdx.x]);
+        if (s_peak[threadIdx.x]) atomicAdd(&tally.peak[threadIdx.x], (unsigned long long)s_peak[threadIdx.x]);
+    }
+    if (threadIdx.x >= 4 && threadIdx.x < 14 && s_cnt[threadIdx.x])
+        atomicAdd(&((unsigned long long *)tally.counters)[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
+}
+
+// ---------------------------------------------------------------- ray-cast hook with dynamic fetch
+// Persistent warps take chunks of ray indices from one global counter; a lane whose ray ends stores the result and
+// takes the next ray of its warp's chunk once `k_fetch` lanes are idle.
+__global__ void __launch_bounds__(256)
+gd_k_trace_wave(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ dir, long long n, int filter_mat,
+                float t_min, int *__restrict__ tri_out, float *__restrict__ t_out, GdCounters *counters,
+                unsigned long long *next_ray, unsigned chunk, GdWaveTune tune) {
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    int stack[GD_STACK4];
+    GdTrav T;
+    gd_trav_idle(T);
+    long long my_ray = -1;
+    unsigned n_box = 0, n_tri = 0, n_query = 0;
+    long long w_cur = 0, w_end = 0;
+    bool dry = false;                 // the global counter ran past n
+    for (;;) {
+        const unsigned idle_mask = __ballot_sync(0xFFFFFFFFu, T.slot < 0);
+        const int n_idle = __popc(idle_mask);
+        if (n_idle) {
+            if (w_cur >= w_end && !dry) {
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(next_ray, (unsigned long long)chunk);
+                base = __shfl_sync(0xFFFFFFFFu, base, 0);
+                w_cur = (long long)base;
+                w_end = w_cur + chunk < n ? w_cur + chunk : n;
+                if (w_cur >= n) { dry = true; w_cur = w_end = 0; }
+            }
+            const long long avail = w_end - w_cur;
+            if (avail > 0) {
+                if (n_idle >= tune.k_fetch || n_idle == 32) {
+                    const int rank = __popc(idle_mask & lt_mask);
+                    if (T.slot < 0 && rank < avail) {
+                        const long long i = w_cur + rank;
+                        my_ray = i;
+                        gd_trav_begin(T, bvh, org[3 * i], org[3 * i + 1], org[3 * i + 2], dir[3 * i], dir[3 * i + 1],
+                                      dir[3 * i + 2], t_min, GD_INF, filter_mat, -1, -1, -1, 0);
+                        n_query++;
+                    }
+                    w_cur += n_idle < avail ? n_idle : avail;
+                }
+            } else if (n_idle == 32) {
+                break;
+            }
+        }
+        gd_trav_step(T, bvh, stack, tune.n_steps, n_box, n_tri);
+        if (T.slot >= 0 && T.node == GD_TRAV_DONE) {
+            tri_out[my_ray] = T.orig == GD_NO_FACET ? -1 : T.orig;
+            t_out[my_ray] = T.orig == GD_NO_FACET ? GD_INF : T.t;
+            T.slot = -1;
+        }
+    }
+    GdLocalCounters cnt = {};
+    cnt.n_queries = n_query; cnt.n_box_tests = n_box; cnt.n_tri_tests = n_tri;
+    gd_flush_counters(cnt, counters, 0);
+}

@@ -155,6 +155,8 @@ def test_per_history_parity(pkg, orc, cfg, n):
     assert c["n_leak"] == 0 and oc["n_leak"] == 0
     assert (edep <= w.source["line_mev"][(flags >> 8) & 0xFF] * (1 + 1e-6)).all()      # deposit <= source energy
     # event totals track the oracle's to the fraction of diverged histories
+    c = dict(c)
+    c["n_queries"] += c["n_skipped_queries"]       # flights answered by a facet-free sphere are queries the oracle makes
     for k in ("n_queries", "n_crossings", "n_pe", "n_compton", "n_coherent", "n_escaped"):
         assert abs(c[k] - oc[k]) <= 0.01 * oc[k] + 50, (k, c[k], oc[k])
     assert c["n_pair"] == pytest.approx(oc["n_pair"], abs=3 + 0.05 * oc["n_pair"])
@@ -231,19 +233,28 @@ def test_results_do_not_depend_on_partitioning_and_are_deterministic(pkg, orc):
     assert np.array_equal(a, p2) and not np.array_equal(a, p1)
 
 
-def test_both_kernels_give_identical_tallies(pkg, orc):
-    # persistent-lane kernel vs plain history-per-thread kernel: same streams, integer tallies -> bit-identical
-    from paper_2605_25963_b200.binding import RUN_HISTORY_PER_THREAD
+def test_all_kernel_variants_give_identical_tallies(pkg, orc):
+    # warp-resident wavefront (default) vs persistent lanes vs plain history-per-thread: same streams, integer
+    # tallies -> bit-identical spectra and event counts.  The wavefront kernel uses an FMA slab test with its own
+    # conservative padding, so only its box / triangle test counts may differ.
+    from paper_2605_25963_b200.binding import RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES
     for cfg, n in ((1, 400_000), (3, 20_000)):
         w, g, s = _setup(pkg, orc, cfg)
         a = g.run(n, 5, w.n_bins, w.spectrum_e_max_mev).copy()
         ca = g.get_counters()
         b = g.run(n, 5, w.n_bins, w.spectrum_e_max_mev, flags=RUN_HISTORY_PER_THREAD).copy()
         cb = g.get_counters()
-        assert np.array_equal(a, b)
-        for k in ("n_histories", "n_queries", "n_box_tests", "n_tri_tests", "n_crossings", "n_pe", "n_compton", "n_coherent",
-                  "n_pair", "n_escaped", "emitted", "peak"):
-            assert ca[k] == cb[k], k
+        c = g.run(n, 5, w.n_bins, w.spectrum_e_max_mev, flags=RUN_PERSISTENT_LANES).copy()
+        cc = g.get_counters()
+        assert np.array_equal(a, b) and np.array_equal(a, c)
+        for k in ("n_histories", "n_crossings", "n_pe", "n_compton", "n_coherent",
+                  "n_pair", "n_escaped", "n_leak", "n_cutoff", "emitted", "peak"):
+            assert ca[k] == cb[k] == cc[k], k
+        for k in ("n_queries", "n_box_tests", "n_tri_tests"):
+            assert cb[k] == cc[k], k
+        # a flight covered by a facet-free sphere is answered without a BVH query: every query is accounted for
+        assert ca["n_queries"] + ca["n_skipped_queries"] == cb["n_queries"]
+        assert ca["n_box_tests"] <= 1.25 * cb["n_box_tests"] and ca["n_tri_tests"] <= 1.25 * cb["n_tri_tests"]
         assert ca["n_histories"] == n
 
 
