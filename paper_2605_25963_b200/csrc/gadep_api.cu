@@ -637,6 +637,11 @@ extern "C" int gadep_philox_raw(gadep_ctx *c, const unsigned *ctr4, const unsign
 }
 
 #ifdef GD_DIAG
+extern "C" int gadep_debug_read_warps(unsigned long long *out) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out, gd_diag_warp, sizeof(unsigned long long) * 4096 * 8);
+    return 0;
+}
 extern "C" int gadep_debug_read(unsigned long long *out128, int reset) {
     cudaDeviceSynchronize();
     cudaMemcpyFromSymbol(out128, gd_diag, sizeof(unsigned long long) * 128);

@@ -184,15 +184,19 @@ GD_HD bool gd_lane_next_photon(GdLane &L, unsigned long long seed) {
 }
 
 // consume the query result; returns true when the history is finished (out is then valid)
-GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const GdSource &S, unsigned long long seed, const GdHit &hit,
-                        GdHistory &out, GdLocalCounters &cnt) {
+GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const GdSource &S, unsigned long long seed,
+                        const GdHit &hit_in, GdHistory &out, GdLocalCounters &cnt) {
+    GdHit hit = hit_in;
     bool photon_done = false;
     if (L.mode == GD_MODE_LOCATE) {                                                         // O5
         L.m = hit.leaf < 0 ? M.world_material : (hit.leaving ? gd_mat_inside(hit.mats) : gd_mat_outside(hit.mats));
         L.tau = -logf(gd_rng_next(L.g));                                                    // O7.1
-        L.need_mu = 1;
         L.mode = GD_MODE_FLIGHT;
-        return false;
+        // The first flight runs along the same ray as the localisation query, and the nearest facet ahead is by
+        // construction the first one whose from-side is the start material: one traversal answers both (O5 + O7.3).
+        L.mu_tot = gd_mu_lookup(M, tab, L.m, L.e, L.mu); L.need_mu = 0;                     // O2
+        L.sdist = L.mu_tot > 0.0f ? L.tau / L.mu_tot : GD_INF;                              // O7.2
+        if (hit.leaf >= 0 && !(hit.t <= L.sdist)) hit.leaf = -1;
     }
     if (hit.leaf >= 0) {                                                                    // O7.6 boundary first
         float t = fmaxf(hit.t, 0.0f);
@@ -277,6 +281,6 @@ GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *t
         gd_ray_setup(ray, L.pos, L.dir);
         cnt.n_queries++;
         gd_nearest_hit<false>(bvh, ray, t_min, t_max, filter, L.ex, true, hit, cnt.n_box_tests, cnt.n_tri_tests);
-        if (gd_lane_post(L, M, S, seed, hit, out, cnt)) return;
+        if (gd_lane_post(L, M, tab, S, seed, hit, out, cnt)) return;
     }
 }

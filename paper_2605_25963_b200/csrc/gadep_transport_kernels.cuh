@@ -168,7 +168,7 @@ gd_k_transport_refill(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src
         gd_nearest_hit<true>(bvh, ray, t_min, t_max, filter, L.ex, live, hit, cnt.n_box_tests, cnt.n_tri_tests);
         if (live) {
             GdHistory r;
-            if (gd_lane_post(L, M, s_src, seed, hit, r, cnt)) {
+            if (gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt)) {
                 n_done++;
                 atomicAdd(&s_emitted[r.line], 1u);
                 if (r.flags & GD_F_PEAK) {

@@ -23,6 +23,7 @@
 
 #ifdef GD_DIAG
 __device__ unsigned long long gd_diag[128];
+__device__ unsigned long long gd_diag_warp[4096][8];
 #define GD_DIAG_ADD(k, v) do { dacc[k] += (unsigned long long)(v); } while (0)
 #else
 #define GD_DIAG_ADD(k, v) do {} while (0)
@@ -79,23 +80,29 @@ GD_D void gd_slot_load(const float *sl, int s, GdLane &L, unsigned long long see
 #define GD_PLAN_RAY 0
 #define GD_PLAN_SAFETY 1
 #define GD_PLAN_SKIP 2
+#ifdef GD_DIAG
+#define GD_PLAN_RET(reason, plan) do { atomicAdd(&gd_diag[32 + (L.m < 0 ? 0 : L.m) * 8 + (reason)], 1ull); return (plan); } while (0)
+#else
+#define GD_PLAN_RET(reason, plan) return (plan)
+#endif
 GD_D int gd_wave_plan(GdLane &L, const GdWaveTune &tune, float &r2_cap) {
-    if (L.mode != GD_MODE_FLIGHT || !(L.sdist < GD_INF) || !(tune.lam_max > 0.0f)) return GD_PLAN_RAY;
+    if (L.mode != GD_MODE_FLIGHT || !(L.sdist < GD_INF) || !(tune.lam_max > 0.0f)) GD_PLAN_RET(0, GD_PLAN_RAY);
     float d = 0.0f;
     if (L.sr > 0.0f) {
         const float dx = L.pos.x - L.sc.x, dy = L.pos.y - L.sc.y, dz = L.pos.z - L.sc.z;
         d = sqrtf(dx * dx + dy * dy + dz * dz);
-        if (d * 1.0001f + L.sdist * 1.0001f + 4.0f * GD_TBACK < L.sr) return GD_PLAN_SKIP;
+        if (d * 1.0001f + L.sdist * 1.0001f + 4.0f * GD_TBACK < L.sr) GD_PLAN_RET(1, GD_PLAN_SKIP);
     }
     // a safety query only right after an interaction (never on a surface), in an optically thick medium, and not
     // while an earlier sphere still covers the neighbourhood or an earlier query came back too small to pay off
     const float lam = 1.0f / L.mu_tot;
-    if (L.ex.a >= 0 || !(lam < tune.lam_max)) return GD_PLAN_RAY;
-    if (L.sr > 0.0f && d < 0.5f * L.sr) return GD_PLAN_RAY;
-    if (L.cool > 0) { L.cool--; return GD_PLAN_RAY; }
+    if (!(lam < tune.lam_max)) GD_PLAN_RET(2, GD_PLAN_RAY);
+    if (L.ex.a >= 0) GD_PLAN_RET(3, GD_PLAN_RAY);
+    if (L.sr > 0.0f && d < 0.5f * L.sr) GD_PLAN_RET(4, GD_PLAN_RAY);
+    if (L.cool > 0) { L.cool--; GD_PLAN_RET(5, GD_PLAN_RAY); }
     const float r = tune.cap_mfp * lam;
     r2_cap = r * r;
-    return GD_PLAN_SAFETY;
+    GD_PLAN_RET(6, GD_PLAN_SAFETY);
 }
 
 GD_D void gd_tally_history(const GdHistory &r, const GdSource &S, const GdTally &tally, unsigned *s_spec,
@@ -153,6 +160,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #ifdef GD_DIAG
     unsigned d_steps = 0;
     unsigned long long dacc[20] = {};
+    const long long d_start = clock64();
 #endif
     __syncwarp();
 
@@ -204,7 +212,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                     } else {
                         const int was_pending = L.pending;
                         GdHistory r;
-                        if (gd_lane_post(L, M, s_src, seed, hit, r, cnt)) {
+                        if (gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt)) {
                             n_done++;
                             gd_tally_history(r, s_src, tally, s_spec, s_emitted, s_peak);
                             const unsigned long long hrel = L.history - first;
@@ -343,6 +351,10 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     }
 #ifdef GD_DIAG
     if (lane == 0) for (int k = 0; k < 20; ++k) atomicAdd(&gd_diag[k], dacc[k]);
+    if (lane == 0) {
+        unsigned long long *dw = gd_diag_warp[(blockIdx.x * GD_W_WARPS + warp) & 4095];
+        dw[0] = clock64() - d_start; dw[1] = dacc[8]; dw[2] = dacc[0]; dw[3] = dacc[16]; dw[4] = dacc[17]; dw[5] = dacc[9]; dw[6] = dacc[4]; dw[7] = dacc[5];
+    }
 #endif
     // ---- flush: per-lane 32-bit work counters straight to the 64-bit global totals
     {
