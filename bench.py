@@ -121,7 +121,7 @@ def main():
     ap.add_argument("--histories", type=float, default=0, help="per GPU per step; 0 = the config's own count")
     ap.add_argument("--impl", default="gadep")
     ap.add_argument("--ref-sample", type=float, default=60000)
-    ap.add_argument("--cpu-sample", type=float, default=120000)
+    ap.add_argument("--cpu-sample", type=float, default=0, help="oracle histories; 0 = sized for ~15 s from a pilot run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
 
@@ -233,7 +233,7 @@ def main():
                         "steps": e2e_steps, "fepe": fepe},
                 "gpu_launches": launches,
                 "clocks": clocks,
-                "roofline": {"bound": "alu", "kernel": "gd_k_transport", "achieved": achieved, "peak": alu_peak,
+                "roofline": {"bound": "alu", "kernel": "gd_k_transport_wave", "achieved": achieved, "peak": alu_peak,
                              "unit": "Tinstr/s (FP32 lane-instructions)", "frac": achieved / alu_peak,
                              "traffic": None, "peak_source": f"{n_sm} SMs x 128 lanes x sm_max_mhz ({peak_src})",
                              "kernel_ms_per_step": sum(kern_ms) / args.steps,
@@ -244,6 +244,9 @@ def main():
                 "paper_context": "RTX 4090: 1e8 particles in 66.08 s = 1.51e6 /s (PAPER.md:270), other physics"}
         if not args.no_cpu_baseline and world == 1:
             n_s = int(args.cpu_sample)
+            if n_s <= 0:                                         # pilot -> about 15 s of CPU work
+                r0, dt0, _ = oracle_rate(w, 20000)
+                n_s = int(min(max(15.0 * r0, 20000), 5e7))
             r, dt, cores = oracle_rate(w, n_s)
             line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"first {n_s} histories of {w.name} ({dt:.1f} s)"}

@@ -50,7 +50,7 @@ struct gadep_ctx {
     int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
-    GdWaveTune tune = {8, 8, 4, 4.0f, 8.0f};
+    GdWaveTune tune = {8, 16, 4, 0.0f, 8.0f};   // safety spheres off by default (GADEP_TUNE enables them)
     int n_bins = 0;
     float spec_e_max = 0;
     bool results_stale = false, have_results = false;

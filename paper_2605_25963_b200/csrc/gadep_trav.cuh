@@ -10,6 +10,9 @@
 
 #define GD_TRAV_DONE ((int)0x80000000)     // node value: traversal finished (leaf codes are ~index > GD_TRAV_DONE)
 #define GD_NO_FACET 0x7FFFFFFF
+#ifndef GD_WITH_SAFETY
+#define GD_WITH_SAFETY 0          // facet-free-sphere queries inside the traversal loop (costs loop-body size)
+#endif
 #define GD_TINF __int_as_float(0x7F800000)
 
 struct GdTrav {
@@ -249,8 +252,11 @@ GD_D void gd_trav_step(GdTrav &T, const GdBvh &bvh, int *stack, int n_steps, uns
 #pragma unroll 1
     for (int k = 0; k < n_steps; ++k) {
         if (T.node >= 0) {
+#if GD_WITH_SAFETY
             if (T.filter == GD_FILTER_SAFETY) gd_trav_node4_safety(T, bvh, stack, n_box_tests);
-            else gd_trav_node4(T, bvh, stack, n_box_tests);
+            else
+#endif
+            gd_trav_node4(T, bvh, stack, n_box_tests);
         }
     }
     if (T.node < 0 && T.node != GD_TRAV_DONE) {

@@ -86,7 +86,7 @@ GD_D void gd_slot_load(const float *sl, int s, GdLane &L, unsigned long long see
 #define GD_PLAN_RET(reason, plan) return (plan)
 #endif
 GD_D int gd_wave_plan(GdLane &L, const GdWaveTune &tune, float &r2_cap) {
-    if (L.mode != GD_MODE_FLIGHT || !(L.sdist < GD_INF) || !(tune.lam_max > 0.0f)) GD_PLAN_RET(0, GD_PLAN_RAY);
+    if (!GD_WITH_SAFETY || L.mode != GD_MODE_FLIGHT || !(L.sdist < GD_INF) || !(tune.lam_max > 0.0f)) GD_PLAN_RET(0, GD_PLAN_RAY);
     float d = 0.0f;
     if (L.sr > 0.0f) {
         const float dx = L.pos.x - L.sc.x, dy = L.pos.y - L.sc.y, dz = L.pos.z - L.sc.z;
@@ -302,9 +302,12 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                         if (T.slot < 0 && rank < n_ready) {
                             const int s = (int)q_ready[n_ready - 1 - rank];
                             const unsigned st = __float_as_uint(GD_SF(14));
+#if GD_WITH_SAFETY
                             if ((st >> 27) & 1u) {
                                 gd_trav_begin_safety(T, bvh, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(22), s);
-                            } else {
+                            } else
+#endif
+                            {
                                 const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
                                 gd_trav_begin(T, bvh, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
                                               loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
