@@ -90,8 +90,9 @@ GD_HD GdVec3 gd_make(float x, float y, float z) { GdVec3 v = {x, y, z}; return v
 GD_HD float gd_get(const GdVec3 &v, int k) { return k == 0 ? v.x : (k == 1 ? v.y : v.z); }
 
 // ---------------------------------------------------------------- Philox4x32-10 (Salmon et al., SC'11)
-GD_HD void gd_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
-                            uint32_t out[4]) {
+struct GdU4 { uint32_t x, y, z, w; };
+#define GD_HD_NI __host__ __device__ __noinline__   // one copy in the instruction cache instead of one per call site
+GD_HD_NI GdU4 gd_philox4x32_10v(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
 #ifdef __CUDA_ARCH__
@@ -105,7 +106,13 @@ GD_HD void gd_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, 
         c0 = n0; c1 = l1; c2 = n2; c3 = l0;
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
-    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+    GdU4 o = {c0, c1, c2, c3};
+    return o;
+}
+GD_HD void gd_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                            uint32_t out[4]) {
+    GdU4 o = gd_philox4x32_10v(c0, c1, c2, c3, k0, k1);
+    out[0] = o.x; out[1] = o.y; out[2] = o.z; out[3] = o.w;
 }
 
 // Counter-based stream: key = seed, counter = (history_lo, history_hi, draw/4, stream); draw k = word k%4.

@@ -11,27 +11,38 @@ GD_HD float __int_as_float_inf() { return gd_as_float(0x7F800000); }
 
 // ---------------------------------------------------------------- O2: attenuation lookup
 // tab: [n_mat][4][n_grid]; channels 0..2 hold ln(mu) (-1e30 for zero), channel 3 holds mu.
-GD_HD float gd_mu_lookup(const GdMaterials &M, const float *tab, int m, float e, float mu[4]) {
-    float x = (logf(e) - M.ln_e0) * M.inv_dln;
+struct GdF4 { float a, b, c, d; };
+GD_HD_NI GdF4 gd_mu_lookup_v(int n_grid, float ln_e0, float inv_dln, const float *tab, int m, float e) {
+    float x = (logf(e) - ln_e0) * inv_dln;
     int j = (int)floorf(x);
-    j = j < 0 ? 0 : (j > M.n_grid - 2 ? M.n_grid - 2 : j);
+    j = j < 0 ? 0 : (j > n_grid - 2 ? n_grid - 2 : j);
     float f = x - (float)j;
     float g = 1.0f - f;
-    const float *t = tab + (m * 4) * M.n_grid + j;
-    mu[0] = expf(g * t[0] + f * t[1]);
-    mu[1] = expf(g * t[M.n_grid] + f * t[M.n_grid + 1]);
-    mu[2] = expf(g * t[2 * M.n_grid] + f * t[2 * M.n_grid + 1]);
-    mu[3] = g * t[3 * M.n_grid] + f * t[3 * M.n_grid + 1];
+    const float *t = tab + (m * 4) * n_grid + j;
+    GdF4 mu;
+    mu.a = expf(g * t[0] + f * t[1]);
+    mu.b = expf(g * t[n_grid] + f * t[n_grid + 1]);
+    mu.c = expf(g * t[2 * n_grid] + f * t[2 * n_grid + 1]);
+    mu.d = g * t[3 * n_grid] + f * t[3 * n_grid + 1];
+    return mu;
+}
+GD_HD float gd_mu_lookup(const GdMaterials &M, const float *tab, int m, float e, float mu[4]) {
+    GdF4 r = gd_mu_lookup_v(M.n_grid, M.ln_e0, M.inv_dln, tab, m, e);
+    mu[0] = r.a; mu[1] = r.b; mu[2] = r.c; mu[3] = r.d;
     return ((mu[0] + mu[1]) + mu[2]) + mu[3];
 }
 
-GD_HD void gd_sincos_2pi(float u, float &s, float &c) {
+struct GdF2 { float s, c; };
+GD_HD_NI GdF2 gd_sincos_2pi_v(float u) {
+    GdF2 r;
 #ifdef __CUDA_ARCH__
-    sincospif(2.0f * u, &s, &c);
+    sincospif(2.0f * u, &r.s, &r.c);
 #else
-    s = sinf(GD_TWO_PI * u); c = cosf(GD_TWO_PI * u);
+    r.s = sinf(GD_TWO_PI * u); r.c = cosf(GD_TWO_PI * u);
 #endif
+    return r;
 }
+GD_HD void gd_sincos_2pi(float u, float &s, float &c) { GdF2 r = gd_sincos_2pi_v(u); s = r.s; c = r.c; }
 
 // O4 / O12: isotropic direction from 2 draws
 GD_HD GdVec3 gd_sample_isotropic(GdRng &g) {
@@ -44,7 +55,7 @@ GD_HD GdVec3 gd_sample_isotropic(GdRng &g) {
 }
 
 // O13: rotate d by polar cosine c and azimuth 2*pi*u_phi
-GD_HD GdVec3 gd_rotate(GdVec3 d, float c, float u_phi) {
+GD_HD_NI GdVec3 gd_rotate(GdVec3 d, float c, float u_phi) {
     float sp, cp;
     gd_sincos_2pi(u_phi, sp, cp);
     float s = sqrtf(fmaxf(0.0f, 1.0f - c * c));

@@ -99,6 +99,17 @@ GD_D void gd_trav_node_safety(GdTrav &T, const GdBvh &bvh, int *stack, unsigned 
     }
 }
 
+struct GdEdge3 { float u, v, w; int ok; };
+__device__ __noinline__ GdEdge3 gd_edges_double(float ax, float ay, float bx, float by, float cx, float cy) {
+    const double du = GD_DSUB(GD_DMUL((double)cx, (double)by), GD_DMUL((double)cy, (double)bx));
+    const double dv = GD_DSUB(GD_DMUL((double)ax, (double)cy), GD_DMUL((double)ay, (double)cx));
+    const double dw = GD_DSUB(GD_DMUL((double)bx, (double)ay), GD_DMUL((double)by, (double)ax));
+    GdEdge3 e;
+    e.u = (float)du; e.v = (float)dv; e.w = (float)dw;
+    e.ok = !((du < 0.0 || dv < 0.0 || dw < 0.0) && (du > 0.0 || dv > 0.0 || dw > 0.0));
+    return e;
+}
+
 GD_D float gd_sel3(float x, float y, float z, int k) { return k == 0 ? x : (k == 1 ? y : z); }
 
 // same arithmetic as gd_ray_tri / gd_test_leaf (gadep_bvh.cuh), on the register-resident ray
@@ -119,12 +130,10 @@ GD_D void gd_trav_leaf(GdTrav &T, const GdBvh &bvh, int leaf, unsigned &n_tri_te
     float u = GD_SUB(GD_MUL(cx, by), GD_MUL(cy, bx));
     float v = GD_SUB(GD_MUL(ax, cy), GD_MUL(ay, cx));
     float w = GD_SUB(GD_MUL(bx, ay), GD_MUL(by, ax));
-    if (u == 0.0f || v == 0.0f || w == 0.0f) {          // on an edge in float: decide in double
-        double du = GD_DSUB(GD_DMUL((double)cx, (double)by), GD_DMUL((double)cy, (double)bx));
-        double dv = GD_DSUB(GD_DMUL((double)ax, (double)cy), GD_DMUL((double)ay, (double)cx));
-        double dw = GD_DSUB(GD_DMUL((double)bx, (double)ay), GD_DMUL((double)by, (double)ax));
-        u = (float)du; v = (float)dv; w = (float)dw;
-        if ((du < 0.0 || dv < 0.0 || dw < 0.0) && (du > 0.0 || dv > 0.0 || dw > 0.0)) return;
+    if (u == 0.0f || v == 0.0f || w == 0.0f) {          // on an edge in float: decide in double (out of line: rare)
+        const GdEdge3 e = gd_edges_double(ax, ay, bx, by, cx, cy);
+        u = e.u; v = e.v; w = e.w;
+        if (!e.ok) return;
     } else if ((u < 0.0f || v < 0.0f || w < 0.0f) && (u > 0.0f || v > 0.0f || w > 0.0f)) {
         return;
     }

@@ -20,6 +20,9 @@
 #define GD_W_WARPS (GD_W_THREADS / 32)
 #define GD_W_SLOTS 64
 #define GD_W_NF 29
+#ifndef GD_W_SYNC
+#define GD_W_SYNC 0            // the warps of a block run their physics / traversal bursts in lock-step
+#endif
 
 #ifdef GD_DIAG
 __device__ unsigned long long gd_diag[128];
@@ -33,6 +36,8 @@ struct GdWaveTune {
     int k_fetch, k_exit, n_steps;
     float lam_max;      // safety queries only where the mean free path is below this [mm]; 0 disables them
     float cap_mfp;      // search radius of a safety query in mean free paths
+    int sparse_max;     // ... and only while the warp has at most this many live photons
+    int t_burst;        // phase-locked mode: traversal rounds per T-burst
 };
 
 // ---- slot <-> registers
@@ -85,7 +90,7 @@ GD_D void gd_slot_load(const float *sl, int s, GdLane &L, unsigned long long see
 #else
 #define GD_PLAN_RET(reason, plan) return (plan)
 #endif
-GD_D int gd_wave_plan(GdLane &L, const GdWaveTune &tune, float &r2_cap) {
+GD_D int gd_wave_plan(GdLane &L, const GdWaveTune &tune, bool allow_safety, float &r2_cap) {
     if (!GD_WITH_SAFETY || L.mode != GD_MODE_FLIGHT || !(L.sdist < GD_INF) || !(tune.lam_max > 0.0f)) GD_PLAN_RET(0, GD_PLAN_RAY);
     float d = 0.0f;
     if (L.sr > 0.0f) {
@@ -96,7 +101,7 @@ GD_D int gd_wave_plan(GdLane &L, const GdWaveTune &tune, float &r2_cap) {
     // a safety query only right after an interaction (never on a surface), in an optically thick medium, and not
     // while an earlier sphere still covers the neighbourhood or an earlier query came back too small to pay off
     const float lam = 1.0f / L.mu_tot;
-    if (!(lam < tune.lam_max)) GD_PLAN_RET(2, GD_PLAN_RAY);
+    if (!allow_safety || !(lam < tune.lam_max)) GD_PLAN_RET(2, GD_PLAN_RAY);
     if (L.ex.a >= 0) GD_PLAN_RET(3, GD_PLAN_RAY);
     if (L.sr > 0.0f && d < 0.5f * L.sr) GD_PLAN_RET(4, GD_PLAN_RAY);
     if (L.cool > 0) { L.cool--; GD_PLAN_RET(5, GD_PLAN_RAY); }
@@ -129,6 +134,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     __shared__ GdSource s_src;
     __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];
     __shared__ unsigned s_cnt[14];
+    __shared__ int s_live_warps;
     __shared__ unsigned char s_qready[GD_W_WARPS][GD_W_SLOTS], s_qres[GD_W_WARPS][GD_W_SLOTS];
     const int n_tab = M.n_mat * 4 * M.n_grid;
     float *s_tab = (float *)gd_smem;
@@ -139,6 +145,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i];
     if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }
     if (threadIdx.x < 14) s_cnt[threadIdx.x] = 0;
+    if (threadIdx.x == 0) s_live_warps = GD_W_WARPS;
     __syncthreads();
 
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -164,20 +171,29 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #endif
     __syncwarp();
 
+    bool alive = true;
     for (;;) {
+#if GD_W_SYNC
+        // all warps of the block change phase together: one instruction-cache fill serves 16 warps
+        __syncthreads();
+        if (*(volatile int *)&s_live_warps == 0) break;
+#endif
         // ================================================================ P-burst
 #ifdef GD_DIAG
         long long d_t0 = clock64();
 #endif
         // full batches first; a partial batch only when the warp would otherwise starve
         bool did_full = false;
-        while (n_res >= 32 || (n_res > 0 && n_ready == 0 && !did_full)) {
+        while (alive && (n_res >= 32 || (n_res > 0 && n_ready == 0 && !did_full))) {
             const int take = n_res < 32 ? n_res : 32;
             did_full = take == 32;
             GD_DIAG_ADD(8, 1); GD_DIAG_ADD(9, take);
             bool act = (int)lane < take;           // this lane still works on slot s in this batch
             const int s = act ? (int)q_res[n_res - 1 - (int)lane] : 0;
             n_res -= take;
+            // facet-free-sphere queries only while the warp is sparse (drain of a launch, few long scattering chains):
+            // there they shorten the chains; in a full warp they would only add divergence to the traversal loop
+            const bool sparse = take + n_res + n_ready + __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0)) <= tune.sparse_max;
             GdLane L;
             L.mode = GD_MODE_DONE;
             GdHit hit;
@@ -223,11 +239,10 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                             p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
                             p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
                         }
-                        if (cnt.n_crossings) atomicAdd(&s_cnt[4], 1u);
-                        if (cnt.n_pe) atomicAdd(&s_cnt[5], 1u);
-                        if (cnt.n_compton) atomicAdd(&s_cnt[6], 1u);
-                        if (cnt.n_coherent) atomicAdd(&s_cnt[7], 1u);
-                        if (cnt.n_pair) atomicAdd(&s_cnt[8], 1u);
+                        {   // one event kind per visit (crossing / PE / Compton / coherent / pair), rarer flags apart
+                            const int kind = cnt.n_crossings ? 4 : (cnt.n_coherent ? 7 : (cnt.n_compton ? 6 : (cnt.n_pe ? 5 : (cnt.n_pair ? 8 : -1))));
+                            if (kind >= 0) atomicAdd(&s_cnt[kind], 1u);
+                        }
                         if (cnt.n_escaped) atomicAdd(&s_cnt[9], cnt.n_escaped);
                         if (cnt.n_leak) atomicAdd(&s_cnt[10], cnt.n_leak);
                         if (cnt.n_cutoff) atomicAdd(&s_cnt[11], cnt.n_cutoff);
@@ -261,7 +276,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                     float t_min, t_max;
                     int filter;
                     gd_lane_query(L, M, s_tab, t_min, t_max, filter);
-                    plan = gd_wave_plan(L, tune, r2_cap);
+                    plan = gd_wave_plan(L, tune, sparse, r2_cap);
                     L.qkind = plan == GD_PLAN_SAFETY ? 1 : 0;
                 }
                 const bool skip = live && plan == GD_PLAN_SKIP;
@@ -286,13 +301,28 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #ifdef GD_DIAG
         long long d_t1 = clock64(); GD_DIAG_ADD(16, d_t1 - d_t0);
 #endif
+#if GD_W_SYNC
+        __syncthreads();
+        if (!alive) continue;
+#endif
         const unsigned busy_mask = __ballot_sync(0xFFFFFFFFu, T.slot >= 0);
         if (n_ready == 0 && busy_mask == 0u) {
-            if (n_res == 0) break;                           // every slot is dead
+            if (n_res == 0) {                                // every slot is dead
+#if GD_W_SYNC
+                alive = false;
+                if (lane == 0) atomicSub(&s_live_warps, 1);
+                continue;
+#else
+                break;
+#endif
+            }
             continue;
         }
         // ================================================================ T-burst
-        for (;;) {
+        for (int t_it = 0;; ++t_it) {
+#if GD_W_SYNC
+            if (t_it >= tune.t_burst) break;
+#endif
             const unsigned idle_mask = __ballot_sync(0xFFFFFFFFu, T.slot < 0);
             const int n_idle = __popc(idle_mask);
             if (n_idle) {
@@ -318,7 +348,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                         GD_DIAG_ADD(4, 1); GD_DIAG_ADD(5, n_idle < n_ready ? n_idle : n_ready);
                         n_ready -= n_idle < n_ready ? n_idle : n_ready;
                     }
-                } else if ((n_res > 0 && (n_res >= 32 || n_idle >= tune.k_exit)) || n_idle == 32) {
+                } else if ((n_res > 0 && (n_res >= 32 || n_res >= tune.k_exit * (32 - n_idle))) || n_idle == 32) {
                     break;
                 }
             }
