@@ -112,6 +112,34 @@ def run_reference(args, w, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_ray_bench(args, dm):
+    """BASELINE.json configs[4]: seeded isotropic rays from random points inside the endcap's bounding cylinder through
+    the 2 M-facet BVH (device arrays, CUDA events), the check of a sample against brute force is tests/test_gpu_parity.py::test_cfg4_full_size_rays."""
+    import torch
+    import paper_2605_25963_b200 as pkg
+    w = dm.make_config(4)
+    g = pkg.Gadep(0, torch.cuda.current_stream().cuda_stream)
+    g.load_workload(w)
+    n, chunk = int(args.ray_bench), 20_000_000
+    t_ms, boxes, tris, done = 0.0, 0, 0, 0
+    while done < n:
+        m = min(chunk, n - done)
+        org, d = dm.configs.make_rays(m, 1 + done // chunk, 41.9, -101.9, 6.0)
+        to, td = torch.from_numpy(org).cuda(), torch.from_numpy(d).cuda()
+        tri = torch.empty(m, dtype=torch.int32, device="cuda")
+        t = torch.empty(m, dtype=torch.float32, device="cuda")
+        if done == 0:
+            g.trace_rays(to[:100000], td[:100000], tri_out=tri[:100000], t_out=t[:100000])      # warm-up
+        g.trace_rays(to, td, tri_out=tri, t_out=t)
+        c = g.get_counters()
+        t_ms += c["last_run_ms"]; boxes += c["n_box_tests"]; tris += c["n_tri_tests"]
+        done += m
+    line = {"metric": "BVH nearest-hit rays/s", "value": n / (t_ms * 1e-3), "unit": "rays/s", "n_rays": n,
+            "workload": w.name, "n_triangles": w.mesh.n_tri, "kernel_ms": t_ms, "box_tests_per_s": boxes / (t_ms * 1e-3),
+            "tri_tests_per_s": tris / (t_ms * 1e-3), "bvh_build_ms": g.get_counters()["last_build_ms"]}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -123,6 +151,7 @@ def main():
     ap.add_argument("--ref-sample", type=float, default=60000)
     ap.add_argument("--cpu-sample", type=float, default=0, help="oracle histories; 0 = sized for ~15 s from a pilot run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ray-bench", type=float, default=0, help="config-4 ray benchmark: this many seeded rays through gadep_trace_rays")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -144,6 +173,9 @@ def main():
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if args.ray_bench:
+        run_ray_bench(args, dm)
+        return
     n_hist = int(args.histories) if args.histories else w.n_histories
     stream = torch.cuda.current_stream()
     g = pkg.Gadep(local_rank, stream.cuda_stream)

@@ -50,7 +50,8 @@ typedef enum {
 /* per-history flags written by gadep_run_histories */
 #define GADEP_F_ESCAPED 1u        /* some photon of the history left the geometry (no facet ahead, or KILL) */
 #define GADEP_F_PEAK 2u           /* full-absorption history: all energy deposited in scoring material      */
-#define GADEP_F_LEAK 4u           /* no facet ahead while inside a non-world material (numerical leak)      */
+#define GADEP_F_LEAK 4u           /* no facet ahead while inside a non-world material (float32 corner case): */
+                                  /* the photon was localised again from its current point and went on      */
 #define GADEP_F_NONSCORING 8u     /* some energy deposited outside the scoring material                     */
 /* bits 8..15: line index; bits 16..31: number of interactions (saturating) */
 

@@ -20,6 +20,7 @@
 #define GD_F_PEAK 2u
 #define GD_F_LEAK 4u
 #define GD_F_NONSCORING 8u
+#define GD_F_RELOC 0x80u             // internal: a re-localisation query is pending (never leaves the kernel)
 
 // ---------------------------------------------------------------- BVH layout
 // Binary BVH, children's boxes stored in the parent (one 64-byte node = 4 x 16 B loads):

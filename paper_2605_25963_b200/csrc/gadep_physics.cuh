@@ -201,7 +201,8 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
     bool photon_done = false;
     if (L.mode == GD_MODE_LOCATE) {                                                         // O5
         L.m = hit.leaf < 0 ? M.world_material : (hit.leaving ? gd_mat_inside(hit.mats) : gd_mat_outside(hit.mats));
-        L.tau = -logf(gd_rng_next(L.g));                                                    // O7.1
+        if (L.flags & GD_F_RELOC) L.flags &= ~GD_F_RELOC;                                   // re-localisation: tau carries on
+        else L.tau = -logf(gd_rng_next(L.g));                                               // O7.1
         L.mode = GD_MODE_FLIGHT;
         // The first flight runs along the same ray as the localisation query, and the nearest facet ahead is by
         // construction the first one whose from-side is the start material: one traversal answers both (O5 + O7.3).
@@ -216,15 +217,23 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
         L.m = hit.leaving ? gd_mat_outside(hit.mats) : gd_mat_inside(hit.mats);
         cnt.n_crossings++;
         L.need_mu = 1;
-        if (t > GD_TBACK) { L.ex = gd_no_exclude(); L.n_stall = 0; }      // earlier facets left the window
+        // Facets crossed earlier on this straight segment stay excluded whatever the distance: for a grazing ray the
+        // float32 error of t (position ulp / cos) exceeds GD_TBACK, and a facet 1e-4 behind can reappear inside the window.
+        if (t > GD_TBACK) L.n_stall = 0;
         L.ex.c = L.ex.b; L.ex.b = L.ex.a; L.ex.a = hit.orig;
         if (L.m == GD_MAT_KILL) { L.flags |= GD_F_ESCAPED; cnt.n_escaped++; photon_done = true; }
         else if (++L.n_stall > 32) {       // > 32 facets inside 0.1 um: degenerate mesh; stop instead of spinning
             L.flags |= GD_F_ESCAPED | GD_F_LEAK; cnt.n_escaped++; cnt.n_leak++; photon_done = true;
         }
+    } else if (!(L.sdist < GD_INF) && L.m != M.world_material && !(L.flags & GD_F_RELOC)) {
+        // No facet ahead although the photon is not in the world material: a float32 inconsistency at a corner (the
+        // rounded crossing point of one facet lies just outside its neighbour across the shared edge).  Localise again
+        // from the current point and direction (O5), keep the optical depth; counted in n_leak / GD_F_LEAK.
+        L.flags |= GD_F_LEAK | GD_F_RELOC; cnt.n_leak++;
+        L.mode = GD_MODE_LOCATE; L.ex = gd_no_exclude(); L.n_stall = 0;
+        return false;
     } else if (!(L.sdist < GD_INF)) {                                                       // O7.5
         L.flags |= GD_F_ESCAPED; cnt.n_escaped++;
-        if (L.m != M.world_material) { L.flags |= GD_F_LEAK; cnt.n_leak++; }
         photon_done = true;
     } else {                                                                                // O7.4 / O8 interaction
         L.pos.x += L.sdist * L.dir.x; L.pos.y += L.sdist * L.dir.y; L.pos.z += L.sdist * L.dir.z;
@@ -271,6 +280,7 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
     if (!gd_lane_next_photon(L, seed)) return false;
     // ---- O14
     if (!(L.flags & (GD_F_ESCAPED | GD_F_NONSCORING))) { L.flags |= GD_F_PEAK; L.dep = S.line_mev[L.line]; }
+    L.flags &= ~GD_F_RELOC;
     L.flags |= ((unsigned)L.line & 0xFFu) << 8;
     L.flags |= (L.n_events > 0xFFFFu ? 0xFFFFu : L.n_events) << 16;
     out.edep = L.dep; out.flags = L.flags; out.line = L.line;
@@ -292,6 +302,9 @@ GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *t
         gd_ray_setup(ray, L.pos, L.dir);
         cnt.n_queries++;
         gd_nearest_hit<false>(bvh, ray, t_min, t_max, filter, L.ex, true, hit, cnt.n_box_tests, cnt.n_tri_tests);
+#if defined(GD_DIAG) && defined(__CUDA_ARCH__)     // step trace of the history-per-thread kernel (diagnostic builds only)
+        printf("q%u mode %d m %d e %.6f pos (%.7f %.7f %.7f) dir (%.6f %.6f %.6f) tau %.5g mu %.5g sdist %.6g ex (%d %d %d) -> facet %d t %.9g leaving %d in %d out %d\n", cnt.n_queries, L.mode, L.m, L.e, L.pos.x, L.pos.y, L.pos.z, L.dir.x, L.dir.y, L.dir.z, L.tau, L.mu_tot, L.sdist, L.ex.a, L.ex.b, L.ex.c, hit.leaf < 0 ? -1 : hit.orig, hit.t, hit.leaving, gd_mat_inside(hit.mats), gd_mat_outside(hit.mats));
+#endif
         if (gd_lane_post(L, M, tab, S, seed, hit, out, cnt)) return;
     }
 }
