@@ -201,25 +201,31 @@ GD_D void gd_trav_descend4(GdTrav &T, int *stack, float k0, float k1, float k2, 
     T.node = c0 != GD_NO_CHILD ? c0 : gd_trav_pop(T, stack);
 }
 
-// one 4-wide node visit of a ray: FMA slab tests, far sides padded by the FMA error bound and ~3 ulp
+// one 4-wide node visit of a ray: FMA slab tests, far sides padded by the FMA error bound and ~3 ulp.
+// The near / far plane of every slab is picked by address from the sign of the direction component (lo and hi are
+// 16 bytes apart in GdNode4), which equals min / max of the two plane distances (fma is monotonic in its first
+// operand) and saves 24 min/max per visit.
 GD_D void gd_trav_node4(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
-    const GdNode4 &nd = bvh.nodes4[T.node];
-    const float4 lox = nd.lox, hix = nd.hix, loy = nd.loy, hiy = nd.hiy, loz = nd.loz, hiz = nd.hiz;
-    const int4 ch = nd.child;
+    const char *nd = (const char *)(bvh.nodes4 + T.node);
+    const int sx = (__float_as_int(T.ix) >> 31) & 16, sy = (__float_as_int(T.iy) >> 31) & 16, sz = (__float_as_int(T.iz) >> 31) & 16;
+    const float4 nx = *(const float4 *)(nd + sx), fx = *(const float4 *)(nd + (16 - sx));
+    const float4 ny = *(const float4 *)(nd + 32 + sy), fy = *(const float4 *)(nd + 32 + (16 - sy));
+    const float4 nz = *(const float4 *)(nd + 64 + sz), fz = *(const float4 *)(nd + 64 + (16 - sz));
+    const int4 ch = *(const int4 *)(nd + 96);
     n_box_tests += 4;
     const float pad = 4.0e-7f, tlo = T.tmin + T.err, e2 = 2.0f * T.err;
     float key[4];
     int cc[4] = {ch.x, ch.y, ch.z, ch.w};
-    const float lx[4] = {lox.x, lox.y, lox.z, lox.w}, hx[4] = {hix.x, hix.y, hix.z, hix.w};
-    const float ly[4] = {loy.x, loy.y, loy.z, loy.w}, hy[4] = {hiy.x, hiy.y, hiy.z, hiy.w};
-    const float lz[4] = {loz.x, loz.y, loz.z, loz.w}, hz[4] = {hiz.x, hiz.y, hiz.z, hiz.w};
+    const float ax[4] = {nx.x, nx.y, nx.z, nx.w}, bx[4] = {fx.x, fx.y, fx.z, fx.w};
+    const float ay[4] = {ny.x, ny.y, ny.z, ny.w}, by[4] = {fy.x, fy.y, fy.z, fy.w};
+    const float az[4] = {nz.x, nz.y, nz.z, nz.w}, bz[4] = {fz.x, fz.y, fz.z, fz.w};
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        float x0 = fmaf(lx[k], T.ix, -T.bx), x1 = fmaf(hx[k], T.ix, -T.bx);
-        float y0 = fmaf(ly[k], T.iy, -T.by), y1 = fmaf(hy[k], T.iy, -T.by);
-        float z0 = fmaf(lz[k], T.iz, -T.bz), z1 = fmaf(hz[k], T.iz, -T.bz);
-        float n = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), tlo));
-        float f = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fminf(fmaxf(z0, z1), T.t));
+        const float x0 = fmaf(ax[k], T.ix, -T.bx), x1 = fmaf(bx[k], T.ix, -T.bx);
+        const float y0 = fmaf(ay[k], T.iy, -T.by), y1 = fmaf(by[k], T.iy, -T.by);
+        const float z0 = fmaf(az[k], T.iz, -T.bz), z1 = fmaf(bz[k], T.iz, -T.bz);
+        const float n = fmaxf(fmaxf(x0, y0), fmaxf(z0, tlo));
+        float f = fminf(fminf(x1, y1), fminf(z1, T.t));
         f = fmaf(fabsf(f), pad, f) + e2;
         const bool h = n <= f && cc[k] != GD_NO_CHILD;
         key[k] = h ? n : GD_TINF;
