@@ -14,6 +14,9 @@
 #define GD_WITH_SAFETY 0          // facet-free-sphere queries inside the traversal loop (costs loop-body size)
 #endif
 #define GD_TINF __int_as_float(0x7F800000)
+#ifndef GD_FULL_SORT
+#define GD_FULL_SORT 1
+#endif
 
 struct GdTrav {
     float ox, oy, oz;        // origin (ray-triangle test)
@@ -193,8 +196,13 @@ GD_D void gd_trav_node(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_
 
 // order the four (key, child) pairs, push the valid ones farthest first, continue with the nearest
 GD_D void gd_trav_descend4(GdTrav &T, int *stack, float k0, float k1, float k2, float k3, int c0, int c1, int c2, int c3) {
+#if GD_FULL_SORT
     GD_CSWAP(k0, c0, k1, c1); GD_CSWAP(k2, c2, k3, c3); GD_CSWAP(k0, c0, k2, c2); GD_CSWAP(k1, c1, k3, c3);
     GD_CSWAP(k1, c1, k2, c2);
+#else
+    // nearest child first; the others (usually none or one) in stored order, farther of a pair pushed first
+    GD_CSWAP(k0, c0, k1, c1); GD_CSWAP(k2, c2, k3, c3); GD_CSWAP(k0, c0, k2, c2);
+#endif
     if (c3 != GD_NO_CHILD) stack[T.sp++] = c3;
     if (c2 != GD_NO_CHILD) stack[T.sp++] = c2;
     if (c1 != GD_NO_CHILD) stack[T.sp++] = c1;

@@ -163,7 +163,10 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
         GD_SF(14) = __uint_as_float((unsigned)GD_MODE_NEED << 5);
         q_res[s] = (unsigned char)s;
     }
-    int n_res = GD_W_SLOTS, n_ready = 0;
+    // both queues are rings (first in, first out): a slot of a long scattering chain is served every round instead of
+    // waiting at the bottom of a stack while fresh histories stream over it -- the chains are the critical path
+    int n_res = GD_W_SLOTS, n_ready = 0, h_res = 0, h_ready = 0;
+    static_assert((GD_W_SLOTS & (GD_W_SLOTS - 1)) == 0, "slot count must be a power of two");
 #ifdef GD_DIAG
     unsigned d_steps = 0;
     unsigned long long dacc[20] = {};
@@ -189,8 +192,8 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
             did_full = take == 32;
             GD_DIAG_ADD(8, 1); GD_DIAG_ADD(9, take);
             bool act = (int)lane < take;           // this lane still works on slot s in this batch
-            const int s = act ? (int)q_res[n_res - 1 - (int)lane] : 0;
-            n_res -= take;
+            const int s = act ? (int)q_res[(h_res + (int)lane) & (GD_W_SLOTS - 1)] : 0;
+            h_res = (h_res + take) & (GD_W_SLOTS - 1); n_res -= take;
             // facet-free-sphere queries only while the warp is sparse (drain of a launch, few long scattering chains):
             // there they shorten the chains; in a full warp they would only add divergence to the traversal loop
             const bool sparse = take + n_res + n_ready + __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0)) <= tune.sparse_max;
@@ -287,8 +290,8 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                     gd_slot_store(sl, s, L, first);
                     if (plan == GD_PLAN_SAFETY) { GD_SF(22) = r2_cap; atomicAdd(&s_cnt[12], 1u); }
                     else if (skip) { GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
-                    if (skip) q_res[n_res + __popc(skip_mask & lt_mask)] = (unsigned char)s;
-                    else q_ready[n_ready + __popc(ready_mask & lt_mask)] = (unsigned char)s;
+                    if (skip) q_res[(h_res + n_res + __popc(skip_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
+                    else q_ready[(h_ready + n_ready + __popc(ready_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
                 }
                 if (skip) atomicAdd(&s_cnt[13], 1u);
                 n_ready += __popc(ready_mask);
@@ -330,7 +333,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                     if (n_idle >= tune.k_fetch || n_idle == 32) {
                         const int rank = __popc(idle_mask & lt_mask);
                         if (T.slot < 0 && rank < n_ready) {
-                            const int s = (int)q_ready[n_ready - 1 - rank];
+                            const int s = (int)q_ready[(h_ready + rank) & (GD_W_SLOTS - 1)];
                             const unsigned st = __float_as_uint(GD_SF(14));
 #if GD_WITH_SAFETY
                             if ((st >> 27) & 1u) {
@@ -346,7 +349,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                             }
                         }
                         GD_DIAG_ADD(4, 1); GD_DIAG_ADD(5, n_idle < n_ready ? n_idle : n_ready);
-                        n_ready -= n_idle < n_ready ? n_idle : n_ready;
+                        { const int tk = n_idle < n_ready ? n_idle : n_ready; h_ready = (h_ready + tk) & (GD_W_SLOTS - 1); n_ready -= tk; }
                     }
                 } else if ((n_res > 0 && (n_res >= 32 || n_res >= tune.k_exit * (32 - n_idle))) || n_idle == 32) {
                     break;
@@ -371,7 +374,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                 if (fin) {
                     const int s = T.slot;
                     GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
-                    q_res[n_res + __popc(fin_mask & lt_mask)] = (unsigned char)s;
+                    q_res[(h_res + n_res + __popc(fin_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
                     T.slot = -1;
                 }
                 n_res += __popc(fin_mask);
