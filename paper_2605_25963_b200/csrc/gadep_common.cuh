@@ -128,7 +128,17 @@ GD_HD void gd_rng_init(GdRng &g, unsigned long long seed, unsigned long long his
     g.stream = stream; g.draw = draw; g.block = 0xFFFFFFFFu;
 }
 // u = ((w >> 9) + 0.5) * 2^-23 in (0,1): k + 0.5 with k < 2^23 is exact in float32
+#ifndef GD_RNG_CACHE
+#define GD_RNG_CACHE 0      // 1: keep the last Philox block in registers (4 draws per block, ~30 instructions per call site)
+#endif
+GD_HD_NI float gd_rng_uniform_v(uint32_t k0, uint32_t k1, uint32_t h0, uint32_t h1, uint32_t stream, uint32_t draw) {
+    const GdU4 o = gd_philox4x32_10v(h0, h1, draw >> 2, stream, k0, k1);
+    const uint32_t k = draw & 3u;
+    const uint32_t w = k == 0 ? o.x : (k == 1 ? o.y : (k == 2 ? o.z : o.w));
+    return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f);
+}
 GD_HD float gd_rng_next(GdRng &g) {
+#if GD_RNG_CACHE
     uint32_t b = g.draw >> 2;
     if (b != g.block) {
         gd_philox4x32_10(g.h0, g.h1, b, g.stream, g.k0, g.k1, g.w);
@@ -138,4 +148,8 @@ GD_HD float gd_rng_next(GdRng &g) {
     uint32_t w = k == 0 ? g.w[0] : (k == 1 ? g.w[1] : (k == 2 ? g.w[2] : g.w[3]));
     g.draw++;
     return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f);
+#else
+    // one out-of-line copy of the generator for all call sites (the transport kernels are instruction-fetch bound)
+    return gd_rng_uniform_v(g.k0, g.k1, g.h0, g.h1, g.stream, g.draw++);
+#endif
 }
