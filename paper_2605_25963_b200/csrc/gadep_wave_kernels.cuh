@@ -419,7 +419,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 // ---------------------------------------------------------------- ray-cast hook with dynamic fetch
 // Persistent warps take chunks of ray indices from one global counter; a lane whose ray ends stores the result and
 // takes the next ray of its warp's chunk once `k_fetch` lanes are idle.
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 gd_k_trace_wave(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ dir, long long n, int filter_mat,
                 float t_min, int *__restrict__ tri_out, float *__restrict__ t_out, GdCounters *counters,
                 unsigned long long *next_ray, unsigned chunk, GdWaveTune tune) {
