@@ -51,6 +51,7 @@ struct gadep_ctx {
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
     GdWaveTune tune = {8, 4, 4, 4.0f, 8.0f, 12, 8};
+    double split_budget = 8.0;                // extra BVH references per facet handed out by the splitting budget
     int n_bins = 0;
     float spec_e_max = 0;
     bool results_stale = false, have_results = false;
@@ -115,6 +116,7 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb1);
     if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
+    if (const char *t = getenv("GADEP_SPLIT_BUDGET")) { double b = atof(t); if (b >= 0 && b <= 15) c->split_budget = b; }
     if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,leaf_thresh" (measurement sweeps)
         int a, b, d;
         float lm = c->tune.lam_max, cm = c->tune.cap_mfp;
@@ -255,9 +257,11 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     if (cudaMalloc(&scene, 4 * 16) != cudaSuccess) { cudaFree(counts); return gd_fail(c, GADEP_E_CUDA, "cudaMalloc failed"); }
     cudaEventRecord(c->evb0, st);
     gd_k_init_scene<<<1, 32, 0, st>>>(scene);
-    gd_k_ref_count<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts);
+    gd_k_split_prio<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts, (unsigned long long *)(scene + 10));
+    gd_k_ref_count<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts, (const unsigned long long *)(scene + 10),
+                                       (unsigned long long)(c->split_budget * (double)n_tri));
     gd_k_scan<<<1, 1024, 0, st>>>(counts, n_tri, (unsigned *)(scene + 8));
-    launches += 3;
+    launches += 4;
     unsigned n_ref_u = 0;
     cudaError_t e = cudaMemcpyAsync(&n_ref_u, scene + 8, 4, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -294,7 +298,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         int *child_l = (int *)(arena + o_cl), *child_r = (int *)(arena + o_cr);
         int *parent_int = (int *)(arena + o_pi), *parent_leaf = (int *)(arena + o_pl);
         int *visits = (int *)(arena + o_vis), *ref_tri = (int *)(arena + o_rt);
-        gd_k_make_refs<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts, ref_lo, ref_hi, ref_tri, scene);
+        gd_k_make_refs<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts, (unsigned)n, ref_lo, ref_hi, ref_tri, scene);
         gd_k_morton<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, scene, keys[0], vals[0]);
         launches += 2;
         int cur = 0;
@@ -326,7 +330,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     } while (0);
     cudaFree(arena); cudaFree(counts); cudaFree(scene);
     if (e != cudaSuccess) rc = gd_fail(c, GADEP_E_CUDA, "BVH build failed: %s", cudaGetErrorString(e));
-    else if (depth >= GD_STACK || 3 * ((depth + 1) / 2) + 4 > GD_STACK4) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
+    else if (depth >= GD_STACK || 3 * depth + 4 > GD_STACK4) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
     if (rc != GADEP_OK) return rc;
     c->bvh_depth = depth;
     c->n_ref = n;

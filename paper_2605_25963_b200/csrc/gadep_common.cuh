@@ -14,7 +14,7 @@
 #define GD_MAX_LINES 64
 #define GD_MAX_MAT 16
 #define GD_STACK 96                 // LBVH depth bound: 63 Morton bits + index tie-break bits
-#define GD_STACK4 148                // 4-wide traversal: up to 3 pushes per two binary levels
+#define GD_STACK4 196                // 4-wide traversal: up to 3 pushes per binary level descended (depth <= 64)
 
 #define GD_F_ESCAPED 1u
 #define GD_F_PEAK 2u
