@@ -140,6 +140,38 @@ def run_ray_bench(args, dm):
     print(json.dumps(line), flush=True)
 
 
+def run_locate_bench(args, dm):
+    """cost of the paper's reworked localisation (parity counting over all facets hit, an
+    all-hits BVH traversal) against its original side-id rule (nearest facet), on the config-1 detector at the
+    standard tessellation and at 3x the angular segments (the paper's facet-count sensitivity experiment)."""
+    import torch
+    import paper_2605_25963_b200 as pkg
+    n = int(args.locate_bench)
+    out = {"metric": "localisation queries/s", "unit": "queries/s", "n_points": n, "cases": []}
+    for nt in (256, 768):
+        w = dm.make_config(1, n_theta=nt)
+        g = pkg.Gadep(0, torch.cuda.current_stream().cuda_stream)
+        g.load_workload(w)
+        org, d = dm.configs.make_rays(n, 3, 45.0, -105.0, 10.0)
+        to, td = torch.from_numpy(org).cuda(), torch.from_numpy(d).cuda()
+        mat = torch.empty(n, dtype=torch.int32, device="cuda")
+        case = {"n_theta": nt, "n_triangles": w.mesh.n_tri}
+        res = {}
+        for mode, name in ((0, "side_id"), (1, "parity")):
+            g.locate(to[:10000], td[:10000], mode, material_out=mat[:10000])
+            g.locate(to, td, mode, material_out=mat)
+            c = g.get_counters()
+            res[name] = mat.cpu().numpy().copy()
+            case[name] = {"queries_per_s": n / (c["last_run_ms"] * 1e-3), "kernel_ms": c["last_run_ms"],
+                          "box_tests_per_query": c["n_box_tests"] / n, "tri_tests_per_query": c["n_tri_tests"] / n}
+        case["parity_over_side_id_time"] = case["parity"]["kernel_ms"] / case["side_id"]["kernel_ms"]
+        case["rules_disagree"] = int((res["side_id"] != res["parity"]).sum())
+        out["cases"].append(case)
+    a, b = out["cases"]
+    out["facets_x3_time_increase"] = {k: b[k]["kernel_ms"] / a[k]["kernel_ms"] - 1.0 for k in ("side_id", "parity")}
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -151,6 +183,7 @@ def main():
     ap.add_argument("--ref-sample", type=float, default=60000)
     ap.add_argument("--cpu-sample", type=float, default=0, help="oracle histories; 0 = sized for ~15 s from a pilot run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--locate-bench", type=float, default=0, help="localisation benchmark: side-id vs parity rule (PAPER.md:191-193)")
     ap.add_argument("--ray-bench", type=float, default=0, help="config-4 ray benchmark: this many seeded rays through gadep_trace_rays")
     args = ap.parse_args()
 
@@ -175,6 +208,9 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     if args.ray_bench:
         run_ray_bench(args, dm)
+        return
+    if args.locate_bench:
+        run_locate_bench(args, dm)
         return
     n_hist = int(args.histories) if args.histories else w.n_histories
     stream = torch.cuda.current_stream()

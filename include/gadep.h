@@ -141,6 +141,21 @@ int gadep_fepe(const gadep_ctx *ctx, int line, int mode, double *fepe, double *s
 int gadep_trace_rays(gadep_ctx *ctx, const float *org, const float *dir, long long n_rays, int filter_material,
                      float t_min, int *tri_out, float *t_out);
 
+/*
+ * Material in which each point lies (sec 2.4.2), found from a ray cast along dir.
+ *   mode GADEP_LOCATE_SIDE_ID  the paper's original rule: nearest facet ahead; its normal tells entering from leaving and
+ *                              the facet's side ids give the material (what gadep_run uses).
+ *   mode GADEP_LOCATE_PARITY   the paper's reworked rule: intersections with every closed surface are counted (all-hits
+ *                              BVH traversal); among the surfaces with an odd count the one whose first intersection
+ *                              is nearest contains the point and its inside material is returned; none -> world.
+ * org, dir: HOST-or-DEVICE float[n][3]; material_out int[n] in the same memory space.  A ray that meets more than 96
+ * facets returns GADEP_LOCATE_OVERFLOW (-3) in parity mode.  Counters (box / triangle tests) as for gadep_trace_rays.
+ */
+#define GADEP_LOCATE_SIDE_ID 0
+#define GADEP_LOCATE_PARITY 1
+#define GADEP_LOCATE_OVERFLOW (-3)
+int gadep_locate(gadep_ctx *ctx, const float *org, const float *dir, long long n, int mode, int *material_out);
+
 /* Per-history dump (same arithmetic as gadep_run): edep_out float[n] scoring deposit (line energy for
  * full-absorption histories), flags_out unsigned[n] (GADEP_F_*).  HOST-or-DEVICE, either may be NULL. */
 int gadep_run_histories(gadep_ctx *ctx, unsigned long long first, long long n, unsigned long long seed,

@@ -20,7 +20,7 @@ RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES = 1, 2, 
 
 EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_set_materials", "gadep_load_mesh",
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
-                    "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw")
+                    "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw", "gadep_locate")
 
 
 class GadepError(RuntimeError):
@@ -97,6 +97,7 @@ def load_library(build_if_missing: bool = True):
     L.gadep_run_histories.argtypes = [vp, ull, ll, ull, vp, vp]
     L.gadep_get_counters.argtypes = [vp, C.POINTER(GadepCounters)]
     L.gadep_philox_raw.argtypes = [vp, vp, vp, i32, vp]
+    L.gadep_locate.argtypes = [vp, vp, vp, ll, i32, vp]
     _lib = L
     return L
 
@@ -215,6 +216,17 @@ class Gadep:
         self._check(self.L.gadep_trace_rays(self.h, _ptr(org), _ptr(dir), n, int(filter_material), float(t_min),
                                             _ptr(tri_out), _ptr(t_out)))
         return tri_out, t_out
+
+    def locate(self, org, dir, mode=0, material_out=None):
+        """Material containing each point (mode 0 side-id rule, 1 parity rule)."""
+        if isinstance(org, np.ndarray):
+            org = np.ascontiguousarray(org, dtype=np.float32)
+            dir = np.ascontiguousarray(dir, dtype=np.float32)
+            material_out = np.empty(org.shape[0], dtype=np.int32) if material_out is None else material_out
+        elif material_out is None:
+            raise ValueError("device inputs need a device output")
+        self._check(self.L.gadep_locate(self.h, _ptr(org), _ptr(dir), org.shape[0], int(mode), _ptr(material_out)))
+        return material_out
 
     def run_histories(self, first, n, seed):
         edep = np.empty(n, dtype=np.float32)

@@ -16,6 +16,7 @@
 #include "gadep_build_kernels.cuh"
 #include "gadep_transport_kernels.cuh"
 #include "gadep_wave_kernels.cuh"
+#include "gadep_locate_kernels.cuh"
 
 struct gadep_ctx {
     int device = 0;
@@ -568,6 +569,43 @@ extern "C" int gadep_trace_rays(gadep_ctx *c, const float *org, const float *dir
     if (e == cudaSuccess) e = cudaMemcpy(&c->h_counters, c->d_counters, sizeof(GdCounters), cudaMemcpyDeviceToHost);
     cudaFree(stage);
     if (e != cudaSuccess) return gd_fail(c, GADEP_E_CUDA, "trace failed: %s", cudaGetErrorString(e));
+    cudaEventElapsedTime(&c->last_run_ms, c->ev0, c->ev1);
+    c->run_timed = false;
+    return GADEP_OK;
+}
+
+extern "C" int gadep_locate(gadep_ctx *c, const float *org, const float *dir, long long n, int mode, int *material_out) {
+    if (!c) return GADEP_E_NULL;
+    if (!org || !dir || !material_out) return gd_fail(c, GADEP_E_NULL, "null array");
+    if (!c->have_bvh) return gd_fail(c, GADEP_E_ORDER, "gadep_locate before gadep_build_bvh");
+    if (n < 0 || (mode != GADEP_LOCATE_SIDE_ID && mode != GADEP_LOCATE_PARITY)) return gd_fail(c, GADEP_E_ARG, "bad count or mode");
+    if (n == 0) return GADEP_OK;
+    GD_CUDA(c, cudaSetDevice(c->device));
+    const bool dev = gd_is_device_ptr(org);
+    if (dev != gd_is_device_ptr(dir) || dev != gd_is_device_ptr(material_out))
+        return gd_fail(c, GADEP_E_ARG, "arrays must live in one memory space");
+    cudaStream_t st = c->stream;
+    const float *d_org = org, *d_dir = dir;
+    int *d_mat = material_out;
+    float *stage = nullptr;
+    const size_t nb3 = sizeof(float) * 3 * (size_t)n;
+    if (!dev) {
+        GD_CUDA(c, cudaMalloc(&stage, 2 * nb3 + sizeof(int) * (size_t)n));
+        d_org = stage; d_dir = stage + 3 * n; d_mat = (int *)(stage + 6 * n);
+        cudaMemcpyAsync(stage, org, nb3, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(stage + 3 * n, dir, nb3, cudaMemcpyHostToDevice, st);
+    }
+    cudaMemsetAsync(c->d_counters, 0, sizeof(GdCounters), st);
+    cudaEventRecord(c->ev0, st);
+    gd_k_locate<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n, mode, c->world, d_mat, c->d_counters);
+    cudaEventRecord(c->ev1, st);
+    c->last_run_launches = 1;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && !dev) cudaMemcpyAsync(material_out, d_mat, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaMemcpy(&c->h_counters, c->d_counters, sizeof(GdCounters), cudaMemcpyDeviceToHost);
+    cudaFree(stage);
+    if (e != cudaSuccess) return gd_fail(c, GADEP_E_CUDA, "locate failed: %s", cudaGetErrorString(e));
     cudaEventElapsedTime(&c->last_run_ms, c->ev0, c->ev1);
     c->run_timed = false;
     return GADEP_OK;

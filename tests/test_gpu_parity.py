@@ -148,6 +148,29 @@ def test_cfg4_full_size_rays(pkg, orc):
     _check_rays(w, g, s, org[:k], d[:k])
 
 
+@pytest.mark.parametrize("cfg,n", [(1, 4000), (3, 2000)])
+def test_localisation_side_id_and_parity_rules(pkg, orc, cfg, n):
+    # the original side-id rule and the reworked parity rule (all-hits traversal) must name the same
+    # material for every point, and both must agree with the oracle's brute-force versions of the two rules.
+    w, g, s = _setup(pkg, orc, cfg)
+    r, z0, z1 = (45.0, -105.0, 10.0) if cfg == 1 else (60.0, -235.0, 45.0)
+    org, d = make_rays(n, 11, r, z0, z1)
+    m_side = g.locate(org, d, 0)
+    c0 = g.get_counters()
+    m_par = g.locate(org, d, 1)
+    c1 = g.get_counters()
+    o_side = np.array([s.locate_sideid(org[i].astype(np.float64), d[i].astype(np.float64)) for i in range(n)])
+    o_par = np.array([s.locate_parity(org[i].astype(np.float64), d[i].astype(np.float64)) for i in range(n)])
+    assert (m_par != -3).all()                               # no ray met more facets than the hit list holds
+    # a ray through an edge or vertex is counted twice by any edge-inclusive test: allow a handful of such rays
+    for a, b in ((m_side, o_side), (m_par, o_par), (m_side, m_par)):
+        assert (a != b).sum() <= 2 + 1e-3 * n, int((a != b).sum())
+    assert set(np.unique(m_par)) <= set(range(len(w.is_scoring)))
+    assert len(np.unique(m_par)) >= 5                        # the sample really visits the nested regions
+    # the all-hits traversal visits more of the hierarchy than the nearest-hit one
+    assert c1["n_box_tests"] >= c0["n_box_tests"] and c1["n_tri_tests"] >= c0["n_tri_tests"]
+
+
 def test_filtered_trace_with_negative_window(pkg, orc):
     w, g, s = _setup(pkg, orc, 1)
     org, d = make_rays(60_000, 5, 36.0, -72.0, 1.0)
