@@ -51,7 +51,7 @@ struct gadep_ctx {
     int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
-    GdWaveTune tune = {8, 4, 4, 4.0f, 8.0f, 12, 8};
+    GdWaveTune tune = {8, 4, 4, 4.0f, 8.0f, 12};
     double split_budget = 8.0;                // extra BVH references per facet handed out by the splitting budget
     int n_bins = 0;
     float spec_e_max = 0;
@@ -121,9 +121,9 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,leaf_thresh" (measurement sweeps)
         int a, b, d;
         float lm = c->tune.lam_max, cm = c->tune.cap_mfp;
-        int sp = c->tune.sparse_max, tb = c->tune.t_burst;
-        int k = sscanf(t, "%d,%d,%d,%f,%f,%d,%d", &a, &b, &d, &lm, &cm, &sp, &tb);
-        if (k >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && lm >= 0 && cm > 0 && tb >= 1) c->tune = {a, b, d, lm, cm, sp, tb};
+        int sp = c->tune.sparse_max;
+        int k = sscanf(t, "%d,%d,%d,%f,%f,%d", &a, &b, &d, &lm, &cm, &sp);
+        if (k >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && lm >= 0 && cm > 0) c->tune = {a, b, d, lm, cm, sp};
     }
     *out = c;
     return GADEP_OK;

@@ -20,9 +20,6 @@
 #define GD_W_WARPS (GD_W_THREADS / 32)
 #define GD_W_SLOTS 64
 #define GD_W_NF 29
-#ifndef GD_W_SYNC
-#define GD_W_SYNC 0            // the warps of a block run their physics / traversal bursts in lock-step
-#endif
 
 #ifdef GD_DIAG
 __device__ unsigned long long gd_diag[128];
@@ -37,7 +34,6 @@ struct GdWaveTune {
     float lam_max;      // safety queries only where the mean free path is below this [mm]; 0 disables them
     float cap_mfp;      // search radius of a safety query in mean free paths
     int sparse_max;     // ... and only while the warp has at most this many live photons
-    int t_burst;        // phase-locked mode: traversal rounds per T-burst
 };
 
 // ---- slot <-> registers
@@ -134,7 +130,6 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     __shared__ GdSource s_src;
     __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];
     __shared__ unsigned s_cnt[14];
-    __shared__ int s_live_warps;
     __shared__ unsigned char s_qready[GD_W_WARPS][GD_W_SLOTS], s_qres[GD_W_WARPS][GD_W_SLOTS];
     const int n_tab = M.n_mat * 4 * M.n_grid;
     float *s_tab = (float *)gd_smem;
@@ -145,7 +140,6 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i];
     if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }
     if (threadIdx.x < 14) s_cnt[threadIdx.x] = 0;
-    if (threadIdx.x == 0) s_live_warps = GD_W_WARPS;
     __syncthreads();
 
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -174,20 +168,14 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #endif
     __syncwarp();
 
-    bool alive = true;
     for (;;) {
-#if GD_W_SYNC
-        // all warps of the block change phase together: one instruction-cache fill serves 16 warps
-        __syncthreads();
-        if (*(volatile int *)&s_live_warps == 0) break;
-#endif
         // ================================================================ P-burst
 #ifdef GD_DIAG
         long long d_t0 = clock64();
 #endif
         // full batches first; a partial batch only when the warp would otherwise starve
         bool did_full = false;
-        while (alive && (n_res >= 32 || (n_res > 0 && n_ready == 0 && !did_full))) {
+        while (n_res >= 32 || (n_res > 0 && n_ready == 0 && !did_full)) {
             const int take = n_res < 32 ? n_res : 32;
             did_full = take == 32;
             GD_DIAG_ADD(8, 1); GD_DIAG_ADD(9, take);
@@ -304,28 +292,15 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #ifdef GD_DIAG
         long long d_t1 = clock64(); GD_DIAG_ADD(16, d_t1 - d_t0);
 #endif
-#if GD_W_SYNC
-        __syncthreads();
-        if (!alive) continue;
-#endif
         const unsigned busy_mask = __ballot_sync(0xFFFFFFFFu, T.slot >= 0);
         if (n_ready == 0 && busy_mask == 0u) {
             if (n_res == 0) {                                // every slot is dead
-#if GD_W_SYNC
-                alive = false;
-                if (lane == 0) atomicSub(&s_live_warps, 1);
-                continue;
-#else
                 break;
-#endif
             }
             continue;
         }
         // ================================================================ T-burst
-        for (int t_it = 0;; ++t_it) {
-#if GD_W_SYNC
-            if (t_it >= tune.t_burst) break;
-#endif
+        for (;;) {
             const unsigned idle_mask = __ballot_sync(0xFFFFFFFFu, T.slot < 0);
             const int n_idle = __popc(idle_mask);
             if (n_idle) {
