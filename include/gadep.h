@@ -108,6 +108,9 @@ int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
 #define GADEP_RUN_HISTORY_PER_THREAD 4  /* measurement: the plain one-history-per-thread kernel instead of the   */
                                    /* warp-resident wavefront kernel (same results, bit for bit)                */
 #define GADEP_RUN_PERSISTENT_LANES 8    /* measurement: one history per lane with refill (same results)           */
+#define GADEP_RUN_PARITY_LOCALISATION 16 /* the paper's reworked localisation: the material at the  */
+                                   /* start and after every boundary crossing comes from parity counting over  */
+                                   /* all facets ahead (history-per-thread kernel); the side ids only mark KILL */
 typedef struct {
     int n_bins;                    /* spectrum bins over [0, e_max_mev); one extra overflow slot follows        */
     float e_max_mev;
@@ -171,6 +174,8 @@ typedef struct {
     int last_run_launches, last_build_launches;
     unsigned long long n_safety_queries;   /* wavefront kernel: facet-free-sphere queries issued                 */
     unsigned long long n_skipped_queries;  /* flights whose nearest-hit query was answered by such a sphere      */
+    unsigned long long n_parity_queries;   /* GADEP_RUN_PARITY_LOCALISATION: all-hits localisation queries       */
+    unsigned long long n_parity_mismatch;  /* ... of which the parity rule and the side ids named different media */
 } gadep_counters;
 /* Counters of the last gadep_run / gadep_run_histories / gadep_trace_rays (HOST output). */
 int gadep_get_counters(const gadep_ctx *ctx, gadep_counters *out);

@@ -16,7 +16,7 @@ F_ESCAPED, F_PEAK, F_LEAK, F_NONSCORING = 1, 2, 4, 8
 FILTER_NONE = -2
 MAT_KILL = -1
 MAX_LINES = 64
-RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES = 1, 2, 4, 8
+RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES, RUN_PARITY_LOCALISATION = 1, 2, 4, 8, 16
 
 EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_set_materials", "gadep_load_mesh",
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
@@ -47,7 +47,8 @@ class GadepCounters(C.Structure):
                [("emitted", C.c_ulonglong * MAX_LINES), ("peak", C.c_ulonglong * MAX_LINES), ("n_lines", C.c_int),
                 ("n_bvh_nodes", C.c_int), ("bvh_max_depth", C.c_int), ("last_run_ms", C.c_float),
                 ("last_build_ms", C.c_float), ("last_run_launches", C.c_int), ("last_build_launches", C.c_int),
-                ("n_safety_queries", C.c_ulonglong), ("n_skipped_queries", C.c_ulonglong)]
+                ("n_safety_queries", C.c_ulonglong), ("n_skipped_queries", C.c_ulonglong),
+                ("n_parity_queries", C.c_ulonglong), ("n_parity_mismatch", C.c_ulonglong)]
 
     def as_dict(self):
         d = {n: int(getattr(self, n)) for n, _ in self._fields_[:12]}
@@ -56,7 +57,8 @@ class GadepCounters(C.Structure):
                  n_bvh_nodes=int(self.n_bvh_nodes), bvh_max_depth=int(self.bvh_max_depth),
                  last_run_ms=float(self.last_run_ms), last_build_ms=float(self.last_build_ms),
                  last_run_launches=int(self.last_run_launches), last_build_launches=int(self.last_build_launches),
-                 n_safety_queries=int(self.n_safety_queries), n_skipped_queries=int(self.n_skipped_queries))
+                 n_safety_queries=int(self.n_safety_queries), n_skipped_queries=int(self.n_skipped_queries),
+                 n_parity_queries=int(self.n_parity_queries), n_parity_mismatch=int(self.n_parity_mismatch))
         return d
 
 

@@ -427,7 +427,8 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (variant == 2) smem += sizeof(float) * (size_t)GD_W_WARPS * GD_W_NF * GD_W_SLOTS;
     if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
     const void *kern = variant == 2 ? (const void *)gd_k_transport_wave
-                                    : (variant == 1 ? (const void *)gd_k_transport_refill : (const void *)gd_k_transport);
+                                    : (variant == 1 ? (const void *)gd_k_transport_refill
+                                                  : (variant == 3 ? (const void *)gd_k_transport<true> : (const void *)gd_k_transport<false>));
     GD_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
@@ -448,15 +449,17 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0) {
         unsigned long long warps = (unsigned long long)grid * (threads / 32);
         unsigned chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / (warps * 16)));
-        if (variant != 0) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
+        if (variant == 1 || variant == 2) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
         if (variant == 2) {
             gd_k_transport_wave<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
                                                              c->d_next, chunk, c->d_pair, c->tune);
         } else if (variant == 1) {
             gd_k_transport_refill<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
                                                                d_flags, c->d_next, chunk);
+        } else if (variant == 3) {
+            gd_k_transport<true><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
         } else {
-            gd_k_transport<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+            gd_k_transport<false><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
         }
         c->last_run_launches = 1;
     }
@@ -490,7 +493,7 @@ extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned 
     bool dev_out = gd_is_device_ptr(spectrum);
     if ((opts->flags & GADEP_RUN_ASYNC) && spectrum && !dev_out)
         return gd_fail(c, GADEP_E_ARG, "GADEP_RUN_ASYNC needs a device spectrum pointer");
-    c->kernel_variant = (opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((opts->flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2);
+    c->kernel_variant = (opts->flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((opts->flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
     int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
                                  (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
     if (rc) return rc;
@@ -644,6 +647,7 @@ extern "C" int gadep_get_counters(const gadep_ctx *cc, gadep_counters *out) {
     out->n_tri_tests = h.n_tri_tests; out->n_crossings = h.n_crossings; out->n_pe = h.n_pe; out->n_compton = h.n_compton;
     out->n_coherent = h.n_coherent; out->n_pair = h.n_pair; out->n_escaped = h.n_escaped; out->n_leak = h.n_leak;
     out->n_cutoff = h.n_cutoff; out->n_safety_queries = h.n_safety; out->n_skipped_queries = h.n_skipped;
+    out->n_parity_queries = h.n_parity; out->n_parity_mismatch = h.n_parity_mismatch;
     memcpy(out->emitted, c->h_emitted, sizeof(out->emitted));
     memcpy(out->peak, c->h_peak, sizeof(out->peak));
     out->n_lines = c->src.n_lines;

@@ -58,7 +58,7 @@ struct GdBvh {
 
 struct GdCounters {    // device-side totals, 64-bit
     unsigned long long n_histories, n_queries, n_box_tests, n_tri_tests, n_crossings, n_pe, n_compton, n_coherent,
-        n_pair, n_escaped, n_leak, n_cutoff, n_safety, n_skipped;
+        n_pair, n_escaped, n_leak, n_cutoff, n_safety, n_skipped, n_parity, n_parity_mismatch;
 };
 
 struct GdLocalCounters {  // per-thread, 32-bit

@@ -288,9 +288,89 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
     return true;
 }
 
-// One whole history on one lane (history-per-thread kernel, host emulation)
-GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *tab, const GdSource &S,
-                          unsigned long long seed, unsigned long long history, GdHistory &out, GdLocalCounters &cnt) {
+// ---------------------------------------------------------------- parity localisation inside the transport loop
+// intersections of the ray from the photon with every closed surface are counted (all hits, binary BVH);
+// among the surfaces with an odd count the one with the nearest first intersection contains the photon.  Facets the
+// photon has just crossed (ex) lie at t ~ 0 and are skipped -- the crossing itself already moved the photon to their
+// far side.  Returns the material, or -3 when the hit list overflows.
+#define GD_PAR_MAX_HITS 64
+GD_HD int gd_locate_parity(const GdBvh &bvh, const GdRay &ray, const GdExclude &ex, int world, unsigned &n_box_tests,
+                           unsigned &n_tri_tests) {
+    int h_facet[GD_PAR_MAX_HITS], h_surf[GD_PAR_MAX_HITS], h_in[GD_PAR_MAX_HITS];
+    float h_t[GD_PAR_MAX_HITS];
+    int nh = 0;
+    if (!bvh.root_is_leaf) {
+        int stack[GD_STACK];
+        int sp = 0, node = 0;
+        for (;;) {
+            if (node >= 0) {
+                const GdNode &nd = bvh.nodes[node];
+                const float4 a = nd.n0xy, b = nd.n1xy, z = nd.nz;
+                const int4 lk = nd.link;
+                n_box_tests += 2;
+                float x0 = (a.x - ray.o.x) * ray.inv.x, x1 = (a.y - ray.o.x) * ray.inv.x;
+                float y0 = (a.z - ray.o.y) * ray.inv.y, y1 = (a.w - ray.o.y) * ray.inv.y;
+                float z0 = (z.x - ray.o.z) * ray.inv.z, z1 = (z.y - ray.o.z) * ray.inv.z;
+                const float n0 = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), 0.0f));
+                float f0 = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fmaxf(z0, z1));
+                f0 = f0 + fabsf(f0) * 4.0e-7f;
+                x0 = (b.x - ray.o.x) * ray.inv.x; x1 = (b.y - ray.o.x) * ray.inv.x;
+                y0 = (b.z - ray.o.y) * ray.inv.y; y1 = (b.w - ray.o.y) * ray.inv.y;
+                z0 = (z.z - ray.o.z) * ray.inv.z; z1 = (z.w - ray.o.z) * ray.inv.z;
+                const float n1 = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), 0.0f));
+                float f1 = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fmaxf(z0, z1));
+                f1 = f1 + fabsf(f1) * 4.0e-7f;
+                const bool g0 = n0 <= f0, g1 = n1 <= f1;
+                if (g0 && g1) { stack[sp++] = lk.y; node = lk.x; }
+                else if (g0) node = lk.x;
+                else if (g1) node = lk.y;
+                else if (sp == 0) break;
+                else node = stack[--sp];
+                continue;
+            }
+            const GdTri &tr = bvh.tris[~node];
+            const int facet = gd_as_int(tr.v0.w);
+            if (facet != ex.a && facet != ex.b && facet != ex.c) {
+                float t, det;
+                n_tri_tests++;
+                if (gd_ray_tri(ray, tr.v0, tr.v1, tr.v2, t, det) && t > 0.0f) {
+                    bool seen = false;
+                    for (int k = 0; k < nh; ++k) seen = seen || h_facet[k] == facet;
+                    if (!seen) {
+                        if (nh == GD_PAR_MAX_HITS) return -3;
+                        h_facet[nh] = facet; h_t[nh] = t; h_surf[nh] = gd_as_int(tr.v2.w);
+                        h_in[nh] = gd_mat_inside(gd_as_int(tr.v1.w));
+                        nh++;
+                    }
+                }
+            }
+            if (sp == 0) break;
+            node = stack[--sp];
+        }
+    }
+    int result = world;
+    float best = GD_INF;
+    for (int a = 0; a < nh; ++a) {
+        bool first_of_surface = true;
+        for (int b = 0; b < a; ++b) first_of_surface = first_of_surface && h_surf[b] != h_surf[a];
+        if (!first_of_surface) continue;
+        int count = 0;
+        float first = GD_INF;
+        for (int b = a; b < nh; ++b)
+            if (h_surf[b] == h_surf[a]) { count++; first = fminf(first, h_t[b]); }
+        if ((count & 1) && first < best) { best = first; result = h_in[a]; }
+    }
+    return result;
+}
+
+// One whole history on one lane (history-per-thread kernel, host emulation).
+// PARITY: after the start localisation and after every boundary crossing the material comes from the parity rule
+// instead of the facet's side ids (the side ids still say where the KILL boundary is); mismatches between the two
+// rules are counted in cnt.n_cutoff's neighbour fields by the caller.
+template <bool PARITY>
+GD_HD void gd_run_history_t(const GdBvh &bvh, const GdMaterials &M, const float *tab, const GdSource &S,
+                            unsigned long long seed, unsigned long long history, GdHistory &out, GdLocalCounters &cnt,
+                            unsigned &n_parity, unsigned &n_mismatch) {
     GdLane L;
     gd_lane_start(L, S, seed, history);
     GdRay ray;
@@ -302,9 +382,33 @@ GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *t
         gd_ray_setup(ray, L.pos, L.dir);
         cnt.n_queries++;
         gd_nearest_hit<false>(bvh, ray, t_min, t_max, filter, L.ex, true, hit, cnt.n_box_tests, cnt.n_tri_tests);
-#if defined(GD_DIAG) && defined(__CUDA_ARCH__)     // step trace of the history-per-thread kernel (diagnostic builds only)
-        printf("q%u mode %d m %d e %.6f pos (%.7f %.7f %.7f) dir (%.6f %.6f %.6f) tau %.5g mu %.5g sdist %.6g ex (%d %d %d) -> facet %d t %.9g leaving %d in %d out %d\n", cnt.n_queries, L.mode, L.m, L.e, L.pos.x, L.pos.y, L.pos.z, L.dir.x, L.dir.y, L.dir.z, L.tau, L.mu_tot, L.sdist, L.ex.a, L.ex.b, L.ex.c, hit.leaf < 0 ? -1 : hit.orig, hit.t, hit.leaving, gd_mat_inside(hit.mats), gd_mat_outside(hit.mats));
-#endif
+        const unsigned crossings_before = cnt.n_crossings;
+        const bool was_locate = L.mode == GD_MODE_LOCATE;
+        if (PARITY && was_locate) {
+            // start material from the parity rule: present it as the from-side of the hit (or as the world material)
+            const int m_par = gd_locate_parity(bvh, ray, L.ex, M.world_material, cnt.n_box_tests, cnt.n_tri_tests);
+            n_parity++;
+            const int m_side = hit.leaf < 0 ? M.world_material : (hit.leaving ? gd_mat_inside(hit.mats) : gd_mat_outside(hit.mats));
+            if (m_par != m_side) {
+                n_mismatch++;
+                if (m_par >= 0 && hit.leaf >= 0) {      // the parity rule decides: present it as the facet's from-side
+                    if (hit.leaving) hit.mats = (m_par & 0xFFFF) | (int)((unsigned)hit.mats & 0xFFFF0000u);
+                    else hit.mats = (hit.mats & 0xFFFF) | (int)((unsigned)(m_par & 0xFFFF) << 16);
+                }
+            }
+        }
         if (gd_lane_post(L, M, tab, S, seed, hit, out, cnt)) return;
+        if (PARITY && cnt.n_crossings != crossings_before && L.mode == GD_MODE_FLIGHT) {
+            gd_ray_setup(ray, L.pos, L.dir);
+            const int m_par = gd_locate_parity(bvh, ray, L.ex, M.world_material, cnt.n_box_tests, cnt.n_tri_tests);
+            n_parity++;
+            if (m_par != L.m) { n_mismatch++; if (m_par >= 0) { L.m = m_par; L.need_mu = 1; } }
+        }
     }
+}
+
+GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *tab, const GdSource &S,
+                          unsigned long long seed, unsigned long long history, GdHistory &out, GdLocalCounters &cnt) {
+    unsigned a = 0, b = 0;
+    gd_run_history_t<false>(bvh, M, tab, S, seed, history, out, cnt, a, b);
 }

@@ -54,6 +54,8 @@ gd_k_trace(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ d
 }
 
 // dynamic shared memory: [table floats][spectrum u32 (n_bins+1)]
+// PARITY: material after the start and after every crossing from the paper's parity rule
+template <bool PARITY>
 __global__ void __launch_bounds__(GD_RUN_THREADS)
 gd_k_transport(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
                unsigned long long n_hist, unsigned long long seed, GdTally tally, float *__restrict__ edep_out,
@@ -71,11 +73,11 @@ gd_k_transport(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsig
     __syncthreads();
 
     GdLocalCounters cnt = {};
-    unsigned n_done = 0;
+    unsigned n_done = 0, n_parity = 0, n_mismatch = 0;
     const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
     for (unsigned long long h = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; h < n_hist; h += stride) {
         GdHistory r;
-        gd_run_history(bvh, M, s_tab, s_src, seed, first + h, r, cnt);
+        gd_run_history_t<PARITY>(bvh, M, s_tab, s_src, seed, first + h, r, cnt, n_parity, n_mismatch);
         n_done++;
         atomicAdd(&s_emitted[r.line], 1u);
         if (r.flags & GD_F_PEAK) {
@@ -99,6 +101,10 @@ gd_k_transport(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsig
         if (s_peak[threadIdx.x]) atomicAdd(&tally.peak[threadIdx.x], (unsigned long long)s_peak[threadIdx.x]);
     }
     gd_flush_counters(cnt, tally.counters, n_done);
+    if (PARITY) {
+        if (n_parity) atomicAdd(&tally.counters->n_parity, (unsigned long long)n_parity);
+        if (n_mismatch) atomicAdd(&tally.counters->n_parity_mismatch, (unsigned long long)n_mismatch);
+    }
 }
 
 // ---------------------------------------------------------------- v1: persistent lanes with refill

@@ -171,6 +171,24 @@ def test_localisation_side_id_and_parity_rules(pkg, orc, cfg, n):
     assert c1["n_box_tests"] >= c0["n_box_tests"] and c1["n_tri_tests"] >= c0["n_tri_tests"]
 
 
+@pytest.mark.parametrize("cfg,n", [(1, 300_000), (3, 20_000)])
+def test_transport_with_parity_localisation(pkg, orc, cfg, n):
+    # GADEP_RUN_PARITY_LOCALISATION: the material after the start and after every crossing comes from the paper's parity
+    # rule instead of the facet's side ids.  On a valid mesh the two rules name the same medium, so the
+    # tallies must coincide except for the rare rays through an edge, which the counters report.
+    from paper_2605_25963_b200.binding import RUN_HISTORY_PER_THREAD, RUN_PARITY_LOCALISATION
+    w, g, s = _setup(pkg, orc, cfg)
+    a = g.run(n, 3, w.n_bins, w.spectrum_e_max_mev, flags=RUN_HISTORY_PER_THREAD).copy()
+    ca = g.get_counters()
+    b = g.run(n, 3, w.n_bins, w.spectrum_e_max_mev, flags=RUN_PARITY_LOCALISATION).copy()
+    cb = g.get_counters()
+    assert cb["n_parity_queries"] >= n and cb["n_parity_mismatch"] <= 2e-5 * cb["n_parity_queries"] + 2
+    assert ca["n_parity_queries"] == 0
+    assert abs(int(a.sum()) - int(b.sum())) <= 5 * cb["n_parity_mismatch"] + 2
+    assert np.abs(a.astype(np.int64) - b.astype(np.int64)).sum() <= 10 * cb["n_parity_mismatch"] + 4
+    assert sum(cb["emitted"]) == n and cb["n_box_tests"] > ca["n_box_tests"]
+
+
 def test_filtered_trace_with_negative_window(pkg, orc):
     w, g, s = _setup(pkg, orc, 1)
     org, d = make_rays(60_000, 5, 36.0, -72.0, 1.0)
