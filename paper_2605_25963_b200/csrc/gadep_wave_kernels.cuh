@@ -3,11 +3,14 @@
 // Every warp owns GD_W_SLOTS photon slots in shared memory (SoA, GD_W_NF words per slot).  A slot is in one of
 // three places: the READY queue (its next nearest-hit query is prepared), in flight on a lane (GdTrav registers),
 // or the RESULT queue (hit known, physics pending).  The warp alternates
-//   T-burst: lanes traverse; a lane whose ray ends writes the hit to its slot, pushes it to RESULT and -- as soon as
-//            `k_fetch` lanes are idle -- takes a READY slot (dynamic fetch).  The burst ends when READY is empty and
-//            `k_exit` lanes idle; unfinished rays stay in their lanes' registers.
+//   T-burst: lanes traverse in rounds of `n_steps` 4-wide node visits + one leaf step; a lane whose ray ends writes
+//            the hit to its slot, pushes it to RESULT and -- as soon as `k_fetch` lanes are idle -- takes a READY slot
+//            (dynamic fetch).  The burst ends when READY is empty and 32 results wait (or `k_exit` times as many
+//            results as rays still in flight: sparse warps batch their few chains); unfinished rays stay in their
+//            lanes' registers across the physics burst.
 //   P-burst: RESULT slots are processed 32 at a time by all lanes (boundary crossing / interaction / tally /
-//            refill from the history counter / attenuation lookup) and pushed to READY.
+//            refill from the history counter / attenuation lookup) and pushed to READY.  Both queues are rings
+//            (first in, first out), so every slot is served once per cycle.
 // There is no block-level barrier inside the loop and no particle state in global memory (only the two pending
 // annihilation photons of a pair event, which are rare, sit in a global side buffer).  Results do not depend on any
 // of this scheduling: random streams are keyed by the history index and the tallies are integers.
@@ -29,8 +32,12 @@ __device__ unsigned long long gd_diag_warp[4096][8];
 #define GD_DIAG_ADD(k, v) do {} while (0)
 #endif
 
+// scheduling knobs (defaults in gadep_api.cu; GADEP_TUNE="k_fetch,k_exit,n_steps[,lam_max,cap_mfp,sparse_max]" overrides
+// them for measurement sweeps).  None of them can change a result.
 struct GdWaveTune {
-    int k_fetch, k_exit, n_steps;
+    int k_fetch;        // idle lanes needed before READY slots are fetched
+    int k_exit;         // T-burst ends when n_results >= k_exit * rays in flight (or 32 results) and READY is empty
+    int n_steps;        // node visits per traversal round
     float lam_max;      // safety queries only where the mean free path is below this [mm]; 0 disables them
     float cap_mfp;      // search radius of a safety query in mean free paths
     int sparse_max;     // ... and only while the warp has at most this many live photons
