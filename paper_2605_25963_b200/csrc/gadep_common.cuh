@@ -137,6 +137,27 @@ GD_HD_NI float gd_rng_uniform_v(uint32_t k0, uint32_t k1, uint32_t h0, uint32_t 
     const uint32_t w = k == 0 ? o.x : (k == 1 ? o.y : (k == 2 ? o.z : o.w));
     return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f);
 }
+// the next four uniforms of the stream (draws d .. d+3) from one or two Philox blocks, without advancing the counter:
+// an interaction that knows it will use several draws in a row peeks them with one call and then advances by what
+// it used -- the stream is a pure function of the draw index, so the values are those gd_rng_next would return
+struct GdF4u { float a, b, c, d; };
+GD_HD_NI GdF4u gd_rng_peek4_v(uint32_t k0, uint32_t k1, uint32_t h0, uint32_t h1, uint32_t stream, uint32_t draw) {
+    const uint32_t b = draw >> 2, o = draw & 3u;
+    const GdU4 A = gd_philox4x32_10v(h0, h1, b, stream, k0, k1);
+    uint32_t w0 = A.x, w1 = A.y, w2 = A.z, w3 = A.w;
+    if (o) {
+        const GdU4 B = gd_philox4x32_10v(h0, h1, b + 1u, stream, k0, k1);
+        if (o == 1) { w0 = A.y; w1 = A.z; w2 = A.w; w3 = B.x; }
+        else if (o == 2) { w0 = A.z; w1 = A.w; w2 = B.x; w3 = B.y; }
+        else { w0 = A.w; w1 = B.x; w2 = B.y; w3 = B.z; }
+    }
+    const float s = 1.0f / 8388608.0f;
+    GdF4u u = {((float)(w0 >> 9) + 0.5f) * s, ((float)(w1 >> 9) + 0.5f) * s, ((float)(w2 >> 9) + 0.5f) * s,
+               ((float)(w3 >> 9) + 0.5f) * s};
+    return u;
+}
+GD_HD GdF4u gd_rng_peek4(const GdRng &g) { return gd_rng_peek4_v(g.k0, g.k1, g.h0, g.h1, g.stream, g.draw); }
+
 GD_HD float gd_rng_next(GdRng &g) {
 #if GD_RNG_CACHE
     uint32_t b = g.draw >> 2;

@@ -45,6 +45,13 @@ GD_HD_NI GdF2 gd_sincos_2pi_v(float u) {
 GD_HD void gd_sincos_2pi(float u, float &s, float &c) { GdF2 r = gd_sincos_2pi_v(u); s = r.s; c = r.c; }
 
 // O4 / O12: isotropic direction from 2 draws
+GD_HD GdVec3 gd_isotropic_from(float u1, float u2) {
+    float w = 1.0f - 2.0f * u1;
+    float st = sqrtf(fmaxf(0.0f, 1.0f - w * w));
+    float s, c;
+    gd_sincos_2pi(u2, s, c);
+    return gd_make(st * c, st * s, w);
+}
 GD_HD GdVec3 gd_sample_isotropic(GdRng &g) {
     float u1 = gd_rng_next(g), u2 = gd_rng_next(g);
     float w = 1.0f - 2.0f * u1;
@@ -95,8 +102,7 @@ GD_HD float gd_sample_compton(GdRng &g, float e, float &cos_t) {
 }
 
 // O11: Thomson (1 + cos^2) law by exact inversion of the CDF (3c + c^3 + 4)/8
-GD_HD float gd_sample_thomson(GdRng &g) {
-    float u = gd_rng_next(g);
+GD_HD float gd_thomson_from(float u) {
     float c = 8.0f * u - 4.0f;
     float r = sqrtf(0.25f * c * c + 1.0f);
     return cbrtf(0.5f * c + r) + cbrtf(0.5f * c - r);
@@ -144,7 +150,8 @@ GD_HD void gd_lane_start(GdLane &L, const GdSource &S, unsigned long long seed, 
     L.history = history;
     gd_rng_init(L.g, seed, history, 0, 0);
     int nl = S.n_lines;
-    float ul = gd_rng_next(L.g) * S.line_cum[nl - 1];
+    const GdF4u u4 = gd_rng_peek4(L.g);               // draws 0..3: line, then (point source) the direction
+    float ul = u4.a * S.line_cum[nl - 1]; L.g.draw += 1;
     int line = nl - 1;
     for (int l = 0; l < nl; ++l) if (ul < S.line_cum[l]) { line = l; break; }
     L.line = line;
@@ -164,6 +171,7 @@ GD_HD void gd_lane_start(GdLane &L, const GdSource &S, unsigned long long seed, 
         L.pos = gd_make(S.pos[0], S.pos[1], S.pos[2]);
     }
     if (S.kind == 2) L.dir = gd_make(S.dir[0], S.dir[1], S.dir[2]);
+    else if (S.kind == 0) { L.dir = gd_isotropic_from(u4.b, u4.c); L.g.draw += 2; }
     else L.dir = gd_sample_isotropic(L.g);
     L.dep = 0.0f; L.flags = 0; L.n_events = 0; L.pending = 0;
     L.m = 0; L.need_mu = 1; L.mu_tot = 0.0f; L.tau = 0.0f; L.sdist = 0.0f;
@@ -241,7 +249,9 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
         L.ex = gd_no_exclude(); L.n_stall = 0;                            // new flight segment
         if (L.e < M.e_cut) { gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_cutoff++; photon_done = true; }
         else {
-            float us = gd_rng_next(L.g) * L.mu_tot;
+            const GdF4u u4 = gd_rng_peek4(L.g);       // selection draw + the three draws of a coherent event
+            bool tau_done = false;
+            float us = u4.a * L.mu_tot; L.g.draw += 1;
             int ch = -1;
             float acc = 0.0f;
 #pragma unroll
@@ -262,9 +272,10 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
                 L.need_mu = 1;
                 if (L.e < M.e_cut) { gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_cutoff++; photon_done = true; }
             } else if (ch == 2) {                                                           // O11 coherent
-                float cost = gd_sample_thomson(L.g);
-                float uphi = gd_rng_next(L.g);
-                L.dir = gd_rotate(L.dir, cost, uphi);
+                const float cost = gd_thomson_from(u4.b);
+                L.dir = gd_rotate(L.dir, cost, u4.c);
+                L.tau = -logf(u4.d); tau_done = true;                                        // O7.1
+                L.g.draw += 3;
                 cnt.n_coherent++;
             } else {                                                                        // O12 pair
                 gd_deposit(M, L.m, L.e - GD_TWO_MEC2, L.dep, L.flags);
@@ -273,7 +284,7 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
                 cnt.n_pair++;
                 photon_done = true;
             }
-            if (!photon_done) L.tau = -logf(gd_rng_next(L.g));                              // O7.1
+            if (!photon_done && !tau_done) L.tau = -logf(gd_rng_next(L.g));                 // O7.1
         }
     }
     if (!photon_done) return false;
