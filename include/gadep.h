@@ -111,6 +111,9 @@ int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
 #define GADEP_RUN_PARITY_LOCALISATION 16 /* the paper's reworked localisation: the material at the  */
                                    /* start and after every boundary crossing comes from parity counting over  */
                                    /* all facets ahead (history-per-thread kernel); the side ids only mark KILL */
+#define GADEP_RUN_PARTIAL_XS 32     /* the paper's "partial cross-section method": one remaining    */
+                                   /* optical depth per process instead of total-mu sampling + a selection draw  */
+                                   /* (history-per-thread kernel; same distribution, different random streams)   */
 typedef struct {
     int n_bins;                    /* spectrum bins over [0, e_max_mev); one extra overflow slot follows        */
     float e_max_mev;

@@ -428,7 +428,8 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
     const void *kern = variant == 2 ? (const void *)gd_k_transport_wave
                                     : (variant == 1 ? (const void *)gd_k_transport_refill
-                                                  : (variant == 3 ? (const void *)gd_k_transport<true> : (const void *)gd_k_transport<false>));
+                                                  : (variant == 3 ? (const void *)gd_k_transport<true, false>
+                                                     : (variant == 4 ? (const void *)gd_k_transport<false, true> : (const void *)gd_k_transport<false, false>)));
     GD_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
@@ -457,9 +458,11 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
             gd_k_transport_refill<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
                                                                d_flags, c->d_next, chunk);
         } else if (variant == 3) {
-            gd_k_transport<true><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+            gd_k_transport<true, false><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+        } else if (variant == 4) {
+            gd_k_transport<false, true><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
         } else {
-            gd_k_transport<false><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+            gd_k_transport<false, false><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
         }
         c->last_run_launches = 1;
     }
@@ -493,7 +496,7 @@ extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned 
     bool dev_out = gd_is_device_ptr(spectrum);
     if ((opts->flags & GADEP_RUN_ASYNC) && spectrum && !dev_out)
         return gd_fail(c, GADEP_E_ARG, "GADEP_RUN_ASYNC needs a device spectrum pointer");
-    c->kernel_variant = (opts->flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((opts->flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
+    c->kernel_variant = (opts->flags & GADEP_RUN_PARTIAL_XS) ? 4 : (opts->flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((opts->flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
     int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
                                  (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
     if (rc) return rc;

@@ -143,6 +143,9 @@ struct GdLane {
     GdVec3 sc;
     float sr;
     int cool, qkind;       // safety-query back-off; kind of the pending query (0 ray, 1 safety)
+    // partial cross-section method only: remaining optical depth of every process, process that fires next
+    float tau_c[4];
+    int sel;
 };
 
 // O4: source sampling on stream 0; leaves the lane in mode LOCATE
@@ -180,16 +183,44 @@ GD_HD void gd_lane_start(GdLane &L, const GdSource &S, unsigned long long seed, 
     L.mode = GD_MODE_LOCATE;
 }
 
+// ---- "partial cross-section method" (R2 / section 13): every process c keeps its own remaining
+// optical depth tau_c; the flight ends where the first budget runs out (s = min_c tau_c / mu_c), that process fires, and
+// only its budget is sampled again.  Same distribution as total-mu sampling + a selection draw, one draw fewer per event.
+GD_HD void gd_partial_birth(GdLane &L) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) L.tau_c[c] = -logf(gd_rng_next(L.g));
+}
+GD_HD void gd_partial_step(GdLane &L) {
+    float best = GD_INF;
+    int sel = 0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const float sc = L.mu[c] > 0.0f ? L.tau_c[c] / L.mu[c] : GD_INF;
+        if (sc < best) { best = sc; sel = c; }
+    }
+    L.sdist = best; L.sel = sel;
+}
+GD_HD void gd_partial_advance(GdLane &L, float t) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) L.tau_c[c] -= L.mu[c] * t;
+}
+
 // parameters of the lane's next query
-GD_HD void gd_lane_query(GdLane &L, const GdMaterials &M, const float *tab, float &t_min, float &t_max, int &filter) {
+template <bool PARTIAL>
+GD_HD void gd_lane_query_t(GdLane &L, const GdMaterials &M, const float *tab, float &t_min, float &t_max, int &filter) {
     if (L.mode == GD_MODE_LOCATE) { t_min = 0.0f; t_max = GD_INF; filter = -2; return; }
     if (L.need_mu) { L.mu_tot = gd_mu_lookup(M, tab, L.m, L.e, L.mu); L.need_mu = 0; }     // O2
-    L.sdist = L.mu_tot > 0.0f ? L.tau / L.mu_tot : GD_INF;                                  // O7.2
+    if (PARTIAL) gd_partial_step(L);
+    else L.sdist = L.mu_tot > 0.0f ? L.tau / L.mu_tot : GD_INF;                             // O7.2
     t_min = -GD_TBACK; t_max = L.sdist; filter = L.m;                                       // O7.3
+}
+GD_HD void gd_lane_query(GdLane &L, const GdMaterials &M, const float *tab, float &t_min, float &t_max, int &filter) {
+    gd_lane_query_t<false>(L, M, tab, t_min, t_max, filter);
 }
 
 // the current photon ended: start the next annihilation photon if one waits; returns true when the history is over
-GD_HD bool gd_lane_next_photon(GdLane &L, unsigned long long seed) {
+template <bool PARTIAL>
+GD_HD bool gd_lane_next_photon_t(GdLane &L, unsigned long long seed) {
     if (L.pending == 0) return true;
     L.pos = L.p_pos; L.m = L.p_m; L.e = GD_MEC2; L.need_mu = 1;
     unsigned stream;
@@ -197,31 +228,36 @@ GD_HD bool gd_lane_next_photon(GdLane &L, unsigned long long seed) {
     else { L.dir = gd_make(-L.p_axis.x, -L.p_axis.y, -L.p_axis.z); stream = 2; }
     L.pending--;
     gd_rng_init(L.g, seed, L.history, stream, 0);
-    L.tau = -logf(gd_rng_next(L.g));                                                        // O7.1
+    if (PARTIAL) gd_partial_birth(L);
+    else L.tau = -logf(gd_rng_next(L.g));                                                   // O7.1
     L.ex = gd_no_exclude(); L.n_stall = 0;
     return false;
 }
 
 // consume the query result; returns true when the history is finished (out is then valid)
-GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const GdSource &S, unsigned long long seed,
-                        const GdHit &hit_in, GdHistory &out, GdLocalCounters &cnt) {
+template <bool PARTIAL>
+GD_HD bool gd_lane_post_t(GdLane &L, const GdMaterials &M, const float *tab, const GdSource &S, unsigned long long seed,
+                          const GdHit &hit_in, GdHistory &out, GdLocalCounters &cnt) {
     GdHit hit = hit_in;
     bool photon_done = false;
     if (L.mode == GD_MODE_LOCATE) {                                                         // O5
         L.m = hit.leaf < 0 ? M.world_material : (hit.leaving ? gd_mat_inside(hit.mats) : gd_mat_outside(hit.mats));
         if (L.flags & GD_F_RELOC) L.flags &= ~GD_F_RELOC;                                   // re-localisation: tau carries on
+        else if (PARTIAL) gd_partial_birth(L);
         else L.tau = -logf(gd_rng_next(L.g));                                               // O7.1
         L.mode = GD_MODE_FLIGHT;
         // The first flight runs along the same ray as the localisation query, and the nearest facet ahead is by
         // construction the first one whose from-side is the start material: one traversal answers both (O5 + O7.3).
         L.mu_tot = gd_mu_lookup(M, tab, L.m, L.e, L.mu); L.need_mu = 0;                     // O2
-        L.sdist = L.mu_tot > 0.0f ? L.tau / L.mu_tot : GD_INF;                              // O7.2
+        if (PARTIAL) gd_partial_step(L);
+        else L.sdist = L.mu_tot > 0.0f ? L.tau / L.mu_tot : GD_INF;                         // O7.2
         if (hit.leaf >= 0 && !(hit.t <= L.sdist)) hit.leaf = -1;
     }
     if (hit.leaf >= 0) {                                                                    // O7.6 boundary first
         float t = fmaxf(hit.t, 0.0f);
         L.pos.x += t * L.dir.x; L.pos.y += t * L.dir.y; L.pos.z += t * L.dir.z;
-        L.tau -= L.mu_tot * t;
+        if (PARTIAL) gd_partial_advance(L, t);
+        else L.tau -= L.mu_tot * t;
         L.m = hit.leaving ? gd_mat_outside(hit.mats) : gd_mat_inside(hit.mats);
         cnt.n_crossings++;
         L.need_mu = 1;
@@ -249,14 +285,20 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
         L.ex = gd_no_exclude(); L.n_stall = 0;                            // new flight segment
         if (L.e < M.e_cut) { gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_cutoff++; photon_done = true; }
         else {
-            const GdF4u u4 = gd_rng_peek4(L.g);       // selection draw + the three draws of a coherent event
+            GdF4u u4 = gd_rng_peek4(L.g);             // selection draw + the three draws of a coherent event
             bool tau_done = false;
-            float us = u4.a * L.mu_tot; L.g.draw += 1;
             int ch = -1;
-            float acc = 0.0f;
+            if (PARTIAL) {                            // the process whose budget ran out fires; the others pay for the flight
+                ch = L.sel;
+                gd_partial_advance(L, L.sdist);
+                u4.d = u4.c; u4.c = u4.b; u4.b = u4.a;    // no selection draw: the event's own draws start at once
+            } else {
+                float us = u4.a * L.mu_tot; L.g.draw += 1;
+                float acc = 0.0f;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) { acc += L.mu[c]; if (ch < 0 && us < acc) ch = c; }
-            if (ch < 0) ch = L.mu[3] > 0.0f ? 3 : (L.mu[2] > 0.0f ? 2 : (L.mu[1] > 0.0f ? 1 : 0));
+                for (int c = 0; c < 4; ++c) { acc += L.mu[c]; if (ch < 0 && us < acc) ch = c; }
+                if (ch < 0) ch = L.mu[3] > 0.0f ? 3 : (L.mu[2] > 0.0f ? 2 : (L.mu[1] > 0.0f ? 1 : 0));
+            }
             if (ch == 0) {                                                                  // O9 photoelectric
                 gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_pe++;
                 photon_done = true;
@@ -274,7 +316,8 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
             } else if (ch == 2) {                                                           // O11 coherent
                 const float cost = gd_thomson_from(u4.b);
                 L.dir = gd_rotate(L.dir, cost, u4.c);
-                L.tau = -logf(u4.d); tau_done = true;                                        // O7.1
+                if (PARTIAL) L.tau_c[2] = -logf(u4.d); else L.tau = -logf(u4.d);             // O7.1
+                tau_done = true;
                 L.g.draw += 3;
                 cnt.n_coherent++;
             } else {                                                                        // O12 pair
@@ -284,11 +327,13 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
                 cnt.n_pair++;
                 photon_done = true;
             }
-            if (!photon_done && !tau_done) L.tau = -logf(gd_rng_next(L.g));                 // O7.1
+            if (!photon_done && !tau_done) {                                                // O7.1
+                if (PARTIAL) L.tau_c[ch] = -logf(gd_rng_next(L.g)); else L.tau = -logf(gd_rng_next(L.g));
+            }
         }
     }
     if (!photon_done) return false;
-    if (!gd_lane_next_photon(L, seed)) return false;
+    if (!gd_lane_next_photon_t<PARTIAL>(L, seed)) return false;
     // ---- O14
     if (!(L.flags & (GD_F_ESCAPED | GD_F_NONSCORING))) { L.flags |= GD_F_PEAK; L.dep = S.line_mev[L.line]; }
     L.flags &= ~GD_F_RELOC;
@@ -297,6 +342,10 @@ GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const
     out.edep = L.dep; out.flags = L.flags; out.line = L.line;
     L.mode = GD_MODE_NEED;
     return true;
+}
+GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const GdSource &S, unsigned long long seed,
+                        const GdHit &hit, GdHistory &out, GdLocalCounters &cnt) {
+    return gd_lane_post_t<false>(L, M, tab, S, seed, hit, out, cnt);
 }
 
 // ---------------------------------------------------------------- parity localisation inside the transport loop
@@ -378,7 +427,7 @@ GD_HD int gd_locate_parity(const GdBvh &bvh, const GdRay &ray, const GdExclude &
 // PARITY: after the start localisation and after every boundary crossing the material comes from the parity rule
 // instead of the facet's side ids (the side ids still say where the KILL boundary is); mismatches between the two
 // rules are counted in cnt.n_cutoff's neighbour fields by the caller.
-template <bool PARITY>
+template <bool PARITY, bool PARTIAL>
 GD_HD void gd_run_history_t(const GdBvh &bvh, const GdMaterials &M, const float *tab, const GdSource &S,
                             unsigned long long seed, unsigned long long history, GdHistory &out, GdLocalCounters &cnt,
                             unsigned &n_parity, unsigned &n_mismatch) {
@@ -389,7 +438,7 @@ GD_HD void gd_run_history_t(const GdBvh &bvh, const GdMaterials &M, const float 
     for (;;) {
         float t_min, t_max;
         int filter;
-        gd_lane_query(L, M, tab, t_min, t_max, filter);
+        gd_lane_query_t<PARTIAL>(L, M, tab, t_min, t_max, filter);
         gd_ray_setup(ray, L.pos, L.dir);
         cnt.n_queries++;
         gd_nearest_hit<false>(bvh, ray, t_min, t_max, filter, L.ex, true, hit, cnt.n_box_tests, cnt.n_tri_tests);
@@ -408,7 +457,7 @@ GD_HD void gd_run_history_t(const GdBvh &bvh, const GdMaterials &M, const float 
                 }
             }
         }
-        if (gd_lane_post(L, M, tab, S, seed, hit, out, cnt)) return;
+        if (gd_lane_post_t<PARTIAL>(L, M, tab, S, seed, hit, out, cnt)) return;
         if (PARITY && cnt.n_crossings != crossings_before && L.mode == GD_MODE_FLIGHT) {
             gd_ray_setup(ray, L.pos, L.dir);
             const int m_par = gd_locate_parity(bvh, ray, L.ex, M.world_material, cnt.n_box_tests, cnt.n_tri_tests);
@@ -421,5 +470,5 @@ GD_HD void gd_run_history_t(const GdBvh &bvh, const GdMaterials &M, const float 
 GD_HD void gd_run_history(const GdBvh &bvh, const GdMaterials &M, const float *tab, const GdSource &S,
                           unsigned long long seed, unsigned long long history, GdHistory &out, GdLocalCounters &cnt) {
     unsigned a = 0, b = 0;
-    gd_run_history_t<false>(bvh, M, tab, S, seed, history, out, cnt, a, b);
+    gd_run_history_t<false, false>(bvh, M, tab, S, seed, history, out, cnt, a, b);
 }
