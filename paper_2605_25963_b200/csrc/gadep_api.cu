@@ -631,6 +631,7 @@ extern "C" int gadep_run_histories(gadep_ctx *c, unsigned long long first, long 
     if (flags_out && !dev_f && n > 0) { GD_CUDA(c, cudaMalloc(&stage_f, sizeof(unsigned) * (size_t)n)); d_f = stage_f; }
     int n_bins = c->n_bins > 0 ? c->n_bins : 4096;
     float e_max = c->spec_e_max > 0 ? c->spec_e_max : 2.0f;
+    c->kernel_variant = 2;       // always the default kernel, whatever the last gadep_run asked for
     int rc = gd_launch_transport(c, first, (unsigned long long)n, seed, n_bins, e_max, false, d_e, d_f);
     if (rc == GADEP_OK) rc = gd_fetch_results(c);
     if (rc == GADEP_OK && stage_e) cudaMemcpy(edep_out, stage_e, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost);
