@@ -140,6 +140,27 @@ def run_ray_bench(args, dm):
     print(json.dumps(line), flush=True)
 
 
+def run_calibration(args, dm):
+    """the paper's calibration use-case (Table 3, Fig. 11): one launch of 1e7
+    histories per detector gives the full-energy-peak efficiency at the 13 calibration energies."""
+    import torch
+    import paper_2605_25963_b200 as pkg
+    out = {"metric": "FEPE curves (13 energies per launch)", "energies_kev": list(dm.TABLE3_KEV), "detectors": []}
+    for k in range(len(dm.CALIBRATION_DETECTORS)):
+        w = dm.make_calibration(k, n_histories=int(args.histories) if args.histories else 10_000_000)
+        g = pkg.Gadep(0, torch.cuda.current_stream().cuda_stream)
+        g.load_workload(w)
+        g.run(200_000, w.seed, w.n_bins, w.spectrum_e_max_mev)
+        g.run(w.n_histories, w.seed, w.n_bins, w.spectrum_e_max_mev)
+        c = g.get_counters()
+        fe = [g.fepe(l) for l in range(13)]
+        out["detectors"].append({"name": w.name, "n_triangles": w.mesh.n_tri, "histories": w.n_histories,
+                                 "kernel_ms": c["last_run_ms"], "bvh_build_ms": c["last_build_ms"],
+                                 "histories_per_s": w.n_histories / (c["last_run_ms"] * 1e-3),
+                                 "fepe": [f for f, _ in fe], "fepe_std_err": [s_ for _, s_ in fe]})
+    print(json.dumps(out), flush=True)
+
+
 def run_locate_bench(args, dm):
     """cost of the paper's reworked localisation (parity counting over all facets hit, an
     all-hits BVH traversal) against its original side-id rule (nearest facet), on the config-1 detector at the
@@ -183,6 +204,7 @@ def main():
     ap.add_argument("--ref-sample", type=float, default=60000)
     ap.add_argument("--cpu-sample", type=float, default=0, help="oracle histories; 0 = sized for ~15 s from a pilot run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--calibration", action="store_true", help="FEPE curves: 13 Table-3 energies x 3 parametric detectors")
     ap.add_argument("--locate-bench", type=float, default=0, help="localisation benchmark: side-id vs parity rule (PAPER.md:191-193)")
     ap.add_argument("--ray-bench", type=float, default=0, help="config-4 ray benchmark: this many seeded rays through gadep_trace_rays")
     args = ap.parse_args()
@@ -211,6 +233,9 @@ def main():
         return
     if args.locate_bench:
         run_locate_bench(args, dm)
+        return
+    if args.calibration:
+        run_calibration(args, dm)
         return
     n_hist = int(args.histories) if args.histories else w.n_histories
     stream = torch.cuda.current_stream()

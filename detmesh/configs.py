@@ -193,3 +193,49 @@ def make_rays(n: int, seed: int, cyl_r: float, z0: float, z1: float):
     ps = 2 * np.pi * u[:, 4]
     d = np.stack([s * np.cos(ps), s * np.sin(ps), w], axis=1)
     return np.ascontiguousarray(org, dtype=np.float32), np.ascontiguousarray(d, dtype=np.float32)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Calibration sweep (Table 3, Fig. 11): 13 calibration energies from a point
+# source 250 mm above the endcap, one FEPE curve per detector.  The paper's six ORTEC detectors are not specified in
+# print (parameters d1-d10), so three synthetic coaxial p-type detectors span the same range of sizes.
+TABLE3_KEV = (59.54, 81.00, 121.78, 244.70, 344.28, 356.02, 411.13, 443.97, 778.90, 964.06, 1112.09, 1332.49, 1408.02)
+
+CALIBRATION_DETECTORS = (
+    # crystal radius / length / front rounding, bore radius / depth of its apex, outer dead layer, endcap gap
+    dict(name="cal_d60", R=30.0, L=60.0, r_ch=6.0, bore_r=4.5, bore_apex=-14.0, dead=0.5, gap=4.0),
+    dict(name="cal_d70", R=35.0, L=70.0, r_ch=8.0, bore_r=5.0, bore_apex=-15.0, dead=0.7, gap=5.0),
+    dict(name="cal_d85", R=42.5, L=80.0, r_ch=8.0, bore_r=5.5, bore_apex=-18.0, dead=1.0, gap=5.0),
+)
+
+
+def _param_detector_segment_lists(p, n_phi, side_bands):
+    """Coaxial p-type HPGe from a parameter set: same surface recipe as configs[1] (Eq. 1-6)."""
+    d = DELTA
+    G_A, G_D, AL, CU, AIR, VAC = (MAT["Ge_active"], MAT["Ge_dead"], MAT["Al"], MAT["Cu"], MAT["air"], MAT["vacuum"])
+    R, L, r, dl = p["R"], p["L"], p["r_ch"], p["dead"]
+    shell = 0.0003                                   # inner bore dead layer, 0.3 um
+    cup_in, cup_out = R + 0.1, R + 0.9               # 0.1 mm clearance, 0.8 mm Cu
+    cav_r = cup_out + 5.0                            # cup outer + 5 mm
+    cav_top, cav_bot = p["gap"], -(L + 0.9) - 30.0   # front gap; 30 mm rear vacuum
+    return [
+        ("S0_crystal_outer", _rounded_cyl_segments(R, 0.0, -L, r, n_phi, side_bands), G_D, VAC),
+        ("S1_active", _rounded_cyl_segments(R - dl, -dl, -L + d, r - dl, n_phi, side_bands), G_A, G_D),
+        ("S2_bore_shell", _bore_segments(p["bore_r"] + shell, p["bore_apex"] + shell, -L + 2 * d, n_phi, side_bands), G_D, G_A),
+        ("S3_bore", _bore_segments(p["bore_r"], p["bore_apex"], -L + 3 * d, n_phi, side_bands), VAC, G_D),
+        ("S4_cu_cup", _cup_segments(cup_in, cup_out, 0.0, -L - 0.1, -L - 0.9, side_bands), CU, VAC),
+        ("S5_endcap_outer", _cyl_segments(cav_r + 1.0, cav_top + 1.0, cav_bot - 1.0, side_bands), AL, AIR),
+        ("S6_endcap_cavity", _cyl_segments(cav_r, cav_top, cav_bot, side_bands), VAC, AL),
+        ("S7_world", _cyl_segments(300.0, 400.0, -300.0, side_bands), AIR, MAT_KILL),
+    ]
+
+
+def make_calibration(detector: int, n_histories: int = 10_000_000, n_theta: int = 256) -> Workload:
+    """Point source 250 mm above the endcap of CALIBRATION_DETECTORS[detector], the 13 energies of PAPER.md Table 3
+    at equal intensity, 1e7 histories (Fig. 11)."""
+    p = CALIBRATION_DETECTORS[detector]
+    mu, sc, _ = make_tables(coh_coeff=7.0e-27)
+    mesh = _build(_param_detector_segment_lists(p, 8, 4), n_theta, MAT["air"])
+    src = _source(SRC_POINT, pos=(0, 0, p["gap"] + 1.0 + 250.0), lines_kev=TABLE3_KEV)
+    return Workload(p["name"] + "_point250_13lines", mesh, mu, sc, E_MIN_MEV, E_MAX_MEV, src, n_histories, 1,
+                    notes={"detector": dict(p)})

@@ -136,6 +136,15 @@ int gadep_run(gadep_ctx *ctx, unsigned long long n_histories, unsigned long long
  */
 int gadep_fepe(const gadep_ctx *ctx, int line, int mode, double *fepe, double *std_err);
 
+/*
+ * Detector-resolution broadening of the spectrum of the last gadep_run (the paper's spectra are
+ * unbroadened, PAPER.md:253-259 reads the FEPE from exact peaks).  FWHM(E)^2 = fwhm_a + fwhm_b E + fwhm_c E^2 [MeV^2,
+ * E in MeV]; every bin's counts are spread as a Gaussian centred on the bin middle.  out: HOST-or-DEVICE
+ * double[n_bins + 1]; bin 0 also takes the mass below 0, the last slot the overflow counts and the mass above e_max,
+ * so the total is conserved.
+ */
+int gadep_broaden(gadep_ctx *ctx, double fwhm_a, double fwhm_b, double fwhm_c, double *out);
+
 /* ---- test / measurement hooks ------------------------------------------------------------------------------ */
 
 /*

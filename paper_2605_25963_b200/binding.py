@@ -21,7 +21,7 @@ RUN_PARTIAL_XS = 32
 
 EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_set_materials", "gadep_load_mesh",
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
-                    "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw", "gadep_locate")
+                    "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw", "gadep_locate", "gadep_broaden")
 
 
 class GadepError(RuntimeError):
@@ -101,6 +101,7 @@ def load_library(build_if_missing: bool = True):
     L.gadep_get_counters.argtypes = [vp, C.POINTER(GadepCounters)]
     L.gadep_philox_raw.argtypes = [vp, vp, vp, i32, vp]
     L.gadep_locate.argtypes = [vp, vp, vp, ll, i32, vp]
+    L.gadep_broaden.argtypes = [vp, dbl, dbl, dbl, vp]
     _lib = L
     return L
 
@@ -194,6 +195,7 @@ class Gadep:
     def run(self, n_histories, seed, n_bins=4096, e_max_mev=2.0, first_history=0, flags=0, spectrum=None):
         """spectrum: None -> a new host uint64 array is returned; numpy array or device tensor/pointer -> filled."""
         opts = GadepRunOpts(int(n_bins), float(e_max_mev), int(first_history), int(flags))
+        self._last_bins = int(n_bins)
         out = spectrum
         if out is None:
             out = np.zeros(n_bins + 1, dtype=np.uint64)
@@ -219,6 +221,13 @@ class Gadep:
         self._check(self.L.gadep_trace_rays(self.h, _ptr(org), _ptr(dir), n, int(filter_material), float(t_min),
                                             _ptr(tri_out), _ptr(t_out)))
         return tri_out, t_out
+
+    def broaden(self, fwhm_a, fwhm_b=0.0, fwhm_c=0.0, out=None):
+        """Spectrum of the last run with Gaussian resolution FWHM(E)^2 = a + b E + c E^2 (MeV); float64[n_bins+1]."""
+        if out is None:
+            out = np.empty(self._last_bins + 1, dtype=np.float64)
+        self._check(self.L.gadep_broaden(self.h, float(fwhm_a), float(fwhm_b), float(fwhm_c), _ptr(out)))
+        return out
 
     def locate(self, org, dir, mode=0, material_out=None):
         """Material containing each point (mode 0 side-id rule, 1 parity rule)."""

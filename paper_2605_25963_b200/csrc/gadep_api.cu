@@ -617,6 +617,49 @@ extern "C" int gadep_locate(gadep_ctx *c, const float *org, const float *dir, lo
     return GADEP_OK;
 }
 
+// ---------------------------------------------------------------- detector-resolution broadening
+// out[j] = sum_i S[i] * P(bin j | Gaussian centred on the middle of bin i, FWHM(E)^2 = a + b E + c E^2); bin 0 also takes
+// the mass below 0, the overflow slot the mass above e_max (and the unbroadened overflow counts): the total is kept.
+__global__ void gd_k_broaden(const unsigned long long *__restrict__ spec, int n_bins, double e_max, double a, double b,
+                             double c, double *__restrict__ out) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j > n_bins) return;
+    const double de = e_max / n_bins;
+    const double lo = j == 0 ? -1.0e300 : (j == n_bins ? e_max : j * de);
+    const double hi = j == n_bins ? 1.0e300 : (j + 1) * de;
+    double acc = j == n_bins ? (double)spec[n_bins] : 0.0;
+    for (int i = 0; i < n_bins; ++i) {
+        const unsigned long long s = spec[i];
+        if (!s) continue;
+        const double e = (i + 0.5) * de;
+        const double fwhm2 = a + b * e + c * e * e;
+        if (!(fwhm2 > 0.0)) { if (i == j) acc += (double)s; continue; }
+        const double inv = 2.3548200450309493 / sqrt(2.0 * fwhm2);          // 1 / (sigma sqrt 2)
+        acc += (double)s * 0.5 * (erf((hi - e) * inv) - erf((lo - e) * inv));
+    }
+    out[j] = acc;
+}
+
+extern "C" int gadep_broaden(gadep_ctx *c, double fwhm_a, double fwhm_b, double fwhm_c, double *out) {
+    if (!c) return GADEP_E_NULL;
+    if (!out) return gd_fail(c, GADEP_E_NULL, "null output");
+    if (!c->have_results || !c->d_tally || c->n_bins <= 0) return gd_fail(c, GADEP_E_ORDER, "gadep_broaden before gadep_run");
+    if (!(fwhm_a >= 0) || !std::isfinite(fwhm_b) || !std::isfinite(fwhm_c)) return gd_fail(c, GADEP_E_ARG, "bad resolution parameters");
+    GD_CUDA(c, cudaSetDevice(c->device));
+    const bool dev = gd_is_device_ptr(out);
+    const size_t bytes = sizeof(double) * ((size_t)c->n_bins + 1);
+    double *d_out = out;
+    if (!dev) GD_CUDA(c, cudaMalloc(&d_out, bytes));
+    gd_k_broaden<<<(c->n_bins + 1 + 127) / 128, 128, 0, c->stream>>>(c->d_tally, c->n_bins, (double)c->spec_e_max, fwhm_a, fwhm_b,
+                                                                    fwhm_c, d_out);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && !dev) e = cudaMemcpyAsync(out, d_out, bytes, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (!dev) cudaFree(d_out);
+    if (e != cudaSuccess) return gd_fail(c, GADEP_E_CUDA, "broaden failed: %s", cudaGetErrorString(e));
+    return GADEP_OK;
+}
+
 extern "C" int gadep_run_histories(gadep_ctx *c, unsigned long long first, long long n, unsigned long long seed,
                                    float *edep_out, unsigned *flags_out) {
     if (!c) return GADEP_E_NULL;
