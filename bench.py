@@ -291,18 +291,21 @@ def main():
               + m.surf_inside.nbytes + m.surf_outside.nbytes + w.source["line_mev"].nbytes * 2)
     d2h = int(8 * n_tally)
     g2 = pkg.Gadep(local_rank, stream.cuda_stream)
-    e2e_steps = max(1, min(args.steps, 2))
+    e2e_steps = max(1, min(args.steps, 3))
     g2.load_workload(w); g2.run(min(n_hist, 100000), w.seed)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    t0 = time.perf_counter()
+    e2e_times = []
     for k in range(e2e_steps):
+        t0 = time.perf_counter()
         g2.load_workload(w)                                      # host arrays -> device, validation, BVH build
         h_spec = g2.run(n_hist, w.seed, w.n_bins, w.spectrum_e_max_mev, first_history=first)   # host spectrum out
         fepe = [g2.fepe(l)[0] for l in range(len(w.source["line_mev"]))]
-    torch.cuda.synchronize()
-    e2e_t = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize()
+        e2e_times.append(time.perf_counter() - t0)
+    # wall clock on a shared host: the median step, times the number of steps, guards against a single hiccup
+    e2e_t = torch.tensor([float(np.median(e2e_times)) * e2e_steps], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
     e2e_value = world * n_hist * e2e_steps / float(e2e_t.item())

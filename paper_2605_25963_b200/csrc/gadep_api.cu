@@ -39,6 +39,11 @@ struct gadep_ctx {
     GdTri *d_leaf_tris = nullptr;
     int bvh_depth = 0;
     int n_ref = 0;                 // leaves of the BVH: facet references after splitting
+    // build buffers are kept between builds (no cudaMalloc / cudaFree, and none of their implicit synchronisations,
+    // inside a step that rebuilds the BVH every time): [0] counts [1] scene [2] scratch arena [3] nodes [4] leaf
+    // triangles [5] 4-wide nodes
+    void *pool[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    size_t pool_cap[6] = {0, 0, 0, 0, 0, 0};
     // source
     bool have_src = false;
     GdSource src;
@@ -129,9 +134,21 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     return GADEP_OK;
 }
 
+static cudaError_t gd_pool_get(gadep_ctx *c, int k, size_t bytes, void **out) {
+    if (c->pool_cap[k] < bytes) {
+        cudaFree(c->pool[k]); c->pool[k] = nullptr; c->pool_cap[k] = 0;
+        const size_t want = bytes + bytes / 8 + 256;
+        cudaError_t e = cudaMalloc(&c->pool[k], want);
+        if (e != cudaSuccess) { *out = nullptr; return e; }
+        c->pool_cap[k] = want;
+    }
+    *out = c->pool[k];
+    return cudaSuccess;
+}
+
 static void gd_free_mesh(gadep_ctx *c) {
     cudaFree(c->d_verts); cudaFree(c->d_tris); cudaFree(c->d_tri_mats); cudaFree(c->d_tri_surf);
-    cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris); cudaFree(c->d_nodes4); c->d_nodes4 = nullptr;
+    c->d_nodes4 = nullptr;
     c->d_verts = nullptr; c->d_tris = c->d_tri_mats = c->d_tri_surf = nullptr;
     c->d_nodes = nullptr; c->d_leaf_tris = nullptr;
     c->have_mesh = c->have_bvh = false;
@@ -142,6 +159,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
+    for (int k = 0; k < 6; ++k) cudaFree(c->pool[k]);
     cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -247,15 +265,14 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     GD_CUDA(c, cudaSetDevice(c->device));
     const int n_tri = c->n_tri;
     cudaStream_t st = c->stream;
-    cudaFree(c->d_nodes); cudaFree(c->d_leaf_tris); cudaFree(c->d_nodes4);
     c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->d_nodes4 = nullptr; c->have_bvh = false;
     const int tb = 256, nbt = (n_tri + tb - 1) / tb;
     int launches = 0;
     // ---- phase A: how many references (reference splitting) -> one 4-byte read-back sizes the arena
     unsigned *counts = nullptr;
     int *scene = nullptr;
-    GD_CUDA(c, cudaMalloc(&counts, 4 * (size_t)n_tri));
-    if (cudaMalloc(&scene, 4 * 16) != cudaSuccess) { cudaFree(counts); return gd_fail(c, GADEP_E_CUDA, "cudaMalloc failed"); }
+    GD_CUDA(c, gd_pool_get(c, 0, 4 * (size_t)n_tri, (void **)&counts));
+    GD_CUDA(c, gd_pool_get(c, 1, 4 * 16, (void **)&scene));
     cudaEventRecord(c->evb0, st);
     gd_k_init_scene<<<1, 32, 0, st>>>(scene);
     gd_k_split_prio<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts, (unsigned long long *)(scene + 10));
@@ -267,7 +284,6 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     cudaError_t e = cudaMemcpyAsync(&n_ref_u, scene + 8, 4, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess || n_ref_u < (unsigned)n_tri || n_ref_u > (unsigned)n_tri * GD_MAX_SPLITS) {
-        cudaFree(counts); cudaFree(scene);
         return gd_fail(c, GADEP_E_CUDA, "BVH build (reference count) failed: %s", cudaGetErrorString(e));
     }
     const int n = (int)n_ref_u;
@@ -284,13 +300,13 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     size_t o_cl = take(4 * (size_t)n), o_cr = take(4 * (size_t)n), o_pi = take(4 * (size_t)n), o_pl = take(4 * (size_t)n);
     size_t o_vis = take(4 * (size_t)n), o_rt = take(4 * (size_t)n);
     unsigned char *arena = nullptr;
-    if (cudaMalloc(&arena, off) != cudaSuccess) { cudaFree(counts); cudaFree(scene); return gd_fail(c, GADEP_E_NOMEM, "BVH scratch (%zu B)", off); }
+    if (gd_pool_get(c, 2, off, (void **)&arena) != cudaSuccess) return gd_fail(c, GADEP_E_NOMEM, "BVH scratch (%zu B)", off);
     int rc = GADEP_OK;
     int depth = 0;
     do {
-        if ((e = cudaMalloc(&c->d_nodes, sizeof(GdNode) * (size_t)std::max(n - 1, 1))) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_leaf_tris, sizeof(GdTri) * (size_t)n)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_nodes4, sizeof(GdNode4) * (size_t)std::max(n - 1, 1))) != cudaSuccess) break;
+        if ((e = gd_pool_get(c, 3, sizeof(GdNode) * (size_t)std::max(n - 1, 1), (void **)&c->d_nodes)) != cudaSuccess) break;
+        if ((e = gd_pool_get(c, 4, sizeof(GdTri) * (size_t)n, (void **)&c->d_leaf_tris)) != cudaSuccess) break;
+        if ((e = gd_pool_get(c, 5, sizeof(GdNode4) * (size_t)std::max(n - 1, 1), (void **)&c->d_nodes4)) != cudaSuccess) break;
         float4 *ref_lo = (float4 *)(arena + o_tlo), *ref_hi = (float4 *)(arena + o_thi);
         float4 *node_lo = (float4 *)(arena + o_nlo), *node_hi = (float4 *)(arena + o_nhi);
         unsigned long long *keys[2] = {(unsigned long long *)(arena + o_k0), (unsigned long long *)(arena + o_k1)};
@@ -329,7 +345,6 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         if (n > 1 && (e = cudaMemcpy(&depth, scene + 6, sizeof(int), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
         cudaEventElapsedTime(&c->last_build_ms, c->evb0, c->evb1);
     } while (0);
-    cudaFree(arena); cudaFree(counts); cudaFree(scene);
     if (e != cudaSuccess) rc = gd_fail(c, GADEP_E_CUDA, "BVH build failed: %s", cudaGetErrorString(e));
     else if (depth >= GD_STACK || 3 * depth + 4 > GD_STACK4) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
     if (rc != GADEP_OK) return rc;
