@@ -42,8 +42,9 @@ struct gadep_ctx {
     // build buffers are kept between builds (no cudaMalloc / cudaFree, and none of their implicit synchronisations,
     // inside a step that rebuilds the BVH every time): [0] counts [1] scene [2] scratch arena [3] nodes [4] leaf
     // triangles [5] 4-wide nodes
-    void *pool[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    size_t pool_cap[6] = {0, 0, 0, 0, 0, 0};
+    // [6..9] the mesh copies (vertices, triangles, side materials, surface ids)
+    void *pool[10] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    size_t pool_cap[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     // source
     bool have_src = false;
     GdSource src;
@@ -147,7 +148,6 @@ static cudaError_t gd_pool_get(gadep_ctx *c, int k, size_t bytes, void **out) {
 }
 
 static void gd_free_mesh(gadep_ctx *c) {
-    cudaFree(c->d_verts); cudaFree(c->d_tris); cudaFree(c->d_tri_mats); cudaFree(c->d_tri_surf);
     c->d_nodes4 = nullptr;
     c->d_verts = nullptr; c->d_tris = c->d_tri_mats = c->d_tri_surf = nullptr;
     c->d_nodes = nullptr; c->d_leaf_tris = nullptr;
@@ -159,7 +159,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    for (int k = 0; k < 6; ++k) cudaFree(c->pool[k]);
+    for (int k = 0; k < 10; ++k) cudaFree(c->pool[k]);
     cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -213,7 +213,16 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
     for (size_t i = 0; i < (size_t)n_vert * 3; ++i)
         if (!std::isfinite(vertices[i])) return gd_fail(c, GADEP_E_NONFINITE, "vertex %zu is not finite", i / 3);
     std::vector<int> mats(n_tri);
-    std::vector<std::vector<unsigned long long>> edges(n_surf);
+    // closed + consistently oriented (PAPER.md:193 needs closed geometry): every directed edge of a surface occurs once
+    // and its reverse once, in the same surface.  One open-addressing table over all directed edges (O(n)).
+    size_t cap = 16;
+    int cap_log2 = 4;
+    while (cap < (size_t)n_tri * 6) { cap <<= 1; cap_log2++; }
+    const unsigned long long EMPTY = ~0ull;
+    std::vector<unsigned long long> ekey(cap, EMPTY);
+    std::vector<int> esurf(cap, -1);
+    const int shift = 64 - cap_log2;
+    auto slot_of = [&](unsigned long long k) { return (size_t)((k * 0x9E3779B97F4A7C15ull) >> shift); };
     for (int t = 0; t < n_tri; ++t) {
         int s = tri_surface[t];
         if (s < 0 || s >= n_surf) return gd_fail(c, GADEP_E_INDEX, "triangle %d: surface %d out of range", t, s);
@@ -227,26 +236,31 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
         if (v[0] == v[1] || v[1] == v[2] || v[0] == v[2] || nx * nx + ny * ny + nz * nz == 0.0)
             return gd_fail(c, GADEP_E_DEGENERATE, "triangle %d has zero area", t);
         mats[t] = (surf_inside[s] & 0xFFFF) | (int)((unsigned)(surf_outside[s] & 0xFFFF) << 16);
-        for (int k = 0; k < 3; ++k)
-            edges[s].push_back(((unsigned long long)(unsigned)v[k] << 32) | (unsigned)v[(k + 1) % 3]);
-    }
-    // closed + consistently oriented: every directed edge once, its reverse once (PAPER.md:193 needs closed geometry)
-    for (int s = 0; s < n_surf; ++s) {
-        std::vector<unsigned long long> &e = edges[s];
-        std::sort(e.begin(), e.end());
-        for (size_t i = 1; i < e.size(); ++i)
-            if (e[i] == e[i - 1]) return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %d: directed edge used twice (non-manifold or inconsistent winding)", s);
-        for (size_t i = 0; i < e.size(); ++i) {
-            unsigned long long rev = (e[i] << 32) | (e[i] >> 32);
-            if (!std::binary_search(e.begin(), e.end(), rev)) return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %d is not closed (open edge)", s);
+        for (int k = 0; k < 3; ++k) {
+            const unsigned long long key = ((unsigned long long)(unsigned)v[k] << 32) | (unsigned)v[(k + 1) % 3];
+            size_t i = slot_of(key);
+            while (ekey[i] != EMPTY) {
+                if (ekey[i] == key)
+                    return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %d: directed edge used twice (non-manifold or inconsistent winding)", s);
+                i = (i + 1) & (cap - 1);
+            }
+            ekey[i] = key; esurf[i] = s;
         }
+    }
+    for (size_t i = 0; i < cap; ++i) {
+        if (ekey[i] == EMPTY) continue;
+        const unsigned long long rev = (ekey[i] << 32) | (ekey[i] >> 32);
+        size_t j = slot_of(rev);
+        while (ekey[j] != EMPTY && ekey[j] != rev) j = (j + 1) & (cap - 1);
+        if (ekey[j] == EMPTY || esurf[j] != esurf[i])
+            return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %d is not closed (open edge)", esurf[i]);
     }
     GD_CUDA(c, cudaSetDevice(c->device));
     gd_free_mesh(c);
-    GD_CUDA(c, cudaMalloc(&c->d_verts, sizeof(float) * 3 * (size_t)n_vert));
-    GD_CUDA(c, cudaMalloc(&c->d_tris, sizeof(int) * 3 * (size_t)n_tri));
-    GD_CUDA(c, cudaMalloc(&c->d_tri_mats, sizeof(int) * (size_t)n_tri));
-    GD_CUDA(c, cudaMalloc(&c->d_tri_surf, sizeof(int) * (size_t)n_tri));
+    GD_CUDA(c, gd_pool_get(c, 6, sizeof(float) * 3 * (size_t)n_vert, (void **)&c->d_verts));
+    GD_CUDA(c, gd_pool_get(c, 7, sizeof(int) * 3 * (size_t)n_tri, (void **)&c->d_tris));
+    GD_CUDA(c, gd_pool_get(c, 8, sizeof(int) * (size_t)n_tri, (void **)&c->d_tri_mats));
+    GD_CUDA(c, gd_pool_get(c, 9, sizeof(int) * (size_t)n_tri, (void **)&c->d_tri_surf));
     GD_CUDA(c, cudaMemcpyAsync(c->d_verts, vertices, sizeof(float) * 3 * (size_t)n_vert, cudaMemcpyHostToDevice, c->stream));
     GD_CUDA(c, cudaMemcpyAsync(c->d_tris, triangles, sizeof(int) * 3 * (size_t)n_tri, cudaMemcpyHostToDevice, c->stream));
     GD_CUDA(c, cudaMemcpyAsync(c->d_tri_mats, mats.data(), sizeof(int) * (size_t)n_tri, cudaMemcpyHostToDevice, c->stream));
