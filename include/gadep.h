@@ -114,6 +114,7 @@ int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
 #define GADEP_RUN_PARTIAL_XS 32     /* the paper's "partial cross-section method": one remaining    */
                                    /* optical depth per process instead of total-mu sampling + a selection draw  */
                                    /* (history-per-thread kernel; same distribution, different random streams)   */
+#define GADEP_RUN_WARP_SPECIALISED 64 /* measurement: physics and traversal on separate warps of a block (same results) */
 typedef struct {
     int n_bins;                    /* spectrum bins over [0, e_max_mev); one extra overflow slot follows        */
     float e_max_mev;

@@ -17,6 +17,7 @@
 #include "gadep_transport_kernels.cuh"
 #include "gadep_wave_kernels.cuh"
 #include "gadep_locate_kernels.cuh"
+#include "gadep_ws_kernels.cuh"
 
 struct gadep_ctx {
     int device = 0;
@@ -452,10 +453,11 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0xFFFFFFFFull) return gd_fail(c, GADEP_E_ARG, "more than 2^32-1 histories in one launch");
     size_t smem = sizeof(float) * (size_t)c->n_mat * 4 * c->n_grid + sizeof(unsigned) * ((size_t)n_bins + 1);
     const int variant = c->kernel_variant;
-    const int threads = variant == 2 ? GD_W_THREADS : GD_RUN_THREADS;
+    const int threads = variant == 2 ? GD_W_THREADS : (variant == 5 ? GD_WS_THREADS : GD_RUN_THREADS);
     if (variant == 2) smem += sizeof(float) * (size_t)GD_W_WARPS * GD_W_NF * GD_W_SLOTS;
+    if (variant == 5) smem += sizeof(float) * (size_t)GD_WS_TEAMS * GD_WS_NF * GD_WS_SLOTS;
     if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
-    const void *kern = variant == 2 ? (const void *)gd_k_transport_wave
+    const void *kern = variant == 5 ? (const void *)gd_k_transport_ws : variant == 2 ? (const void *)gd_k_transport_wave
                                     : (variant == 1 ? (const void *)gd_k_transport_refill
                                                   : (variant == 3 ? (const void *)gd_k_transport<true, false>
                                                      : (variant == 4 ? (const void *)gd_k_transport<false, true> : (const void *)gd_k_transport<false, false>)));
@@ -463,11 +465,12 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     int per_sm = 1;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return gd_fail(c, GADEP_E_CUDA, "transport kernel does not fit on an SM (%zu B shared memory)", smem);
-    const unsigned long long per_block = variant == 2 ? (unsigned long long)GD_W_WARPS * GD_W_SLOTS : GD_RUN_THREADS;
+    const unsigned long long per_block = variant == 2 ? (unsigned long long)GD_W_WARPS * GD_W_SLOTS
+                                         : (variant == 5 ? (unsigned long long)GD_WS_TEAMS * GD_WS_SLOTS : GD_RUN_THREADS);
     unsigned long long want = (n + per_block - 1) / per_block;
     int grid = (int)std::min<unsigned long long>((unsigned long long)c->n_sm * per_sm, std::max<unsigned long long>(want, 1));
-    if (variant == 2) {
-        size_t need = (size_t)grid * GD_W_WARPS * GD_W_SLOTS * 8;
+    if (variant == 2 || variant == 5) {
+        size_t need = variant == 2 ? (size_t)grid * GD_W_WARPS * GD_W_SLOTS * 8 : (size_t)grid * GD_WS_TEAMS * GD_WS_SLOTS * 8;
         if (need > c->pair_floats) {
             cudaFree(c->d_pair); c->d_pair = nullptr; c->pair_floats = 0;
             GD_CUDA(c, cudaMalloc(&c->d_pair, need * sizeof(float)));
@@ -479,8 +482,12 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0) {
         unsigned long long warps = (unsigned long long)grid * (threads / 32);
         unsigned chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / (warps * 16)));
-        if (variant == 1 || variant == 2) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
-        if (variant == 2) {
+        if (variant == 1 || variant == 2 || variant == 5) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
+        if (variant == 5) {
+            unsigned ws_chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / ((unsigned long long)grid * GD_WS_TEAMS * 16)));
+            gd_k_transport_ws<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
+                                                           c->d_next, ws_chunk, c->d_pair, c->tune);
+        } else if (variant == 2) {
             gd_k_transport_wave<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
                                                              c->d_next, chunk, c->d_pair, c->tune);
         } else if (variant == 1) {
@@ -525,7 +532,7 @@ extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned 
     bool dev_out = gd_is_device_ptr(spectrum);
     if ((opts->flags & GADEP_RUN_ASYNC) && spectrum && !dev_out)
         return gd_fail(c, GADEP_E_ARG, "GADEP_RUN_ASYNC needs a device spectrum pointer");
-    c->kernel_variant = (opts->flags & GADEP_RUN_PARTIAL_XS) ? 4 : (opts->flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((opts->flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
+    c->kernel_variant = (opts->flags & GADEP_RUN_WARP_SPECIALISED) ? 5 : (opts->flags & GADEP_RUN_PARTIAL_XS) ? 4 : (opts->flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((opts->flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
     int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
                                  (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
     if (rc) return rc;

@@ -421,7 +421,7 @@ def test_all_kernel_variants_give_identical_tallies(pkg, orc):
     # warp-resident wavefront (default) vs persistent lanes vs plain history-per-thread: same streams, integer
     # tallies -> bit-identical spectra and event counts.  The wavefront kernel uses an FMA slab test with its own
     # conservative padding, so only its box / triangle test counts may differ.
-    from paper_2605_25963_b200.binding import RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES
+    from paper_2605_25963_b200.binding import RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES, RUN_WARP_SPECIALISED
     for cfg, n in ((1, 400_000), (3, 20_000)):
         w, g, s = _setup(pkg, orc, cfg)
         a = g.run(n, 5, w.n_bins, w.spectrum_e_max_mev).copy()
@@ -430,6 +430,12 @@ def test_all_kernel_variants_give_identical_tallies(pkg, orc):
         cb = g.get_counters()
         c = g.run(n, 5, w.n_bins, w.spectrum_e_max_mev, flags=RUN_PERSISTENT_LANES).copy()
         cc = g.get_counters()
+        d = g.run(n, 5, w.n_bins, w.spectrum_e_max_mev, flags=RUN_WARP_SPECIALISED).copy()      # physics / traversal warps
+        cd = g.get_counters()
+        assert np.array_equal(a, d)
+        for k in ("n_histories", "n_queries", "n_box_tests", "n_tri_tests", "n_crossings", "n_pe", "n_compton", "n_coherent",
+                  "n_pair", "n_escaped", "n_leak", "n_cutoff", "emitted", "peak"):
+            assert ca[k] == cd[k], k
         assert np.array_equal(a, b) and np.array_equal(a, c)
         for k in ("n_histories", "n_crossings", "n_pe", "n_compton", "n_coherent",
                   "n_pair", "n_escaped", "n_leak", "n_cutoff", "emitted", "peak"):
