@@ -79,7 +79,8 @@ int gadep_set_materials(gadep_ctx *ctx, int n_mat, int n_grid, double e_min_mev,
  *   surf_inside / surf_outside   HOST int[n_surf] material id on the inner / outer side, or GADEP_MAT_KILL
  *   world_material  material where no facet lies ahead
  * Checks: finite vertices, index ranges, zero-area facets, and per surface that every directed edge is matched by
- * exactly one opposite edge (closed + oriented; the side-id rule of PAPER.md:191 is only valid then).
+ * exactly one opposite edge (closed + oriented; the side-id rule of PAPER.md:191 is only valid then).  The arrays are
+ * copied to the device first and checked there; a rejected mesh leaves the context without a mesh.
  * Invalidates a previously built BVH.
  */
 int gadep_load_mesh(gadep_ctx *ctx, const float *vertices, int n_vert, const int *triangles, const int *tri_surface,

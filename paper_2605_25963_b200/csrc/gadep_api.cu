@@ -44,8 +44,9 @@ struct gadep_ctx {
     // inside a step that rebuilds the BVH every time): [0] counts [1] scene [2] scratch arena [3] nodes [4] leaf
     // triangles [5] 4-wide nodes
     // [6..9] the mesh copies (vertices, triangles, side materials, surface ids)
-    void *pool[10] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    size_t pool_cap[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    // [10..12] mesh validation: edge table keys, edge table surfaces, error record + surface sides
+    void *pool[13] = {};
+    size_t pool_cap[13] = {};
     // source
     bool have_src = false;
     GdSource src;
@@ -160,7 +161,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    for (int k = 0; k < 10; ++k) cudaFree(c->pool[k]);
+    for (int k = 0; k < 13; ++k) cudaFree(c->pool[k]);
     cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -211,62 +212,55 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
         if (surf_inside[s] < GADEP_MAT_KILL || surf_inside[s] >= mat_hi || surf_outside[s] < GADEP_MAT_KILL || surf_outside[s] >= mat_hi)
             return gd_fail(c, GADEP_E_INDEX, "surface %d: material id out of range", s);
     }
-    for (size_t i = 0; i < (size_t)n_vert * 3; ++i)
-        if (!std::isfinite(vertices[i])) return gd_fail(c, GADEP_E_NONFINITE, "vertex %zu is not finite", i / 3);
-    std::vector<int> mats(n_tri);
-    // closed + consistently oriented (PAPER.md:193 needs closed geometry): every directed edge of a surface occurs once
-    // and its reverse once, in the same surface.  One open-addressing table over all directed edges (O(n)).
+    // copies first, then the checks on the device (gadep_build_kernels.cuh): O(n) hash-table pass over the directed
+    // edges at device rate instead of host rate; one 32-byte read-back carries the verdict
     size_t cap = 16;
     int cap_log2 = 4;
     while (cap < (size_t)n_tri * 6) { cap <<= 1; cap_log2++; }
-    const unsigned long long EMPTY = ~0ull;
-    std::vector<unsigned long long> ekey(cap, EMPTY);
-    std::vector<int> esurf(cap, -1);
-    const int shift = 64 - cap_log2;
-    auto slot_of = [&](unsigned long long k) { return (size_t)((k * 0x9E3779B97F4A7C15ull) >> shift); };
-    for (int t = 0; t < n_tri; ++t) {
-        int s = tri_surface[t];
-        if (s < 0 || s >= n_surf) return gd_fail(c, GADEP_E_INDEX, "triangle %d: surface %d out of range", t, s);
-        int v[3] = {triangles[3 * t], triangles[3 * t + 1], triangles[3 * t + 2]};
-        for (int k = 0; k < 3; ++k)
-            if (v[k] < 0 || v[k] >= n_vert) return gd_fail(c, GADEP_E_INDEX, "triangle %d: vertex %d out of range", t, v[k]);
-        const float *a = vertices + 3 * (size_t)v[0], *b = vertices + 3 * (size_t)v[1], *q = vertices + 3 * (size_t)v[2];
-        double e1[3] = {(double)b[0] - a[0], (double)b[1] - a[1], (double)b[2] - a[2]};
-        double e2[3] = {(double)q[0] - a[0], (double)q[1] - a[1], (double)q[2] - a[2]};
-        double nx = e1[1] * e2[2] - e1[2] * e2[1], ny = e1[2] * e2[0] - e1[0] * e2[2], nz = e1[0] * e2[1] - e1[1] * e2[0];
-        if (v[0] == v[1] || v[1] == v[2] || v[0] == v[2] || nx * nx + ny * ny + nz * nz == 0.0)
-            return gd_fail(c, GADEP_E_DEGENERATE, "triangle %d has zero area", t);
-        mats[t] = (surf_inside[s] & 0xFFFF) | (int)((unsigned)(surf_outside[s] & 0xFFFF) << 16);
-        for (int k = 0; k < 3; ++k) {
-            const unsigned long long key = ((unsigned long long)(unsigned)v[k] << 32) | (unsigned)v[(k + 1) % 3];
-            size_t i = slot_of(key);
-            while (ekey[i] != EMPTY) {
-                if (ekey[i] == key)
-                    return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %d: directed edge used twice (non-manifold or inconsistent winding)", s);
-                i = (i + 1) & (cap - 1);
-            }
-            ekey[i] = key; esurf[i] = s;
-        }
-    }
-    for (size_t i = 0; i < cap; ++i) {
-        if (ekey[i] == EMPTY) continue;
-        const unsigned long long rev = (ekey[i] << 32) | (ekey[i] >> 32);
-        size_t j = slot_of(rev);
-        while (ekey[j] != EMPTY && ekey[j] != rev) j = (j + 1) & (cap - 1);
-        if (ekey[j] == EMPTY || esurf[j] != esurf[i])
-            return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %d is not closed (open edge)", esurf[i]);
-    }
     GD_CUDA(c, cudaSetDevice(c->device));
     gd_free_mesh(c);
+    cudaStream_t st = c->stream;
+    unsigned long long *ekey = nullptr;
+    int *esurf = nullptr, *sides = nullptr;
+    unsigned *err = nullptr;
     GD_CUDA(c, gd_pool_get(c, 6, sizeof(float) * 3 * (size_t)n_vert, (void **)&c->d_verts));
     GD_CUDA(c, gd_pool_get(c, 7, sizeof(int) * 3 * (size_t)n_tri, (void **)&c->d_tris));
     GD_CUDA(c, gd_pool_get(c, 8, sizeof(int) * (size_t)n_tri, (void **)&c->d_tri_mats));
     GD_CUDA(c, gd_pool_get(c, 9, sizeof(int) * (size_t)n_tri, (void **)&c->d_tri_surf));
-    GD_CUDA(c, cudaMemcpyAsync(c->d_verts, vertices, sizeof(float) * 3 * (size_t)n_vert, cudaMemcpyHostToDevice, c->stream));
-    GD_CUDA(c, cudaMemcpyAsync(c->d_tris, triangles, sizeof(int) * 3 * (size_t)n_tri, cudaMemcpyHostToDevice, c->stream));
-    GD_CUDA(c, cudaMemcpyAsync(c->d_tri_mats, mats.data(), sizeof(int) * (size_t)n_tri, cudaMemcpyHostToDevice, c->stream));
-    GD_CUDA(c, cudaMemcpyAsync(c->d_tri_surf, tri_surface, sizeof(int) * (size_t)n_tri, cudaMemcpyHostToDevice, c->stream));
-    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    GD_CUDA(c, gd_pool_get(c, 10, sizeof(unsigned long long) * cap, (void **)&ekey));
+    GD_CUDA(c, gd_pool_get(c, 11, sizeof(int) * cap, (void **)&esurf));
+    GD_CUDA(c, gd_pool_get(c, 12, sizeof(int) * 2 * (size_t)n_surf + sizeof(unsigned) * GD_ERR_N, (void **)&err));
+    sides = (int *)(err + GD_ERR_N);
+    std::vector<int> h_sides(2 * (size_t)n_surf);
+    for (int s = 0; s < n_surf; ++s) { h_sides[2 * s] = surf_inside[s]; h_sides[2 * s + 1] = surf_outside[s]; }
+    GD_CUDA(c, cudaMemcpyAsync(c->d_verts, vertices, sizeof(float) * 3 * (size_t)n_vert, cudaMemcpyHostToDevice, st));
+    GD_CUDA(c, cudaMemcpyAsync(c->d_tris, triangles, sizeof(int) * 3 * (size_t)n_tri, cudaMemcpyHostToDevice, st));
+    GD_CUDA(c, cudaMemcpyAsync(c->d_tri_surf, tri_surface, sizeof(int) * (size_t)n_tri, cudaMemcpyHostToDevice, st));
+    GD_CUDA(c, cudaMemcpyAsync(sides, h_sides.data(), sizeof(int) * 2 * (size_t)n_surf, cudaMemcpyHostToDevice, st));
+    GD_CUDA(c, cudaMemsetAsync(ekey, 0xFF, sizeof(unsigned long long) * cap, st));
+    GD_CUDA(c, cudaMemsetAsync(err, 0xFF, sizeof(unsigned) * GD_ERR_N, st));
+    const int shift = 64 - cap_log2;
+    gd_k_check_verts<<<(unsigned)(((size_t)n_vert * 3 + 255) / 256), 256, 0, st>>>(c->d_verts, (size_t)n_vert * 3, err);
+    gd_k_check_tris<<<(n_tri + 255) / 256, 256, 0, st>>>(c->d_verts, c->d_tris, c->d_tri_surf, n_tri, n_vert, n_surf, sides,
+                                                         c->d_tri_mats, ekey, esurf, cap - 1, shift, err);
+    gd_k_check_closed<<<(unsigned)((cap + 255) / 256), 256, 0, st>>>(ekey, esurf, cap, shift, err);
+    unsigned h_err[GD_ERR_N];
+    GD_CUDA(c, cudaMemcpyAsync(h_err, err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
+    GD_CUDA(c, cudaStreamSynchronize(st));
+    GD_CUDA(c, cudaGetLastError());
+    const unsigned NONE = 0xFFFFFFFFu;
+    if (h_err[GD_ERR_NONFINITE] != NONE) return gd_fail(c, GADEP_E_NONFINITE, "vertex %u is not finite", h_err[GD_ERR_NONFINITE]);
+    {   // the first offending triangle decides, classes in the order they are checked within a triangle
+        int best = -1;
+        for (int k = GD_ERR_SURFACE; k <= GD_ERR_EDGE_TWICE; ++k)
+            if (h_err[k] != NONE && (best < 0 || h_err[k] < h_err[best])) best = k;
+        if (best == GD_ERR_SURFACE) return gd_fail(c, GADEP_E_INDEX, "triangle %u: surface id out of range", h_err[best]);
+        if (best == GD_ERR_VERTEX) return gd_fail(c, GADEP_E_INDEX, "triangle %u: vertex id out of range", h_err[best]);
+        if (best == GD_ERR_DEGENERATE) return gd_fail(c, GADEP_E_DEGENERATE, "triangle %u has zero area", h_err[best]);
+        if (best == GD_ERR_EDGE_TWICE)
+            return gd_fail(c, GADEP_E_NOT_CLOSED, "triangle %u: directed edge used twice (non-manifold or inconsistent winding)", h_err[best]);
+    }
+    if (h_err[GD_ERR_OPEN] != NONE) return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %u is not closed (open edge)", h_err[GD_ERR_OPEN]);
     c->n_vert = n_vert; c->n_tri = n_tri; c->n_surf = n_surf; c->world = world_material;
     c->have_mesh = true;
     return GADEP_OK;

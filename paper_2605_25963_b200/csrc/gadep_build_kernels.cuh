@@ -18,6 +18,71 @@ __global__ void gd_k_init_scene(int *scene) {
     else if (threadIdx.x < 16) scene[threadIdx.x] = 0;
 }
 
+// ---------------------------------------------------------------- mesh validation (gadep_load_mesh)
+// Everything gadep_load_mesh promises to reject is found on the device, in the copies the BVH build will read: vertex
+// coordinates that are not finite, surface / vertex indices out of range, zero-area triangles, and surfaces that are
+// not closed and consistently oriented (PAPER.md:193 needs closed geometry): every directed edge of a surface must
+// occur once and its reverse once, in the same surface -- one open-addressing table over all directed edges.
+// err[k] = smallest offending index of class k (0xFFFFFFFF = none).
+#define GD_ERR_NONFINITE 0    // vertex index
+#define GD_ERR_SURFACE 1      // triangle index: surface id out of range
+#define GD_ERR_VERTEX 2       // triangle index: vertex id out of range
+#define GD_ERR_DEGENERATE 3   // triangle index
+#define GD_ERR_EDGE_TWICE 4   // triangle index: a directed edge used twice
+#define GD_ERR_OPEN 5         // surface id: an edge without its reverse in the same surface
+#define GD_ERR_N 8
+#define GD_EDGE_EMPTY (~0ull)
+
+GD_D size_t gd_edge_slot(unsigned long long key, int shift) { return (size_t)((key * 0x9E3779B97F4A7C15ull) >> shift); }
+
+__global__ void gd_k_check_verts(const float *__restrict__ verts, size_t n3, unsigned *err) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n3 && !isfinite(verts[i])) atomicMin(&err[GD_ERR_NONFINITE], (unsigned)(i / 3));
+}
+
+__global__ void gd_k_check_tris(const float *__restrict__ verts, const int *__restrict__ tris, const int *__restrict__ tri_surf,
+                                int n_tri, int n_vert, int n_surf, const int *__restrict__ surf_sides, int *__restrict__ mats,
+                                unsigned long long *ekey, int *esurf, size_t cap_mask, int shift, unsigned *err) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_tri) return;
+    const int s = tri_surf[t];
+    if (s < 0 || s >= n_surf) { atomicMin(&err[GD_ERR_SURFACE], (unsigned)t); return; }
+    const int v[3] = {tris[3 * t], tris[3 * t + 1], tris[3 * t + 2]};
+    for (int k = 0; k < 3; ++k)
+        if (v[k] < 0 || v[k] >= n_vert) { atomicMin(&err[GD_ERR_VERTEX], (unsigned)t); return; }
+    const float *a = verts + 3 * (size_t)v[0], *b = verts + 3 * (size_t)v[1], *q = verts + 3 * (size_t)v[2];
+    const double e1[3] = {(double)b[0] - a[0], (double)b[1] - a[1], (double)b[2] - a[2]};
+    const double e2[3] = {(double)q[0] - a[0], (double)q[1] - a[1], (double)q[2] - a[2]};
+    const double nx = e1[1] * e2[2] - e1[2] * e2[1], ny = e1[2] * e2[0] - e1[0] * e2[2], nz = e1[0] * e2[1] - e1[1] * e2[0];
+    if (v[0] == v[1] || v[1] == v[2] || v[0] == v[2] || !(nx * nx + ny * ny + nz * nz > 0.0)) {
+        atomicMin(&err[GD_ERR_DEGENERATE], (unsigned)t);
+        return;
+    }
+    mats[t] = (surf_sides[2 * s] & 0xFFFF) | (int)((unsigned)(surf_sides[2 * s + 1] & 0xFFFF) << 16);
+    for (int k = 0; k < 3; ++k) {
+        const unsigned long long key = ((unsigned long long)(unsigned)v[k] << 32) | (unsigned)v[(k + 1) % 3];
+        size_t i = gd_edge_slot(key, shift);
+        for (;;) {
+            const unsigned long long seen = atomicCAS(&ekey[i], GD_EDGE_EMPTY, key);
+            if (seen == GD_EDGE_EMPTY) { esurf[i] = s; break; }
+            if (seen == key) { atomicMin(&err[GD_ERR_EDGE_TWICE], (unsigned)t); break; }
+            i = (i + 1) & cap_mask;
+        }
+    }
+}
+
+__global__ void gd_k_check_closed(const unsigned long long *__restrict__ ekey, const int *__restrict__ esurf, size_t cap,
+                                  int shift, unsigned *err) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= cap) return;
+    const unsigned long long key = ekey[i];
+    if (key == GD_EDGE_EMPTY) return;
+    const unsigned long long rev = (key << 32) | (key >> 32);
+    size_t j = gd_edge_slot(rev, shift);
+    while (ekey[j] != GD_EDGE_EMPTY && ekey[j] != rev) j = (j + 1) & (cap - 1);
+    if (ekey[j] == GD_EDGE_EMPTY || esurf[j] != esurf[i]) atomicMin(&err[GD_ERR_OPEN], (unsigned)esurf[i]);
+}
+
 #define GD_MAX_SPLITS 16
 
 GD_D void gd_load_tri(const float *__restrict__ verts, const int *__restrict__ tris, int i, float p[3][3], float lo[3],
