@@ -60,6 +60,10 @@ struct gadep_ctx {
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
     GdWaveTune tune = {8, 4, 4, 4.0f, 8.0f, 12};
+    // two-level BVH entry (GdBvh): box of the facets that are not on the KILL boundary, links of the root's children
+    bool two_level = false;
+    float inner_lo[3] = {0, 0, 0}, inner_hi[3] = {0, 0, 0};
+    int entry_inner = 0, entry_outer = 0;
     double split_budget = 8.0;                // extra BVH references per facet handed out by the splitting budget
     int n_bins = 0;
     float spec_e_max = 0;
@@ -238,11 +242,13 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
     GD_CUDA(c, cudaMemcpyAsync(c->d_tri_surf, tri_surface, sizeof(int) * (size_t)n_tri, cudaMemcpyHostToDevice, st));
     GD_CUDA(c, cudaMemcpyAsync(sides, h_sides.data(), sizeof(int) * 2 * (size_t)n_surf, cudaMemcpyHostToDevice, st));
     GD_CUDA(c, cudaMemsetAsync(ekey, 0xFF, sizeof(unsigned long long) * cap, st));
-    GD_CUDA(c, cudaMemsetAsync(err, 0xFF, sizeof(unsigned) * GD_ERR_N, st));
+    GD_CUDA(c, cudaMemsetAsync(err, 0xFF, sizeof(unsigned) * GD_ERR_BOX_MAX, st));
+    GD_CUDA(c, cudaMemsetAsync(err + GD_ERR_BOX_MAX, 0, sizeof(unsigned) * (GD_ERR_N - GD_ERR_BOX_MAX), st));
     const int shift = 64 - cap_log2;
     gd_k_check_verts<<<(unsigned)(((size_t)n_vert * 3 + 255) / 256), 256, 0, st>>>(c->d_verts, (size_t)n_vert * 3, err);
     gd_k_check_tris<<<(n_tri + 255) / 256, 256, 0, st>>>(c->d_verts, c->d_tris, c->d_tri_surf, n_tri, n_vert, n_surf, sides,
                                                          c->d_tri_mats, ekey, esurf, cap - 1, shift, err);
+    gd_k_check_boundary<<<(n_tri + 255) / 256, 256, 0, st>>>(c->d_verts, c->d_tris, c->d_tri_mats, n_tri, err);
     gd_k_check_closed<<<(unsigned)((cap + 255) / 256), 256, 0, st>>>(ekey, esurf, cap, shift, err);
     unsigned h_err[GD_ERR_N];
     GD_CUDA(c, cudaMemcpyAsync(h_err, err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
@@ -261,6 +267,15 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
             return gd_fail(c, GADEP_E_NOT_CLOSED, "triangle %u: directed edge used twice (non-manifold or inconsistent winding)", h_err[best]);
     }
     if (h_err[GD_ERR_OPEN] != NONE) return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %u is not closed (open edge)", h_err[GD_ERR_OPEN]);
+    {   // two-level BVH entry: needs both kinds of facets, and no boundary facet reaching into the box of the others
+        auto u2f = [](unsigned u) { int o = (int)(u ^ 0x80000000u); int b = o >= 0 ? o : o ^ 0x7FFFFFFF; float f; memcpy(&f, &b, 4); return f; };
+        c->two_level = h_err[GD_ERR_HAS_BOUNDARY] == 0 && h_err[GD_ERR_BOX_MIN] != NONE && h_err[GD_ERR_OVERLAP] == 0;
+        for (int d = 0; d < 3; ++d) {
+            c->inner_lo[d] = c->two_level ? u2f(h_err[GD_ERR_BOX_MIN + d]) : 0.0f;
+            c->inner_hi[d] = c->two_level ? u2f(h_err[GD_ERR_BOX_MAX + d]) : 0.0f;
+        }
+        if (getenv("GADEP_NO_TWO_LEVEL")) c->two_level = false;      // measurement switch
+    }
     c->n_vert = n_vert; c->n_tri = n_tri; c->n_surf = n_surf; c->world = world_material;
     c->have_mesh = true;
     return GADEP_OK;
@@ -325,7 +340,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         int *parent_int = (int *)(arena + o_pi), *parent_leaf = (int *)(arena + o_pl);
         int *visits = (int *)(arena + o_vis), *ref_tri = (int *)(arena + o_rt);
         gd_k_make_refs<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts, (unsigned)n, ref_lo, ref_hi, ref_tri, scene);
-        gd_k_morton<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, scene, keys[0], vals[0]);
+        gd_k_morton<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, scene, keys[0], vals[0], ref_tri, c->d_tri_mats, c->two_level ? 1 : 0);
         launches += 2;
         int cur = 0;
         for (int shift = 0; shift < 64; shift += 8) {
@@ -342,7 +357,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         if (n > 1) {
             cudaMemsetAsync(visits, 0, 4 * (size_t)n, st);
             cudaMemsetAsync(parent_leaf, 0xFF, 4 * (size_t)n, st);
-            gd_k_karras<<<nb, tb, 0, st>>>(keys[cur], n, child_l, child_r, parent_int, parent_leaf);
+            gd_k_karras<<<nb, tb, 0, st>>>(keys[cur], n, child_l, child_r, parent_int, parent_leaf, scene + 12);
             gd_k_refit<<<nb, tb, 0, st>>>(n, child_l, child_r, parent_int, parent_leaf, ref_lo, ref_hi, vals[cur], node_lo,
                                           node_hi, visits, c->d_nodes, scene + 6);
             gd_k_collapse4<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes4);
@@ -351,7 +366,10 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         cudaEventRecord(c->evb1, st);
         if ((e = cudaGetLastError()) != cudaSuccess) break;
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
-        if (n > 1 && (e = cudaMemcpy(&depth, scene + 6, sizeof(int), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
+        int tail[8] = {0, 0, 0, 0, 0, 0, 0, 0};      // scene[6] depth, scene[12..13] links of the root's children
+        if (n > 1 && (e = cudaMemcpy(tail, scene + 6, sizeof(tail), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
+        depth = tail[0];
+        c->entry_inner = tail[6]; c->entry_outer = tail[7];
         cudaEventElapsedTime(&c->last_build_ms, c->evb0, c->evb1);
     } while (0);
     if (e != cudaSuccess) rc = gd_fail(c, GADEP_E_CUDA, "BVH build failed: %s", cudaGetErrorString(e));
@@ -367,6 +385,14 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
 static GdBvh gd_bvh_view(const gadep_ctx *c) {
     GdBvh b;
     b.nodes = c->d_nodes; b.nodes4 = c->d_nodes4; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
+    b.two_level = c->two_level && c->n_ref > 1;
+    b.entry_inner = c->entry_inner; b.entry_outer = c->entry_outer;
+    for (int d = 0; d < 3; ++d) {
+        // margins: far above the step back to t_min (1e-4 mm) and the rounding of a point on the box, far below a facet
+        const float m = 1.0e-3f + 1.0e-5f * std::max(std::fabs(c->inner_lo[d]), std::fabs(c->inner_hi[d]));
+        b.in_small[d] = c->inner_lo[d] + m; b.in_small[3 + d] = c->inner_hi[d] - m;
+        b.in_big[d] = c->inner_lo[d] - m; b.in_big[3 + d] = c->inner_hi[d] + m;
+    }
     return b;
 }
 

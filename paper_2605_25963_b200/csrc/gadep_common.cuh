@@ -54,6 +54,12 @@ struct GdBvh {
     const GdTri *tris;
     int n_tri;
     int root_is_leaf;   // n_tri == 1
+    // two-level entry (gadep_build_bvh): the references of the facets on the KILL boundary sort behind all others, so the
+    // two children of the root are "inner geometry" and "boundary".  A segment that stays inside the (shrunk) box of the
+    // inner geometry starts at entry_inner, a ray that misses the (grown) box at entry_outer, everything else at the root.
+    int two_level;
+    int entry_inner, entry_outer;       // links as stored in the nodes (>= 0 node, < 0 ~leaf)
+    float in_small[6], in_big[6];       // lo xyz, hi xyz
 };
 
 struct GdCounters {    // device-side totals, 64-bit

@@ -55,6 +55,25 @@ GD_D void gd_trav_begin(GdTrav &T, const GdBvh &bvh, float px, float py, float p
     T.filter = filter; T.exa = exa; T.exb = exb; T.exc = exc;
     T.sp = 0; T.node = bvh.root_is_leaf ? ~0 : 0;
     T.slot = slot;
+    if (bvh.two_level) {
+        const float *a = bvh.in_small, *b = bvh.in_big;
+        if (px > a[0] && px < a[3] && py > a[1] && py < a[4] && pz > a[2] && pz < a[5]) {
+            // origin inside: the flight ends inside as well -> no boundary facet can be met (the box is convex and no
+            // boundary facet reaches into it; the shrink margin covers the step back to t_min and the rounding here)
+            if (t_max < GD_TINF) {
+                const float ex = fmaf(dx, t_max, px), ey = fmaf(dy, t_max, py), ez = fmaf(dz, t_max, pz);
+                if (ex > a[0] && ex < a[3] && ey > a[1] && ey < a[4] && ez > a[2] && ez < a[5]) T.node = bvh.entry_inner;
+            }
+        } else {
+            // ray misses the grown box of the inner geometry -> only boundary facets can be met
+            const float x0 = (b[0] - px) * T.ix, x1 = (b[3] - px) * T.ix;
+            const float y0 = (b[1] - py) * T.iy, y1 = (b[4] - py) * T.iy;
+            const float z0 = (b[2] - pz) * T.iz, z1 = (b[5] - pz) * T.iz;
+            const float tn = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), t_min));
+            const float tf = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fminf(fmaxf(z0, z1), t_max));
+            if (tn > tf) T.node = bvh.entry_outer;
+        }
+    }
 }
 
 // Safety query (filter == GD_FILTER_SAFETY): lower bound of the distance from a point to the nearest facet, as the
