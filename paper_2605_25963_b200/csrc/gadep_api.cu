@@ -60,10 +60,11 @@ struct gadep_ctx {
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
     GdWaveTune tune = {8, 4, 4, 4.0f, 8.0f, 12};
-    // two-level BVH entry (GdBvh): box of the facets that are not on the KILL boundary, links of the root's children
-    bool two_level = false;
-    float inner_lo[3] = {0, 0, 0}, inner_hi[3] = {0, 0, 0};
-    int entry_inner = 0, entry_outer = 0;
+    // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
+    std::vector<int> h_sides;                 // [n_surf][2] inside, outside
+    int *d_mat_entry = nullptr;               // [GADEP_MAX_MATERIALS][1 + GD_ENTRY_MAX], see GdBvh
+    bool have_entries = false;
+    bool cluster_surfaces = true;             // GADEP_NO_SURFACE_CLUSTERS=1 switches it off (measurement)
     double split_budget = 8.0;                // extra BVH references per facet handed out by the splitting budget
     int n_bins = 0;
     float spec_e_max = 0;
@@ -129,6 +130,7 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb1);
     if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
+    if (getenv("GADEP_NO_SURFACE_CLUSTERS")) c->cluster_surfaces = false;
     if (const char *t = getenv("GADEP_SPLIT_BUDGET")) { double b = atof(t); if (b >= 0 && b <= 15) c->split_budget = b; }
     if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,leaf_thresh" (measurement sweeps)
         int a, b, d;
@@ -166,7 +168,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
     for (int k = 0; k < 13; ++k) cudaFree(c->pool[k]);
-    cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair);
+    cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair); cudaFree(c->d_mat_entry);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     if (c->evb0) cudaEventDestroy(c->evb0);
@@ -235,20 +237,19 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
     GD_CUDA(c, gd_pool_get(c, 11, sizeof(int) * cap, (void **)&esurf));
     GD_CUDA(c, gd_pool_get(c, 12, sizeof(int) * 2 * (size_t)n_surf + sizeof(unsigned) * GD_ERR_N, (void **)&err));
     sides = (int *)(err + GD_ERR_N);
-    std::vector<int> h_sides(2 * (size_t)n_surf);
+    std::vector<int> &h_sides = c->h_sides;
+    h_sides.resize(2 * (size_t)n_surf);
     for (int s = 0; s < n_surf; ++s) { h_sides[2 * s] = surf_inside[s]; h_sides[2 * s + 1] = surf_outside[s]; }
     GD_CUDA(c, cudaMemcpyAsync(c->d_verts, vertices, sizeof(float) * 3 * (size_t)n_vert, cudaMemcpyHostToDevice, st));
     GD_CUDA(c, cudaMemcpyAsync(c->d_tris, triangles, sizeof(int) * 3 * (size_t)n_tri, cudaMemcpyHostToDevice, st));
     GD_CUDA(c, cudaMemcpyAsync(c->d_tri_surf, tri_surface, sizeof(int) * (size_t)n_tri, cudaMemcpyHostToDevice, st));
     GD_CUDA(c, cudaMemcpyAsync(sides, h_sides.data(), sizeof(int) * 2 * (size_t)n_surf, cudaMemcpyHostToDevice, st));
     GD_CUDA(c, cudaMemsetAsync(ekey, 0xFF, sizeof(unsigned long long) * cap, st));
-    GD_CUDA(c, cudaMemsetAsync(err, 0xFF, sizeof(unsigned) * GD_ERR_BOX_MAX, st));
-    GD_CUDA(c, cudaMemsetAsync(err + GD_ERR_BOX_MAX, 0, sizeof(unsigned) * (GD_ERR_N - GD_ERR_BOX_MAX), st));
+    GD_CUDA(c, cudaMemsetAsync(err, 0xFF, sizeof(unsigned) * GD_ERR_N, st));
     const int shift = 64 - cap_log2;
     gd_k_check_verts<<<(unsigned)(((size_t)n_vert * 3 + 255) / 256), 256, 0, st>>>(c->d_verts, (size_t)n_vert * 3, err);
     gd_k_check_tris<<<(n_tri + 255) / 256, 256, 0, st>>>(c->d_verts, c->d_tris, c->d_tri_surf, n_tri, n_vert, n_surf, sides,
                                                          c->d_tri_mats, ekey, esurf, cap - 1, shift, err);
-    gd_k_check_boundary<<<(n_tri + 255) / 256, 256, 0, st>>>(c->d_verts, c->d_tris, c->d_tri_mats, n_tri, err);
     gd_k_check_closed<<<(unsigned)((cap + 255) / 256), 256, 0, st>>>(ekey, esurf, cap, shift, err);
     unsigned h_err[GD_ERR_N];
     GD_CUDA(c, cudaMemcpyAsync(h_err, err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
@@ -267,15 +268,6 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
             return gd_fail(c, GADEP_E_NOT_CLOSED, "triangle %u: directed edge used twice (non-manifold or inconsistent winding)", h_err[best]);
     }
     if (h_err[GD_ERR_OPEN] != NONE) return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %u is not closed (open edge)", h_err[GD_ERR_OPEN]);
-    {   // two-level BVH entry: needs both kinds of facets, and no boundary facet reaching into the box of the others
-        auto u2f = [](unsigned u) { int o = (int)(u ^ 0x80000000u); int b = o >= 0 ? o : o ^ 0x7FFFFFFF; float f; memcpy(&f, &b, 4); return f; };
-        c->two_level = h_err[GD_ERR_HAS_BOUNDARY] == 0 && h_err[GD_ERR_BOX_MIN] != NONE && h_err[GD_ERR_OVERLAP] == 0;
-        for (int d = 0; d < 3; ++d) {
-            c->inner_lo[d] = c->two_level ? u2f(h_err[GD_ERR_BOX_MIN + d]) : 0.0f;
-            c->inner_hi[d] = c->two_level ? u2f(h_err[GD_ERR_BOX_MAX + d]) : 0.0f;
-        }
-        if (getenv("GADEP_NO_TWO_LEVEL")) c->two_level = false;      // measurement switch
-    }
     c->n_vert = n_vert; c->n_tri = n_tri; c->n_surf = n_surf; c->world = world_material;
     c->have_mesh = true;
     return GADEP_OK;
@@ -323,6 +315,10 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     size_t o_hist = take(4 * (size_t)256 * n_tiles);
     size_t o_cl = take(4 * (size_t)n), o_cr = take(4 * (size_t)n), o_pi = take(4 * (size_t)n), o_pl = take(4 * (size_t)n);
     size_t o_vis = take(4 * (size_t)n), o_rt = take(4 * (size_t)n);
+    // surface clusters: class bits above the Morton code, one entry node per surface
+    int cls_bits = 0;
+    if (c->cluster_surfaces && c->n_surf >= 2 && c->n_surf <= 256 && n > 1) while ((1 << cls_bits) < c->n_surf) cls_bits++;
+    size_t o_se = take(4 * (size_t)std::max(c->n_surf, 1));
     unsigned char *arena = nullptr;
     if (gd_pool_get(c, 2, off, (void **)&arena) != cudaSuccess) return gd_fail(c, GADEP_E_NOMEM, "BVH scratch (%zu B)", off);
     int rc = GADEP_OK;
@@ -339,8 +335,9 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         int *child_l = (int *)(arena + o_cl), *child_r = (int *)(arena + o_cr);
         int *parent_int = (int *)(arena + o_pi), *parent_leaf = (int *)(arena + o_pl);
         int *visits = (int *)(arena + o_vis), *ref_tri = (int *)(arena + o_rt);
+        int *surf_entry = (int *)(arena + o_se);
         gd_k_make_refs<<<nbt, tb, 0, st>>>(c->d_verts, c->d_tris, n_tri, counts, (unsigned)n, ref_lo, ref_hi, ref_tri, scene);
-        gd_k_morton<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, scene, keys[0], vals[0], ref_tri, c->d_tri_mats, c->two_level ? 1 : 0);
+        gd_k_morton<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, scene, keys[0], vals[0], ref_tri, c->d_tri_surf, cls_bits);
         launches += 2;
         int cur = 0;
         for (int shift = 0; shift < 64; shift += 8) {
@@ -357,7 +354,8 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         if (n > 1) {
             cudaMemsetAsync(visits, 0, 4 * (size_t)n, st);
             cudaMemsetAsync(parent_leaf, 0xFF, 4 * (size_t)n, st);
-            gd_k_karras<<<nb, tb, 0, st>>>(keys[cur], n, child_l, child_r, parent_int, parent_leaf, scene + 12);
+            cudaMemsetAsync(surf_entry, 0xFF, 4 * (size_t)std::max(c->n_surf, 1), st);        // -1 = no entry node
+            gd_k_karras<<<nb, tb, 0, st>>>(keys[cur], n, child_l, child_r, parent_int, parent_leaf, cls_bits, surf_entry);
             gd_k_refit<<<nb, tb, 0, st>>>(n, child_l, child_r, parent_int, parent_leaf, ref_lo, ref_hi, vals[cur], node_lo,
                                           node_hi, visits, c->d_nodes, scene + 6);
             gd_k_collapse4<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes4);
@@ -366,14 +364,33 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         cudaEventRecord(c->evb1, st);
         if ((e = cudaGetLastError()) != cudaSuccess) break;
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
-        int tail[8] = {0, 0, 0, 0, 0, 0, 0, 0};      // scene[6] depth, scene[12..13] links of the root's children
-        if (n > 1 && (e = cudaMemcpy(tail, scene + 6, sizeof(tail), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
-        depth = tail[0];
-        c->entry_inner = tail[6]; c->entry_outer = tail[7];
+        if (n > 1 && (e = cudaMemcpy(&depth, scene + 6, sizeof(int), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
         cudaEventElapsedTime(&c->last_build_ms, c->evb0, c->evb1);
+        // per-material entry table: the surfaces that have the material on one side.  A surface without an entry node
+        // (never for a closed surface of >= 2 references) or too many surfaces around one material -> root for it.
+        c->have_entries = false;
+        if (cls_bits > 0) {
+            std::vector<int> se(c->n_surf);
+            if ((e = cudaMemcpy(se.data(), surf_entry, 4 * (size_t)c->n_surf, cudaMemcpyDeviceToHost)) != cudaSuccess) break;
+            int table[GADEP_MAX_MATERIALS][1 + GD_ENTRY_MAX];
+            memset(table, 0, sizeof(table));
+            for (int m = 0; m < GADEP_MAX_MATERIALS; ++m) {
+                int cnt = 0;
+                bool ok = true;
+                for (int s2 = 0; s2 < c->n_surf && ok; ++s2) {
+                    if (c->h_sides[2 * s2] != m && c->h_sides[2 * s2 + 1] != m) continue;
+                    if (se[s2] < 0 || cnt == GD_ENTRY_MAX) ok = false;
+                    else table[m][1 + cnt++] = se[s2];
+                }
+                table[m][0] = ok ? cnt : 0;
+            }
+            if (!c->d_mat_entry && (e = cudaMalloc(&c->d_mat_entry, sizeof(table))) != cudaSuccess) break;
+            if ((e = cudaMemcpy(c->d_mat_entry, table, sizeof(table), cudaMemcpyHostToDevice)) != cudaSuccess) break;
+            c->have_entries = true;
+        }
     } while (0);
     if (e != cudaSuccess) rc = gd_fail(c, GADEP_E_CUDA, "BVH build failed: %s", cudaGetErrorString(e));
-    else if (depth >= GD_STACK || 3 * depth + 4 > GD_STACK4) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
+    else if (depth >= GD_STACK || 3 * depth + 4 + GD_ENTRY_MAX > GD_STACK4) rc = gd_fail(c, GADEP_E_ARG, "BVH depth %d exceeds the traversal stack (%d)", depth, GD_STACK);
     if (rc != GADEP_OK) return rc;
     c->bvh_depth = depth;
     c->n_ref = n;
@@ -385,14 +402,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
 static GdBvh gd_bvh_view(const gadep_ctx *c) {
     GdBvh b;
     b.nodes = c->d_nodes; b.nodes4 = c->d_nodes4; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
-    b.two_level = c->two_level && c->n_ref > 1;
-    b.entry_inner = c->entry_inner; b.entry_outer = c->entry_outer;
-    for (int d = 0; d < 3; ++d) {
-        // margins: far above the step back to t_min (1e-4 mm) and the rounding of a point on the box, far below a facet
-        const float m = 1.0e-3f + 1.0e-5f * std::max(std::fabs(c->inner_lo[d]), std::fabs(c->inner_hi[d]));
-        b.in_small[d] = c->inner_lo[d] + m; b.in_small[3 + d] = c->inner_hi[d] - m;
-        b.in_big[d] = c->inner_lo[d] - m; b.in_big[3 + d] = c->inner_hi[d] + m;
-    }
+    b.mat_entry = c->have_entries ? c->d_mat_entry : nullptr;
     return b;
 }
 

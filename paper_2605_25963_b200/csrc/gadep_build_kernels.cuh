@@ -30,13 +30,8 @@ __global__ void gd_k_init_scene(int *scene) {
 #define GD_ERR_DEGENERATE 3   // triangle index
 #define GD_ERR_EDGE_TWICE 4   // triangle index: a directed edge used twice
 #define GD_ERR_OPEN 5         // surface id: an edge without its reverse in the same surface
-#define GD_ERR_HAS_BOUNDARY 6 // 0 if some facet lies on the KILL boundary
-#define GD_ERR_BOX_MIN 8      // [8..10] box of the facets that do not: min corner as ordered unsigned
-#define GD_ERR_BOX_MAX 12     // [12..14] max corner (initialised to 0)
-#define GD_ERR_OVERLAP 15     // 1 if a boundary facet's box reaches into that box
-#define GD_ERR_N 16
+#define GD_ERR_N 8
 #define GD_EDGE_EMPTY (~0ull)
-GD_D unsigned gd_f2u(float f) { return (unsigned)gd_f2o(f) ^ 0x80000000u; }   // order-preserving float -> unsigned
 
 GD_D size_t gd_edge_slot(unsigned long long key, int shift) { return (size_t)((key * 0x9E3779B97F4A7C15ull) >> shift); }
 
@@ -64,12 +59,6 @@ __global__ void gd_k_check_tris(const float *__restrict__ verts, const int *__re
         return;
     }
     mats[t] = (surf_sides[2 * s] & 0xFFFF) | (int)((unsigned)(surf_sides[2 * s + 1] & 0xFFFF) << 16);
-    if (surf_sides[2 * s] < 0 || surf_sides[2 * s + 1] < 0) err[GD_ERR_HAS_BOUNDARY] = 0;
-    else
-        for (int d = 0; d < 3; ++d) {
-            atomicMin(&err[GD_ERR_BOX_MIN + d], gd_f2u(fminf(fminf(a[d], b[d]), q[d])));
-            atomicMax(&err[GD_ERR_BOX_MAX + d], gd_f2u(fmaxf(fmaxf(a[d], b[d]), q[d])));
-        }
     for (int k = 0; k < 3; ++k) {
         const unsigned long long key = ((unsigned long long)(unsigned)v[k] << 32) | (unsigned)v[(k + 1) % 3];
         size_t i = gd_edge_slot(key, shift);
@@ -80,22 +69,6 @@ __global__ void gd_k_check_tris(const float *__restrict__ verts, const int *__re
             i = (i + 1) & cap_mask;
         }
     }
-}
-
-// after gd_k_check_tris: does a facet on the KILL boundary reach into the box of the other facets?
-__global__ void gd_k_check_boundary(const float *__restrict__ verts, const int *__restrict__ tris, const int *__restrict__ mats,
-                                    int n_tri, unsigned *err) {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= n_tri || err[GD_ERR_SURFACE] != 0xFFFFFFFFu || err[GD_ERR_VERTEX] != 0xFFFFFFFFu) return;
-    const int m = mats[t];
-    if ((m & 0xFFFF) != 0xFFFF && ((unsigned)m >> 16) != 0xFFFFu) return;
-    bool overlap = true;
-    for (int d = 0; d < 3; ++d) {
-        const float x0 = verts[3 * (size_t)tris[3 * t] + d], x1 = verts[3 * (size_t)tris[3 * t + 1] + d], x2 = verts[3 * (size_t)tris[3 * t + 2] + d];
-        const unsigned lo = gd_f2u(fminf(fminf(x0, x1), x2)), hi = gd_f2u(fmaxf(fmaxf(x0, x1), x2));
-        overlap = overlap && lo <= err[GD_ERR_BOX_MAX + d] && hi >= err[GD_ERR_BOX_MIN + d];
-    }
-    if (overlap) err[GD_ERR_OVERLAP] = 1;
 }
 
 __global__ void gd_k_check_closed(const unsigned long long *__restrict__ ekey, const int *__restrict__ esurf, size_t cap,
@@ -221,8 +194,8 @@ __global__ void gd_k_make_refs(const float *__restrict__ verts, const int *__res
 
 __global__ void gd_k_morton(const float4 *__restrict__ tri_lo, const float4 *__restrict__ tri_hi, int n_tri,
                             const int *__restrict__ scene, unsigned long long *__restrict__ keys,
-                            unsigned *__restrict__ vals, const int *__restrict__ ref_tri, const int *__restrict__ tri_mats,
-                            int two_level) {
+                            unsigned *__restrict__ vals, const int *__restrict__ ref_tri, const int *__restrict__ tri_surf,
+                            int cls_bits) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_tri) return;
     float sx = gd_o2f(scene[0]), sy = gd_o2f(scene[1]), sz = gd_o2f(scene[2]);
@@ -233,10 +206,8 @@ __global__ void gd_k_morton(const float4 *__restrict__ tri_lo, const float4 *__r
     float ny = ey > 0.0f ? (cy - sy) / ey : 0.0f;
     float nz = ez > 0.0f ? (cz - sz) / ez : 0.0f;
     unsigned long long key = gd_morton63(nx, ny, nz);
-    if (two_level) {                    // facets on the KILL boundary behind all others: the root splits between the two
-        const int m = tri_mats[ref_tri[i]];
-        if ((m & 0xFFFF) == 0xFFFF || ((unsigned)m >> 16) == 0xFFFFu) key |= 1ull << 63;
-    }
+    // surface id above the Morton code: every closed surface becomes one subtree of the radix tree
+    if (cls_bits > 0) key = (key >> (cls_bits - 1)) | ((unsigned long long)tri_surf[ref_tri[i]] << (64 - cls_bits));
     keys[i] = key;
     vals[i] = (unsigned)i;
 }
@@ -331,7 +302,7 @@ __global__ void gd_k_sort_scatter(const unsigned long long *__restrict__ keys_in
 // internal node i in [0, n-1); children encoded >= 0 internal, < 0 leaf (~sorted index)
 __global__ void gd_k_karras(const unsigned long long *__restrict__ keys, int n, int *__restrict__ child_l,
                             int *__restrict__ child_r, int *__restrict__ parent_int, int *__restrict__ parent_leaf,
-                            int *__restrict__ root_links) {
+                            int cls_bits, int *__restrict__ surf_entry) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n - 1) return;
     int first, last, split;
@@ -341,7 +312,13 @@ __global__ void gd_k_karras(const unsigned long long *__restrict__ keys, int n, 
     if (last == split + 1) { r = ~(split + 1); parent_leaf[split + 1] = i; } else { r = split + 1; parent_int[split + 1] = i; }
     child_l[i] = l;
     child_r[i] = r;
-    if (i == 0) { parent_int[0] = -1; root_links[0] = l; root_links[1] = r; }
+    if (i == 0) parent_int[0] = -1;
+    if (cls_bits > 0) {        // the node that covers exactly the references of one surface is that surface's entry
+        const int sh = 64 - cls_bits;
+        const unsigned long long ca = keys[first] >> sh, cb = keys[last] >> sh;
+        if (ca == cb && (first == 0 || (keys[first - 1] >> sh) != ca) && (last == n - 1 || (keys[last + 1] >> sh) != ca))
+            surf_entry[ca] = i;
+    }
 }
 
 // leaf-ordered triangle records

@@ -54,13 +54,12 @@ struct GdBvh {
     const GdTri *tris;
     int n_tri;
     int root_is_leaf;   // n_tri == 1
-    // two-level entry (gadep_build_bvh): the references of the facets on the KILL boundary sort behind all others, so the
-    // two children of the root are "inner geometry" and "boundary".  A segment that stays inside the (shrunk) box of the
-    // inner geometry starts at entry_inner, a ray that misses the (grown) box at entry_outer, everything else at the root.
-    int two_level;
-    int entry_inner, entry_outer;       // links as stored in the nodes (>= 0 node, < 0 ~leaf)
-    float in_small[6], in_big[6];       // lo xyz, hi xyz
+    // Surface-clustered hierarchy (gadep_build_bvh): the references sort by surface first, so every closed surface is one
+    // subtree.  A flight in a known material can only meet the surfaces that have it on one side: mat_entry (device,
+    // [material][1 + GD_ENTRY_MAX]: count, links) names their subtrees; count 0 = start at the root.  nullptr = off.
+    const int *mat_entry;
 };
+#define GD_ENTRY_MAX 8
 
 struct GdCounters {    // device-side totals, 64-bit
     unsigned long long n_histories, n_queries, n_box_tests, n_tri_tests, n_crossings, n_pe, n_compton, n_coherent,

@@ -20,7 +20,7 @@ gd_k_locate(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ 
     if (i < n) {
         int stack[GD_STACK4];
         GdTrav T;
-        gd_trav_begin(T, bvh, org[3 * i], org[3 * i + 1], org[3 * i + 2], dir[3 * i], dir[3 * i + 1], dir[3 * i + 2], 0.0f,
+        gd_trav_begin(T, bvh, stack, org[3 * i], org[3 * i + 1], org[3 * i + 2], dir[3 * i], dir[3 * i + 1], dir[3 * i + 2], 0.0f,
                       GD_TINF, -2, -1, -1, -1, 0);
         int result = world_material;
         if (mode == 0) {

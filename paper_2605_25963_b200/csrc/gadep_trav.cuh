@@ -35,7 +35,7 @@ struct GdTrav {
 
 GD_D void gd_trav_idle(GdTrav &T) { T.slot = -1; T.node = GD_TRAV_DONE; T.sp = 0; }
 
-GD_D void gd_trav_begin(GdTrav &T, const GdBvh &bvh, float px, float py, float pz, float dx, float dy, float dz,
+GD_D void gd_trav_begin(GdTrav &T, const GdBvh &bvh, int *stack, float px, float py, float pz, float dx, float dy, float dz,
                         float t_min, float t_max, int filter, int exa, int exb, int exc, int slot) {
     T.ox = px; T.oy = py; T.oz = pz;
     T.ix = gd_safe_rcp(dx); T.iy = gd_safe_rcp(dy); T.iz = gd_safe_rcp(dz);
@@ -55,23 +55,14 @@ GD_D void gd_trav_begin(GdTrav &T, const GdBvh &bvh, float px, float py, float p
     T.filter = filter; T.exa = exa; T.exb = exb; T.exc = exc;
     T.sp = 0; T.node = bvh.root_is_leaf ? ~0 : 0;
     T.slot = slot;
-    if (bvh.two_level) {
-        const float *a = bvh.in_small, *b = bvh.in_big;
-        if (px > a[0] && px < a[3] && py > a[1] && py < a[4] && pz > a[2] && pz < a[5]) {
-            // origin inside: the flight ends inside as well -> no boundary facet can be met (the box is convex and no
-            // boundary facet reaches into it; the shrink margin covers the step back to t_min and the rounding here)
-            if (t_max < GD_TINF) {
-                const float ex = fmaf(dx, t_max, px), ey = fmaf(dy, t_max, py), ez = fmaf(dz, t_max, pz);
-                if (ex > a[0] && ex < a[3] && ey > a[1] && ey < a[4] && ez > a[2] && ez < a[5]) T.node = bvh.entry_inner;
-            }
-        } else {
-            // ray misses the grown box of the inner geometry -> only boundary facets can be met
-            const float x0 = (b[0] - px) * T.ix, x1 = (b[3] - px) * T.ix;
-            const float y0 = (b[1] - py) * T.iy, y1 = (b[4] - py) * T.iy;
-            const float z0 = (b[2] - pz) * T.iz, z1 = (b[5] - pz) * T.iz;
-            const float tn = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), t_min));
-            const float tf = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fminf(fmaxf(z0, z1), t_max));
-            if (tn > tf) T.node = bvh.entry_outer;
+    if (bvh.mat_entry && filter >= 0) {
+        // only facets with `filter` on their from-side can be accepted: start at the subtrees of the surfaces that have
+        // this material on one side
+        const int *e = bvh.mat_entry + filter * (1 + GD_ENTRY_MAX);
+        const int ne = __ldg(e);
+        if (ne > 0) {
+            T.node = __ldg(e + 1);
+            for (int k = 2; k <= ne; ++k) stack[T.sp++] = __ldg(e + k);
         }
     }
 }

@@ -324,7 +324,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #endif
                             {
                                 const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
-                                gd_trav_begin(T, bvh, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
+                                gd_trav_begin(T, bvh, stack, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
                                               loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
                                               __float_as_int(GD_SF(19)), __float_as_int(GD_SF(20)), __float_as_int(GD_SF(21)), s);
                                 n_query++;
@@ -433,7 +433,7 @@ gd_k_trace_wave(GdBvh bvh, const float *__restrict__ org, const float *__restric
                     if (T.slot < 0 && rank < avail) {
                         const long long i = w_cur + rank;
                         my_ray = i;
-                        gd_trav_begin(T, bvh, org[3 * i], org[3 * i + 1], org[3 * i + 2], dir[3 * i], dir[3 * i + 1],
+                        gd_trav_begin(T, bvh, stack, org[3 * i], org[3 * i + 1], org[3 * i + 2], dir[3 * i], dir[3 * i + 1],
                                       dir[3 * i + 2], t_min, GD_INF, filter_mat, -1, -1, -1, 0);
                         n_query++;
                     }

@@ -222,7 +222,7 @@ GD_D void gd_ws_traverse(GdWsTeam *tm, float *sl, const GdBvh &bvh, const GdWave
             const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
             const float mu_tot = GD_WSF(12);
             const float sdist = mu_tot > 0.0f ? GD_WSF(7) / mu_tot : GD_TINF;
-            gd_trav_begin(T, bvh, GD_WSF(0), GD_WSF(1), GD_WSF(2), GD_WSF(3), GD_WSF(4), GD_WSF(5), loc ? 0.0f : -GD_TBACK,
+            gd_trav_begin(T, bvh, stack, GD_WSF(0), GD_WSF(1), GD_WSF(2), GD_WSF(3), GD_WSF(4), GD_WSF(5), loc ? 0.0f : -GD_TBACK,
                           loc ? GD_TINF : sdist, loc ? -2 : (int)(st & 31u) - 1, __float_as_int(GD_WSF(18)),
                           __float_as_int(GD_WSF(19)), __float_as_int(GD_WSF(20)), s);
             n_query++;
