@@ -88,30 +88,6 @@ GD_D float gd_box_dist2(float px, float py, float pz, float lx, float hx, float 
     return fmaf(dx, dx, fmaf(dy, dy, dz * dz));
 }
 
-GD_D void gd_trav_node_safety(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
-    const GdNode &nd = bvh.nodes[T.node];
-    const float4 a = nd.n0xy, b = nd.n1xy, z = nd.nz;
-    const int4 lk = nd.link;
-    n_box_tests += 2;
-    const float d0 = gd_box_dist2(T.ox, T.oy, T.oz, a.x, a.y, a.z, a.w, z.x, z.y);
-    const float d1 = gd_box_dist2(T.ox, T.oy, T.oz, b.x, b.y, b.z, b.w, z.z, z.w);
-    bool v0 = d0 < T.t, v1 = d1 < T.t;
-    if (v0 && lk.x < 0) { T.t = d0; v0 = false; v1 = v1 && d1 < T.t; }
-    if (v1 && lk.y < 0) { T.t = d1; v1 = false; v0 = v0 && d0 < T.t; }
-    if (v0 && v1) {
-        int near_c = lk.x, far_c = lk.y;
-        if (d1 < d0) { near_c = lk.y; far_c = lk.x; }
-        stack[T.sp++] = far_c;
-        T.node = near_c;
-    } else if (v0) {
-        T.node = lk.x;
-    } else if (v1) {
-        T.node = lk.y;
-    } else {
-        T.node = T.sp == 0 ? GD_TRAV_DONE : stack[--T.sp];
-    }
-}
-
 struct GdEdge3 { float u, v, w; int ok; };
 __device__ __noinline__ GdEdge3 gd_edges_double(float ax, float ay, float bx, float by, float cx, float cy) {
     const double du = GD_DSUB(GD_DMUL((double)cx, (double)by), GD_DMUL((double)cy, (double)bx));
@@ -167,40 +143,6 @@ GD_D void gd_trav_leaf(GdTrav &T, const GdBvh &bvh, int leaf, unsigned &n_tri_te
 }
 
 GD_D int gd_trav_pop(GdTrav &T, const int *stack) { return T.sp == 0 ? GD_TRAV_DONE : stack[--T.sp]; }
-
-// one inner-node visit (two child boxes); far sides padded by the FMA error bound and ~3 ulp
-GD_D void gd_trav_node(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
-    const GdNode &nd = bvh.nodes[T.node];
-    const float4 a = nd.n0xy, b = nd.n1xy, z = nd.nz;
-    const int4 lk = nd.link;
-    n_box_tests += 2;
-    const float pad = 4.0e-7f;
-    float x0 = fmaf(a.x, T.ix, -T.bx), x1 = fmaf(a.y, T.ix, -T.bx);
-    float y0 = fmaf(a.z, T.iy, -T.by), y1 = fmaf(a.w, T.iy, -T.by);
-    float z0 = fmaf(z.x, T.iz, -T.bz), z1 = fmaf(z.y, T.iz, -T.bz);
-    float n0 = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), T.tmin + T.err));
-    float f0 = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fminf(fmaxf(z0, z1), T.t));
-    f0 = fmaf(fabsf(f0), pad, f0) + 2.0f * T.err;
-    x0 = fmaf(b.x, T.ix, -T.bx); x1 = fmaf(b.y, T.ix, -T.bx);
-    y0 = fmaf(b.z, T.iy, -T.by); y1 = fmaf(b.w, T.iy, -T.by);
-    z0 = fmaf(z.z, T.iz, -T.bz); z1 = fmaf(z.w, T.iz, -T.bz);
-    float n1 = fmaxf(fmaxf(fminf(x0, x1), fminf(y0, y1)), fmaxf(fminf(z0, z1), T.tmin + T.err));
-    float f1 = fminf(fminf(fmaxf(x0, x1), fmaxf(y0, y1)), fminf(fmaxf(z0, z1), T.t));
-    f1 = fmaf(fabsf(f1), pad, f1) + 2.0f * T.err;
-    const bool h0 = n0 <= f0, h1 = n1 <= f1;
-    if (h0 && h1) {
-        int near_c = lk.x, far_c = lk.y;
-        if (n1 < n0) { near_c = lk.y; far_c = lk.x; }
-        stack[T.sp++] = far_c;
-        T.node = near_c;
-    } else if (h0) {
-        T.node = lk.x;
-    } else if (h1) {
-        T.node = lk.y;
-    } else {
-        T.node = gd_trav_pop(T, stack);
-    }
-}
 
 #define GD_CSWAP(ka, ca, kb, cb) do { if (kb < ka) { float tk = ka; ka = kb; kb = tk; int tc = ca; ca = cb; cb = tc; } } while (0)
 
