@@ -180,6 +180,24 @@ def make_config(i: int, n_theta: int | None = None, total_bands: int | None = No
     raise ValueError(f"no config {i}")
 
 
+def make_pellet_stack(n_pellets: int, n_theta: int = 24, n_histories: int = 20_000) -> Workload:
+    """Test scene for the per-material BVH entries: `n_pellets` disjoint cylinders (r = 6 mm, 4 mm tall, 2 mm apart)
+    stacked on the axis in air, materials cycling Ge_active / Cu / water, point source above the stack.  Air touches
+    every pellet and the world (n_pellets + 1 surfaces), each pellet material n_pellets / 3 of them."""
+    mats = [MAT["Ge_active"], MAT["Cu"], MAT["water"]]
+    segl = []
+    for k in range(n_pellets):
+        z_top = -6.0 * k
+        segl.append((f"P{k}", _cyl_segments(6.0, z_top, z_top - 4.0, 1), mats[k % 3], MAT["air"]))
+    depth = 6.0 * n_pellets
+    segl.append(("world", _cyl_segments(40.0, 30.0, -depth - 30.0, 2), MAT["air"], -1))
+    mesh = _build(segl, n_theta, MAT["air"])
+    mu, sc, _ = make_tables(coh_coeff=7.0e-27)
+    src = _source(SRC_POINT, pos=(0, 0, 12.0), lines_kev=[122.1, 661.7])
+    return Workload(f"pellet_stack_{n_pellets}", mesh, mu, sc, E_MIN_MEV, E_MAX_MEV, src, n_histories, 3,
+                    notes={"ray_box": (8.0, -depth - 2.0, 2.0)})
+
+
 def make_rays(n: int, seed: int, cyl_r: float, z0: float, z1: float):
     """Seeded isotropic rays from uniform points in a z-axis cylinder (BASELINE.json configs[4] ray test).
     Returns (org f32[n,3], dir f32[n,3]); directions are unit in float32 to 1 ulp."""

@@ -18,6 +18,22 @@ def test_surfaces_closed_oriented_positive_volume(cfg):
         assert dm.mesh_signed_volume(m.vertices, tri) > 0
 
 
+def test_pellet_stack_scene_is_closed_disjoint_and_of_known_volume():
+    # the test scene of the per-material BVH entries: n disjoint cylinders r = 6, h = 4 on the axis, 2 mm apart
+    m = dm.make_pellet_stack(12, n_theta=96).mesh
+    assert m.n_surf == 13
+    for s in range(12):
+        tri = m.triangles[m.tri_surface == s]
+        c = dm.check_closed_oriented(tri)
+        assert c["ok"] and c["euler"] == 2
+        vol = dm.mesh_signed_volume(m.vertices, tri)
+        prism = 0.5 * 96 * 36.0 * np.sin(2 * np.pi / 96) * 4.0      # regular 96-gon prism
+        assert vol == pytest.approx(prism, rel=1e-5)
+        z = m.vertices[np.unique(tri)][:, 2]
+        assert z.max() == pytest.approx(-6.0 * s) and z.min() == pytest.approx(-6.0 * s - 4.0)
+    assert (m.surf_outside[:12] == dm.MAT["air"]).all() and m.surf_outside[12] == -1
+
+
 def test_triangle_counts():
     assert dm.make_config(0).mesh.n_tri == 256           # BASELINE.json configs[0]: "~256 triangles"
     assert dm.make_config(1).mesh.n_tri == 38400

@@ -259,6 +259,34 @@ def test_filtered_trace_with_negative_window(pkg, orc):
         _check_rays(w, g, s, org, d, filter_mat=mat, t_min=-1e-4)
 
 
+@pytest.mark.parametrize("n_pellets", [6, 12, 300])
+def test_material_entry_table_and_its_fallbacks(pkg, orc, n_pellets):
+    # The clustered hierarchy starts a flight at the subtrees of the surfaces around its material.  6 pellets: every
+    # material has an entry list (air: 7 surfaces).  12 pellets: air touches 13 surfaces, more than the table holds ->
+    # root for air, entry lists for the pellet materials.  300 pellets: more surfaces than class bits -> plain order.
+    # In every case filtered and unfiltered rays and whole histories must agree with the oracle.
+    w = dm.make_pellet_stack(n_pellets)
+    g = pkg.Gadep(0)
+    g.load_workload(w)
+    s = orc.OracleScene(w)
+    assert dm.check_closed_oriented(w.mesh.triangles)["ok"]
+    r, z0, z1 = w.notes["ray_box"]
+    n_rays = 20_000 if n_pellets < 100 else 3_000
+    org, d = make_rays(n_rays, 11, r, z0, z1)
+    _check_rays(w, g, s, org, d)
+    for mat in (dm.MAT["air"], dm.MAT["Ge_active"], dm.MAT["Cu"], dm.MAT["water"]):
+        _check_rays(w, g, s, org, d, filter_mat=mat, t_min=-1e-4)
+    n = 20_000 if n_pellets < 100 else 2_000
+    edep, flags = g.run_histories(0, n, w.seed)
+    oe, of, oc = s.run_histories(0, n, w.seed)
+    same = (flags == of) & (np.abs(edep.astype(np.float64) - oe) <= 2e-6 + 1e-5 * oe)
+    assert same.mean() >= 0.998, same.mean()
+    c = g.get_counters()
+    assert c["n_leak"] == 0 and oc["n_leak"] == 0
+    for k in ("n_crossings", "n_pe", "n_compton", "n_coherent", "n_escaped"):
+        assert abs(c[k] - oc[k]) <= 0.01 * oc[k] + 20, (k, c[k], oc[k])
+
+
 # ------------------------------------------------------------------ histories, same random streams
 @pytest.mark.parametrize("cfg,n", [(0, 400_000), (1, 40_000), (2, 6_000), (3, 6_000)])
 def test_per_history_parity(pkg, orc, cfg, n):
