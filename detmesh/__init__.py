@@ -7,14 +7,14 @@ set-ups of BASELINE.json.  Nothing in here performs transport arithmetic.
 """
 from .geometry import (Line, Arc, discretise, revolve, Mesh, merge_surfaces,
                        mesh_signed_volume, mesh_area, check_closed_oriented)
-from .materials import (ELEMENTS, MATERIALS, MAT, energy_grid, sigma_kn_total,
+from .materials import (ELEMENTS, MATERIALS, MAT, DENSITY_G_CM3, energy_grid, sigma_kn_total,
                         make_tables, N_GRID, E_MIN_MEV, E_MAX_MEV)
 from .configs import make_config, make_calibration, make_pellet_stack, Workload, philox_u01_host, TABLE3_KEV, CALIBRATION_DETECTORS
 
 __all__ = [
     "Line", "Arc", "discretise", "revolve", "Mesh", "merge_surfaces",
     "mesh_signed_volume", "mesh_area", "check_closed_oriented",
-    "ELEMENTS", "MATERIALS", "MAT", "energy_grid", "sigma_kn_total", "make_tables",
+    "ELEMENTS", "MATERIALS", "MAT", "DENSITY_G_CM3", "energy_grid", "sigma_kn_total", "make_tables",
     "N_GRID", "E_MIN_MEV", "E_MAX_MEV", "make_config", "make_calibration", "make_pellet_stack", "Workload", "philox_u01_host",
     "TABLE3_KEV", "CALIBRATION_DETECTORS",
 ]

@@ -42,6 +42,7 @@ MATERIALS = [
     ("SiO2", 2.0, {"Si": 0.46744, "O": 0.53256}, 0),
 ]
 MAT = {name: i for i, (name, _, _, _) in enumerate(MATERIALS)}
+DENSITY_G_CM3 = np.array([rho for (_, rho, _, _) in MATERIALS], dtype=np.float32)   # input of the electron-range mode
 MAT_KILL = -1
 
 

@@ -13,11 +13,14 @@
  *   - parity (Jordan) localisation, used here as a cross-check only
  *   - photoelectric, Compton, pair production (+ coherent per BASELINE.json configs[1])
  *   - scoring of deposited energy in the sensitive Ge volume -> FEPE
+ *   - optional (orc_set_electron_mode): the electrons of PAPER.md:179's coupled photon-electron physics as straight
+ *     segments of the Katz-Penfold range instead of a local deposit (reading R16)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors; ray-triangle vs a second
  * formulation and hand-computed rays; slab transmission exp(-mu x); on-axis solid angle of the N-gon
  * cylinder; Klein-Nishina / Thomson moments vs quadrature; energy accounting per history; parity rule ==
- * side-id rule; pair escape peaks.  FEPE values themselves: parity unpinned by the paper (it prints no
+ * side-id rule; pair escape peaks; electron mode: range values, kept fraction below a plane face (closed form),
+ * photon trajectories untouched.  FEPE values themselves: parity unpinned by the paper (it prints no
  * numeric FEPE, Fig. 11 is an image); they are pinned only through the closed forms above.
  */
 #include <math.h>
@@ -57,6 +60,9 @@ typedef struct {
     double src_pos[3], src_dir[3], cyl_r, cyl_z0, cyl_z1, ex_r, ex_z0, ex_z1;
     int n_lines;
     double *line_mev, *line_int, line_int_sum;
+    /* NEXT-4 ("coupled photon-electron"): straight CSDA electron segments, see deposit() */
+    int electron_mode;
+    double rho[16];          /* g/cm^3 per material */
 } orc_scene;
 
 typedef struct {
@@ -428,10 +434,50 @@ void orc_test_rotate(const double *d_in, double c, double phi, double *d_out) {
 /* ------------------------------------------------------------------ one history (O4 .. O14) */
 typedef struct {
     double dep_scoring, dep_other, e_escaped;
-    uint32_t flags, n_events;
+    uint32_t flags, n_events, n_electrons;
 } orc_hist;
 
 typedef struct { double pos[3], dir[3], e; int m; uint32_t stream; } orc_photon;
+
+/* Electron range, Katz & Penfold (1952): R [mg/cm^2] = 412 T^n, n = 1.265 - 0.0954 ln T, T in MeV; in mm for the
+ * material's density.  DESIGN.md reading R16. */
+double orc_electron_range_mm(double t_mev, double rho_g_cm3) {
+    if (!(t_mev > 0.0) || !(rho_g_cm3 > 0.0)) return 0.0;
+    double n = 1.265 - 0.0954 * log(t_mev);
+    return 412.0 * pow(t_mev, n) / (100.0 * rho_g_cm3);
+}
+
+/* Energy `t_kin` set free as one electron at `pos` in material m.  Local deposit (O9/O10/O12) unless the electron mode
+ * is on: then the energy is laid down uniformly along a straight segment of the CSDA range in a direction drawn
+ * isotropically from stream 3 of the history (draws 2k, 2k+1 for the k-th electron); the segment is cut at the first
+ * facet that has m on its from-side, what is left goes to the material behind that facet, on the spot (lost if KILL). */
+static void deposit(const orc_scene *s, orc_hist *h, const double pos[3], int m, double t_kin, uint64_t seed,
+                    uint64_t history, uint32_t *n_electrons, orc_counters *cnt) {
+    double in_m = t_kin, beyond = 0.0;
+    int m2 = m;
+    if (s->electron_mode) {
+        double range = orc_electron_range_mm(t_kin, s->rho[m]);
+        orc_rng g = {seed, history, 3, 2u * (*n_electrons)};
+        (*n_electrons)++;
+        double u[3];
+        sample_isotropic(&g, u);
+        if (range > 0.0) {
+            double t = INFINITY; int leaving = 0;
+            cnt->n_queries++;
+            int hit = nearest_hit(s, pos, u, m, 0.0, &t, &leaving, cnt);
+            if (hit >= 0 && t < range) {
+                in_m = t_kin * (t / range); beyond = t_kin - in_m;
+                int k = s->tri_surface[hit];
+                m2 = leaving ? s->surf_out[k] : s->surf_in[k];
+            }
+        }
+    }
+    if (s->is_scoring[m]) h->dep_scoring += in_m; else { h->dep_other += in_m; h->flags |= ORC_F_NONSCORING; }
+    if (beyond > 0.0) {
+        if (m2 != ORC_MAT_KILL && s->is_scoring[m2]) h->dep_scoring += beyond;
+        else { h->dep_other += beyond; h->flags |= ORC_F_NONSCORING; }
+    }
+}
 
 /* O7-O12 for one photon; secondaries (pair) are appended to `stack` */
 static void transport_photon(const orc_scene *s, orc_photon ph, uint64_t seed, uint64_t history, uint32_t draw0,
@@ -462,10 +508,9 @@ static void transport_photon(const orc_scene *s, orc_photon ph, uint64_t seed, u
         }
         /* O7.4 interaction at pos + s d */
         for (int a = 0; a < 3; ++a) ph.pos[a] += sdist * ph.dir[a];
-        int scoring = s->is_scoring[ph.m];
         h->n_events++;
         if (ph.e < ORC_ECUT) {                                          /* O8 cut-off */
-            if (scoring) h->dep_scoring += ph.e; else { h->dep_other += ph.e; h->flags |= ORC_F_NONSCORING; }
+            deposit(s, h, ph.pos, ph.m, ph.e, seed, history, &h->n_electrons, cnt);
             cnt->n_cutoff++;
             return;
         }
@@ -474,7 +519,7 @@ static void transport_photon(const orc_scene *s, orc_photon ph, uint64_t seed, u
         for (int c = 0; c < 4; ++c) { acc += mu[c]; if (u < acc) { ch = c; break; } }
         if (ch < 0) { for (int c = 3; c >= 0; --c) if (mu[c] > 0.0) { ch = c; break; } }
         if (ch == 0) {                                                  /* O9 photoelectric */
-            if (scoring) h->dep_scoring += ph.e; else { h->dep_other += ph.e; h->flags |= ORC_F_NONSCORING; }
+            deposit(s, h, ph.pos, ph.m, ph.e, seed, history, &h->n_electrons, cnt);
             cnt->n_pe++;
             return;
         } else if (ch == 1) {                                           /* O10 Compton */
@@ -482,12 +527,12 @@ static void transport_photon(const orc_scene *s, orc_photon ph, uint64_t seed, u
             double eps = sample_compton(&g, ph.e, &cost);
             double phi = ORC_TWO_PI * rng_next(&g);
             double e_new = eps * ph.e, dep = ph.e - e_new;
-            if (scoring) h->dep_scoring += dep; else { h->dep_other += dep; h->flags |= ORC_F_NONSCORING; }
+            deposit(s, h, ph.pos, ph.m, dep, seed, history, &h->n_electrons, cnt);
             rotate_dir(ph.dir, cost, phi);
             ph.e = e_new;
             cnt->n_compton++;
             if (ph.e < ORC_ECUT) {
-                if (scoring) h->dep_scoring += ph.e; else { h->dep_other += ph.e; h->flags |= ORC_F_NONSCORING; }
+                deposit(s, h, ph.pos, ph.m, ph.e, seed, history, &h->n_electrons, cnt);
                 cnt->n_cutoff++;
                 return;
             }
@@ -498,7 +543,7 @@ static void transport_photon(const orc_scene *s, orc_photon ph, uint64_t seed, u
             cnt->n_coherent++;
         } else {                                                        /* O12 pair */
             double dep = ph.e - 2.0 * ORC_MEC2;
-            if (scoring) h->dep_scoring += dep; else { h->dep_other += dep; h->flags |= ORC_F_NONSCORING; }
+            deposit(s, h, ph.pos, ph.m, dep, seed, history, &h->n_electrons, cnt);
             double ax[3];
             sample_isotropic(&g, ax);
             cnt->n_pair++;
@@ -554,6 +599,26 @@ static int run_history(const orc_scene *s, uint64_t seed, uint64_t history, orc_
 static void add_counters(orc_counters *a, const orc_counters *b) {
     uint64_t *x = (uint64_t *)a; const uint64_t *y = (const uint64_t *)b;
     for (size_t i = 0; i < sizeof(orc_counters) / sizeof(uint64_t); ++i) x[i] += y[i];
+}
+
+/* NEXT-4: switch the straight-segment electron model on (densities in g/cm^3 per material) or off (rho == NULL) */
+int orc_set_electron_mode(orc_scene *s, const double *rho, int n_mat) {
+    if (!s || n_mat > 16) return -1;
+    s->electron_mode = rho != NULL;
+    for (int m = 0; m < n_mat && rho; ++m) s->rho[m] = rho[m];
+    return 0;
+}
+
+/* test hook: fraction of t_kin that stays in material m for electrons number 0 of histories first .. first+n-1 */
+void orc_test_electron_split(const orc_scene *s, const double *pos, int m, double t_kin, uint64_t seed, uint64_t first,
+                             long long n, double *frac_in_m) {
+    orc_counters cnt; memset(&cnt, 0, sizeof(cnt));
+    for (long long i = 0; i < n; ++i) {
+        orc_hist h; memset(&h, 0, sizeof(h));
+        deposit(s, &h, pos, m, t_kin, seed, first + (uint64_t)i, &h.n_electrons, &cnt);
+        /* in_m is whichever of the two tallies material m feeds; the rest went beyond the facet */
+        frac_in_m[i] = (s->is_scoring[m] ? h.dep_scoring : h.dep_other) / t_kin;
+    }
 }
 
 /* per-history dump (parity T4).  Any output pointer may be NULL. */

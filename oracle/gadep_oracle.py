@@ -62,7 +62,17 @@ def lib():
         L.orc_run_histories.argtypes = [vp, u64, ll, u64, vp, vp, vp, vp, vp]
         L.orc_run.argtypes = [vp, u64, ll, u64, i32, dbl, vp, vp, vp, vp]
         L.orc_num_threads.restype = i32
+        L.orc_set_electron_mode.argtypes = [vp, vp, i32]
+        L.orc_electron_range_mm.argtypes = [dbl, dbl]
+        L.orc_electron_range_mm.restype = dbl
+        L.orc_test_electron_split.argtypes = [vp, vp, i32, dbl, u64, u64, ll, vp]
+        L.orc_test_electron_split.restype = None
     return _lib
+
+
+def electron_range_mm(t_mev: float, rho_g_cm3: float) -> float:
+    """Katz-Penfold range of an electron of kinetic energy t_mev in a material of that density (R16)."""
+    return float(lib().orc_electron_range_mm(float(t_mev), float(rho_g_cm3)))
 
 
 def _p(a):
@@ -198,6 +208,21 @@ class OracleScene:
         o = np.ascontiguousarray(o, dtype=np.float64)
         d = np.ascontiguousarray(d, dtype=np.float64)
         return self.L.orc_locate_parity(self.h, _p(o), _p(d))
+
+    def set_electron_mode(self, rho):
+        """NEXT-4: straight CSDA electron segments instead of local deposit; rho = g/cm^3 per material, None = off."""
+        if rho is None:
+            assert self.L.orc_set_electron_mode(self.h, None, 0) == 0
+        else:
+            r = np.ascontiguousarray(rho, dtype=np.float64)
+            assert self.L.orc_set_electron_mode(self.h, _p(r), len(r)) == 0
+
+    def electron_split(self, pos, m, t_kin, seed, first, n):
+        """Fraction of t_kin that stays in material m for electron 0 of histories first .. first+n-1 (test hook)."""
+        out = np.empty(n)
+        p = np.ascontiguousarray(pos, dtype=np.float64)
+        self.L.orc_test_electron_split(self.h, _p(p), int(m), float(t_kin), seed, first, n, _p(out))
+        return out
 
     def run_histories(self, first, n, seed, details=False):
         edep = np.empty(n)

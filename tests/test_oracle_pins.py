@@ -414,3 +414,64 @@ def test_two_seeds_agree_statistically():
     m = (a + b) >= 20
     chi2 = ((a[m] - b[m]) ** 2 / (a[m] + b[m])).sum() / m.sum()
     assert chi2 < 1.8
+
+
+# ------------------------------------------------------------------ NEXT-4: straight CSDA electron segments (R16)
+def test_electron_range_katz_penfold_values():
+    # R = 412 T^(1.265 - 0.0954 ln T) mg/cm^2: at 1 MeV the exponent does not matter (412 mg/cm^2), at 0.5 MeV the
+    # textbook value is 0.164 g/cm^2 (aluminium range tables: 0.16 - 0.17), the range scales with 1/density
+    assert orc.electron_range_mm(1.0, 1.0) == pytest.approx(4.12, rel=1e-12)            # 412 mg/cm^2 = 4.12 mm of water
+    assert orc.electron_range_mm(1.0, 5.323) == pytest.approx(4.12 / 5.323, rel=1e-12)
+    assert orc.electron_range_mm(0.5, 1.0) == pytest.approx(1.637, rel=2e-3)
+    assert orc.electron_range_mm(0.1, 1.0) == pytest.approx(0.1350, rel=2e-3)
+    assert orc.electron_range_mm(0.0, 1.0) == 0.0 and orc.electron_range_mm(1.0, 0.0) == 0.0
+    r = [orc.electron_range_mm(t, 2.7) for t in np.geomspace(0.01, 2.5, 40)]
+    assert (np.diff(r) > 0).all()                                                        # monotonic in the energy
+
+
+def test_electron_split_below_a_plane_face_matches_closed_form():
+    # A point at depth d below the flat top of the bare Ge cylinder (config 0; the range is far below its radius).
+    # Isotropic straight segments of length R, uniform energy loss: a direction with cosine c towards the face keeps
+    # the fraction min(1, a / c), a = d / R, inside; averaged over the sphere: 1/2 + a (1 - ln a) / 2 for a < 1.
+    w = dm.make_config(0)
+    s = orc.OracleScene(w)
+    s.set_electron_mode(dm.DENSITY_G_CM3)
+    t_kin = 1.0
+    R = orc.electron_range_mm(t_kin, 5.323)
+    n = 40_000
+    for a in (0.1, 0.35, 0.8):
+        f = s.electron_split([0.3, -0.2, -a * R], dm.MAT["Ge_active"], t_kin, 5, 0, n)
+        assert (f >= 0).all() and (f <= 1 + 1e-12).all()
+        exact = 0.5 + 0.5 * a * (1.0 - math.log(a))
+        # variance of the kept fraction is below 1/4
+        assert f.mean() == pytest.approx(exact, abs=4 * 0.5 / math.sqrt(n)), (a, f.mean(), exact)
+        assert (f < 1 - 1e-9).mean() == pytest.approx(0.5 * (1 - a), abs=4 * 0.5 / math.sqrt(n))   # solid angle of c > a
+    f = s.electron_split([0.0, 0.0, -30.0], dm.MAT["Ge_active"], t_kin, 5, 0, 2000)      # deep inside: nothing leaves
+    assert (f == 1.0).all()
+    s.set_electron_mode(None)
+    f = s.electron_split([0.0, 0.0, -0.1 * R], dm.MAT["Ge_active"], t_kin, 5, 0, 2000)   # mode off: local deposit
+    assert (f == 1.0).all()
+
+
+def test_electron_mode_leaves_the_photons_alone_and_only_removes_energy():
+    # The electrons draw from their own stream: same photon trajectories, so per history the flags other than
+    # PEAK / NONSCORING, the event count and the escaped energy are unchanged, and with a single scoring volume in
+    # vacuum the scored energy can only go down.
+    w = dm.make_config(0)
+    s = orc.OracleScene(w)
+    n = 600_000
+    e0, f0, o0, x0, c0 = s.run_histories(0, n, w.seed, details=True)
+    s.set_electron_mode(dm.DENSITY_G_CM3)
+    e1, f1, o1, x1, c1 = s.run_histories(0, n, w.seed, details=True)
+    keep = ~np.uint32(orc.F_PEAK | orc.F_NONSCORING)
+    assert np.array_equal(f0 & keep, f1 & keep) and np.array_equal(x0, x1)
+    for k in ("n_pe", "n_compton", "n_coherent", "n_pair", "n_crossings", "n_escaped"):
+        assert c0[k] == c1[k]
+    line = w.source["line_mev"][0]
+    d0 = np.where(f0 & orc.F_PEAK, line, e0)
+    d1 = np.where(f1 & orc.F_PEAK, line, e1)
+    assert (d1 <= d0 + 1e-12).all()
+    lost = d0 - d1
+    assert (lost > 1e-9).sum() >= 5                          # some electrons do reach the surface (R = 0.5 mm at 662 keV)
+    assert np.allclose(d1 + o1 + x1, d0 + o0 + x0, atol=1e-9)    # energy is moved between tallies, not created
+    assert ((f1 & orc.F_PEAK) != 0).sum() < ((f0 & orc.F_PEAK) != 0).sum()
