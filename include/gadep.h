@@ -116,6 +116,11 @@ int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
                                    /* optical depth per process instead of total-mu sampling + a selection draw  */
                                    /* (history-per-thread kernel; same distribution, different random streams)   */
 #define GADEP_RUN_WARP_SPECIALISED 64 /* measurement: physics and traversal on separate warps of a block (same results) */
+#define GADEP_RUN_ELECTRON_RANGE 128 /* SURVEY.md 8(f) NEXT-4 (coupled photon-electron physics): every   */
+                                   /* energy deposit becomes one electron, a straight segment of the Katz-Penfold   */
+                                   /* range in an isotropic direction (Philox stream 3), cut at the first facet of  */
+                                   /* its material; the rest goes to the material behind it.  History-per-thread    */
+                                   /* kernel; needs gadep_set_densities.  DESIGN.md reading R16.                    */
 typedef struct {
     int n_bins;                    /* spectrum bins over [0, e_max_mev); one extra overflow slot follows        */
     float e_max_mev;
@@ -173,10 +178,19 @@ int gadep_trace_rays(gadep_ctx *ctx, const float *org, const float *dir, long lo
 #define GADEP_LOCATE_OVERFLOW (-3)
 int gadep_locate(gadep_ctx *ctx, const float *org, const float *dir, long long n, int mode, int *material_out);
 
+/*
+ * Densities of the materials [g/cm^3], HOST float[n_mat] (n_mat as in gadep_set_materials); used only by
+ * GADEP_RUN_ELECTRON_RANGE to turn the Katz-Penfold range (mg/cm^2) into millimetres.  0 = no electron transport there.
+ */
+int gadep_set_densities(gadep_ctx *ctx, int n_mat, const float *rho_g_cm3);
+
 /* Per-history dump (same arithmetic as gadep_run): edep_out float[n] scoring deposit (line energy for
  * full-absorption histories), flags_out unsigned[n] (GADEP_F_*).  HOST-or-DEVICE, either may be NULL. */
 int gadep_run_histories(gadep_ctx *ctx, unsigned long long first, long long n, unsigned long long seed,
                         float *edep_out, unsigned *flags_out);
+/* The same with the kernel-selecting GADEP_RUN_* flags of gadep_run (ASYNC and ACCUMULATE are ignored). */
+int gadep_run_histories_ex(gadep_ctx *ctx, unsigned long long first, long long n, unsigned long long seed,
+                           int run_flags, float *edep_out, unsigned *flags_out);
 
 typedef struct {
     unsigned long long n_histories, n_queries, n_box_tests, n_tri_tests, n_crossings, n_pe, n_compton, n_coherent,

@@ -19,10 +19,12 @@ MAX_LINES = 64
 RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES, RUN_PARITY_LOCALISATION = 1, 2, 4, 8, 16
 RUN_PARTIAL_XS = 32
 RUN_WARP_SPECIALISED = 64
+RUN_ELECTRON_RANGE = 128
 
 EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_set_materials", "gadep_load_mesh",
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
-                    "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw", "gadep_locate", "gadep_broaden")
+                    "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw", "gadep_locate", "gadep_broaden",
+                    "gadep_set_densities", "gadep_run_histories_ex")
 
 
 class GadepError(RuntimeError):
@@ -99,6 +101,8 @@ def load_library(build_if_missing: bool = True):
     L.gadep_fepe.argtypes = [vp, i32, i32, C.POINTER(dbl), C.POINTER(dbl)]
     L.gadep_trace_rays.argtypes = [vp, vp, vp, ll, i32, f32, vp, vp]
     L.gadep_run_histories.argtypes = [vp, ull, ll, ull, vp, vp]
+    L.gadep_run_histories_ex.argtypes = [vp, ull, ll, ull, C.c_int, vp, vp]
+    L.gadep_set_densities.argtypes = [vp, C.c_int, vp]
     L.gadep_get_counters.argtypes = [vp, C.POINTER(GadepCounters)]
     L.gadep_philox_raw.argtypes = [vp, vp, vp, i32, vp]
     L.gadep_locate.argtypes = [vp, vp, vp, ll, i32, vp]
@@ -241,10 +245,16 @@ class Gadep:
         self._check(self.L.gadep_locate(self.h, _ptr(org), _ptr(dir), org.shape[0], int(mode), _ptr(material_out)))
         return material_out
 
-    def run_histories(self, first, n, seed):
+    def set_densities(self, rho_g_cm3):
+        rho = np.ascontiguousarray(rho_g_cm3, dtype=np.float32)
+        self._check(self.L.gadep_set_densities(self.h, int(len(rho)), _np_ptr(rho)))
+
+    def run_histories(self, first, n, seed, flags=0):
         edep = np.empty(n, dtype=np.float32)
+        run_flags = int(flags)
         flags = np.empty(n, dtype=np.uint32)
-        self._check(self.L.gadep_run_histories(self.h, int(first), int(n), int(seed), _np_ptr(edep), _np_ptr(flags)))
+        self._check(self.L.gadep_run_histories_ex(self.h, int(first), int(n), int(seed), run_flags, _np_ptr(edep),
+                                                  _np_ptr(flags)))
         return edep, flags
 
     def get_counters(self) -> dict:

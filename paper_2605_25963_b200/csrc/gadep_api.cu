@@ -60,6 +60,8 @@ struct gadep_ctx {
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
     GdWaveTune tune = {8, 4, 4, 4.0f, 8.0f, 12};
+    float rho[GADEP_MAX_MATERIALS] = {};      // g/cm^3, electron-range mode
+    bool have_rho = false;
     // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
     std::vector<int> h_sides;                 // [n_surf][2] inside, outside
     int *d_mat_entry = nullptr;               // [GADEP_MAX_MATERIALS][1 + GD_ENTRY_MAX], see GdBvh
@@ -477,6 +479,7 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     M.inv_dln = (float)((c->n_grid - 1) / (std::log(c->e_max) - std::log(c->e_min)));
     M.e_cut = (float)c->e_min;
     M.table = c->d_table; M.scoring_mask = c->scoring_mask; M.world_material = c->world;
+    for (int m = 0; m < GADEP_MAX_MATERIALS; ++m) M.rho[m] = c->rho[m];
     GdTally T;
     T.spectrum = c->d_tally; T.emitted = c->d_tally + n_bins + 1; T.peak = T.emitted + GADEP_MAX_LINES;
     T.counters = c->d_counters; T.n_bins = n_bins; T.inv_de = (float)((double)n_bins / (double)e_max);
@@ -490,7 +493,8 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     const void *kern = variant == 5 ? (const void *)gd_k_transport_ws : variant == 2 ? (const void *)gd_k_transport_wave
                                     : (variant == 1 ? (const void *)gd_k_transport_refill
                                                   : (variant == 3 ? (const void *)gd_k_transport<true, false>
-                                                     : (variant == 4 ? (const void *)gd_k_transport<false, true> : (const void *)gd_k_transport<false, false>)));
+                                                     : (variant == 4 ? (const void *)gd_k_transport<false, true>
+                                                        : (variant == 6 ? (const void *)gd_k_transport<false, false, true> : (const void *)gd_k_transport<false, false>))));
     GD_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
@@ -527,6 +531,8 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
             gd_k_transport<true, false><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
         } else if (variant == 4) {
             gd_k_transport<false, true><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
+        } else if (variant == 6) {
+            gd_k_transport<false, false, true><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
         } else {
             gd_k_transport<false, false><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags);
         }
@@ -555,6 +561,23 @@ static int gd_fetch_results(gadep_ctx *c) {
     return GADEP_OK;
 }
 
+static int gd_variant_of(int flags) {
+    return (flags & GADEP_RUN_ELECTRON_RANGE) ? 6 : (flags & GADEP_RUN_WARP_SPECIALISED) ? 5 : (flags & GADEP_RUN_PARTIAL_XS) ? 4
+           : (flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
+}
+
+extern "C" int gadep_set_densities(gadep_ctx *c, int n_mat, const float *rho_g_cm3) {
+    if (!c) return GADEP_E_NULL;
+    if (!rho_g_cm3) return gd_fail(c, GADEP_E_NULL, "null density array");
+    if (n_mat <= 0 || n_mat > GADEP_MAX_MATERIALS || (c->have_mat && n_mat != c->n_mat))
+        return gd_fail(c, GADEP_E_ARG, "n_mat %d does not match the materials", n_mat);
+    for (int m = 0; m < n_mat; ++m)
+        if (!(rho_g_cm3[m] >= 0.0f) || !std::isfinite(rho_g_cm3[m])) return gd_fail(c, GADEP_E_ARG, "material %d: bad density", m);
+    for (int m = 0; m < GADEP_MAX_MATERIALS; ++m) c->rho[m] = m < n_mat ? rho_g_cm3[m] : 0.0f;
+    c->have_rho = true;
+    return GADEP_OK;
+}
+
 extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned long long seed, const gadep_run_opts *opts,
                          unsigned long long *spectrum) {
     if (!c) return GADEP_E_NULL;
@@ -562,7 +585,9 @@ extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned 
     bool dev_out = gd_is_device_ptr(spectrum);
     if ((opts->flags & GADEP_RUN_ASYNC) && spectrum && !dev_out)
         return gd_fail(c, GADEP_E_ARG, "GADEP_RUN_ASYNC needs a device spectrum pointer");
-    c->kernel_variant = (opts->flags & GADEP_RUN_WARP_SPECIALISED) ? 5 : (opts->flags & GADEP_RUN_PARTIAL_XS) ? 4 : (opts->flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((opts->flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((opts->flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
+    if ((opts->flags & GADEP_RUN_ELECTRON_RANGE) && !c->have_rho)
+        return gd_fail(c, GADEP_E_ORDER, "GADEP_RUN_ELECTRON_RANGE needs gadep_set_densities");
+    c->kernel_variant = gd_variant_of(opts->flags);
     int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
                                  (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
     if (rc) return rc;
@@ -726,10 +751,19 @@ extern "C" int gadep_broaden(gadep_ctx *c, double fwhm_a, double fwhm_b, double 
     return GADEP_OK;
 }
 
+extern "C" int gadep_run_histories_ex(gadep_ctx *c, unsigned long long first, long long n, unsigned long long seed,
+                                      int run_flags, float *edep_out, unsigned *flags_out);
 extern "C" int gadep_run_histories(gadep_ctx *c, unsigned long long first, long long n, unsigned long long seed,
                                    float *edep_out, unsigned *flags_out) {
+    return gadep_run_histories_ex(c, first, n, seed, 0, edep_out, flags_out);
+}
+
+extern "C" int gadep_run_histories_ex(gadep_ctx *c, unsigned long long first, long long n, unsigned long long seed,
+                                      int run_flags, float *edep_out, unsigned *flags_out) {
     if (!c) return GADEP_E_NULL;
     if (n < 0) return gd_fail(c, GADEP_E_ARG, "negative history count");
+    if ((run_flags & GADEP_RUN_ELECTRON_RANGE) && !c->have_rho)
+        return gd_fail(c, GADEP_E_ORDER, "GADEP_RUN_ELECTRON_RANGE needs gadep_set_densities");
     GD_CUDA(c, cudaSetDevice(c->device));
     bool dev_e = gd_is_device_ptr(edep_out), dev_f = gd_is_device_ptr(flags_out);
     float *d_e = edep_out;
@@ -740,7 +774,7 @@ extern "C" int gadep_run_histories(gadep_ctx *c, unsigned long long first, long 
     if (flags_out && !dev_f && n > 0) { GD_CUDA(c, cudaMalloc(&stage_f, sizeof(unsigned) * (size_t)n)); d_f = stage_f; }
     int n_bins = c->n_bins > 0 ? c->n_bins : 4096;
     float e_max = c->spec_e_max > 0 ? c->spec_e_max : 2.0f;
-    c->kernel_variant = 2;       // always the default kernel, whatever the last gadep_run asked for
+    c->kernel_variant = gd_variant_of(run_flags & ~(GADEP_RUN_ASYNC | GADEP_RUN_ACCUMULATE));   // 0: the default kernel
     int rc = gd_launch_transport(c, first, (unsigned long long)n, seed, n_bins, e_max, false, d_e, d_f);
     if (rc == GADEP_OK) rc = gd_fetch_results(c);
     if (rc == GADEP_OK && stage_e) cudaMemcpy(edep_out, stage_e, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost);

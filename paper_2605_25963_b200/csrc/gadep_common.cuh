@@ -87,6 +87,7 @@ struct GdMaterials {
     const float *table;             // device [n_mat][4][n_grid]: ln(mu) for channels 0..2 (-1e30 = zero), mu for 3
     unsigned scoring_mask;          // bit m set = material m scores
     int world_material;
+    float rho[16];                  // g/cm^3 per material (electron-range mode only, R16)
 };
 
 struct GdVec3 {

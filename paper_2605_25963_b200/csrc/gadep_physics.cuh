@@ -118,6 +118,12 @@ GD_HD void gd_deposit(const GdMaterials &M, int m, float e, float &dep, unsigned
     if ((M.scoring_mask >> m) & 1u) dep += e;
     else flags |= GD_F_NONSCORING;
 }
+// Katz & Penfold: R [mg/cm^2] = 412 T^(1.265 - 0.0954 ln T); in mm for the material's density (R16)
+GD_HD float gd_electron_range_mm(float t_mev, float rho) {
+    if (!(t_mev > 0.0f) || !(rho > 0.0f)) return 0.0f;
+    const float lt = logf(t_mev);
+    return 412.0f * expf((1.265f - 0.0954f * lt) * lt) / (100.0f * rho);
+}
 
 // ---------------------------------------------------------------- lane state machine
 // One lane carries one history at a time; every step of a live lane issues exactly one nearest-hit query
@@ -146,6 +152,12 @@ struct GdLane {
     // partial cross-section method only: remaining optical depth of every process, process that fires next
     float tau_c[4];
     int sel;
+    // electron-range mode only (R16): energies set free at el_pos in material el_m by the last
+    // gd_lane_post call, waiting for their segments; running number of the history's electrons
+    int el_n, el_m;
+    float el_T[2];
+    GdVec3 el_pos;
+    unsigned el_count;
 };
 
 // O4: source sampling on stream 0; leaves the lane in mode LOCATE
@@ -234,8 +246,26 @@ GD_HD bool gd_lane_next_photon_t(GdLane &L, unsigned long long seed) {
     return false;
 }
 
-// consume the query result; returns true when the history is finished (out is then valid)
-template <bool PARTIAL>
+// O14: flags and scoring deposit of a finished history
+GD_HD void gd_lane_finish(GdLane &L, const GdSource &S, GdHistory &out) {
+    if (!(L.flags & (GD_F_ESCAPED | GD_F_NONSCORING))) { L.flags |= GD_F_PEAK; L.dep = S.line_mev[L.line]; }
+    L.flags &= ~GD_F_RELOC;
+    L.flags |= ((unsigned)L.line & 0xFFu) << 8;
+    L.flags |= (L.n_events > 0xFFFFu ? 0xFFFFu : L.n_events) << 16;
+    out.edep = L.dep; out.flags = L.flags; out.line = L.line;
+    L.mode = GD_MODE_NEED;
+}
+
+// an energy deposit: at once, or (ELECTRON, R16) noted for the caller, who lays it along an electron segment
+#define GD_DEPOSIT(e_)                                                                         \
+    do {                                                                                       \
+        if (ELECTRON) { L.el_T[L.el_n++] = (e_); L.el_m = L.m; L.el_pos = L.pos; }             \
+        else gd_deposit(M, L.m, (e_), L.dep, L.flags);                                         \
+    } while (0)
+
+// consume the query result; returns true when the history is finished (out is then valid; with ELECTRON the caller
+// first resolves the noted deposits and then calls gd_lane_finish itself)
+template <bool PARTIAL, bool ELECTRON = false>
 GD_HD bool gd_lane_post_t(GdLane &L, const GdMaterials &M, const float *tab, const GdSource &S, unsigned long long seed,
                           const GdHit &hit_in, GdHistory &out, GdLocalCounters &cnt) {
     GdHit hit = hit_in;
@@ -283,7 +313,7 @@ GD_HD bool gd_lane_post_t(GdLane &L, const GdMaterials &M, const float *tab, con
         L.pos.x += L.sdist * L.dir.x; L.pos.y += L.sdist * L.dir.y; L.pos.z += L.sdist * L.dir.z;
         L.n_events++;
         L.ex = gd_no_exclude(); L.n_stall = 0;                            // new flight segment
-        if (L.e < M.e_cut) { gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_cutoff++; photon_done = true; }
+        if (L.e < M.e_cut) { GD_DEPOSIT(L.e); cnt.n_cutoff++; photon_done = true; }
         else {
             GdF4u u4 = gd_rng_peek4(L.g);             // selection draw + the three draws of a coherent event
             bool tau_done = false;
@@ -300,19 +330,19 @@ GD_HD bool gd_lane_post_t(GdLane &L, const GdMaterials &M, const float *tab, con
                 if (ch < 0) ch = L.mu[3] > 0.0f ? 3 : (L.mu[2] > 0.0f ? 2 : (L.mu[1] > 0.0f ? 1 : 0));
             }
             if (ch == 0) {                                                                  // O9 photoelectric
-                gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_pe++;
+                GD_DEPOSIT(L.e); cnt.n_pe++;
                 photon_done = true;
             } else if (ch == 1) {                                                           // O10 Compton
                 float cost;
                 float eps = gd_sample_compton(L.g, L.e, cost);
                 float uphi = gd_rng_next(L.g);
                 float e_new = eps * L.e;
-                gd_deposit(M, L.m, L.e - e_new, L.dep, L.flags);
+                GD_DEPOSIT(L.e - e_new);
                 L.dir = gd_rotate(L.dir, cost, uphi);
                 L.e = e_new;
                 cnt.n_compton++;
                 L.need_mu = 1;
-                if (L.e < M.e_cut) { gd_deposit(M, L.m, L.e, L.dep, L.flags); cnt.n_cutoff++; photon_done = true; }
+                if (L.e < M.e_cut) { GD_DEPOSIT(L.e); cnt.n_cutoff++; photon_done = true; }
             } else if (ch == 2) {                                                           // O11 coherent
                 const float cost = gd_thomson_from(u4.b);
                 L.dir = gd_rotate(L.dir, cost, u4.c);
@@ -321,7 +351,7 @@ GD_HD bool gd_lane_post_t(GdLane &L, const GdMaterials &M, const float *tab, con
                 L.g.draw += 3;
                 cnt.n_coherent++;
             } else {                                                                        // O12 pair
-                gd_deposit(M, L.m, L.e - GD_TWO_MEC2, L.dep, L.flags);
+                GD_DEPOSIT(L.e - GD_TWO_MEC2);
                 L.p_axis = gd_sample_isotropic(L.g);
                 L.p_pos = L.pos; L.p_m = L.m; L.pending = 2;
                 cnt.n_pair++;
@@ -335,12 +365,7 @@ GD_HD bool gd_lane_post_t(GdLane &L, const GdMaterials &M, const float *tab, con
     if (!photon_done) return false;
     if (!gd_lane_next_photon_t<PARTIAL>(L, seed)) return false;
     // ---- O14
-    if (!(L.flags & (GD_F_ESCAPED | GD_F_NONSCORING))) { L.flags |= GD_F_PEAK; L.dep = S.line_mev[L.line]; }
-    L.flags &= ~GD_F_RELOC;
-    L.flags |= ((unsigned)L.line & 0xFFu) << 8;
-    L.flags |= (L.n_events > 0xFFFFu ? 0xFFFFu : L.n_events) << 16;
-    out.edep = L.dep; out.flags = L.flags; out.line = L.line;
-    L.mode = GD_MODE_NEED;
+    if (!ELECTRON) gd_lane_finish(L, S, out);
     return true;
 }
 GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const GdSource &S, unsigned long long seed,
@@ -427,12 +452,14 @@ GD_HD int gd_locate_parity(const GdBvh &bvh, const GdRay &ray, const GdExclude &
 // PARITY: after the start localisation and after every boundary crossing the material comes from the parity rule
 // instead of the facet's side ids (the side ids still say where the KILL boundary is); mismatches between the two
 // rules are counted in cnt.n_cutoff's neighbour fields by the caller.
-template <bool PARITY, bool PARTIAL>
+// ELECTRON: deposits become straight electron segments (R16).
+template <bool PARITY, bool PARTIAL, bool ELECTRON = false>
 GD_HD void gd_run_history_t(const GdBvh &bvh, const GdMaterials &M, const float *tab, const GdSource &S,
                             unsigned long long seed, unsigned long long history, GdHistory &out, GdLocalCounters &cnt,
                             unsigned &n_parity, unsigned &n_mismatch) {
     GdLane L;
     gd_lane_start(L, S, seed, history);
+    L.el_n = 0; L.el_m = 0; L.el_count = 0;
     GdRay ray;
     GdHit hit;
     for (;;) {
@@ -457,7 +484,39 @@ GD_HD void gd_run_history_t(const GdBvh &bvh, const GdMaterials &M, const float 
                 }
             }
         }
-        if (gd_lane_post_t<PARTIAL>(L, M, tab, S, seed, hit, out, cnt)) return;
+        const bool finished = gd_lane_post_t<PARTIAL, ELECTRON>(L, M, tab, S, seed, hit, out, cnt);
+        if (ELECTRON) {
+            for (int k = 0; k < L.el_n; ++k) {
+                // the k-th electron of the history: isotropic direction from stream 3, segment of the CSDA range, cut
+                // at the first facet with the material on its from-side; the rest is left behind that facet
+                const float t_kin = L.el_T[k];
+                const float range = gd_electron_range_mm(t_kin, M.rho[L.el_m]);
+                const float u1 = gd_rng_uniform_v((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)history, (uint32_t)(history >> 32), 3u, 2u * L.el_count);
+                const float u2 = gd_rng_uniform_v((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)history, (uint32_t)(history >> 32), 3u, 2u * L.el_count + 1u);
+                L.el_count++;
+                float in_m = t_kin, beyond = 0.0f;
+                int m2 = L.el_m;
+                if (range > 0.0f) {
+                    GdRay er;
+                    GdHit eh;
+                    gd_ray_setup(er, L.el_pos, gd_isotropic_from(u1, u2));
+                    cnt.n_queries++;
+                    gd_nearest_hit<false>(bvh, er, 0.0f, range, L.el_m, gd_no_exclude(), true, eh, cnt.n_box_tests, cnt.n_tri_tests);
+                    if (eh.leaf >= 0 && eh.t < range) {
+                        in_m = t_kin * (fmaxf(eh.t, 0.0f) / range); beyond = t_kin - in_m;
+                        m2 = eh.leaving ? gd_mat_outside(eh.mats) : gd_mat_inside(eh.mats);
+                    }
+                }
+                gd_deposit(M, L.el_m, in_m, L.dep, L.flags);
+                if (beyond > 0.0f) {
+                    if (m2 >= 0) gd_deposit(M, m2, beyond, L.dep, L.flags);
+                    else L.flags |= GD_F_NONSCORING;          // left through the KILL boundary
+                }
+            }
+            L.el_n = 0;
+            if (finished) gd_lane_finish(L, S, out);
+        }
+        if (finished) return;
         if (PARITY && cnt.n_crossings != crossings_before && L.mode == GD_MODE_FLIGHT) {
             gd_ray_setup(ray, L.pos, L.dir);
             const int m_par = gd_locate_parity(bvh, ray, L.ex, M.world_material, cnt.n_box_tests, cnt.n_tri_tests);

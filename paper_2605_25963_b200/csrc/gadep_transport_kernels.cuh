@@ -55,7 +55,8 @@ gd_k_trace(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ d
 
 // dynamic shared memory: [table floats][spectrum u32 (n_bins+1)]
 // PARITY: material after the start and after every crossing from the paper's parity rule
-template <bool PARITY, bool PARTIAL>
+// ELECTRON: deposits as straight electron segments (R16)
+template <bool PARITY, bool PARTIAL, bool ELECTRON = false>
 __global__ void __launch_bounds__(GD_RUN_THREADS)
 gd_k_transport(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
                unsigned long long n_hist, unsigned long long seed, GdTally tally, float *__restrict__ edep_out,
@@ -77,7 +78,7 @@ gd_k_transport(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsig
     const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
     for (unsigned long long h = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; h < n_hist; h += stride) {
         GdHistory r;
-        gd_run_history_t<PARITY, PARTIAL>(bvh, M, s_tab, s_src, seed, first + h, r, cnt, n_parity, n_mismatch);
+        gd_run_history_t<PARITY, PARTIAL, ELECTRON>(bvh, M, s_tab, s_src, seed, first + h, r, cnt, n_parity, n_mismatch);
         n_done++;
         atomicAdd(&s_emitted[r.line], 1u);
         if (r.flags & GD_F_PEAK) {

@@ -316,6 +316,49 @@ def test_per_history_parity(pkg, orc, cfg, n):
         assert abs(pg - po) <= 3 + 0.01 * po
 
 
+@pytest.mark.parametrize("scene,n", [("cfg0", 400_000), ("cfg1", 40_000), ("pellets", 40_000)])
+def test_electron_range_mode_per_history_parity(pkg, orc, scene, n):
+    # deposits as straight electron segments of the Katz-Penfold range.  The
+    # electrons draw from their own Philox stream, so the photon side is the per-history parity above; here the split
+    # of every deposit at the first facet must agree too (float32 range and hit distance against double).
+    from paper_2605_25963_b200.binding import RUN_ELECTRON_RANGE
+    w = dm.make_pellet_stack(9, n_histories=n) if scene == "pellets" else dm.make_config(int(scene[3]))
+    g = pkg.Gadep(0)
+    g.load_workload(w)
+    s = orc.OracleScene(w)
+    with pytest.raises(pkg.GadepError) as e:                      # densities first
+        g.run_histories(0, 10, w.seed, flags=RUN_ELECTRON_RANGE)
+    assert e.value.code == -2
+    g.set_densities(dm.DENSITY_G_CM3)
+    s.set_electron_mode(dm.DENSITY_G_CM3)
+    edep0, flags0 = g.run_histories(0, n, w.seed)                 # local deposit, default kernel
+    edep, flags = g.run_histories(0, n, w.seed, flags=RUN_ELECTRON_RANGE)
+    c = g.get_counters()
+    oe, of, oc = s.run_histories(0, n, w.seed)
+    same = (flags == of) & (np.abs(edep.astype(np.float64) - oe) <= 2e-6 + 1e-5 * oe)
+    assert same.mean() >= 0.999, same.mean()
+    for k in ("n_queries", "n_crossings", "n_pe", "n_compton", "n_coherent", "n_escaped"):
+        assert abs(c[k] + (n if k == "n_queries" else 0) - oc[k]) <= 0.01 * oc[k] + 50, (k, c[k], oc[k])
+    # against the local-deposit run of the same histories: same photons (event count, line, escape bit) ...
+    keep = ~np.uint32(2 | 8)
+    assert np.array_equal(flags & keep, flags0 & keep)
+    # ... and electrons that leave the scoring volume do show up
+    changed = (np.abs(edep - edep0) > 1e-6) | ((flags ^ flags0) & 2 != 0)
+    assert changed.sum() >= 3, changed.sum()
+    if scene == "cfg0":                                           # one volume in vacuum: energy can only be lost
+        line = w.source["line_mev"][(flags >> 8) & 0xFF]
+        assert (edep <= edep0 + 1e-6).all() and (edep <= line * (1 + 1e-6)).all()
+    # the spectrum of gadep_run in this mode is the histogram of the dump
+    spec = g.run(n, w.seed, w.n_bins, w.spectrum_e_max_mev, flags=RUN_ELECTRON_RANGE)
+    de = w.spectrum_e_max_mev / w.n_bins
+    line, peak = (flags >> 8) & 0xFF, (flags & 2) != 0
+    bins = np.minimum(np.floor(np.float32(edep) * np.float32(w.n_bins / w.spectrum_e_max_mev)).astype(np.int64), w.n_bins)
+    lb = np.minimum(np.floor(w.source["line_mev"].astype(np.float64) / de).astype(np.int64), w.n_bins)
+    bins[peak] = lb[line[peak]]
+    ref = np.bincount(bins[edep.astype(np.float64) > 0], minlength=w.n_bins + 1)
+    assert np.array_equal(ref.astype(np.uint64), spec)
+
+
 def test_run_spectrum_equals_histogram_of_history_dump(pkg, orc):
     w, g, s = _setup(pkg, orc, 1)
     n = 200_000
