@@ -134,7 +134,7 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
     if (getenv("GADEP_NO_SURFACE_CLUSTERS")) c->cluster_surfaces = false;
     if (const char *t = getenv("GADEP_SPLIT_BUDGET")) { double b = atof(t); if (b >= 0 && b <= 15) c->split_budget = b; }
-    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,leaf_thresh" (measurement sweeps)
+    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,n_steps[,lam_max,cap_mfp,sparse_max]" (measurement sweeps)
         int a, b, d;
         float lm = c->tune.lam_max, cm = c->tune.cap_mfp;
         int sp = c->tune.sparse_max;
