@@ -22,7 +22,9 @@
 #define GD_W_THREADS 512
 #define GD_W_WARPS (GD_W_THREADS / 32)
 #define GD_W_SLOTS 64
-#define GD_W_NF 29
+// fields per slot; the facet-free sphere (25..28) only exists with GD_WITH_SAFETY.  Without it the block's shared
+// memory stays under the 164 KB carve-out for up to 9 materials, which leaves the SM a 64 KB L1 instead of 32 KB.
+#define GD_W_NF (GD_WITH_SAFETY ? 29 : 25)
 
 #ifdef GD_DIAG
 __device__ unsigned long long gd_diag[128];
@@ -62,7 +64,7 @@ GD_D void gd_slot_store(float *sl, int s, const GdLane &L, unsigned long long fi
     GD_SF(17) = L.dep;
     GD_SF(18) = __uint_as_float((L.flags & 0xFFu) | ((L.n_events > 0xFFFFu ? 0xFFFFu : L.n_events) << 16));
     GD_SF(19) = __int_as_float(L.ex.a); GD_SF(20) = __int_as_float(L.ex.b); GD_SF(21) = __int_as_float(L.ex.c);
-    GD_SF(25) = L.sc.x; GD_SF(26) = L.sc.y; GD_SF(27) = L.sc.z; GD_SF(28) = L.sr;
+    if (GD_WITH_SAFETY) { GD_SF(25) = L.sc.x; GD_SF(26) = L.sc.y; GD_SF(27) = L.sc.z; GD_SF(28) = L.sr; }
 }
 GD_D void gd_slot_load(const float *sl, int s, GdLane &L, unsigned long long seed, unsigned long long first) {
     L.pos = gd_make(GD_SF(0), GD_SF(1), GD_SF(2));
@@ -80,7 +82,8 @@ GD_D void gd_slot_load(const float *sl, int s, GdLane &L, unsigned long long see
     L.flags = fe & 0xFFu; L.n_events = fe >> 16;
     L.ex.a = __float_as_int(GD_SF(19)); L.ex.b = __float_as_int(GD_SF(20)); L.ex.c = __float_as_int(GD_SF(21));
     L.cool = (int)((st >> 24) & 7u); L.qkind = (int)((st >> 27) & 1u);
-    L.sc = gd_make(GD_SF(25), GD_SF(26), GD_SF(27)); L.sr = GD_SF(28);
+    if (GD_WITH_SAFETY) { L.sc = gd_make(GD_SF(25), GD_SF(26), GD_SF(27)); L.sr = GD_SF(28); }
+    else { L.sc = L.pos; L.sr = 0.0f; }
 }
 
 // What the slot does next (mode FLIGHT, sdist known).  Purely a scheduling decision: a skipped query is one whose
