@@ -256,9 +256,19 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                     const unsigned n_need = __popc(need_mask);
                     unsigned long long new_base = 0;
                     const bool refill = w_cur + n_need > w_end;
+                    unsigned my_chunk = chunk;
                     if (refill) {
-                        if (lane == 0) new_base = atomicAdd(next_history, (unsigned long long)chunk);
+                        // guided: towards the end of the launch the chunks shrink with what is left, so that the last
+                        // histories spread over all warps instead of going to the few that ask last
+                        if (lane == 0) {
+                            const unsigned long long cur = *(volatile unsigned long long *)next_history;
+                            const unsigned long long rem = cur < n_hist ? n_hist - cur : 0ull;
+                            const unsigned long long g = rem / ((unsigned long long)gridDim.x * GD_W_WARPS * 2ull);
+                            if (g < my_chunk) my_chunk = g < 32ull ? 32u : (unsigned)g;
+                            new_base = atomicAdd(next_history, (unsigned long long)my_chunk);
+                        }
                         new_base = __shfl_sync(0xFFFFFFFFu, new_base, 0);
+                        my_chunk = __shfl_sync(0xFFFFFFFFu, my_chunk, 0);
                     }
                     if (act && L.mode == GD_MODE_NEED) {
                         unsigned long long h = w_cur + __popc(need_mask & lt_mask);
@@ -266,7 +276,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                         if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
                         else L.mode = GD_MODE_DONE;
                     }
-                    if (refill) { w_cur = new_base + (w_cur + n_need - w_end); w_end = new_base + chunk; }
+                    if (refill) { w_cur = new_base + (w_cur + n_need - w_end); w_end = new_base + my_chunk; }
                     else w_cur += n_need;
                 }
                 // ---- prepare the next query: READY (ray / safety query), or the known answer "no facet"
