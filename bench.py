@@ -331,8 +331,8 @@ def main():
                 "clocks": clocks,
                 "roofline": {"bound": "alu", "kernel": "gd_k_transport_wave", "achieved": achieved, "peak": alu_peak,
                              "unit": "Tinstr/s (FP32 lane-instructions)", "frac": achieved / alu_peak,
-                             "traffic": 14558464 if args.config == 1 and n_hist == 10_000_000 else None,
-                             "traffic_source": "profiles/r01h_wave_kernel.md (ncu dram bytes of one launch)",
+                             "traffic": 14633984 if args.config == 1 and n_hist == 10_000_000 else None,
+                             "traffic_source": "profiles/r01k_wave_kernel.md (ncu dram bytes of one launch)",
                              "limiter": "L1 data pipe: l1tex__throughput 84 % of peak in the stand-alone traversal kernel, "
                                         "51 % over a whole 1e7-history launch (ncu, profiles/r01f_trace_kernel.md, r01h)",
                              "peak_source": f"{n_sm} SMs x 128 lanes x sm_max_mhz ({peak_src})",
