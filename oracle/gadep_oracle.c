@@ -224,7 +224,13 @@ static double mu_channel(const orc_scene *s, int m, int ch, double e) {
     double f = (log(e) - (s->ln_e0 + j * s->dln_e)) / s->dln_e;
     const double *t = s->mu + ((size_t)m * 4 + ch) * s->n_grid;
     double a = t[j], b = t[j + 1];
-    if (ch == 3) return (1.0 - f) * a + f * b;
+    if (ch == 3) {
+        /* pair production needs E > 2 m_e c^2 (PAPER.md:179 names the process; BASELINE.json configs[0]: "pair
+         * production 0 below 1.022 MeV").  The grid cell 1.00949-1.03885 MeV straddles the threshold, so the linear
+         * interpolation alone would leave mu_pair > 0 just below it (reading R17). */
+        if (e <= 2.0 * ORC_MEC2) return 0.0;
+        return (1.0 - f) * a + f * b;
+    }
     if (a <= 0.0 || b <= 0.0) return 0.0;
     return exp((1.0 - f) * log(a) + f * log(b));
 }
@@ -559,29 +565,49 @@ static void transport_photon(const orc_scene *s, orc_photon ph, uint64_t seed, u
     }
 }
 
-static int run_history(const orc_scene *s, uint64_t seed, uint64_t history, orc_hist *h, orc_counters *cnt) {
-    memset(h, 0, sizeof(*h));
-    orc_rng g = {seed, history, 0, 0};
-    /* O4 source */
-    double ul = rng_next(&g) * s->line_int_sum;
+/* O4: line by cumulative intensity (draw 0, always consumed), emission point, direction.  Returns the line. */
+static int sample_source(const orc_scene *s, orc_rng *g, orc_photon *ph) {
+    double ul = rng_next(g) * s->line_int_sum;
     int line = s->n_lines - 1; double acc = 0.0;
     for (int l = 0; l < s->n_lines; ++l) { acc += s->line_int[l]; if (ul < acc) { line = l; break; } }
-    orc_photon ph;
-    ph.e = s->line_mev[line]; ph.stream = 0;
+    ph->e = s->line_mev[line]; ph->stream = 0;
     if (s->src_kind == 1) {
         for (;;) {
-            double u1 = rng_next(&g), u2 = rng_next(&g), u3 = rng_next(&g);
+            double u1 = rng_next(g), u2 = rng_next(g), u3 = rng_next(g);
             double r = s->cyl_r * sqrt(u1), phi = ORC_TWO_PI * u2;
             double z = s->cyl_z0 + (s->cyl_z1 - s->cyl_z0) * u3;
             if (s->ex_r > 0.0 && r < s->ex_r && z >= s->ex_z0 && z <= s->ex_z1) continue;
-            ph.pos[0] = r * cos(phi); ph.pos[1] = r * sin(phi); ph.pos[2] = z;
+            ph->pos[0] = r * cos(phi); ph->pos[1] = r * sin(phi); ph->pos[2] = z;
             break;
         }
     } else {
-        memcpy(ph.pos, s->src_pos, sizeof(ph.pos));
+        memcpy(ph->pos, s->src_pos, sizeof(ph->pos));
     }
-    if (s->src_kind == 2) memcpy(ph.dir, s->src_dir, sizeof(ph.dir));
-    else sample_isotropic(&g, ph.dir);
+    if (s->src_kind == 2) memcpy(ph->dir, s->src_dir, sizeof(ph->dir));
+    else sample_isotropic(g, ph->dir);
+    return line;
+}
+
+/* test hook (pins of O4): line, emission point, direction and the index of the first draw after the source
+ * sampling (= draw of the first optical depth) for histories first .. first+n-1.  Any output may be NULL. */
+void orc_test_source(const orc_scene *s, uint64_t seed, uint64_t first, long long n, int *line_out, double *pos_out,
+                     double *dir_out, uint32_t *draw_out) {
+    for (long long i = 0; i < n; ++i) {
+        orc_rng g = {seed, first + (uint64_t)i, 0, 0};
+        orc_photon ph;
+        int line = sample_source(s, &g, &ph);
+        if (line_out) line_out[i] = line;
+        if (pos_out) memcpy(pos_out + 3 * i, ph.pos, sizeof(ph.pos));
+        if (dir_out) memcpy(dir_out + 3 * i, ph.dir, sizeof(ph.dir));
+        if (draw_out) draw_out[i] = g.draw;
+    }
+}
+
+static int run_history(const orc_scene *s, uint64_t seed, uint64_t history, orc_hist *h, orc_counters *cnt) {
+    memset(h, 0, sizeof(*h));
+    orc_rng g = {seed, history, 0, 0};
+    orc_photon ph;
+    int line = sample_source(s, &g, &ph);                               /* O4 */
     ph.m = locate_sideid(s, ph.pos, ph.dir, cnt);                       /* O5 */
     orc_photon stack[4]; int n_stack = 0;
     transport_photon(s, ph, seed, history, g.draw, h, stack, &n_stack, cnt);

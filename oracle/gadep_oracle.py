@@ -59,6 +59,8 @@ def lib():
         L.orc_test_isotropic.restype = None
         L.orc_test_rotate.argtypes = [vp, dbl, dbl, vp]
         L.orc_test_rotate.restype = None
+        L.orc_test_source.argtypes = [vp, u64, u64, ll, vp, vp, vp, vp]
+        L.orc_test_source.restype = None
         L.orc_run_histories.argtypes = [vp, u64, ll, u64, vp, vp, vp, vp, vp]
         L.orc_run.argtypes = [vp, u64, ll, u64, i32, dbl, vp, vp, vp, vp]
         L.orc_num_threads.restype = i32
@@ -224,6 +226,16 @@ class OracleScene:
         self.L.orc_test_electron_split(self.h, _p(p), int(m), float(t_kin), seed, first, n, _p(out))
         return out
 
+    def sample_source(self, seed, first, n):
+        """O4 test hook: (line i32[n], pos f64[n,3], dir f64[n,3], draw u32[n]) of histories first .. first+n-1;
+        draw = index of the first stream-0 draw after the source sampling."""
+        line = np.empty(n, dtype=np.int32)
+        pos = np.empty((n, 3))
+        d = np.empty((n, 3))
+        draw = np.empty(n, dtype=np.uint32)
+        self.L.orc_test_source(self.h, seed, first, n, _p(line), _p(pos), _p(d), _p(draw))
+        return line, pos, d, draw
+
     def run_histories(self, first, n, seed, details=False):
         edep = np.empty(n)
         flags = np.empty(n, dtype=np.uint32)
@@ -245,3 +257,37 @@ class OracleScene:
         rc = self.L.orc_run(self.h, first, n, seed, n_bins, e_max_mev, _p(spec), _p(emitted), _p(peak), _p(cnt))
         assert rc == 0, rc
         return spec, emitted, peak, dict(zip(COUNTER_NAMES, (int(x) for x in cnt)))
+
+
+def fepe(spectrum, emitted, peak, line_mev, line, mode=0, e_max_mev=2.0):
+    """O14: full-energy-peak efficiency of one line and its binomial standard error.
+    mode 0: exact counters, peak[l] / emitted[l].  mode 1: read from the spectrum, the line's bin b_l = floor(E_l / dE)
+    (computed in double) minus the mean of its two neighbours, over emitted[l]."""
+    em = float(emitted[line])
+    if em <= 0:
+        return 0.0, 0.0
+    if mode == 0:
+        p = float(peak[line]) / em
+    else:
+        n_bins = len(spectrum) - 1
+        b = int(np.floor(float(line_mev[line]) / (e_max_mev / n_bins)))
+        assert 1 <= b < n_bins - 1
+        p = (float(spectrum[b]) - 0.5 * (float(spectrum[b - 1]) + float(spectrum[b + 1]))) / em
+    return p, float(np.sqrt(max(p * (1.0 - p), 0.0) / em))
+
+
+def tally(edep, flags, line_mev, n_bins=4096, e_max_mev=2.0):
+    """O14 on a per-history dump (what orc_run does inside C, restated for dumps that were produced in chunks):
+    emitted[l] counts every history of line l, peak[l] the full-absorption ones; a history with E_dep > 0 goes to bin
+    floor(E_dep / dE), the last slot takes E_dep >= e_max.  `edep` is the dump's value: E_line for a peak history."""
+    edep = np.asarray(edep, dtype=np.float64)
+    flags = np.asarray(flags, dtype=np.uint32)
+    n_lines = len(line_mev)
+    line = ((flags >> 8) & 0xFF).astype(np.int64)
+    emitted = np.bincount(line, minlength=n_lines).astype(np.uint64)
+    peak = np.bincount(line[(flags & F_PEAK) != 0], minlength=n_lines).astype(np.uint64)
+    pos = edep > 0.0
+    b = np.floor(edep[pos] / (e_max_mev / n_bins))
+    b = np.where(b >= n_bins, n_bins, b).astype(np.int64)
+    spectrum = np.bincount(b, minlength=n_bins + 1).astype(np.uint64)
+    return spectrum, emitted, peak

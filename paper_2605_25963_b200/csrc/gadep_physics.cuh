@@ -23,7 +23,8 @@ GD_HD_NI GdF4 gd_mu_lookup_v(int n_grid, float ln_e0, float inv_dln, const float
     mu.a = expf(g * t[0] + f * t[1]);
     mu.b = expf(g * t[n_grid] + f * t[n_grid + 1]);
     mu.c = expf(g * t[2 * n_grid] + f * t[2 * n_grid + 1]);
-    mu.d = g * t[3 * n_grid] + f * t[3 * n_grid + 1];
+    // pair production only above 2 m_e c^2: the grid cell that straddles the threshold would interpolate to > 0 (R17)
+    mu.d = e > GD_TWO_MEC2 ? g * t[3 * n_grid] + f * t[3 * n_grid + 1] : 0.0f;
     return mu;
 }
 GD_HD float gd_mu_lookup(const GdMaterials &M, const float *tab, int m, float e, float mu[4]) {

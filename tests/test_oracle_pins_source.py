@@ -1,0 +1,341 @@
+"""Pins of the oracle's source sampling, pair threshold (R17), cut-off branch (O8/O10),
+FEPE read-out (O14, both modes) and resolution broadening (oracle/broaden.py) against closed
+forms and invariants.  None of these compares the oracle with itself or with the CUDA path."""
+import math
+
+import numpy as np
+import pytest
+
+import detmesh as dm
+from detmesh.configs import SRC_BEAM, SRC_POINT, SRC_VOLUME
+from detmesh.geometry import Line, discretise, merge_surfaces, revolve
+from oracle import gadep_oracle as orc
+from oracle.broaden import broaden
+
+MEC2 = 0.51099895
+
+
+def _cyl(R, z_top, z_bot, n_theta=32):
+    return revolve(discretise([Line(0, z_top, R, z_top, 1), Line(R, z_top, R, z_bot, 1), Line(R, z_bot, 0, z_bot, 1)]),
+                   n_theta)
+
+
+def _scene(surfaces, mu, is_scoring, source):
+    mesh = merge_surfaces(surfaces, 0)
+    s = orc.OracleScene()
+    s.set_materials(mu, is_scoring, dm.E_MIN_MEV, dm.E_MAX_MEV)
+    s.load_mesh(mesh.vertices, mesh.triangles, mesh.tri_surface, mesh.surf_inside, mesh.surf_outside, 0)
+    s.set_source(**source)
+    return s
+
+
+def _beam(e_kev, pos=(1.234, 0.567, 50.0)):
+    return {"kind": SRC_BEAM, "pos": pos, "dir": (0, 0, -1), "line_mev": [e_kev * 1e-3], "line_intensity": [1.0]}
+
+
+def _source_only_scene(source):
+    s = orc.OracleScene()
+    s.set_source(**source)
+    return s
+
+
+# ------------------------------------------------------------------ O4: line selection by cumulative intensity
+def test_line_frequencies_follow_the_intensities_of_config2():
+    w = dm.make_config(2)
+    inten = np.asarray(w.source["line_intensity"], dtype=np.float64)
+    assert len(inten) == 8 and inten.min() >= 0.5 and inten.max() <= 1.0 and len(set(inten)) == 8   # unequal, Q16
+    s = _source_only_scene(w.source)
+    n = 800_000
+    line, _, _, _ = s.sample_source(w.seed, 0, n)
+    p = inten / inten.sum()
+    cnt = np.bincount(line, minlength=8)
+    assert cnt.sum() == n
+    assert (np.abs(cnt - n * p) < 4 * np.sqrt(n * p * (1 - p))).all()
+    # a plausible off-by-one (lines shifted by one) must fail this: the nearest pair of intensities differs by > 4 sigma
+    shifted = np.roll(p, 1)
+    assert (np.abs(cnt - n * shifted) > 4 * np.sqrt(n * p * (1 - p))).any()
+
+
+def test_zero_intensity_lines_are_never_emitted_and_ratios_hold():
+    src = {"kind": SRC_POINT, "pos": (0, 0, 1), "dir": (0, 0, -1), "line_mev": [0.1, 0.2, 0.3, 0.4],
+           "line_intensity": [0.0, 1.0, 0.0, 3.0]}
+    s = _source_only_scene(src)
+    n = 200_000
+    line, pos, d, draw = s.sample_source(5, 1000, n)
+    cnt = np.bincount(line, minlength=4)
+    assert cnt[0] == 0 and cnt[2] == 0
+    assert abs(cnt[1] - 0.25 * n) < 4 * math.sqrt(n * 0.25 * 0.75)
+    # POINT source: fixed position, 1 (line) + 2 (direction) draws
+    assert (pos == np.array([0, 0, 1.0])).all() and (draw == 3).all()
+    # the line is a function of draw 0 of stream 0 only: u < 1/4 -> line 1, else line 3
+    u0 = np.array([orc.u01(5, 1000 + i, 0, 0) for i in range(2000)])
+    assert np.array_equal(line[:2000], np.where(u0 < 0.25, 1, 3))
+
+
+def test_beam_source_is_fixed_and_consumes_one_draw():
+    s = _source_only_scene(_beam(661.7))
+    line, pos, d, draw = s.sample_source(1, 0, 100)
+    assert (line == 0).all() and (draw == 1).all()
+    assert np.allclose(pos, np.float32([1.234, 0.567, 50.0])) and (d == np.array([0, 0, -1.0])).all()
+
+
+# ------------------------------------------------------------------ O4: volume source, uniform in the cylinder
+def test_volume_source_of_config2_is_uniform_in_the_cylinder_and_isotropic():
+    w = dm.make_config(2)
+    R, z0, z1 = 35.0, 7.01, 47.01
+    s = _source_only_scene(w.source)
+    n = 600_000
+    _, pos, d, draw = s.sample_source(w.seed, 0, n)
+    r2 = pos[:, 0] ** 2 + pos[:, 1] ** 2
+    z = pos[:, 2]
+    assert r2.max() <= R * R * (1 + 1e-12) and z.min() >= z0 - 1e-5 and z.max() <= z1 + 1e-5
+    # uniform in area: r^2 ~ U(0, R^2): <r^2> = R^2/2 (r = R u would give R^2/3), <r^4> = R^4/3
+    assert abs(r2.mean() / R ** 2 - 0.5) < 4 * math.sqrt(1 / 12 / n)
+    assert abs((r2 ** 2).mean() / R ** 4 - 1 / 3) < 4 * math.sqrt((1 / 5 - 1 / 9) / n)
+    # uniform z: mean and variance of U(z0, z1)
+    dz = z1 - z0
+    assert abs(z.mean() - 0.5 * (z0 + z1)) < 4 * dz / math.sqrt(12 * n)
+    assert abs(z.var() / (dz * dz / 12) - 1) < 4 * math.sqrt(0.8 / n)       # var of the variance estimate of a uniform
+    # uniform azimuth: first two Fourier moments vanish
+    phi = np.arctan2(pos[:, 1], pos[:, 0])
+    for k in (1, 2):
+        assert abs(np.cos(k * phi).mean()) < 4 * math.sqrt(0.5 / n) and abs(np.sin(k * phi).mean()) < 4 * math.sqrt(0.5 / n)
+    # r, phi, z independent of each other: equal-volume cells (4 x 4 x 4) are equally filled
+    cell = (np.minimum((r2 / R ** 2 * 4).astype(int), 3) * 16 + np.minimum(((phi + np.pi) / (2 * np.pi) * 4).astype(int), 3) * 4
+            + np.minimum(((z - z0) / dz * 4).astype(int), 3))
+    c = np.bincount(cell, minlength=64).astype(float)
+    chi2 = ((c - n / 64) ** 2 / (n / 64)).sum()
+    assert chi2 < 63 + 5 * math.sqrt(2 * 63)
+    # no rejection without an exclusion cylinder: 1 + 3 + 2 draws
+    assert (draw == 6).all()
+    # isotropic direction, independent of the position
+    assert (np.abs(np.linalg.norm(d, axis=1) - 1) < 1e-12).all()
+    assert (np.abs(d.mean(axis=0)) < 4 * math.sqrt(1 / 3 / n)).all()
+    assert (np.abs((d ** 2).mean(axis=0) - 1 / 3) < 4 * math.sqrt(4 / 45 / n)).all()
+    assert abs(np.corrcoef(z, d[:, 2])[0, 1]) < 4 / math.sqrt(n)
+
+
+def test_volume_source_of_config3_respects_the_exclusion_cylinder():
+    w = dm.make_config(3)
+    R, z0, z1 = 53.9, -228.35, 38.0                      # matrix outline ...
+    r_ex, e0, e1 = 43.9, -228.35, 8.0                    # ... minus the well
+    src = w.source
+    assert (src["cyl_r"], src["ex_r"]) == (R, r_ex)
+    s = _source_only_scene(src)
+    n = 600_000
+    _, pos, d, draw = s.sample_source(w.seed, 0, n)
+    r = np.hypot(pos[:, 0], pos[:, 1])
+    z = pos[:, 2]
+    # nothing inside the well, everything inside the outline
+    assert not ((r < r_ex * (1 - 1e-12)) & (z > e0) & (z < e1 * (1 - 1e-7))).any()
+    assert r.max() <= R * (1 + 1e-12) and z.min() >= z0 - 1e-4 and z.max() <= z1 + 1e-4
+    # uniform in the remaining volume: share of the top slab = V_top / (V_top + V_annulus)
+    v_top = math.pi * R * R * (z1 - e1)
+    v_ann = math.pi * (R * R - r_ex * r_ex) * (e1 - z0)
+    assert (v_top + v_ann) * 1e-6 == pytest.approx(1.000, abs=2e-3)          # the 1.0 L matrix of BASELINE configs[3]
+    p_top = v_top / (v_top + v_ann)
+    top = z > e1
+    assert abs(top.mean() - p_top) < 4 * math.sqrt(p_top * (1 - p_top) / n)
+    # <r^2> in the slab R^2/2, in the annulus (R^2 + r_ex^2)/2
+    assert abs((r[top] ** 2).mean() / (R * R / 2) - 1) < 4 * math.sqrt(1 / 3 / top.sum())
+    ann = ~top
+    m_ann = (R * R + r_ex * r_ex) / 2
+    assert abs((r[ann] ** 2).mean() - m_ann) < 4 * (R * R - r_ex * r_ex) / math.sqrt(12 * ann.sum())
+    # z uniform inside each part
+    assert abs(z[ann].mean() - 0.5 * (z0 + e1)) < 4 * (e1 - z0) / math.sqrt(12 * ann.sum())
+    assert abs(z[top].mean() - 0.5 * (e1 + z1)) < 4 * (z1 - e1) / math.sqrt(12 * top.sum())
+    # rejection bookkeeping: 3 draws per trial; P(accepted at once) = 1 - V_ex / V_cyl; trials geometric
+    trials = (draw.astype(np.int64) - 3)
+    assert (trials % 3 == 0).all() and trials.min() == 3
+    trials //= 3
+    p_acc = 1 - (r_ex * r_ex * (e1 - e0)) / (R * R * (z1 - z0))
+    assert abs((trials == 1).mean() - p_acc) < 4 * math.sqrt(p_acc * (1 - p_acc) / n)
+    assert abs(trials.mean() - 1 / p_acc) < 4 * math.sqrt((1 - p_acc) / p_acc ** 2 / n)
+    # isotropy after a varying number of draws
+    assert (np.abs(d.mean(axis=0)) < 4 * math.sqrt(1 / 3 / n)).all()
+    assert (np.abs((d ** 2).mean(axis=0) - 1 / 3) < 4 * math.sqrt(4 / 45 / n)).all()
+
+
+def test_first_flight_uses_the_draw_after_the_source_sampling():
+    # PE-only infinite medium, constant mu: the first flight length is -ln(u_k)/mu with k = the draw index the hook
+    # reports (6 for a volume source without rejections); the deposit point is not observable, but the number of
+    # histories that interact inside a sphere-like block is: use a slab beam instead -> transmission test covers the
+    # point/beam cases (test_oracle_pins.py); here: a volume source inside a huge block must absorb every history.
+    w = dm.make_config(1)
+    mu = np.zeros_like(w.mu); mu[1, 0, :] = 0.05
+    v, t = _cyl(1e4, 1e4, -1e4, 16)
+    src = dict(w.source); src.update(kind=SRC_VOLUME, cyl_r=10.0, cyl_z0=-5.0, cyl_z1=5.0, ex_r=4.0, ex_z0=-5.0, ex_z1=0.0)
+    s = _scene([("block", v, t, 1, 0)], mu, w.is_scoring, src)
+    n = 20000
+    edep, flags, cnt = s.run_histories(0, n, 3)
+    line = (flags >> 8) & 0xFF
+    assert ((flags & orc.F_PEAK) != 0).all() and cnt["n_pe"] == n
+    assert np.allclose(edep, s.line_mev[line], rtol=0, atol=0)
+    # the hook and the history agree on the line (same draw 0)
+    assert np.array_equal(line, s.sample_source(3, 0, n)[0])
+
+
+# ------------------------------------------------------------------ R17: pair production only above 2 m_e c^2
+def test_pair_channel_is_zero_up_to_threshold_and_linear_above():
+    w = dm.make_config(1)
+    s = orc.OracleScene(w)
+    grid = dm.energy_grid()
+    j = int(np.searchsorted(grid, 2 * MEC2)) - 1
+    assert grid[j] < 2 * MEC2 < grid[j + 1]                  # the cell 1.00949-1.03885 MeV of SURVEY.md O2
+    ge = dm.MAT["Ge_active"]
+    assert w.mu[ge, 3, j] == 0.0 and w.mu[ge, 3, j + 1] > 0.0
+    for e in (0.9, grid[j], 1.0150, 2 * MEC2):
+        assert s.mu(ge, 3, e) == 0.0
+    e = 1.030
+    f = (math.log(e) - math.log(grid[j])) / math.log(grid[j + 1] / grid[j])
+    assert s.mu(ge, 3, e) == pytest.approx(f * float(w.mu[ge, 3, j + 1]), rel=1e-9)
+
+
+def test_no_pair_event_and_no_negative_deposit_below_threshold():
+    # a table whose pair channel is strong right above threshold: without the guard of R17 a 1.015 MeV photon would
+    # pair-produce in the straddling cell and deposit E - 1.022 MeV < 0
+    w = dm.make_config(1)
+    grid = dm.energy_grid()
+    mu = w.mu.copy()
+    mu[:, 3, :] = np.where(grid > 2 * MEC2, 0.05, 0.0)[None, :] * (mu[:, 1, :1] > 0)
+    v, t = _cyl(200.0, 0.0, -400.0, 32)
+    for e_kev, expect_pairs in ((1015.0, False), (1030.0, True)):
+        s = _scene([("ge", v, t, 1, 0)], mu, w.is_scoring, _beam(e_kev))
+        edep, flags, other, esc, cnt = s.run_histories(0, 20000, 9, details=True)
+        assert (cnt["n_pair"] > 100) == expect_pairs and (expect_pairs or cnt["n_pair"] == 0)
+        dep = np.where((flags & orc.F_PEAK) != 0, s.line_mev[0], edep)
+        assert (dep >= 0).all() and (other >= 0).all() and (esc >= 0).all()
+        assert np.allclose(dep + other + esc, s.line_mev[0], rtol=1e-12)
+
+
+# ------------------------------------------------------------------ O8/O10: cut-off at 10 keV
+def test_compton_chain_ends_at_the_cut_off_with_local_deposit():
+    # Compton-only infinite Ge: a 12 keV photon loses at most 1 - 1/(1 + 2k) = 4.5 % per scatter, so it needs at least
+    # ceil(ln(12/10)/ln(1 + 2k)) = 4 scatters to fall below E_cut = 10 keV; there it deposits what is left on the spot.
+    w = dm.make_config(1)
+    mu = np.zeros_like(w.mu); mu[1, 1, :] = w.mu[1, 1, :]
+    v, t = _cyl(1e5, 1e5, -1e5, 16)
+    s = _scene([("block", v, t, 1, 0)], mu, w.is_scoring, _beam(12.0, pos=(1.2, 0.5, 1.0)))
+    n = 5000
+    edep, flags, other, esc, cnt = s.run_histories(0, n, 11, details=True)
+    assert cnt["n_cutoff"] == n and cnt["n_pe"] == 0 and cnt["n_escaped"] == 0
+    assert ((flags & orc.F_PEAK) != 0).all()
+    assert (other == 0).all() and (esc == 0).all() and np.allclose(edep, s.line_mev[0], rtol=1e-12)
+    k = 0.012 / MEC2
+    n_min = math.ceil(math.log(12.0 / 10.0) / math.log(1 + 2 * k))
+    assert n_min == 4
+    nev = flags >> 16
+    assert nev.min() >= n_min and nev.sum() == cnt["n_compton"]
+    # mean energy loss per scatter at k << 1 is k E (1 - ...) ~ E k: mean number of scatters ~ ln(1.2)/k = 7.8
+    assert 6.0 < nev.mean() < 10.0
+
+
+# ------------------------------------------------------------------ O14: FEPE, both modes
+def test_fepe_modes_on_a_constructed_spectrum():
+    n_bins, e_max = 4096, 2.0
+    spec = np.full(n_bins + 1, 40, dtype=np.uint64)           # flat continuum
+    line_mev = np.array([0.6617, 1.3325])
+    b0, b1 = 1355, 2728                                       # 661.7 / 0.48828125 = 1355.16; 1332.5 -> 2728.96 (Q13)
+    spec[b0] += 5000
+    spec[b1] += 1200
+    emitted = np.array([100000, 50000], dtype=np.uint64)
+    peak = np.array([5000, 1200], dtype=np.uint64)
+    for l, p in ((0, 0.05), (1, 0.024)):
+        for mode in (0, 1):
+            f, se = orc.fepe(spec, emitted, peak, line_mev, l, mode)
+            assert f == pytest.approx(p, rel=1e-12)
+            assert se == pytest.approx(math.sqrt(p * (1 - p) / float(emitted[l])), rel=1e-12)
+    # a sloped continuum cancels as well (mean of the neighbours); a step does not
+    spec2 = spec.copy(); spec2[b0 - 1] += 10; spec2[b0 + 1] -= 10
+    assert orc.fepe(spec2, emitted, peak, line_mev, 0, 1)[0] == pytest.approx(0.05, rel=1e-12)
+
+
+def test_fepe_mode1_agrees_with_mode0_on_config0():
+    w = dm.make_config(0)
+    s = orc.OracleScene(w)
+    n = 1_000_000
+    spec, em, pk, _ = s.run(n, 1)
+    f0, se0 = orc.fepe(spec, em, pk, s.line_mev, 0, 0)
+    f1, _ = orc.fepe(spec, em, pk, s.line_mev, 0, 1)
+    assert em[0] == n and f0 == pk[0] / n
+    # single line: the peak bin holds the peak plus a continuum count per bin of a few -> mode 1 within 1 % of mode 0
+    assert abs(f1 - f0) < 0.01 * f0
+    # and below the geometric solid angle of the N-gon cylinder (P5)
+    assert f0 < 0.003555923
+
+
+# ------------------------------------------------------------------ broadening (NEXT-3): closed forms of a Gaussian
+def _moments(out, e_max):
+    n = len(out) - 1
+    c = (np.arange(n) + 0.5) * e_max / n
+    tot = out[:n].sum()
+    m = (out[:n] * c).sum() / tot
+    return tot, m, (out[:n] * (c - m) ** 2).sum() / tot
+
+
+def test_broadening_of_one_bin_is_a_gaussian_with_the_stated_width():
+    n, e_max = 4096, 2.0
+    de = e_max / n
+    fwhm = 0.002                                             # 2 keV at every energy
+    sigma = fwhm / 2.3548200450309493
+    spec = np.zeros(n + 1)
+    i = 1355
+    spec[i] = 1e6
+    out = broaden(spec, e_max, fwhm ** 2)
+    tot, mean, var = _moments(out, e_max)
+    assert out.sum() == pytest.approx(1e6, rel=1e-12) and out[n] < 1e-6 and (out >= 0).all()
+    assert mean == pytest.approx((i + 0.5) * de, abs=1e-9)
+    # binned Gaussian: variance = sigma^2 + dE^2/12 (Sheppard), to ~exp(-2 pi^2 sigma^2/dE^2) relative
+    assert var == pytest.approx(sigma ** 2 + de ** 2 / 12, rel=1e-6)
+    # symmetric about the source bin
+    assert np.allclose(out[i - 20:i], out[i + 20:i:-1], rtol=1e-9, atol=1e-9)
+    # the mass of each output bin equals the integral of the normal density over it (Gauss-Legendre, no erf)
+    x, wq = np.polynomial.legendre.leggauss(24)
+    centre = (i + 0.5) * de
+    for j in (i, i + 1, i + 3, i - 5):
+        a, b = j * de, (j + 1) * de
+        e = 0.5 * (b - a) * x + 0.5 * (a + b)
+        mass = 0.5 * (b - a) * (wq * np.exp(-0.5 * ((e - centre) / sigma) ** 2)).sum() / (sigma * math.sqrt(2 * math.pi))
+        assert out[j] == pytest.approx(1e6 * mass, rel=1e-9)
+    # 68.27 % within one sigma (sum of the fine bins of a coarse-sigma case)
+    wide = broaden(spec, e_max, (40 * de * 2.3548200450309493) ** 2)   # sigma = 40 bins
+    assert wide[i - 39:i + 40].sum() + 0.5 * (wide[i - 40] + wide[i + 40]) == pytest.approx(0.682689492e6, rel=2e-4)
+
+
+def test_broadening_width_follows_a_plus_bE_plus_cE2_and_is_linear():
+    n, e_max = 4096, 2.0
+    de = e_max / n
+    a, b, c = 1.0e-6, 2.0e-6, 1.0e-6
+    spec = np.zeros(n + 1)
+    lines = (250, 1355, 2728)
+    for i in lines:
+        spec[i] = 1e5
+    out = broaden(spec, e_max, a, b, c)
+    for i in lines:
+        e = (i + 0.5) * de
+        sigma2 = (a + b * e + c * e * e) / 2.3548200450309493 ** 2
+        lo, hi = i - 60, i + 61
+        seg = np.zeros(n + 1); seg[lo:hi] = out[lo:hi]
+        tot, mean, var = _moments(seg, e_max)
+        assert tot == pytest.approx(1e5, rel=1e-9) and mean == pytest.approx(e, abs=1e-8)
+        assert var == pytest.approx(sigma2 + de * de / 12, rel=1e-5)
+    # superposition
+    s1 = np.zeros(n + 1); s1[250] = 1e5
+    s2 = spec - s1
+    assert np.allclose(broaden(s1, e_max, a, b, c) + broaden(s2, e_max, a, b, c), out, rtol=1e-12, atol=1e-9)
+
+
+def test_broadening_conserves_the_total_at_the_edges():
+    n, e_max = 64, 2.0
+    de = e_max / n
+    spec = np.zeros(n + 1)
+    spec[0] = 1000.0; spec[n - 1] = 2000.0; spec[n] = 77.0      # first bin, last bin, overflow slot
+    sigma = 2 * de
+    out = broaden(spec, e_max, (sigma * 2.3548200450309493) ** 2)
+    assert out.sum() == pytest.approx(3077.0, rel=1e-12)
+    # bin 0 keeps its own share plus everything below 0: P(x < de) for a normal centred at de/2
+    p_low = 0.5 * (1 + math.erf((0.5 * de) / (sigma * math.sqrt(2))))
+    assert out[0] == pytest.approx(1000.0 * p_low, rel=1e-6)
+    # the overflow slot keeps its counts and takes the mass above e_max
+    p_up = 0.5 * (1 - math.erf((0.5 * de) / (sigma * math.sqrt(2))))
+    assert out[n] == pytest.approx(77.0 + 2000.0 * p_up, rel=1e-6)
