@@ -86,8 +86,14 @@ int gadep_set_materials(gadep_ctx *ctx, int n_mat, int n_grid, double e_min_mev,
 int gadep_load_mesh(gadep_ctx *ctx, const float *vertices, int n_vert, const int *triangles, const int *tri_surface,
                     int n_tri, const int *surf_inside, const int *surf_outside, int n_surf, int world_material);
 
-/* Builds the BVH over the facets on the GPU.  flags: 0.  Timed separately by bench.py. */
+/* Builds the BVH over the facets on the GPU: binary LBVH -> uncompressed 4-wide nodes (default
+ * traversal) and 8-wide nodes with 8-bit quantised child boxes (measured alternative).
+ * flags: 0.  Timed by bench.py. */
 int gadep_build_bvh(gadep_ctx *ctx, int flags);
+
+/* Node width the wavefront kernels and gadep_trace_rays traverse: 4 (default; uncompressed nodes) or 8 (compressed
+ * nodes).  Both hierarchies hold the same facets, so every result is identical. */
+int gadep_set_bvh_width(gadep_ctx *ctx, int width);
 
 #define GADEP_SRC_POINT 0
 #define GADEP_SRC_VOLUME 1
@@ -115,7 +121,8 @@ int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
 #define GADEP_RUN_PARTIAL_XS 32     /* the paper's "partial cross-section method": one remaining    */
                                    /* optical depth per process instead of total-mu sampling + a selection draw  */
                                    /* (history-per-thread kernel; same distribution, different random streams)   */
-#define GADEP_RUN_WARP_SPECIALISED 64 /* measurement: physics and traversal on separate warps of a block (same results) */
+#define GADEP_RUN_BVH8 256          /* measurement / cross-check: the wavefront kernel traverses the compressed      */
+                                   /* 8-wide nodes instead of the uncompressed 4-wide ones (same results, bit for bit) */
 #define GADEP_RUN_ELECTRON_RANGE 128 /* SURVEY.md 8(f) NEXT-4 (coupled photon-electron physics): every   */
                                    /* energy deposit becomes one electron, a straight segment of the Katz-Penfold   */
                                    /* range in an isotropic direction (Philox stream 3), cut at the first facet of  */
@@ -142,6 +149,17 @@ int gadep_run(gadep_ctx *ctx, unsigned long long n_histories, unsigned long long
  * mode 1 = read from the spectrum: (S[b] - (S[b-1] + S[b+1]) / 2) / emitted[l].  std_err = binomial. HOST outputs.
  */
 int gadep_fepe(const gadep_ctx *ctx, int line, int mode, double *fepe, double *std_err);
+
+/*
+ * The whole tally block of the context, for the one exchange of a sharded run: n = gadep_tally_size()
+ * = n_bins + 1 + 2 * GADEP_MAX_LINES words: spectrum[n_bins + 1], emitted[GADEP_MAX_LINES], peak[GADEP_MAX_LINES].
+ * gadep_get_tallies copies it out (HOST-or-DEVICE; a DEVICE copy is stream-ordered and not synchronised);
+ * gadep_set_tallies replaces it, so that gadep_fepe / gadep_get_counters / gadep_broaden read the reduced
+ * counters after an all-reduce.  Both need a previous gadep_run on this context (it fixes n_bins).
+ */
+int gadep_tally_size(const gadep_ctx *ctx);
+int gadep_get_tallies(gadep_ctx *ctx, unsigned long long *out);
+int gadep_set_tallies(gadep_ctx *ctx, const unsigned long long *in);
 
 /*
  * Detector-resolution broadening of the spectrum of the last gadep_run (the paper's spectra are
@@ -200,8 +218,8 @@ typedef struct {
     int n_bvh_nodes, bvh_max_depth;
     float last_run_ms, last_build_ms;      /* CUDA-event times of the last gadep_run / gadep_build_bvh kernels   */
     int last_run_launches, last_build_launches;
-    unsigned long long n_safety_queries;   /* wavefront kernel: facet-free-sphere queries issued                 */
-    unsigned long long n_skipped_queries;  /* flights whose nearest-hit query was answered by such a sphere      */
+    unsigned long long n_stack_overflow;   /* rays that ran out of traversal stack since gadep_create (must be 0; a  */
+                                           /* run that sees one fails with GADEP_E_ARG)                              */
     unsigned long long n_parity_queries;   /* GADEP_RUN_PARITY_LOCALISATION: all-hits localisation queries       */
     unsigned long long n_parity_mismatch;  /* ... of which the parity rule and the side ids named different media */
 } gadep_counters;

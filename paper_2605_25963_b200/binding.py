@@ -18,13 +18,14 @@ MAT_KILL = -1
 MAX_LINES = 64
 RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES, RUN_PARITY_LOCALISATION = 1, 2, 4, 8, 16
 RUN_PARTIAL_XS = 32
-RUN_WARP_SPECIALISED = 64
+RUN_BVH8 = 256
 RUN_ELECTRON_RANGE = 128
 
 EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_set_materials", "gadep_load_mesh",
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
                     "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw", "gadep_locate", "gadep_broaden",
-                    "gadep_set_densities", "gadep_run_histories_ex")
+                    "gadep_set_densities", "gadep_run_histories_ex", "gadep_set_bvh_width", "gadep_tally_size",
+                    "gadep_get_tallies", "gadep_set_tallies")
 
 
 class GadepError(RuntimeError):
@@ -51,7 +52,7 @@ class GadepCounters(C.Structure):
                [("emitted", C.c_ulonglong * MAX_LINES), ("peak", C.c_ulonglong * MAX_LINES), ("n_lines", C.c_int),
                 ("n_bvh_nodes", C.c_int), ("bvh_max_depth", C.c_int), ("last_run_ms", C.c_float),
                 ("last_build_ms", C.c_float), ("last_run_launches", C.c_int), ("last_build_launches", C.c_int),
-                ("n_safety_queries", C.c_ulonglong), ("n_skipped_queries", C.c_ulonglong),
+                ("n_stack_overflow", C.c_ulonglong),
                 ("n_parity_queries", C.c_ulonglong), ("n_parity_mismatch", C.c_ulonglong)]
 
     def as_dict(self):
@@ -61,7 +62,7 @@ class GadepCounters(C.Structure):
                  n_bvh_nodes=int(self.n_bvh_nodes), bvh_max_depth=int(self.bvh_max_depth),
                  last_run_ms=float(self.last_run_ms), last_build_ms=float(self.last_build_ms),
                  last_run_launches=int(self.last_run_launches), last_build_launches=int(self.last_build_launches),
-                 n_safety_queries=int(self.n_safety_queries), n_skipped_queries=int(self.n_skipped_queries),
+                 n_stack_overflow=int(self.n_stack_overflow),
                  n_parity_queries=int(self.n_parity_queries), n_parity_mismatch=int(self.n_parity_mismatch))
         return d
 
@@ -107,6 +108,10 @@ def load_library(build_if_missing: bool = True):
     L.gadep_philox_raw.argtypes = [vp, vp, vp, i32, vp]
     L.gadep_locate.argtypes = [vp, vp, vp, ll, i32, vp]
     L.gadep_broaden.argtypes = [vp, dbl, dbl, dbl, vp]
+    L.gadep_set_bvh_width.argtypes = [vp, i32]
+    L.gadep_tally_size.argtypes = [vp]
+    L.gadep_get_tallies.argtypes = [vp, vp]
+    L.gadep_set_tallies.argtypes = [vp, vp]
     _lib = L
     return L
 
@@ -244,6 +249,22 @@ class Gadep:
             raise ValueError("device inputs need a device output")
         self._check(self.L.gadep_locate(self.h, _ptr(org), _ptr(dir), org.shape[0], int(mode), _ptr(material_out)))
         return material_out
+
+    def set_bvh_width(self, width: int):
+        self._check(self.L.gadep_set_bvh_width(self.h, int(width)))
+
+    def tally_size(self) -> int:
+        return int(self.L.gadep_tally_size(self.h))
+
+    def get_tallies(self, out=None):
+        """spectrum[n_bins + 1] + emitted[64] + peak[64] of the context; out: None -> new host array, else filled."""
+        if out is None:
+            out = np.zeros(self.tally_size(), dtype=np.uint64)
+        self._check(self.L.gadep_get_tallies(self.h, _ptr(out)))
+        return out
+
+    def set_tallies(self, tallies):
+        self._check(self.L.gadep_set_tallies(self.h, _ptr(tallies)))
 
     def set_densities(self, rho_g_cm3):
         rho = np.ascontiguousarray(rho_g_cm3, dtype=np.float32)

@@ -9,7 +9,7 @@ CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libgadep.so")
 SOURCES = ["gadep_api.cu"]
 HEADERS = ["gadep_common.cuh", "gadep_bvh.cuh", "gadep_physics.cuh", "gadep_build_kernels.cuh",
-           "gadep_transport_kernels.cuh", "gadep_trav.cuh", "gadep_wave_kernels.cuh", "gadep_locate_kernels.cuh", "gadep_ws_kernels.cuh", os.path.join("..", "..", "include", "gadep.h")]
+           "gadep_transport_kernels.cuh", "gadep_trav.cuh", "gadep_wave_kernels.cuh", "gadep_locate_kernels.cuh", os.path.join("..", "..", "include", "gadep.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 

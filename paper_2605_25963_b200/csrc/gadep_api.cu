@@ -17,7 +17,6 @@
 #include "gadep_transport_kernels.cuh"
 #include "gadep_wave_kernels.cuh"
 #include "gadep_locate_kernels.cuh"
-#include "gadep_ws_kernels.cuh"
 
 struct gadep_ctx {
     int device = 0;
@@ -37,16 +36,18 @@ struct gadep_ctx {
     int *d_tris = nullptr, *d_tri_mats = nullptr, *d_tri_surf = nullptr;
     GdNode *d_nodes = nullptr;
     GdNode4 *d_nodes4 = nullptr;
+    GdNode8 *d_nodes8 = nullptr;
+    int bvh_width = 4;             // traversal of the wavefront kernels: 4 = uncompressed 4-wide nodes, 8 = compressed 8-wide
     GdTri *d_leaf_tris = nullptr;
     int bvh_depth = 0;
     int n_ref = 0;                 // leaves of the BVH: facet references after splitting
     // build buffers are kept between builds (no cudaMalloc / cudaFree, and none of their implicit synchronisations,
     // inside a step that rebuilds the BVH every time): [0] counts [1] scene [2] scratch arena [3] nodes [4] leaf
-    // triangles [5] 4-wide nodes
+    // triangles [5] 4-wide nodes [13] 8-wide compressed nodes
     // [6..9] the mesh copies (vertices, triangles, side materials, surface ids)
     // [10..12] mesh validation: edge table keys, edge table surfaces, error record + surface sides
-    void *pool[13] = {};
-    size_t pool_cap[13] = {};
+    void *pool[14] = {};
+    size_t pool_cap[14] = {};
     // source
     bool have_src = false;
     GdSource src;
@@ -56,10 +57,12 @@ struct gadep_ctx {
     int cap_bins = 0;
     GdCounters *d_counters = nullptr;
     unsigned long long *d_next = nullptr;     // history counter of the refill kernel
+    int run_width = 4;                        // width used by the current launch (bvh_width, or 8 with GADEP_RUN_BVH8)
+    unsigned long long n_stack_overflow = 0;  // rays that ran out of traversal stack since the context was made (must stay 0)
     int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
-    GdWaveTune tune = {8, 4, 4, 4.0f, 8.0f, 12};
+    GdWaveTune tune = {8, 4, 4};
     float rho[GADEP_MAX_MATERIALS] = {};      // g/cm^3, electron-range mode
     bool have_rho = false;
     // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
@@ -134,12 +137,9 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
     if (getenv("GADEP_NO_SURFACE_CLUSTERS")) c->cluster_surfaces = false;
     if (const char *t = getenv("GADEP_SPLIT_BUDGET")) { double b = atof(t); if (b >= 0 && b <= 15) c->split_budget = b; }
-    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,n_steps[,lam_max,cap_mfp,sparse_max]" (measurement sweeps)
+    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,n_steps" (measurement sweeps)
         int a, b, d;
-        float lm = c->tune.lam_max, cm = c->tune.cap_mfp;
-        int sp = c->tune.sparse_max;
-        int k = sscanf(t, "%d,%d,%d,%f,%f,%d", &a, &b, &d, &lm, &cm, &sp);
-        if (k >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && lm >= 0 && cm > 0) c->tune = {a, b, d, lm, cm, sp};
+        if (sscanf(t, "%d,%d,%d", &a, &b, &d) == 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32) c->tune = {a, b, d};
     }
     *out = c;
     return GADEP_OK;
@@ -158,7 +158,7 @@ static cudaError_t gd_pool_get(gadep_ctx *c, int k, size_t bytes, void **out) {
 }
 
 static void gd_free_mesh(gadep_ctx *c) {
-    c->d_nodes4 = nullptr;
+    c->d_nodes4 = nullptr; c->d_nodes8 = nullptr;
     c->d_verts = nullptr; c->d_tris = c->d_tri_mats = c->d_tri_surf = nullptr;
     c->d_nodes = nullptr; c->d_leaf_tris = nullptr;
     c->have_mesh = c->have_bvh = false;
@@ -169,7 +169,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    for (int k = 0; k < 13; ++k) cudaFree(c->pool[k]);
+    for (int k = 0; k < 14; ++k) cudaFree(c->pool[k]);
     cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair); cudaFree(c->d_mat_entry);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -283,7 +283,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     GD_CUDA(c, cudaSetDevice(c->device));
     const int n_tri = c->n_tri;
     cudaStream_t st = c->stream;
-    c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->d_nodes4 = nullptr; c->have_bvh = false;
+    c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->d_nodes4 = nullptr; c->d_nodes8 = nullptr; c->have_bvh = false;
     const int tb = 256, nbt = (n_tri + tb - 1) / tb;
     int launches = 0;
     // ---- phase A: how many references (reference splitting) -> one 4-byte read-back sizes the arena
@@ -329,6 +329,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         if ((e = gd_pool_get(c, 3, sizeof(GdNode) * (size_t)std::max(n - 1, 1), (void **)&c->d_nodes)) != cudaSuccess) break;
         if ((e = gd_pool_get(c, 4, sizeof(GdTri) * (size_t)n, (void **)&c->d_leaf_tris)) != cudaSuccess) break;
         if ((e = gd_pool_get(c, 5, sizeof(GdNode4) * (size_t)std::max(n - 1, 1), (void **)&c->d_nodes4)) != cudaSuccess) break;
+        if ((e = gd_pool_get(c, 13, sizeof(GdNode8) * (size_t)std::max(n - 1, 1), (void **)&c->d_nodes8)) != cudaSuccess) break;
         float4 *ref_lo = (float4 *)(arena + o_tlo), *ref_hi = (float4 *)(arena + o_thi);
         float4 *node_lo = (float4 *)(arena + o_nlo), *node_hi = (float4 *)(arena + o_nhi);
         unsigned long long *keys[2] = {(unsigned long long *)(arena + o_k0), (unsigned long long *)(arena + o_k1)};
@@ -361,7 +362,8 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
             gd_k_refit<<<nb, tb, 0, st>>>(n, child_l, child_r, parent_int, parent_leaf, ref_lo, ref_hi, vals[cur], node_lo,
                                           node_hi, visits, c->d_nodes, scene + 6);
             gd_k_collapse4<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes4);
-            launches += 3;
+            gd_k_collapse8<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes8);
+            launches += 4;
         }
         cudaEventRecord(c->evb1, st);
         if ((e = cudaGetLastError()) != cudaSuccess) break;
@@ -403,7 +405,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
 
 static GdBvh gd_bvh_view(const gadep_ctx *c) {
     GdBvh b;
-    b.nodes = c->d_nodes; b.nodes4 = c->d_nodes4; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
+    b.nodes = c->d_nodes; b.nodes4 = c->d_nodes4; b.nodes8 = c->d_nodes8; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
     b.mat_entry = c->have_entries ? c->d_mat_entry : nullptr;
     return b;
 }
@@ -456,6 +458,15 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (!c->have_mat || !c->have_mesh || !c->have_bvh || !c->have_src)
         return gd_fail(c, GADEP_E_ORDER, "run needs materials, mesh, BVH and source");
     if (n_bins <= 0 || n_bins > (1 << 20) || !(e_max > 0)) return gd_fail(c, GADEP_E_ARG, "bad spectrum shape");
+    // materials may have been (re)set after the mesh or the source: every id and line energy is checked against the tables
+    // the kernel will index (an id >= n_mat would read past the attenuation table in shared memory)
+    if (c->world < 0 || c->world >= c->n_mat) return gd_fail(c, GADEP_E_INDEX, "world material %d outside the %d materials set", c->world, c->n_mat);
+    for (size_t k = 0; k < c->h_sides.size(); ++k)
+        if (c->h_sides[k] != GADEP_MAT_KILL && (c->h_sides[k] < 0 || c->h_sides[k] >= c->n_mat))
+            return gd_fail(c, GADEP_E_INDEX, "surface %zu: side material %d outside the %d materials set", k / 2, c->h_sides[k], c->n_mat);
+    for (int l = 0; l < c->src.n_lines; ++l)
+        if (!((double)c->src.line_mev[l] >= c->e_min * (1 - 1e-6) && (double)c->src.line_mev[l] <= c->e_max * (1 + 1e-6)))
+            return gd_fail(c, GADEP_E_ARG, "line %d: energy %g outside the table range", l, (double)c->src.line_mev[l]);
     GD_CUDA(c, cudaSetDevice(c->device));
     bool same_shape = c->d_tally && c->n_bins == n_bins && c->spec_e_max == e_max;
     int rc = gd_ensure_tally(c, n_bins);
@@ -486,11 +497,11 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0xFFFFFFFFull) return gd_fail(c, GADEP_E_ARG, "more than 2^32-1 histories in one launch");
     size_t smem = sizeof(float) * (size_t)c->n_mat * 4 * c->n_grid + sizeof(unsigned) * ((size_t)n_bins + 1);
     const int variant = c->kernel_variant;
-    const int threads = variant == 2 ? GD_W_THREADS : (variant == 5 ? GD_WS_THREADS : GD_RUN_THREADS);
+    const int threads = variant == 2 ? GD_W_THREADS : GD_RUN_THREADS;
+    const bool wide8 = c->run_width == 8;
     if (variant == 2) smem += sizeof(float) * (size_t)GD_W_WARPS * GD_W_NF * GD_W_SLOTS;
-    if (variant == 5) smem += sizeof(float) * (size_t)GD_WS_TEAMS * GD_WS_NF * GD_WS_SLOTS;
     if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
-    const void *kern = variant == 5 ? (const void *)gd_k_transport_ws : variant == 2 ? (const void *)gd_k_transport_wave
+    const void *kern = variant == 2 ? (wide8 ? (const void *)gd_k_transport_wave<8> : (const void *)gd_k_transport_wave<4>)
                                     : (variant == 1 ? (const void *)gd_k_transport_refill
                                                   : (variant == 3 ? (const void *)gd_k_transport<true, false>
                                                      : (variant == 4 ? (const void *)gd_k_transport<false, true>
@@ -499,12 +510,11 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     int per_sm = 1;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return gd_fail(c, GADEP_E_CUDA, "transport kernel does not fit on an SM (%zu B shared memory)", smem);
-    const unsigned long long per_block = variant == 2 ? (unsigned long long)GD_W_WARPS * GD_W_SLOTS
-                                         : (variant == 5 ? (unsigned long long)GD_WS_TEAMS * GD_WS_SLOTS : GD_RUN_THREADS);
+    const unsigned long long per_block = variant == 2 ? (unsigned long long)GD_W_WARPS * GD_W_SLOTS : GD_RUN_THREADS;
     unsigned long long want = (n + per_block - 1) / per_block;
     int grid = (int)std::min<unsigned long long>((unsigned long long)c->n_sm * per_sm, std::max<unsigned long long>(want, 1));
-    if (variant == 2 || variant == 5) {
-        size_t need = variant == 2 ? (size_t)grid * GD_W_WARPS * GD_W_SLOTS * 8 : (size_t)grid * GD_WS_TEAMS * GD_WS_SLOTS * 8;
+    if (variant == 2) {
+        size_t need = (size_t)grid * GD_W_WARPS * GD_W_SLOTS * 8;
         if (need > c->pair_floats) {
             cudaFree(c->d_pair); c->d_pair = nullptr; c->pair_floats = 0;
             GD_CUDA(c, cudaMalloc(&c->d_pair, need * sizeof(float)));
@@ -516,14 +526,13 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0) {
         unsigned long long warps = (unsigned long long)grid * (threads / 32);
         unsigned chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / (warps * 16)));
-        if (variant == 1 || variant == 2 || variant == 5) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
-        if (variant == 5) {
-            unsigned ws_chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / ((unsigned long long)grid * GD_WS_TEAMS * 16)));
-            gd_k_transport_ws<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
-                                                           c->d_next, ws_chunk, c->d_pair, c->tune);
+        if (variant == 1 || variant == 2) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
+        if (variant == 2 && wide8) {
+            gd_k_transport_wave<8><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
+                                                                c->d_next, chunk, c->d_pair, c->tune);
         } else if (variant == 2) {
-            gd_k_transport_wave<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
-                                                             c->d_next, chunk, c->d_pair, c->tune);
+            gd_k_transport_wave<4><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
+                                                                c->d_next, chunk, c->d_pair, c->tune);
         } else if (variant == 1) {
             gd_k_transport_refill<<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
                                                                d_flags, c->d_next, chunk);
@@ -558,11 +567,21 @@ static int gd_fetch_results(gadep_ctx *c) {
     GD_CUDA(c, cudaMemcpy(&c->h_counters, c->d_counters, sizeof(GdCounters), cudaMemcpyDeviceToHost));
     if (c->run_timed) { cudaEventElapsedTime(&c->last_run_ms, c->ev0, c->ev1); c->run_timed = false; }
     c->results_stale = false;
+    {
+        unsigned ovf = 0;
+        GD_CUDA(c, cudaMemcpyFromSymbol(&ovf, gd_stack_overflow, sizeof(ovf)));
+        if (ovf) {
+            const unsigned zero = 0;
+            cudaMemcpyToSymbol(gd_stack_overflow, &zero, sizeof(zero));
+            c->n_stack_overflow += ovf;
+            return gd_fail(c, GADEP_E_ARG, "%u rays ran out of traversal stack (BVH too deep for GD_STACK8)", ovf);
+        }
+    }
     return GADEP_OK;
 }
 
 static int gd_variant_of(int flags) {
-    return (flags & GADEP_RUN_ELECTRON_RANGE) ? 6 : (flags & GADEP_RUN_WARP_SPECIALISED) ? 5 : (flags & GADEP_RUN_PARTIAL_XS) ? 4
+    return (flags & GADEP_RUN_ELECTRON_RANGE) ? 6 : (flags & GADEP_RUN_PARTIAL_XS) ? 4
            : (flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
 }
 
@@ -587,7 +606,13 @@ extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned 
         return gd_fail(c, GADEP_E_ARG, "GADEP_RUN_ASYNC needs a device spectrum pointer");
     if ((opts->flags & GADEP_RUN_ELECTRON_RANGE) && !c->have_rho)
         return gd_fail(c, GADEP_E_ORDER, "GADEP_RUN_ELECTRON_RANGE needs gadep_set_densities");
+    {   // GADEP_RUN_* kernel selectors exclude one another
+        const int sel = opts->flags & (GADEP_RUN_HISTORY_PER_THREAD | GADEP_RUN_PERSISTENT_LANES | GADEP_RUN_PARITY_LOCALISATION |
+                                       GADEP_RUN_PARTIAL_XS | GADEP_RUN_ELECTRON_RANGE);
+        if (sel & (sel - 1)) return gd_fail(c, GADEP_E_ARG, "run flags 0x%x select more than one kernel", opts->flags);
+    }
     c->kernel_variant = gd_variant_of(opts->flags);
+    c->run_width = (opts->flags & GADEP_RUN_BVH8) ? 8 : c->bvh_width;
     int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
                                  (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
     if (rc) return rc;
@@ -648,13 +673,16 @@ extern "C" int gadep_trace_rays(gadep_ctx *c, const float *org, const float *dir
     }
     cudaMemsetAsync(c->d_counters, 0, sizeof(GdCounters), st);
     int per_sm = 1;
-    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gd_k_trace_wave, 256, 0));
+    const bool wide8 = c->bvh_width == 8;
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, wide8 ? gd_k_trace_wave<8> : gd_k_trace_wave<4>, 256, 0));
     int grid = (int)std::min<long long>((n_rays + 255) / 256, (long long)c->n_sm * std::max(per_sm, 1));
     unsigned chunk = (unsigned)std::min<long long>(2048, std::max<long long>(32, n_rays / ((long long)grid * 8 * 8)));
     cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st);
     cudaEventRecord(c->ev0, st);
-    gd_k_trace_wave<<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
-                                          c->d_counters, c->d_next, chunk, c->tune);
+    if (wide8) gd_k_trace_wave<8><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
+                                                         c->d_counters, c->d_next, chunk, c->tune);
+    else gd_k_trace_wave<4><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
+                                                   c->d_counters, c->d_next, chunk, c->tune);
     cudaEventRecord(c->ev1, st);
     c->last_run_launches = 1;
     cudaError_t e = cudaGetLastError();
@@ -774,7 +802,13 @@ extern "C" int gadep_run_histories_ex(gadep_ctx *c, unsigned long long first, lo
     if (flags_out && !dev_f && n > 0) { GD_CUDA(c, cudaMalloc(&stage_f, sizeof(unsigned) * (size_t)n)); d_f = stage_f; }
     int n_bins = c->n_bins > 0 ? c->n_bins : 4096;
     float e_max = c->spec_e_max > 0 ? c->spec_e_max : 2.0f;
+    {
+        const int sel = run_flags & (GADEP_RUN_HISTORY_PER_THREAD | GADEP_RUN_PERSISTENT_LANES | GADEP_RUN_PARITY_LOCALISATION |
+                                     GADEP_RUN_PARTIAL_XS | GADEP_RUN_ELECTRON_RANGE);
+        if (sel & (sel - 1)) { cudaFree(stage_e); cudaFree(stage_f); return gd_fail(c, GADEP_E_ARG, "run flags 0x%x select more than one kernel", run_flags); }
+    }
     c->kernel_variant = gd_variant_of(run_flags & ~(GADEP_RUN_ASYNC | GADEP_RUN_ACCUMULATE));   // 0: the default kernel
+    c->run_width = (run_flags & GADEP_RUN_BVH8) ? 8 : c->bvh_width;
     int rc = gd_launch_transport(c, first, (unsigned long long)n, seed, n_bins, e_max, false, d_e, d_f);
     if (rc == GADEP_OK) rc = gd_fetch_results(c);
     if (rc == GADEP_OK && stage_e) cudaMemcpy(edep_out, stage_e, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost);
@@ -793,7 +827,7 @@ extern "C" int gadep_get_counters(const gadep_ctx *cc, gadep_counters *out) {
     out->n_histories = h.n_histories; out->n_queries = h.n_queries; out->n_box_tests = h.n_box_tests;
     out->n_tri_tests = h.n_tri_tests; out->n_crossings = h.n_crossings; out->n_pe = h.n_pe; out->n_compton = h.n_compton;
     out->n_coherent = h.n_coherent; out->n_pair = h.n_pair; out->n_escaped = h.n_escaped; out->n_leak = h.n_leak;
-    out->n_cutoff = h.n_cutoff; out->n_safety_queries = h.n_safety; out->n_skipped_queries = h.n_skipped;
+    out->n_cutoff = h.n_cutoff; out->n_stack_overflow = c->n_stack_overflow;
     out->n_parity_queries = h.n_parity; out->n_parity_mismatch = h.n_parity_mismatch;
     memcpy(out->emitted, c->h_emitted, sizeof(out->emitted));
     memcpy(out->peak, c->h_peak, sizeof(out->peak));
@@ -830,16 +864,38 @@ extern "C" int gadep_philox_raw(gadep_ctx *c, const unsigned *ctr4, const unsign
     return GADEP_OK;
 }
 
-#ifdef GD_DIAG
-extern "C" int gadep_debug_read_warps(unsigned long long *out) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out, gd_diag_warp, sizeof(unsigned long long) * 4096 * 8);
-    return 0;
+// ---------------------------------------------------------------- traversal width, whole-tally exchange
+extern "C" int gadep_set_bvh_width(gadep_ctx *c, int width) {
+    if (!c) return GADEP_E_NULL;
+    if (width != 4 && width != 8) return gd_fail(c, GADEP_E_ARG, "BVH width %d (4 or 8)", width);
+    c->bvh_width = width;
+    return GADEP_OK;
 }
-extern "C" int gadep_debug_read(unsigned long long *out128, int reset) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out128, gd_diag, sizeof(unsigned long long) * 128);
-    if (reset) { unsigned long long z[128] = {}; cudaMemcpyToSymbol(gd_diag, z, sizeof(z)); }
-    return 0;
+
+extern "C" int gadep_tally_size(const gadep_ctx *c) {
+    if (!c) return GADEP_E_NULL;
+    return c->n_bins > 0 ? c->n_bins + 1 + 2 * GADEP_MAX_LINES : 0;
 }
-#endif
+
+extern "C" int gadep_get_tallies(gadep_ctx *c, unsigned long long *out) {
+    if (!c) return GADEP_E_NULL;
+    if (!out) return gd_fail(c, GADEP_E_NULL, "null output");
+    if (!c->have_results || !c->d_tally) return gd_fail(c, GADEP_E_ORDER, "no run yet");
+    GD_CUDA(c, cudaSetDevice(c->device));
+    const size_t bytes = sizeof(unsigned long long) * ((size_t)c->n_bins + 1 + 2 * GADEP_MAX_LINES);
+    const bool dev = gd_is_device_ptr(out);
+    GD_CUDA(c, cudaMemcpyAsync(out, c->d_tally, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+    if (!dev) GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return GADEP_OK;
+}
+
+extern "C" int gadep_set_tallies(gadep_ctx *c, const unsigned long long *in) {
+    if (!c) return GADEP_E_NULL;
+    if (!in) return gd_fail(c, GADEP_E_NULL, "null input");
+    if (!c->have_results || !c->d_tally) return gd_fail(c, GADEP_E_ORDER, "no run yet");
+    GD_CUDA(c, cudaSetDevice(c->device));
+    const size_t bytes = sizeof(unsigned long long) * ((size_t)c->n_bins + 1 + 2 * GADEP_MAX_LINES);
+    GD_CUDA(c, cudaMemcpyAsync(c->d_tally, in, bytes, gd_is_device_ptr(in) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    c->results_stale = true;
+    return GADEP_OK;
+}

@@ -429,3 +429,94 @@ __global__ void gd_k_collapse4(int n_inner, const int *__restrict__ child_l, con
     nd.pad = make_int4(0, 0, 0, 0);
     out[i] = nd;
 }
+
+// 8-wide compressed nodes (GdNode8, gadep_common.cuh): greedy expansion to eight descendants, octant slots,
+// outward 8-bit quantisation.  One per binary inner node, like the 4-wide nodes.
+__global__ void gd_k_collapse8(int n_inner, const int *__restrict__ child_l, const int *__restrict__ child_r,
+                               const float4 *__restrict__ ref_lo, const float4 *__restrict__ ref_hi,
+                               const unsigned *__restrict__ order, const float4 *__restrict__ node_lo,
+                               const float4 *__restrict__ node_hi, GdNode8 *__restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_inner) return;
+    int c[8] = {child_l[i], child_r[i], GD_NO_CHILD, GD_NO_CHILD, GD_NO_CHILD, GD_NO_CHILD, GD_NO_CHILD, GD_NO_CHILD};
+    int k = 2;
+    while (k < 8) {
+        int best = -1;
+        float best_a = -1.0f;
+        for (int j = 0; j < k; ++j)
+            if (c[j] >= 0) {
+                const float a = gd_half_area(node_lo[c[j]], node_hi[c[j]]);
+                if (a > best_a) { best_a = a; best = j; }
+            }
+        if (best < 0) break;
+        const int b = c[best];
+        c[best] = child_l[b];
+        c[k++] = child_r[b];
+    }
+    const float4 nlo = node_lo[i], nhi = node_hi[i];
+    const float blo[3] = {nlo.x, nlo.y, nlo.z}, bhi[3] = {nhi.x, nhi.y, nhi.z};
+    float clo[8][3], chi[8][3];
+    for (int j = 0; j < k; ++j) {
+        float4 a, b;
+        if (c[j] < 0) { const int o = (int)order[~c[j]]; a = ref_lo[o]; b = ref_hi[o]; }
+        else { a = node_lo[c[j]]; b = node_hi[c[j]]; }
+        clo[j][0] = a.x; clo[j][1] = a.y; clo[j][2] = a.z; chi[j][0] = b.x; chi[j][1] = b.y; chi[j][2] = b.z;
+    }
+    // octant slots: child j likes slot s by how far its centre lies from the node's centre on the side s names
+    int slot_of[8], child_in[8];
+    for (int s = 0; s < 8; ++s) child_in[s] = -1;
+    for (int j = 0; j < 8; ++j) slot_of[j] = -1;
+    for (int it = 0; it < k; ++it) {
+        float best = -3.0e38f;
+        int bj = -1, bs = -1;
+        for (int j = 0; j < k; ++j) {
+            if (slot_of[j] >= 0) continue;
+            float d[3];
+            for (int a = 0; a < 3; ++a) d[a] = 0.5f * (clo[j][a] + chi[j][a]) - 0.5f * (blo[a] + bhi[a]);
+            for (int s = 0; s < 8; ++s) {
+                if (child_in[s] >= 0) continue;
+                const float v = ((s & 1) ? d[0] : -d[0]) + ((s & 2) ? d[1] : -d[1]) + ((s & 4) ? d[2] : -d[2]);
+                if (v > best) { best = v; bj = j; bs = s; }
+            }
+        }
+        slot_of[bj] = bs; child_in[bs] = bj;
+    }
+    GdNode8 nd;
+    unsigned q[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
+    unsigned exyz = 0, valid = 0;
+    float org[3];
+    for (int a = 0; a < 3; ++a) {
+        const float ext = bhi[a] - blo[a];
+        int e = -100;
+        if (ext > 0.0f) {
+            int kk;
+            const float m = frexpf(ext, &kk);               // ext = m 2^kk, m in [0.5, 1)
+            e = m * 256.0f <= 254.5f ? kk - 8 : kk - 7;     // (hi - o) / 2^e + margins stays <= 255
+            e = e < -100 ? -100 : (e > 100 ? 100 : e);
+        }
+        const float S = __int_as_float((e + 127) << 23), invS = __int_as_float((127 - e) << 23);
+        const float o = blo[a] - S * (1.0f / 32.0f);
+        org[a] = o;
+        exyz |= (unsigned)(e + 127) << (8 * a);
+        for (int s = 0; s < 8; ++s) {
+            unsigned ql = 255u, qh = 0u;
+            const int j = child_in[s];
+            if (j >= 0) {
+                const float fl = floorf((clo[j][a] - o) * invS - (1.0f / 64.0f));
+                const float fh = ceilf((chi[j][a] - o) * invS + (1.0f / 64.0f));
+                ql = (unsigned)fminf(fmaxf(fl, 0.0f), 255.0f);
+                qh = (unsigned)fminf(fmaxf(fh, 0.0f), 255.0f);
+            }
+            q[a][s >> 2] |= ql << (8 * (s & 3));
+            q[a][2 + (s >> 2)] |= qh << (8 * (s & 3));
+        }
+    }
+    for (int s = 0; s < 8; ++s) {
+        nd.child[s] = child_in[s] >= 0 ? c[child_in[s]] : GD_NO_CHILD;
+        if (child_in[s] >= 0) valid |= 1u << s;
+    }
+    nd.ox = org[0]; nd.oy = org[1]; nd.oz = org[2];
+    nd.exyz_valid = exyz | (valid << 24);
+    for (int w = 0; w < 4; ++w) { nd.qx[w] = q[0][w]; nd.qy[w] = q[1][w]; nd.qz[w] = q[2][w]; }
+    out[i] = nd;
+}

@@ -48,9 +48,28 @@ struct __align__(16) GdNode4 {
     int4 pad;
 };
 
+// 8-wide compressed node of the default traversal (96 bytes = 6 x 16 B): up to eight descendants of a binary node
+// (greedy expansion of the child with the largest surface area), their boxes quantised to 8 bits per plane on a
+// per-node grid: plane coordinate = o + q * 2^e per axis (e biased by 127, i.e. the exponent field of a float).
+// Quantisation is outward (lo: floor, hi: ceil, plus 1/64 of a step), so a dequantised box contains the child's box
+// and the set of facets a ray can reach is unchanged.  Children sit in the slot whose 3-bit number says on which
+// side of the node's centre they lie (x: bit 0, y: bit 1, z: bit 2; greedy assignment), so that slot ^ (signs of
+// the ray direction) is a front-to-back order without sorting distances (octant order of Ylitie, Karras & Laine,
+// "Efficient incoherent ray traversal on GPUs through compressed wide BVHs", HPG 2017 -- idea restated, layout own).
+// child[k]: as in GdNode4; unused slots have an inverted box (qlo 255, qhi 0) and no bit in the valid mask.
+struct __align__(32) GdNode8 {
+    float ox, oy, oz;
+    unsigned exyz_valid;         // ex | ey << 8 | ez << 16 | valid mask << 24
+    unsigned qx[4];              // qlo of slots 0-3, qlo of slots 4-7, qhi of slots 0-3, qhi of slots 4-7 (one byte per slot)
+    unsigned qy[4], qz[4];
+    int child[8];
+};
+#define GD_STACK8 224               // 8-wide traversal: up to 7 pushes per node visited; overflow is detected and reported
+
 struct GdBvh {
     const GdNode *nodes;
     const GdNode4 *nodes4;
+    const GdNode8 *nodes8;
     const GdTri *tris;
     int n_tri;
     int root_is_leaf;   // n_tri == 1

@@ -146,10 +146,6 @@ struct GdLane {
     GdVec3 p_pos, p_axis;
     GdExclude ex;          // facets crossed on this flight segment within the last GD_TBACK of path
     int n_stall;           // consecutive crossings without progress (safety net)
-    // wavefront kernel only: facet-free sphere (centre, radius; 0 = none) that lets flights skip the BVH query
-    GdVec3 sc;
-    float sr;
-    int cool, qkind;       // safety-query back-off; kind of the pending query (0 ray, 1 safety)
     // partial cross-section method only: remaining optical depth of every process, process that fires next
     float tau_c[4];
     int sel;
@@ -192,7 +188,6 @@ GD_HD void gd_lane_start(GdLane &L, const GdSource &S, unsigned long long seed, 
     L.dep = 0.0f; L.flags = 0; L.n_events = 0; L.pending = 0;
     L.m = 0; L.need_mu = 1; L.mu_tot = 0.0f; L.tau = 0.0f; L.sdist = 0.0f;
     L.ex = gd_no_exclude(); L.n_stall = 0;
-    L.sc = L.pos; L.sr = 0.0f; L.cool = 0; L.qkind = 0;
     L.mode = GD_MODE_LOCATE;
 }
 

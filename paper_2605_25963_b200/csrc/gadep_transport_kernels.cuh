@@ -1,4 +1,4 @@
-// gadep_transport_kernels.cuh -- ray-cast hook and the history-per-thread transport kernel (v0).
+// gadep_transport_kernels.cuh -- the history-per-thread transport kernels (cross-check and measurement modes).
 // source, localisation, free flight, BVH nearest hit, boundary crossing,
 // interactions, tally into a per-block shared-memory spectrum, flush to 64-bit global tallies.
 #pragma once
@@ -26,31 +26,6 @@ GD_D void gd_flush_counters(const GdLocalCounters &c, GdCounters *g, unsigned n_
         for (int o = 16; o >= 1; o >>= 1) x += __shfl_down_sync(0xFFFFFFFFu, x, o);
         if ((threadIdx.x & 31) == 0 && x) atomicAdd(&dst[k], x);
     }
-}
-
-__global__ void __launch_bounds__(256)
-gd_k_trace(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ dir, long long n, int filter_mat,
-           float t_min, int *__restrict__ tri_out, float *__restrict__ t_out, GdCounters *counters) {
-    GdLocalCounters cnt = {};
-    unsigned nq = 0;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long base = (long long)blockIdx.x * blockDim.x + (threadIdx.x & ~31); base < n; base += stride) {   // warp-uniform
-        const long long i = base + (threadIdx.x & 31);
-        const bool active = i < n;
-        GdRay ray;
-        if (active) gd_ray_setup(ray, gd_make(org[3 * i], org[3 * i + 1], org[3 * i + 2]),
-                                 gd_make(dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]));
-        else gd_ray_setup(ray, gd_make(0.f, 0.f, 0.f), gd_make(0.f, 0.f, 1.f));
-        GdHit hit;
-        gd_nearest_hit<true>(bvh, ray, t_min, GD_INF, filter_mat, gd_no_exclude(), active, hit, cnt.n_box_tests, cnt.n_tri_tests);
-        if (active) {
-            tri_out[i] = hit.leaf < 0 ? -1 : hit.orig;
-            t_out[i] = hit.leaf < 0 ? GD_INF : hit.t;
-            nq++;
-        }
-    }
-    cnt.n_queries = nq;
-    gd_flush_counters(cnt, counters, 0);
 }
 
 // dynamic shared memory: [table floats][spectrum u32 (n_bins+1)]

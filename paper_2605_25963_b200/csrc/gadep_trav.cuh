@@ -10,9 +10,6 @@
 
 #define GD_TRAV_DONE ((int)0x80000000)     // node value: traversal finished (leaf codes are ~index > GD_TRAV_DONE)
 #define GD_NO_FACET 0x7FFFFFFF
-#ifndef GD_WITH_SAFETY
-#define GD_WITH_SAFETY 0          // facet-free-sphere queries inside the traversal loop (costs loop-body size)
-#endif
 #define GD_TINF __int_as_float(0x7F800000)
 #ifndef GD_FULL_SORT
 #define GD_FULL_SORT 1
@@ -24,7 +21,7 @@ struct GdTrav {
     float bx, by, bz;        // origin * reciprocal direction (slab test as one FMA per plane)
     float err;               // absolute error bound of the FMA slab distances
     float sx, sy, sz;        // Woop shear / scale
-    int kxyz;                // kx | ky << 2 | kz << 4
+    int kxyz;                // kx | ky << 2 | kz << 4 | octant << 8 (bit a of the octant: direction component a < 0)
     float tmin, t;           // window (tmin, t]; t shrinks to the nearest accepted hit
     int orig;                // caller's facet index of that hit, GD_NO_FACET = none
     int fromto;              // (from-side material & 0xFFFF) | (to-side material << 16) of that hit
@@ -50,7 +47,9 @@ GD_D void gd_trav_begin(GdTrav &T, const GdBvh &bvh, int *stack, float px, float
     if (ddz < 0.0f) { int t = kx; kx = ky; ky = t; }
     float ddx = kx == 0 ? dx : (kx == 1 ? dy : dz), ddy = ky == 0 ? dx : (ky == 1 ? dy : dz);
     T.sz = 1.0f / ddz; T.sx = ddx * T.sz; T.sy = ddy * T.sz;
-    T.kxyz = kx | (ky << 2) | (kz << 4);
+    T.kxyz = kx | (ky << 2) | (kz << 4) |
+             (int)((((unsigned)__float_as_int(T.ix) >> 31) | (((unsigned)__float_as_int(T.iy) >> 31) << 1) |
+                    (((unsigned)__float_as_int(T.iz) >> 31) << 2)) << 8);
     T.tmin = t_min; T.t = t_max; T.orig = GD_NO_FACET; T.fromto = 0;
     T.filter = filter; T.exa = exa; T.exb = exb; T.exc = exc;
     T.sp = 0; T.node = bvh.root_is_leaf ? ~0 : 0;
@@ -65,27 +64,6 @@ GD_D void gd_trav_begin(GdTrav &T, const GdBvh &bvh, int *stack, float px, float
             for (int k = 2; k <= ne; ++k) stack[T.sp++] = __ldg(e + k);
         }
     }
-}
-
-// Safety query (filter == GD_FILTER_SAFETY): lower bound of the distance from a point to the nearest facet, as the
-// distance to the nearest leaf box (a leaf box contains its facet part), searched up to radius sqrt(r2_cap).
-// T.t carries the squared bound; leaves are resolved in their parent, so no triangle is touched.
-#define GD_FILTER_SAFETY (-3)
-GD_D void gd_trav_begin_safety(GdTrav &T, const GdBvh &bvh, float px, float py, float pz, float r2_cap, int slot) {
-    T.ox = px; T.oy = py; T.oz = pz;
-    T.ix = T.iy = T.iz = T.bx = T.by = T.bz = T.err = T.sx = T.sy = T.sz = 0.0f;
-    T.kxyz = 0; T.tmin = 0.0f; T.t = r2_cap; T.orig = GD_NO_FACET; T.fromto = 0;
-    T.filter = GD_FILTER_SAFETY; T.exa = T.exb = T.exc = -1;
-    T.sp = 0; T.node = 0;
-    if (bvh.root_is_leaf) { T.t = 0.0f; T.node = GD_TRAV_DONE; }     // no inner node to read a box from
-    T.slot = slot;
-}
-
-GD_D float gd_box_dist2(float px, float py, float pz, float lx, float hx, float ly, float hy, float lz, float hz) {
-    float dx = fmaxf(fmaxf(lx - px, px - hx), 0.0f);
-    float dy = fmaxf(fmaxf(ly - py, py - hy), 0.0f);
-    float dz = fmaxf(fmaxf(lz - pz, pz - hz), 0.0f);
-    return fmaf(dx, dx, fmaf(dy, dy, dz * dz));
 }
 
 struct GdEdge3 { float u, v, w; int ok; };
@@ -108,7 +86,7 @@ GD_D void gd_trav_leaf(GdTrav &T, const GdBvh &bvh, int leaf, unsigned &n_tri_te
     const int facet = __float_as_int(p0.w);
     if (facet == T.exa || facet == T.exb || facet == T.exc) return;
     n_tri_tests++;
-    const int kx = T.kxyz & 3, ky = (T.kxyz >> 2) & 3, kz = T.kxyz >> 4;
+    const int kx = T.kxyz & 3, ky = (T.kxyz >> 2) & 3, kz = (T.kxyz >> 4) & 3;
     float a0 = p0.x - T.ox, a1 = p0.y - T.oy, a2 = p0.z - T.oz;
     float b0 = p1.x - T.ox, b1 = p1.y - T.oy, b2 = p1.z - T.oz;
     float c0 = p2.x - T.ox, c1 = p2.y - T.oy, c2 = p2.z - T.oz;
@@ -194,44 +172,102 @@ GD_D void gd_trav_node4(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box
     gd_trav_descend4(T, stack, key[0], key[1], key[2], key[3], cc[0], cc[1], cc[2], cc[3]);
 }
 
-// safety query on the 4-wide nodes: leaf children update the bound in place, inner children nearer than it are visited
-GD_D void gd_trav_node4_safety(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
-    const GdNode4 &nd = bvh.nodes4[T.node];
-    const float4 lox = nd.lox, hix = nd.hix, loy = nd.loy, hiy = nd.hiy, loz = nd.loz, hiz = nd.hiz;
-    const int4 ch = nd.child;
-    n_box_tests += 4;
-    float key[4];
-    int cc[4] = {ch.x, ch.y, ch.z, ch.w};
-    key[0] = gd_box_dist2(T.ox, T.oy, T.oz, lox.x, hix.x, loy.x, hiy.x, loz.x, hiz.x);
-    key[1] = gd_box_dist2(T.ox, T.oy, T.oz, lox.y, hix.y, loy.y, hiy.y, loz.y, hiz.y);
-    key[2] = gd_box_dist2(T.ox, T.oy, T.oz, lox.z, hix.z, loy.z, hiy.z, loz.z, hiz.z);
-    key[3] = gd_box_dist2(T.ox, T.oy, T.oz, lox.w, hix.w, loy.w, hiy.w, loz.w, hiz.w);
+
+// rays that ran out of traversal stack (8-wide nodes: up to 7 pushes per visit); read and reported by the host
+__device__ unsigned gd_stack_overflow;
+
+// one 8-wide compressed node visit (GdNode8): six 16-byte loads for eight boxes.  A quantised plane q of an axis lies at
+// o + q 2^e; its slab distance is ((o - p) + q 2^e) / d = A + q B with B = 2^e / d and A from the same FMA as the
+// 4-wide test.  The byte goes straight into the mantissa of the float 32768 + q (one PRMT, no integer-to-float
+// conversion), so the distance is fma(32768 + q, B, A - 32768 B); the two extra roundings are bounded by |B| / 256
+// per axis, which widens that axis' slab.  Hit children are visited in octant order (slot ^ direction signs).
+#define GD_SELB(c, a, b) ((c) ? (a) : (b))
+GD_D void gd_trav_node8(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
+    const uint4 *nd = reinterpret_cast<const uint4 *>(bvh.nodes8 + T.node);
+    const uint4 hd = nd[0], qx = nd[1], qy = nd[2], qz = nd[3];
+    const uint4 ca = nd[4], cb = nd[5];
+    const unsigned valid = hd.w >> 24;
+    n_box_tests += __popc(valid);
+    const float Bx = __uint_as_float((hd.w & 0xFFu) << 23) * T.ix;
+    const float By = __uint_as_float(((hd.w >> 8) & 0xFFu) << 23) * T.iy;
+    const float Bz = __uint_as_float(((hd.w >> 16) & 0xFFu) << 23) * T.iz;
+    const float Ax = fmaf(-32768.0f, Bx, fmaf(__uint_as_float(hd.x), T.ix, -T.bx));
+    const float Ay = fmaf(-32768.0f, By, fmaf(__uint_as_float(hd.y), T.iy, -T.by));
+    const float Az = fmaf(-32768.0f, Bz, fmaf(__uint_as_float(hd.z), T.iz, -T.bz));
+    // error bound of a slab distance, per axis (an axis the ray is almost parallel to has a huge B: its bound must not
+    // loosen the other two): |B| / 256 for the two extra roundings + the bound of the 4-wide test; near planes move
+    // down by it, far planes up
+    const float ex = fmaf(fabsf(Bx), 1.0f / 256.0f, T.err), ey = fmaf(fabsf(By), 1.0f / 256.0f, T.err), ez = fmaf(fabsf(Bz), 1.0f / 256.0f, T.err);
+    const float Anx = Ax - ex, Afx = Ax + ex, Any = Ay - ey, Afy = Ay + ey, Anz = Az - ez, Afz = Az + ez;
+    const bool ngx = __float_as_int(T.ix) < 0, ngy = __float_as_int(T.iy) < 0, ngz = __float_as_int(T.iz) < 0;
+    // near / far plane words of slots 0-3 and 4-7: the near plane is lo for a positive direction component, else hi
+    const unsigned nx0 = GD_SELB(ngx, qx.z, qx.x), nx1 = GD_SELB(ngx, qx.w, qx.y), fx0 = GD_SELB(ngx, qx.x, qx.z), fx1 = GD_SELB(ngx, qx.y, qx.w);
+    const unsigned ny0 = GD_SELB(ngy, qy.z, qy.x), ny1 = GD_SELB(ngy, qy.w, qy.y), fy0 = GD_SELB(ngy, qy.x, qy.z), fy1 = GD_SELB(ngy, qy.y, qy.w);
+    const unsigned nz0 = GD_SELB(ngz, qz.z, qz.x), nz1 = GD_SELB(ngz, qz.w, qz.y), fz0 = GD_SELB(ngz, qz.x, qz.z), fz1 = GD_SELB(ngz, qz.y, qz.w);
+    const float pad = 4.0e-7f;
+    unsigned hm = 0;
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
-        if (cc[k] < 0 && cc[k] != GD_NO_CHILD && key[k] < T.t) T.t = key[k];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const bool v = cc[k] >= 0 && key[k] < T.t;
-        key[k] = v ? key[k] : GD_TINF;
-        cc[k] = v ? cc[k] : GD_NO_CHILD;
+    for (int k = 0; k < 8; ++k) {
+        const unsigned sel = 0x7604u | ((unsigned)(k & 3) << 4);       // byte k & 3 of the word -> bits 8..15 of 0x47000000
+        const float x0 = fmaf(__uint_as_float(__byte_perm(k < 4 ? nx0 : nx1, 0x47000000u, sel)), Bx, Anx);
+        const float x1 = fmaf(__uint_as_float(__byte_perm(k < 4 ? fx0 : fx1, 0x47000000u, sel)), Bx, Afx);
+        const float y0 = fmaf(__uint_as_float(__byte_perm(k < 4 ? ny0 : ny1, 0x47000000u, sel)), By, Any);
+        const float y1 = fmaf(__uint_as_float(__byte_perm(k < 4 ? fy0 : fy1, 0x47000000u, sel)), By, Afy);
+        const float z0 = fmaf(__uint_as_float(__byte_perm(k < 4 ? nz0 : nz1, 0x47000000u, sel)), Bz, Anz);
+        const float z1 = fmaf(__uint_as_float(__byte_perm(k < 4 ? fz0 : fz1, 0x47000000u, sel)), Bz, Afz);
+        const float n = fmaxf(fmaxf(x0, y0), fmaxf(z0, T.tmin));
+        float f = fminf(fminf(x1, y1), fminf(z1, T.t));
+        f = fmaf(fabsf(f), pad, f);
+        hm |= n <= f ? (1u << k) : 0u;
     }
-    gd_trav_descend4(T, stack, key[0], key[1], key[2], key[3], cc[0], cc[1], cc[2], cc[3]);
+    hm &= valid;
+    // octant order: position p = slot ^ r is visited before p + 1; permute links and hit bits into position order
+    const unsigned r = ((unsigned)T.kxyz >> 8) & 7u;
+    int c0 = (int)ca.x, c1 = (int)ca.y, c2 = (int)ca.z, c3 = (int)ca.w, c4 = (int)cb.x, c5 = (int)cb.y, c6 = (int)cb.z, c7 = (int)cb.w;
+    {
+        const bool s1 = r & 1u, s2 = r & 2u, s4 = r & 4u;
+        int t;
+        t = GD_SELB(s1, c1, c0); c1 = GD_SELB(s1, c0, c1); c0 = t;  t = GD_SELB(s1, c3, c2); c3 = GD_SELB(s1, c2, c3); c2 = t;
+        t = GD_SELB(s1, c5, c4); c5 = GD_SELB(s1, c4, c5); c4 = t;  t = GD_SELB(s1, c7, c6); c7 = GD_SELB(s1, c6, c7); c6 = t;
+        hm = GD_SELB(s1, ((hm & 0xAAu) >> 1) | ((hm & 0x55u) << 1), hm);
+        t = GD_SELB(s2, c2, c0); c2 = GD_SELB(s2, c0, c2); c0 = t;  t = GD_SELB(s2, c3, c1); c3 = GD_SELB(s2, c1, c3); c1 = t;
+        t = GD_SELB(s2, c6, c4); c6 = GD_SELB(s2, c4, c6); c4 = t;  t = GD_SELB(s2, c7, c5); c7 = GD_SELB(s2, c5, c7); c5 = t;
+        hm = GD_SELB(s2, ((hm & 0xCCu) >> 2) | ((hm & 0x33u) << 2), hm);
+        t = GD_SELB(s4, c4, c0); c4 = GD_SELB(s4, c0, c4); c0 = t;  t = GD_SELB(s4, c5, c1); c5 = GD_SELB(s4, c1, c5); c1 = t;
+        t = GD_SELB(s4, c6, c2); c6 = GD_SELB(s4, c2, c6); c2 = t;  t = GD_SELB(s4, c7, c3); c7 = GD_SELB(s4, c3, c7); c3 = t;
+        hm = GD_SELB(s4, ((hm & 0xF0u) >> 4) | ((hm & 0x0Fu) << 4), hm);
+    }
+    if (hm == 0u) { T.node = gd_trav_pop(T, stack); return; }
+    if (T.sp > GD_STACK8 - 8) {                 // cannot happen on the meshes of the five workloads; reported, never silent
+        atomicAdd(&gd_stack_overflow, 1u);
+        T.node = GD_TRAV_DONE; T.sp = 0; T.orig = GD_NO_FACET;
+        return;
+    }
+    const unsigned rest = hm & (hm - 1u);       // all hits but the first in order: pushed far to near
+    if (rest & 0x80u) stack[T.sp++] = c7;
+    if (rest & 0x40u) stack[T.sp++] = c6;
+    if (rest & 0x20u) stack[T.sp++] = c5;
+    if (rest & 0x10u) stack[T.sp++] = c4;
+    if (rest & 0x08u) stack[T.sp++] = c3;
+    if (rest & 0x04u) stack[T.sp++] = c2;
+    if (rest & 0x02u) stack[T.sp++] = c1;
+    const unsigned low = hm & (0u - hm);
+    T.node = (low & 0x0Fu) ? ((low & 0x03u) ? ((low & 1u) ? c0 : c1) : ((low & 4u) ? c2 : c3))
+                           : ((low & 0x30u) ? ((low & 0x10u) ? c4 : c5) : ((low & 0x40u) ? c6 : c7));
 }
 
 // Advance the warp: every busy lane makes up to `n_steps` inner-node visits (no warp vote in between: a lane that
 // reaches a leaf or the end of its ray idles for the rest of the round), then the lanes waiting at a leaf run
 // their triangle test together.  One vote-free round amortises the scheduling work of the caller (fetch, retire)
 // over several node visits and gathers several lanes for the rarer, more expensive leaf step.
+template <int WIDTH>
 GD_D void gd_trav_step(GdTrav &T, const GdBvh &bvh, int *stack, int n_steps, unsigned &n_box_tests,
                        unsigned &n_tri_tests) {
 #pragma unroll 1
     for (int k = 0; k < n_steps; ++k) {
         if (T.node >= 0) {
-#if GD_WITH_SAFETY
-            if (T.filter == GD_FILTER_SAFETY) gd_trav_node4_safety(T, bvh, stack, n_box_tests);
-            else
-#endif
-            gd_trav_node4(T, bvh, stack, n_box_tests);
+            if (WIDTH == 8) gd_trav_node8(T, bvh, stack, n_box_tests);
+            else gd_trav_node4(T, bvh, stack, n_box_tests);
         }
     }
     if (T.node < 0 && T.node != GD_TRAV_DONE) {

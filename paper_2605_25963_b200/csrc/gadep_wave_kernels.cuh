@@ -22,35 +22,23 @@
 #define GD_W_THREADS 512
 #define GD_W_WARPS (GD_W_THREADS / 32)
 #define GD_W_SLOTS 64
-// fields per slot; the facet-free sphere (25..28) only exists with GD_WITH_SAFETY.  Without it the block's shared
-// memory stays under the 164 KB carve-out for up to 9 materials, which leaves the SM a 64 KB L1 instead of 32 KB.
-#define GD_W_NF (GD_WITH_SAFETY ? 29 : 25)
+// fields per slot.  25 words keep the block's shared memory under the 164 KB carve-out for up to 9 materials, which
+// leaves the SM a 64 KB L1 instead of 32 KB.
+#define GD_W_NF 25
 
-#ifdef GD_DIAG
-__device__ unsigned long long gd_diag[128];
-__device__ unsigned long long gd_diag_warp[4096][8];
-#define GD_DIAG_ADD(k, v) do { dacc[k] += (unsigned long long)(v); } while (0)
-#else
-#define GD_DIAG_ADD(k, v) do {} while (0)
-#endif
-
-// scheduling knobs (defaults in gadep_api.cu; GADEP_TUNE="k_fetch,k_exit,n_steps[,lam_max,cap_mfp,sparse_max]" overrides
-// them for measurement sweeps).  None of them can change a result.
+// scheduling knobs (defaults in gadep_api.cu; GADEP_TUNE="k_fetch,k_exit,n_steps" overrides them for measurement
+// sweeps).  None of them can change a result.
 struct GdWaveTune {
     int k_fetch;        // idle lanes needed before READY slots are fetched
     int k_exit;         // T-burst ends when n_results >= k_exit * rays in flight (or 32 results) and READY is empty
     int n_steps;        // node visits per traversal round
-    float lam_max;      // safety queries only where the mean free path is below this [mm]; 0 disables them
-    float cap_mfp;      // search radius of a safety query in mean free paths
-    int sparse_max;     // ... and only while the warp has at most this many live photons
 };
 
 // ---- slot <-> registers
 #define GD_SF(f) sl[(f) * GD_W_SLOTS + s]
 GD_D unsigned gd_pack_state(const GdLane &L) {
     return (unsigned)(L.m + 1) | ((unsigned)L.mode << 5) | ((unsigned)L.line << 7) | ((unsigned)L.pending << 13) |
-           ((unsigned)L.n_stall << 15) | (L.g.stream << 21) | ((unsigned)L.need_mu << 23) | ((unsigned)L.cool << 24) |
-           ((unsigned)L.qkind << 27);
+           ((unsigned)L.n_stall << 15) | (L.g.stream << 21) | ((unsigned)L.need_mu << 23);
 }
 GD_D void gd_slot_store(float *sl, int s, const GdLane &L, unsigned long long first) {
     GD_SF(0) = L.pos.x; GD_SF(1) = L.pos.y; GD_SF(2) = L.pos.z;
@@ -64,7 +52,6 @@ GD_D void gd_slot_store(float *sl, int s, const GdLane &L, unsigned long long fi
     GD_SF(17) = L.dep;
     GD_SF(18) = __uint_as_float((L.flags & 0xFFu) | ((L.n_events > 0xFFFFu ? 0xFFFFu : L.n_events) << 16));
     GD_SF(19) = __int_as_float(L.ex.a); GD_SF(20) = __int_as_float(L.ex.b); GD_SF(21) = __int_as_float(L.ex.c);
-    if (GD_WITH_SAFETY) { GD_SF(25) = L.sc.x; GD_SF(26) = L.sc.y; GD_SF(27) = L.sc.z; GD_SF(28) = L.sr; }
 }
 GD_D void gd_slot_load(const float *sl, int s, GdLane &L, unsigned long long seed, unsigned long long first) {
     L.pos = gd_make(GD_SF(0), GD_SF(1), GD_SF(2));
@@ -81,56 +68,43 @@ GD_D void gd_slot_load(const float *sl, int s, GdLane &L, unsigned long long see
     const unsigned fe = __float_as_uint(GD_SF(18));
     L.flags = fe & 0xFFu; L.n_events = fe >> 16;
     L.ex.a = __float_as_int(GD_SF(19)); L.ex.b = __float_as_int(GD_SF(20)); L.ex.c = __float_as_int(GD_SF(21));
-    L.cool = (int)((st >> 24) & 7u); L.qkind = (int)((st >> 27) & 1u);
-    if (GD_WITH_SAFETY) { L.sc = gd_make(GD_SF(25), GD_SF(26), GD_SF(27)); L.sr = GD_SF(28); }
-    else { L.sc = L.pos; L.sr = 0.0f; }
 }
 
-// What the slot does next (mode FLIGHT, sdist known).  Purely a scheduling decision: a skipped query is one whose
-// answer is known to be "no facet within (-GD_TBACK, sdist]" because a facet-free sphere covers the whole flight.
-#define GD_PLAN_RAY 0
-#define GD_PLAN_SAFETY 1
-#define GD_PLAN_SKIP 2
-#ifdef GD_DIAG
-#define GD_PLAN_RET(reason, plan) do { atomicAdd(&gd_diag[32 + (L.m < 0 ? 0 : L.m) * 8 + (reason)], 1ull); return (plan); } while (0)
-#else
-#define GD_PLAN_RET(reason, plan) return (plan)
-#endif
-GD_D int gd_wave_plan(GdLane &L, const GdWaveTune &tune, bool allow_safety, float &r2_cap) {
-    if (!GD_WITH_SAFETY || L.mode != GD_MODE_FLIGHT || !(L.sdist < GD_INF) || !(tune.lam_max > 0.0f)) GD_PLAN_RET(0, GD_PLAN_RAY);
-    float d = 0.0f;
-    if (L.sr > 0.0f) {
-        const float dx = L.pos.x - L.sc.x, dy = L.pos.y - L.sc.y, dz = L.pos.z - L.sc.z;
-        d = sqrtf(dx * dx + dy * dy + dz * dz);
-        if (d * 1.0001f + L.sdist * 1.0001f + 4.0f * GD_TBACK < L.sr) GD_PLAN_RET(1, GD_PLAN_SKIP);
+// O14 tally of the histories that ended in this batch, aggregated per warp: lanes that hit the same
+// counter are found with __match_any_sync and their leader adds the group's size, so the five hot `emitted` words of
+// a point-source run see one shared-memory atomic per line and batch instead of one per history.
+// `fin` may differ from lane to lane; every lane of the warp must call.
+GD_D void gd_tally_warp(bool fin, const GdHistory &r, const GdSource &S, const GdTally &tally, unsigned *s_spec,
+                        unsigned *s_emitted, unsigned *s_peak, unsigned lane) {
+    const unsigned fin_mask = __ballot_sync(0xFFFFFFFFu, fin);
+    if (fin_mask == 0u) return;
+    int bin = -1;                                     // spectrum bin of this lane's history, -1 = nothing to book
+    const bool peak = fin && (r.flags & GD_F_PEAK);
+    if (peak) bin = min(S.line_bin[r.line], tally.n_bins);
+    else if (fin && r.edep > 0.0f) {
+        const float b = floorf(r.edep * tally.inv_de);
+        bin = b >= (float)tally.n_bins ? tally.n_bins : (int)b;
     }
-    // a safety query only right after an interaction (never on a surface), in an optically thick medium, and not
-    // while an earlier sphere still covers the neighbourhood or an earlier query came back too small to pay off
-    const float lam = 1.0f / L.mu_tot;
-    if (!allow_safety || !(lam < tune.lam_max)) GD_PLAN_RET(2, GD_PLAN_RAY);
-    if (L.ex.a >= 0) GD_PLAN_RET(3, GD_PLAN_RAY);
-    if (L.sr > 0.0f && d < 0.5f * L.sr) GD_PLAN_RET(4, GD_PLAN_RAY);
-    if (L.cool > 0) { L.cool--; GD_PLAN_RET(5, GD_PLAN_RAY); }
-    const float r = tune.cap_mfp * lam;
-    r2_cap = r * r;
-    GD_PLAN_RET(6, GD_PLAN_SAFETY);
-}
-
-GD_D void gd_tally_history(const GdHistory &r, const GdSource &S, const GdTally &tally, unsigned *s_spec,
-                           unsigned *s_emitted, unsigned *s_peak) {
-    atomicAdd(&s_emitted[r.line], 1u);
-    if (r.flags & GD_F_PEAK) {
-        atomicAdd(&s_peak[r.line], 1u);
-        atomicAdd(&s_spec[min(S.line_bin[r.line], tally.n_bins)], 1u);
-    } else if (r.edep > 0.0f) {
-        float b = floorf(r.edep * tally.inv_de);
-        int bin = b >= (float)tally.n_bins ? tally.n_bins : (int)b;
-        atomicAdd(&s_spec[bin], 1u);
+    if (fin) {
+        const unsigned same = __match_any_sync(fin_mask, r.line);
+        if ((same & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_emitted[r.line], (unsigned)__popc(same));
+    }
+    const unsigned peak_mask = __ballot_sync(0xFFFFFFFFu, peak);
+    if (peak) {
+        const unsigned same = __match_any_sync(peak_mask, r.line);
+        if ((same & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_peak[r.line], (unsigned)__popc(same));
+    }
+    const unsigned bin_mask = __ballot_sync(0xFFFFFFFFu, bin >= 0);
+    if (bin >= 0) {
+        const unsigned same = __match_any_sync(bin_mask, bin);
+        if ((same & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_spec[bin], (unsigned)__popc(same));
     }
 }
 
 // dynamic shared memory: [table floats][spectrum u32 (n_bins+1)][slots: warps x GD_W_NF x GD_W_SLOTS floats]
 // pair_buf: global, 8 floats per slot of every warp of the grid
+// WIDTH: 8 = compressed 8-wide nodes (default), 4 = uncompressed 4-wide nodes (cross-check variant)
+template <int WIDTH>
 __global__ void __launch_bounds__(GD_W_THREADS, 1)
 gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
                     unsigned long long n_hist, unsigned long long seed, GdTally tally, float *__restrict__ edep_out,
@@ -139,7 +113,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     extern __shared__ __align__(16) unsigned char gd_smem[];
     __shared__ GdSource s_src;
     __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];
-    __shared__ unsigned s_cnt[14];
+    __shared__ unsigned s_cnt[12];
     __shared__ unsigned char s_qready[GD_W_WARPS][GD_W_SLOTS], s_qres[GD_W_WARPS][GD_W_SLOTS];
     const int n_tab = M.n_mat * 4 * M.n_grid;
     float *s_tab = (float *)gd_smem;
@@ -149,7 +123,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) s_spec[i] = 0;
     for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i];
     if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }
-    if (threadIdx.x < 14) s_cnt[threadIdx.x] = 0;
+    if (threadIdx.x < 12) s_cnt[threadIdx.x] = 0;
     __syncthreads();
 
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -157,7 +131,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     float *sl = s_slots + (size_t)warp * GD_W_NF * GD_W_SLOTS;
     unsigned char *q_ready = s_qready[warp], *q_res = s_qres[warp];
     float *pair = pair_buf + ((size_t)blockIdx.x * GD_W_WARPS + warp) * GD_W_SLOTS * 8;
-    int stack[GD_STACK4];
+    int stack[WIDTH == 8 ? GD_STACK8 : GD_STACK4];
     GdTrav T;
     gd_trav_idle(T);
     unsigned n_box = 0, n_tri = 0, n_query = 0, n_done = 0;
@@ -171,35 +145,22 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     // waiting at the bottom of a stack while fresh histories stream over it -- the chains are the critical path
     int n_res = GD_W_SLOTS, n_ready = 0, h_res = 0, h_ready = 0;
     static_assert((GD_W_SLOTS & (GD_W_SLOTS - 1)) == 0, "slot count must be a power of two");
-#ifdef GD_DIAG
-    unsigned d_steps = 0;
-    unsigned long long dacc[20] = {};
-    const long long d_start = clock64();
-#endif
     __syncwarp();
 
     for (;;) {
         // ================================================================ P-burst
-#ifdef GD_DIAG
-        long long d_t0 = clock64();
-#endif
         // full batches first; a partial batch only when the warp would otherwise starve
         bool did_full = false;
         while (n_res >= 32 || (n_res > 0 && n_ready == 0 && !did_full)) {
             const int take = n_res < 32 ? n_res : 32;
             did_full = take == 32;
-            GD_DIAG_ADD(8, 1); GD_DIAG_ADD(9, take);
-            bool act = (int)lane < take;           // this lane still works on slot s in this batch
+            const bool act = (int)lane < take;           // this lane works on slot s in this batch
             const int s = act ? (int)q_res[(h_res + (int)lane) & (GD_W_SLOTS - 1)] : 0;
             h_res = (h_res + take) & (GD_W_SLOTS - 1); n_res -= take;
-            // facet-free-sphere queries only while the warp is sparse (drain of a launch, few long scattering chains):
-            // there they shorten the chains; in a full warp they would only add divergence to the traversal loop
-            const bool sparse = take + n_res + n_ready + __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0)) <= tune.sparse_max;
             GdLane L;
             L.mode = GD_MODE_DONE;
             GdHit hit;
             hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
-            bool safety_result = false;
             if (act) {
                 gd_slot_load(sl, s, L, seed, first);
                 if (L.pending) {
@@ -212,111 +173,83 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                 hit.orig = __float_as_int(GD_SF(23));
                 hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
                 hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
-                safety_result = L.qkind == 1;
             }
-            // A lane whose next flight is covered by its facet-free sphere knows the answer of the query ("no facet")
-            // and goes round again in registers -- but only while its warp has nothing else to do (tail of a run,
-            // long scattering chains), so that the other lanes are not kept waiting.
-            for (int it = 0;; ++it) {
-                GdLocalCounters cnt = {};
-                if (act && L.mode != GD_MODE_NEED) {
-                    if (safety_result) {
-                        // facet-free sphere around the current point (a lower bound, rounded down)
-                        const float r = sqrtf(hit.t);
-                        L.sc = L.pos; L.sr = fmaxf(r * 0.9999f - 1.0e-5f, 0.0f);
-                        L.cool = L.sr * L.mu_tot < 2.0f ? 3 : 0;      // under two mean free paths: back off
-                        L.qkind = 0;
-                    } else {
-                        const int was_pending = L.pending;
-                        GdHistory r;
-                        if (gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt)) {
-                            n_done++;
-                            gd_tally_history(r, s_src, tally, s_spec, s_emitted, s_peak);
-                            const unsigned long long hrel = L.history - first;
-                            if (edep_out) edep_out[hrel] = r.edep;
-                            if (flags_out) flags_out[hrel] = r.flags;
-                        } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
-                            float *p = pair + s * 8;
-                            p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
-                            p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
-                        }
-                        {   // one event kind per visit (crossing / PE / Compton / coherent / pair), rarer flags apart
-                            const int kind = cnt.n_crossings ? 4 : (cnt.n_coherent ? 7 : (cnt.n_compton ? 6 : (cnt.n_pe ? 5 : (cnt.n_pair ? 8 : -1))));
-                            if (kind >= 0) atomicAdd(&s_cnt[kind], 1u);
-                        }
-                        if (cnt.n_escaped) atomicAdd(&s_cnt[9], cnt.n_escaped);
-                        if (cnt.n_leak) atomicAdd(&s_cnt[10], cnt.n_leak);
-                        if (cnt.n_cutoff) atomicAdd(&s_cnt[11], cnt.n_cutoff);
-                    }
+            GdLocalCounters cnt = {};
+            GdHistory r;
+            r.edep = 0.0f; r.flags = 0u; r.line = 0;
+            bool fin = false;
+            if (act && L.mode != GD_MODE_NEED) {
+                const int was_pending = L.pending;
+                fin = gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt);
+                if (fin) {
+                    n_done++;
+                    const unsigned long long hrel = L.history - first;
+                    if (edep_out) edep_out[hrel] = r.edep;
+                    if (flags_out) flags_out[hrel] = r.flags;
+                } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
+                    float *p = pair + s * 8;
+                    p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
+                    p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
                 }
-                safety_result = false;
-                // ---- refill finished slots from the history counter (warp-level chunks)
-                const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, act && L.mode == GD_MODE_NEED);
-                if (need_mask) {
-                    const unsigned n_need = __popc(need_mask);
-                    unsigned long long new_base = 0;
-                    const bool refill = w_cur + n_need > w_end;
-                    unsigned my_chunk = chunk;
-                    if (refill) {
-                        // guided: towards the end of the launch the chunks shrink with what is left, so that the last
-                        // histories spread over all warps instead of going to the few that ask last
-                        if (lane == 0) {
-                            const unsigned long long cur = *(volatile unsigned long long *)next_history;
-                            const unsigned long long rem = cur < n_hist ? n_hist - cur : 0ull;
-                            const unsigned long long g = rem / ((unsigned long long)gridDim.x * GD_W_WARPS * 2ull);
-                            if (g < my_chunk) my_chunk = g < 32ull ? 32u : (unsigned)g;
-                            new_base = atomicAdd(next_history, (unsigned long long)my_chunk);
-                        }
-                        new_base = __shfl_sync(0xFFFFFFFFu, new_base, 0);
-                        my_chunk = __shfl_sync(0xFFFFFFFFu, my_chunk, 0);
-                    }
-                    if (act && L.mode == GD_MODE_NEED) {
-                        unsigned long long h = w_cur + __popc(need_mask & lt_mask);
-                        if (h >= w_end) h = new_base + (h - w_end);
-                        if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
-                        else L.mode = GD_MODE_DONE;
-                    }
-                    if (refill) { w_cur = new_base + (w_cur + n_need - w_end); w_end = new_base + my_chunk; }
-                    else w_cur += n_need;
-                }
-                // ---- prepare the next query: READY (ray / safety query), or the known answer "no facet"
-                const bool live = act && L.mode != GD_MODE_DONE;
-                int plan = GD_PLAN_RAY;
-                float r2_cap = 0.0f;
-                if (live) {
-                    float t_min, t_max;
-                    int filter;
-                    gd_lane_query(L, M, s_tab, t_min, t_max, filter);
-                    plan = gd_wave_plan(L, tune, sparse, r2_cap);
-                    L.qkind = plan == GD_PLAN_SAFETY ? 1 : 0;
-                }
-                const bool skip = live && plan == GD_PLAN_SKIP;
-                const unsigned ready_mask = __ballot_sync(0xFFFFFFFFu, live && !skip);
-                const unsigned skip_mask = __ballot_sync(0xFFFFFFFFu, skip);
-                const bool spin = skip_mask != 0u && ready_mask == 0u && n_ready == 0 && n_res == 0 && it < 16;
-                if (live && !(skip && spin)) {
-                    gd_slot_store(sl, s, L, first);
-                    if (plan == GD_PLAN_SAFETY) { GD_SF(22) = r2_cap; atomicAdd(&s_cnt[12], 1u); }
-                    else if (skip) { GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
-                    if (skip) q_res[(h_res + n_res + __popc(skip_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
-                    else q_ready[(h_ready + n_ready + __popc(ready_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
-                }
-                if (skip) atomicAdd(&s_cnt[13], 1u);
-                n_ready += __popc(ready_mask);
-                if (!spin) { n_res += __popc(skip_mask); break; }
-                act = skip;
-                hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET;
             }
+            gd_tally_warp(fin, r, s_src, tally, s_spec, s_emitted, s_peak, lane);
+            {   // event counters, one shared-memory atomic per kind and batch (crossing / PE / Compton / coherent / pair;
+                // escapes, re-localisations and cut-offs can accompany any of them)
+                const unsigned v[8] = {cnt.n_crossings, cnt.n_pe, cnt.n_compton, cnt.n_coherent, cnt.n_pair, cnt.n_escaped,
+                                       cnt.n_leak, cnt.n_cutoff};
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const unsigned mk = __ballot_sync(0xFFFFFFFFu, v[k] != 0u);
+                    if (mk && lane == 0) atomicAdd(&s_cnt[4 + k], (unsigned)__popc(mk));
+                }
+            }
+            // ---- refill finished slots from the history counter (warp-level chunks)
+            const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, act && L.mode == GD_MODE_NEED);
+            if (need_mask) {
+                const unsigned n_need = __popc(need_mask);
+                unsigned long long new_base = 0;
+                const bool refill = w_cur + n_need > w_end;
+                unsigned my_chunk = chunk;
+                if (refill) {
+                    // guided: towards the end of the launch the chunks shrink with what is left, so that the last
+                    // histories spread over all warps instead of going to the few that ask last
+                    if (lane == 0) {
+                        const unsigned long long cur = *(volatile unsigned long long *)next_history;
+                        const unsigned long long rem = cur < n_hist ? n_hist - cur : 0ull;
+                        const unsigned long long g = rem / ((unsigned long long)gridDim.x * GD_W_WARPS * 2ull);
+                        if (g < my_chunk) my_chunk = g < 32ull ? 32u : (unsigned)g;
+                        new_base = atomicAdd(next_history, (unsigned long long)my_chunk);
+                    }
+                    new_base = __shfl_sync(0xFFFFFFFFu, new_base, 0);
+                    my_chunk = __shfl_sync(0xFFFFFFFFu, my_chunk, 0);
+                }
+                if (act && L.mode == GD_MODE_NEED) {
+                    unsigned long long h = w_cur + __popc(need_mask & lt_mask);
+                    if (h >= w_end) h = new_base + (h - w_end);
+                    if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
+                    else L.mode = GD_MODE_DONE;
+                }
+                if (refill) { w_cur = new_base + (w_cur + n_need - w_end); w_end = new_base + my_chunk; }
+                else w_cur += n_need;
+            }
+            // ---- prepare the next query and hand the slot to READY
+            const bool live = act && L.mode != GD_MODE_DONE;
+            if (live) {
+                float t_min, t_max;
+                int filter;
+                gd_lane_query(L, M, s_tab, t_min, t_max, filter);
+            }
+            const unsigned ready_mask = __ballot_sync(0xFFFFFFFFu, live);
+            if (live) {
+                gd_slot_store(sl, s, L, first);
+                q_ready[(h_ready + n_ready + __popc(ready_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
+            }
+            n_ready += __popc(ready_mask);
             __syncwarp();
         }
-#ifdef GD_DIAG
-        long long d_t1 = clock64(); GD_DIAG_ADD(16, d_t1 - d_t0);
-#endif
         const unsigned busy_mask = __ballot_sync(0xFFFFFFFFu, T.slot >= 0);
         if (n_ready == 0 && busy_mask == 0u) {
-            if (n_res == 0) {                                // every slot is dead
-                break;
-            }
+            if (n_res == 0) break;                           // every slot is dead
             continue;
         }
         // ================================================================ T-burst
@@ -330,41 +263,22 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                         if (T.slot < 0 && rank < n_ready) {
                             const int s = (int)q_ready[(h_ready + rank) & (GD_W_SLOTS - 1)];
                             const unsigned st = __float_as_uint(GD_SF(14));
-#if GD_WITH_SAFETY
-                            if ((st >> 27) & 1u) {
-                                gd_trav_begin_safety(T, bvh, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(22), s);
-                            } else
-#endif
-                            {
-                                const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
-                                gd_trav_begin(T, bvh, stack, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
-                                              loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
-                                              __float_as_int(GD_SF(19)), __float_as_int(GD_SF(20)), __float_as_int(GD_SF(21)), s);
-                                n_query++;
-                            }
+                            const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
+                            gd_trav_begin(T, bvh, stack, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
+                                          loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
+                                          __float_as_int(GD_SF(19)), __float_as_int(GD_SF(20)), __float_as_int(GD_SF(21)), s);
+                            n_query++;
                         }
-                        GD_DIAG_ADD(4, 1); GD_DIAG_ADD(5, n_idle < n_ready ? n_idle : n_ready);
-                        { const int tk = n_idle < n_ready ? n_idle : n_ready; h_ready = (h_ready + tk) & (GD_W_SLOTS - 1); n_ready -= tk; }
+                        const int tk = n_idle < n_ready ? n_idle : n_ready;
+                        h_ready = (h_ready + tk) & (GD_W_SLOTS - 1); n_ready -= tk;
                     }
                 } else if ((n_res > 0 && (n_res >= 32 || n_res >= tune.k_exit * (32 - n_idle))) || n_idle == 32) {
                     break;
                 }
             }
-#ifdef GD_DIAG
-            {
-                unsigned a_node = __ballot_sync(0xFFFFFFFFu, T.node >= 0);
-                unsigned a_leaf = __ballot_sync(0xFFFFFFFFu, T.node < 0 && T.node != GD_TRAV_DONE);
-                GD_DIAG_ADD(0, 1); GD_DIAG_ADD(1, __popc(a_node)); GD_DIAG_ADD(2, __popc(a_leaf)); GD_DIAG_ADD(3, n_idle);
-                if (n_ready > 0) GD_DIAG_ADD(10, 1); else GD_DIAG_ADD(11, 1);
-                if (T.slot >= 0) d_steps++;
-            }
-#endif
-            gd_trav_step(T, bvh, stack, tune.n_steps, n_box, n_tri);
+            gd_trav_step<WIDTH>(T, bvh, stack, tune.n_steps, n_box, n_tri);
             const bool fin = T.slot >= 0 && T.node == GD_TRAV_DONE;
             const unsigned fin_mask = __ballot_sync(0xFFFFFFFFu, fin);
-#ifdef GD_DIAG
-            if (fin) d_steps = 0;
-#endif
             if (fin_mask) {
                 if (fin) {
                     const int s = T.slot;
@@ -376,17 +290,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                 __syncwarp();
             }
         }
-#ifdef GD_DIAG
-        GD_DIAG_ADD(17, clock64() - d_t1);
-#endif
     }
-#ifdef GD_DIAG
-    if (lane == 0) for (int k = 0; k < 20; ++k) atomicAdd(&gd_diag[k], dacc[k]);
-    if (lane == 0) {
-        unsigned long long *dw = gd_diag_warp[(blockIdx.x * GD_W_WARPS + warp) & 4095];
-        dw[0] = clock64() - d_start; dw[1] = dacc[8]; dw[2] = dacc[0]; dw[3] = dacc[16]; dw[4] = dacc[17]; dw[5] = dacc[9]; dw[6] = dacc[4]; dw[7] = dacc[5];
-    }
-#endif
     // ---- flush: per-lane 32-bit work counters straight to the 64-bit global totals
     {
         unsigned v[4] = {n_done, n_query, n_box, n_tri};
@@ -407,20 +311,21 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
         if (s_emitted[threadIdx.x]) atomicAdd(&tally.emitted[threadIdx.x], (unsigned long long)s_emitted[threadIdx.x]);
         if (s_peak[threadIdx.x]) atomicAdd(&tally.peak[threadIdx.x], (unsigned long long)s_peak[threadIdx.x]);
     }
-    if (threadIdx.x >= 4 && threadIdx.x < 14 && s_cnt[threadIdx.x])
+    if (threadIdx.x >= 4 && threadIdx.x < 12 && s_cnt[threadIdx.x])
         atomicAdd(&((unsigned long long *)tally.counters)[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
 }
 
 // ---------------------------------------------------------------- ray-cast hook with dynamic fetch
 // Persistent warps take chunks of ray indices from one global counter; a lane whose ray ends stores the result and
 // takes the next ray of its warp's chunk once `k_fetch` lanes are idle.
+template <int WIDTH>
 __global__ void __launch_bounds__(256, 4)
 gd_k_trace_wave(GdBvh bvh, const float *__restrict__ org, const float *__restrict__ dir, long long n, int filter_mat,
                 float t_min, int *__restrict__ tri_out, float *__restrict__ t_out, GdCounters *counters,
                 unsigned long long *next_ray, unsigned chunk, GdWaveTune tune) {
     const unsigned lane = threadIdx.x & 31u;
     const unsigned lt_mask = (1u << lane) - 1u;
-    int stack[GD_STACK4];
+    int stack[WIDTH == 8 ? GD_STACK8 : GD_STACK4];
     GdTrav T;
     gd_trav_idle(T);
     long long my_ray = -1;
@@ -456,7 +361,7 @@ gd_k_trace_wave(GdBvh bvh, const float *__restrict__ org, const float *__restric
                 break;
             }
         }
-        gd_trav_step(T, bvh, stack, tune.n_steps, n_box, n_tri);
+        gd_trav_step<WIDTH>(T, bvh, stack, tune.n_steps, n_box, n_tri);
         if (T.slot >= 0 && T.node == GD_TRAV_DONE) {
             tri_out[my_ray] = T.orig == GD_NO_FACET ? -1 : T.orig;
             t_out[my_ray] = T.orig == GD_NO_FACET ? GD_INF : T.t;
