@@ -218,6 +218,8 @@ typedef struct {
     int n_bvh_nodes, bvh_max_depth;
     float last_run_ms, last_build_ms;      /* CUDA-event times of the last gadep_run / gadep_build_bvh kernels   */
     int last_run_launches, last_build_launches;
+    unsigned long long n_skipped_queries;  /* flights that end before the clearance of their grid cell: answered     */
+                                           /* ("no facet") without a BVH query; n_queries counts only BVH queries     */
     unsigned long long n_stack_overflow;   /* rays that ran out of traversal stack since gadep_create (must be 0; a  */
                                            /* run that sees one fails with GADEP_E_ARG)                              */
     unsigned long long n_parity_queries;   /* GADEP_RUN_PARITY_LOCALISATION: all-hits localisation queries       */

@@ -52,7 +52,7 @@ class GadepCounters(C.Structure):
                [("emitted", C.c_ulonglong * MAX_LINES), ("peak", C.c_ulonglong * MAX_LINES), ("n_lines", C.c_int),
                 ("n_bvh_nodes", C.c_int), ("bvh_max_depth", C.c_int), ("last_run_ms", C.c_float),
                 ("last_build_ms", C.c_float), ("last_run_launches", C.c_int), ("last_build_launches", C.c_int),
-                ("n_stack_overflow", C.c_ulonglong),
+                ("n_skipped_queries", C.c_ulonglong), ("n_stack_overflow", C.c_ulonglong),
                 ("n_parity_queries", C.c_ulonglong), ("n_parity_mismatch", C.c_ulonglong)]
 
     def as_dict(self):
@@ -62,7 +62,7 @@ class GadepCounters(C.Structure):
                  n_bvh_nodes=int(self.n_bvh_nodes), bvh_max_depth=int(self.bvh_max_depth),
                  last_run_ms=float(self.last_run_ms), last_build_ms=float(self.last_build_ms),
                  last_run_launches=int(self.last_run_launches), last_build_launches=int(self.last_build_launches),
-                 n_stack_overflow=int(self.n_stack_overflow),
+                 n_skipped_queries=int(self.n_skipped_queries), n_stack_overflow=int(self.n_stack_overflow),
                  n_parity_queries=int(self.n_parity_queries), n_parity_mismatch=int(self.n_parity_mismatch))
         return d
 

@@ -46,8 +46,9 @@ struct gadep_ctx {
     // triangles [5] 4-wide nodes [13] 8-wide compressed nodes
     // [6..9] the mesh copies (vertices, triangles, side materials, surface ids)
     // [10..12] mesh validation: edge table keys, edge table surfaces, error record + surface sides
-    void *pool[14] = {};
-    size_t pool_cap[14] = {};
+    // [14] clearance grid: marks / x distances [15] squared distances after the y pass [16] the grid itself
+    void *pool[17] = {};
+    size_t pool_cap[17] = {};
     // source
     bool have_src = false;
     GdSource src;
@@ -62,13 +63,18 @@ struct gadep_ctx {
     int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
-    GdWaveTune tune = {8, 4, 4};
+    GdWaveTune tune = {8, 4, 4, 16};
     float rho[GADEP_MAX_MATERIALS] = {};      // g/cm^3, electron-range mode
     bool have_rho = false;
     // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
     std::vector<int> h_sides;                 // [n_surf][2] inside, outside
     int *d_mat_entry = nullptr;               // [GADEP_MAX_MATERIALS][1 + GD_ENTRY_MAX], see GdBvh
     bool have_entries = false;
+    // facet-clearance grid: box of all surfaces but the world boundary (host, from gadep_load_mesh), cell budget
+    float roi_lo[3] = {0, 0, 0}, roi_hi[3] = {0, 0, 0};
+    bool have_roi = false;
+    long long grid_cells = 1ll << 23;         // GADEP_GRID_CELLS overrides; 0 = no grid
+    GdGrid grid = {};
     bool cluster_surfaces = true;             // GADEP_NO_SURFACE_CLUSTERS=1 switches it off (measurement)
     double split_budget = 8.0;                // extra BVH references per facet handed out by the splitting budget
     int n_bins = 0;
@@ -136,10 +142,12 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb1);
     if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
     if (getenv("GADEP_NO_SURFACE_CLUSTERS")) c->cluster_surfaces = false;
+    if (const char *t = getenv("GADEP_GRID_CELLS")) { long long v = atoll(t); if (v >= 0 && v <= (1ll << 28)) c->grid_cells = v; }
     if (const char *t = getenv("GADEP_SPLIT_BUDGET")) { double b = atof(t); if (b >= 0 && b <= 15) c->split_budget = b; }
-    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,n_steps" (measurement sweeps)
-        int a, b, d;
-        if (sscanf(t, "%d,%d,%d", &a, &b, &d) == 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32) c->tune = {a, b, d};
+    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,n_steps,p_min" (measurement sweeps)
+        int a, b, d, p = c->tune.p_min;
+        if (sscanf(t, "%d,%d,%d,%d", &a, &b, &d, &p) >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && p >= 1 && p <= 32)
+            c->tune = {a, b, d, p};
     }
     *out = c;
     return GADEP_OK;
@@ -169,7 +177,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    for (int k = 0; k < 14; ++k) cudaFree(c->pool[k]);
+    for (int k = 0; k < 17; ++k) cudaFree(c->pool[k]);
     cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair); cudaFree(c->d_mat_entry);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -271,6 +279,20 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
     }
     if (h_err[GD_ERR_OPEN] != NONE) return gd_fail(c, GADEP_E_NOT_CLOSED, "surface %u is not closed (open edge)", h_err[GD_ERR_OPEN]);
     c->n_vert = n_vert; c->n_tri = n_tri; c->n_surf = n_surf; c->world = world_material;
+    {   // box of every surface that is not a world boundary (outside = KILL): where the clearance grid pays
+        float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+        bool any_inner = false;
+        for (int s2 = 0; s2 < n_surf; ++s2) any_inner = any_inner || surf_outside[s2] != GADEP_MAT_KILL;
+        for (int t = 0; t < n_tri; ++t) {
+            if (any_inner && surf_outside[tri_surface[t]] == GADEP_MAT_KILL) continue;
+            for (int k = 0; k < 3; ++k) {
+                const float *v = vertices + 3 * (size_t)triangles[3 * (size_t)t + k];
+                for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], v[a]); hi[a] = std::max(hi[a], v[a]); }
+            }
+        }
+        for (int a = 0; a < 3; ++a) { c->roi_lo[a] = lo[a]; c->roi_hi[a] = hi[a]; }
+        c->have_roi = lo[0] <= hi[0];
+    }
     c->have_mesh = true;
     return GADEP_OK;
 }
@@ -365,6 +387,38 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
             gd_k_collapse8<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes8);
             launches += 4;
         }
+        // ---- facet-clearance grid over the box of the inner surfaces
+        c->grid = GdGrid{};
+        if (c->grid_cells > 0 && c->have_roi) {
+            double ext[3], vol = 1.0;
+            for (int a = 0; a < 3; ++a) { ext[a] = std::max((double)c->roi_hi[a] - (double)c->roi_lo[a], 1e-3); vol *= ext[a]; }
+            double h = std::cbrt(vol / (double)c->grid_cells);
+            int dim[3];
+            for (;;) {
+                double cells = 1.0;
+                for (int a = 0; a < 3; ++a) { dim[a] = (int)std::ceil(ext[a] / h) + 2; cells *= dim[a]; }
+                if (cells <= (double)c->grid_cells * 1.05 || cells <= 4096.0) break;
+                h *= 1.02;
+            }
+            GdGrid g;
+            g.nx = dim[0]; g.ny = dim[1]; g.nz = dim[2];
+            g.lox = (float)(c->roi_lo[0] - h); g.loy = (float)(c->roi_lo[1] - h); g.loz = (float)(c->roi_lo[2] - h);
+            g.inv_h = (float)(1.0 / h); g.quarter_h = (float)(0.25 * h * (1.0 - 1e-6));
+            const size_t nc = (size_t)g.nx * g.ny * g.nz;
+            unsigned char *occ = nullptr, *cells = nullptr;
+            unsigned short *d2 = nullptr;
+            if ((e = gd_pool_get(c, 14, nc, (void **)&occ)) != cudaSuccess) break;
+            if ((e = gd_pool_get(c, 15, 2 * nc, (void **)&d2)) != cudaSuccess) break;
+            if ((e = gd_pool_get(c, 16, nc, (void **)&cells)) != cudaSuccess) break;
+            g.cells = cells;
+            cudaMemsetAsync(occ, 0, nc, st);
+            gd_k_grid_mark<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, g, occ);
+            gd_k_grid_dt_x<<<(g.ny * g.nz + 127) / 128, 128, 0, st>>>(g, occ);
+            gd_k_grid_dt_y<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, occ, d2);
+            gd_k_grid_dt_z<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, d2, cells);
+            launches += 4;
+            c->grid = g;
+        }
         cudaEventRecord(c->evb1, st);
         if ((e = cudaGetLastError()) != cudaSuccess) break;
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
@@ -405,6 +459,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
 
 static GdBvh gd_bvh_view(const gadep_ctx *c) {
     GdBvh b;
+    b.grid = c->grid;
     b.nodes = c->d_nodes; b.nodes4 = c->d_nodes4; b.nodes8 = c->d_nodes8; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
     b.mat_entry = c->have_entries ? c->d_mat_entry : nullptr;
     return b;
@@ -827,7 +882,7 @@ extern "C" int gadep_get_counters(const gadep_ctx *cc, gadep_counters *out) {
     out->n_histories = h.n_histories; out->n_queries = h.n_queries; out->n_box_tests = h.n_box_tests;
     out->n_tri_tests = h.n_tri_tests; out->n_crossings = h.n_crossings; out->n_pe = h.n_pe; out->n_compton = h.n_compton;
     out->n_coherent = h.n_coherent; out->n_pair = h.n_pair; out->n_escaped = h.n_escaped; out->n_leak = h.n_leak;
-    out->n_cutoff = h.n_cutoff; out->n_stack_overflow = c->n_stack_overflow;
+    out->n_cutoff = h.n_cutoff; out->n_stack_overflow = c->n_stack_overflow; out->n_skipped_queries = h.n_skipped;
     out->n_parity_queries = h.n_parity; out->n_parity_mismatch = h.n_parity_mismatch;
     memcpy(out->emitted, c->h_emitted, sizeof(out->emitted));
     memcpy(out->peak, c->h_peak, sizeof(out->peak));
@@ -899,3 +954,12 @@ extern "C" int gadep_set_tallies(gadep_ctx *c, const unsigned long long *in) {
     c->results_stale = true;
     return GADEP_OK;
 }
+
+#ifdef GD_PROF
+extern "C" int gadep_prof_read(unsigned long long *out16, int reset) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out16, gd_prof, sizeof(unsigned long long) * 16);
+    if (reset) { unsigned long long z[16] = {}; cudaMemcpyToSymbol(gd_prof, z, sizeof(z)); }
+    return 0;
+}
+#endif

@@ -520,3 +520,77 @@ __global__ void gd_k_collapse8(int n_inner, const int *__restrict__ child_l, con
     for (int w = 0; w < 4; ++w) { nd.qx[w] = q[0][w]; nd.qy[w] = q[1][w]; nd.qz[w] = q[2][w]; }
     out[i] = nd;
 }
+
+// ---------------------------------------------------------------- facet-clearance grid (GdGrid, gadep_common.cuh)
+// 1. every cell a reference box touches is marked; 2. exact Euclidean distance transform of the marks in cell units,
+// separable (x by two sweeps per row, then y and z as windowed lower envelopes), capped at GD_GRID_WINDOW + 1 cells;
+// 3. clearance of a cell = (centre-to-centre distance - sqrt(3)) h: two points of the two cells are at least that far
+// apart.  Everything is rounded towards "nearer", so the stored value never exceeds the true clearance.
+#define GD_GRID_WINDOW 24
+__global__ void gd_k_grid_mark(const float4 *__restrict__ ref_lo, const float4 *__restrict__ ref_hi, int n_ref, GdGrid g,
+                               unsigned char *__restrict__ occ) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_ref) return;
+    const float4 lo = ref_lo[i], hi = ref_hi[i];
+    const float pad = 2.0e-4f;          // float32 slack of the boxes and of the cell index computed in the transport kernel
+    const float ex = pad + 1.0e-6f * fmaxf(fabsf(lo.x), fabsf(hi.x)), ey = pad + 1.0e-6f * fmaxf(fabsf(lo.y), fabsf(hi.y)),
+                ez = pad + 1.0e-6f * fmaxf(fabsf(lo.z), fabsf(hi.z));
+    int x0 = (int)floorf((lo.x - ex - g.lox) * g.inv_h), x1 = (int)floorf((hi.x + ex - g.lox) * g.inv_h);
+    int y0 = (int)floorf((lo.y - ey - g.loy) * g.inv_h), y1 = (int)floorf((hi.y + ey - g.loy) * g.inv_h);
+    int z0 = (int)floorf((lo.z - ez - g.loz) * g.inv_h), z1 = (int)floorf((hi.z + ez - g.loz) * g.inv_h);
+    x0 = max(x0, 0); y0 = max(y0, 0); z0 = max(z0, 0);
+    x1 = min(x1, g.nx - 1); y1 = min(y1, g.ny - 1); z1 = min(z1, g.nz - 1);
+    for (int z = z0; z <= z1; ++z)
+        for (int y = y0; y <= y1; ++y) {
+            unsigned char *row = occ + ((size_t)z * g.ny + y) * g.nx;
+            for (int x = x0; x <= x1; ++x) row[x] = 1;
+        }
+}
+// rows along x: occ (1 = marked) -> distance in cells to the nearest marked cell of the row, capped, in place
+__global__ void gd_k_grid_dt_x(GdGrid g, unsigned char *__restrict__ occ) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= g.ny * g.nz) return;
+    unsigned char *row = occ + (size_t)r * g.nx;
+    const int cap = GD_GRID_WINDOW + 1;
+    int d = cap;
+    for (int x = 0; x < g.nx; ++x) { d = row[x] == 1 ? 0 : min(d + 1, cap); row[x] = (unsigned char)(row[x] == 1 ? 0x80 : d); }   // 0x80 = marked
+    d = cap;
+    for (int x = g.nx - 1; x >= 0; --x) {
+        const int v = row[x];
+        d = v == 0x80 ? 0 : min(d + 1, cap);
+        row[x] = (unsigned char)(v == 0x80 ? 0 : min(v, d));
+    }
+}
+__global__ void gd_k_grid_dt_y(GdGrid g, const unsigned char *__restrict__ gx, unsigned short *__restrict__ d2) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t n = (size_t)g.nx * g.ny * g.nz;
+    if (i >= n) return;
+    const int x = (int)(i % g.nx), y = (int)((i / g.nx) % g.ny);
+    const int cap = GD_GRID_WINDOW + 1;
+    int best = cap * cap;
+    const int a = max(y - GD_GRID_WINDOW, 0), b = min(y + GD_GRID_WINDOW, g.ny - 1);
+    const unsigned char *col = gx + (i - (size_t)y * g.nx);
+    for (int yy = a; yy <= b; ++yy) {
+        const int v = col[(size_t)yy * g.nx], dy = yy - y;
+        best = min(best, v * v + dy * dy);
+    }
+    (void)x;
+    d2[i] = (unsigned short)best;
+}
+__global__ void gd_k_grid_dt_z(GdGrid g, const unsigned short *__restrict__ d2, unsigned char *__restrict__ out) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t plane = (size_t)g.nx * g.ny, n = plane * g.nz;
+    if (i >= n) return;
+    const int z = (int)(i / plane);
+    const int cap = GD_GRID_WINDOW + 1;
+    int best = cap * cap;
+    const int a = max(z - GD_GRID_WINDOW, 0), b = min(z + GD_GRID_WINDOW, g.nz - 1);
+    const unsigned short *col = d2 + (i - (size_t)z * plane);
+    for (int zz = a; zz <= b; ++zz) {
+        const int dz = zz - z;
+        best = min(best, (int)col[(size_t)zz * plane] + dz * dz);
+    }
+    // centre distance sqrt(best) cells; any two points of the two cells: at least sqrt(best) - sqrt(3) cells apart
+    const float cl = sqrtf((float)best) * 0.999999f - 1.7320509f;
+    out[i] = (unsigned char)fminf(fmaxf(floorf(cl * 4.0f), 0.0f), 255.0f);
+}

@@ -66,7 +66,18 @@ struct __align__(32) GdNode8 {
 };
 #define GD_STACK8 224               // 8-wide traversal: up to 7 pushes per node visited; overflow is detected and reported
 
+// Facet-clearance grid (built by gadep_build_bvh beside the hierarchy): uniform cells of edge h over the box of all
+// surfaces but the world boundary; a cell holds a lower bound of the distance from any of its points to any facet, in
+// units of h / 4 (0 = unknown / a facet may be near).  A flight that ends before that distance cannot meet a facet, so
+// its nearest-hit query is answered ("none") without touching the BVH -- the answer the traversal would give.
+struct GdGrid {
+    const unsigned char *cells;     // [nz][ny][nx], nullptr = no grid
+    float lox, loy, loz, inv_h, quarter_h;
+    int nx, ny, nz;
+};
+
 struct GdBvh {
+    GdGrid grid;
     const GdNode *nodes;
     const GdNode4 *nodes4;
     const GdNode8 *nodes8;

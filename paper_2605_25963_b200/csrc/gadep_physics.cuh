@@ -109,6 +109,15 @@ GD_HD float gd_thomson_from(float u) {
     return cbrtf(0.5f * c + r) + cbrtf(0.5f * c - r);
 }
 
+// lower bound of the distance from p to the nearest facet, from the clearance grid (0 = unknown)
+GD_D float gd_clearance(const GdGrid &g, const GdVec3 &p) {
+    if (!g.cells) return 0.0f;
+    const int ix = (int)floorf((p.x - g.lox) * g.inv_h), iy = (int)floorf((p.y - g.loy) * g.inv_h),
+              iz = (int)floorf((p.z - g.loz) * g.inv_h);
+    if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) return 0.0f;
+    return (float)__ldg(g.cells + ((size_t)iz * g.ny + iy) * g.nx + ix) * g.quarter_h;
+}
+
 struct GdHistory {
     float edep;        // scoring deposit; line energy for a full-absorption history
     unsigned flags;

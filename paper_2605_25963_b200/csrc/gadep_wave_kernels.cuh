@@ -8,9 +8,10 @@
 //            (dynamic fetch).  The burst ends when READY is empty and 32 results wait (or `k_exit` times as many
 //            results as rays still in flight: sparse warps batch their few chains); unfinished rays stay in their
 //            lanes' registers across the physics burst.
-//   P-burst: RESULT slots are processed 32 at a time by all lanes (boundary crossing / interaction / tally /
-//            refill from the history counter / attenuation lookup) and pushed to READY.  Both queues are rings
-//            (first in, first out), so every slot is served once per cycle.
+//   P-burst: lanes take RESULT slots and process one event each (boundary crossing / interaction / tally / refill
+//            from the history counter / attenuation lookup); a slot whose next flight ends before the clearance of
+//            its grid cell (GdGrid) stays on its lane and goes round again without a query, the others are pushed to
+//            READY and their lanes take the next waiting result.  Both queues are rings (first in, first out).
 // There is no block-level barrier inside the loop and no particle state in global memory (only the two pending
 // annihilation photons of a pair event, which are rare, sit in a global side buffer).  Results do not depend on any
 // of this scheduling: random streams are keyed by the history index and the tallies are integers.
@@ -26,12 +27,21 @@
 // leaves the SM a 64 KB L1 instead of 32 KB.
 #define GD_W_NF 25
 
+// Measurement build only (-DGD_PROF, never in the shipped library): per-warp clocks of the two bursts and lane counts.
+#ifdef GD_PROF
+__device__ unsigned long long gd_prof[16];
+#define GD_PROF_ADD(k, v) do { pacc[k] += (unsigned long long)(v); } while (0)
+#else
+#define GD_PROF_ADD(k, v) do {} while (0)
+#endif
+
 // scheduling knobs (defaults in gadep_api.cu; GADEP_TUNE="k_fetch,k_exit,n_steps" overrides them for measurement
 // sweeps).  None of them can change a result.
 struct GdWaveTune {
     int k_fetch;        // idle lanes needed before READY slots are fetched
     int k_exit;         // T-burst ends when n_results >= k_exit * rays in flight (or 32 results) and READY is empty
     int n_steps;        // node visits per traversal round
+    int p_min;          // a physics pass runs while this many lanes have work (or the warp has nothing else to do)
 };
 
 // ---- slot <-> registers
@@ -134,7 +144,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     int stack[WIDTH == 8 ? GD_STACK8 : GD_STACK4];
     GdTrav T;
     gd_trav_idle(T);
-    unsigned n_box = 0, n_tri = 0, n_query = 0, n_done = 0;
+    unsigned n_box = 0, n_tri = 0, n_query = 0, n_done = 0, n_skip = 0;
     unsigned long long w_cur = 0, w_end = 0;     // warp-uniform chunk of history indices [w_cur, w_end)
     // every slot starts in RESULT with mode NEED: the first P-bursts start the first histories
     for (int s = lane; s < GD_W_SLOTS; s += 32) {
@@ -145,108 +155,148 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     // waiting at the bottom of a stack while fresh histories stream over it -- the chains are the critical path
     int n_res = GD_W_SLOTS, n_ready = 0, h_res = 0, h_ready = 0;
     static_assert((GD_W_SLOTS & (GD_W_SLOTS - 1)) == 0, "slot count must be a power of two");
+#ifdef GD_PROF
+    unsigned long long pacc[16] = {};
+    long long p_t0 = clock64();
+#endif
     __syncwarp();
 
     for (;;) {
         // ================================================================ P-burst
-        // full batches first; a partial batch only when the warp would otherwise starve
-        bool did_full = false;
-        while (n_res >= 32 || (n_res > 0 && n_ready == 0 && !did_full)) {
-            const int take = n_res < 32 ? n_res : 32;
-            did_full = take == 32;
-            const bool act = (int)lane < take;           // this lane works on slot s in this batch
-            const int s = act ? (int)q_res[(h_res + (int)lane) & (GD_W_SLOTS - 1)] : 0;
-            h_res = (h_res + take) & (GD_W_SLOTS - 1); n_res -= take;
+        // Lanes take waiting results, run the physics of one event each, and either hand the slot to READY (the next
+        // flight needs the BVH) or -- when the clearance grid says that no facet lies within the next flight -- keep
+        // it and go round again: the answer of that query is known ("none").  Lanes that gave their slot away take the
+        // next waiting result.  The burst goes on while at least `p_min` lanes have work, or while the warp has
+        // nothing else to do; what is left then is parked in RESULT with its known answer.
+        {
+            bool has = false;
+            int s = 0;
             GdLane L;
             L.mode = GD_MODE_DONE;
             GdHit hit;
             hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
-            if (act) {
-                gd_slot_load(sl, s, L, seed, first);
-                if (L.pending) {
-                    const float *p = pair + s * 8;
-                    L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
-                }
-                // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the
-                // to-side id as "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
-                hit.t = GD_SF(22);
-                hit.orig = __float_as_int(GD_SF(23));
-                hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
-                hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
-            }
-            GdLocalCounters cnt = {};
-            GdHistory r;
-            r.edep = 0.0f; r.flags = 0u; r.line = 0;
-            bool fin = false;
-            if (act && L.mode != GD_MODE_NEED) {
-                const int was_pending = L.pending;
-                fin = gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt);
-                if (fin) {
-                    n_done++;
-                    const unsigned long long hrel = L.history - first;
-                    if (edep_out) edep_out[hrel] = r.edep;
-                    if (flags_out) flags_out[hrel] = r.flags;
-                } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
-                    float *p = pair + s * 8;
-                    p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
-                    p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
-                }
-            }
-            gd_tally_warp(fin, r, s_src, tally, s_spec, s_emitted, s_peak, lane);
-            {   // event counters, one shared-memory atomic per kind and batch (crossing / PE / Compton / coherent / pair;
-                // escapes, re-localisations and cut-offs can accompany any of them)
-                const unsigned v[8] = {cnt.n_crossings, cnt.n_pe, cnt.n_compton, cnt.n_coherent, cnt.n_pair, cnt.n_escaped,
-                                       cnt.n_leak, cnt.n_cutoff};
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    const unsigned mk = __ballot_sync(0xFFFFFFFFu, v[k] != 0u);
-                    if (mk && lane == 0) atomicAdd(&s_cnt[4 + k], (unsigned)__popc(mk));
-                }
-            }
-            // ---- refill finished slots from the history counter (warp-level chunks)
-            const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, act && L.mode == GD_MODE_NEED);
-            if (need_mask) {
-                const unsigned n_need = __popc(need_mask);
-                unsigned long long new_base = 0;
-                const bool refill = w_cur + n_need > w_end;
-                unsigned my_chunk = chunk;
-                if (refill) {
-                    // guided: towards the end of the launch the chunks shrink with what is left, so that the last
-                    // histories spread over all warps instead of going to the few that ask last
-                    if (lane == 0) {
-                        const unsigned long long cur = *(volatile unsigned long long *)next_history;
-                        const unsigned long long rem = cur < n_hist ? n_hist - cur : 0ull;
-                        const unsigned long long g = rem / ((unsigned long long)gridDim.x * GD_W_WARPS * 2ull);
-                        if (g < my_chunk) my_chunk = g < 32ull ? 32u : (unsigned)g;
-                        new_base = atomicAdd(next_history, (unsigned long long)my_chunk);
+            const bool no_rays = __ballot_sync(0xFFFFFFFFu, T.slot >= 0) == 0u;
+            for (bool first_pass = true;; first_pass = false) {
+                // ---- fetch
+                const unsigned free_mask = __ballot_sync(0xFFFFFFFFu, !has);
+                const int n_free = __popc(free_mask), n_has = 32 - n_free;
+                const int take = n_free < n_res ? n_free : n_res;
+                // the first pass takes whatever made the traversal burst end; later passes need p_min lanes with work,
+                // unless the warp has no ray in flight and none prepared
+                if (!(n_has + take > 0 && (first_pass || n_has + take >= tune.p_min || (no_rays && n_ready == 0)))) {
+                    // not worth a pass: park the lanes that still hold a slot (their query is answered: no facet)
+                    if (has) {
+                        gd_slot_store(sl, s, L, first);
+                        GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
+                        q_res[(h_res + n_res + __popc(~free_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
                     }
-                    new_base = __shfl_sync(0xFFFFFFFFu, new_base, 0);
-                    my_chunk = __shfl_sync(0xFFFFFFFFu, my_chunk, 0);
+                    n_res += n_has;
+                    __syncwarp();
+                    break;
                 }
-                if (act && L.mode == GD_MODE_NEED) {
-                    unsigned long long h = w_cur + __popc(need_mask & lt_mask);
-                    if (h >= w_end) h = new_base + (h - w_end);
-                    if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
-                    else L.mode = GD_MODE_DONE;
+                if (take > 0) {
+                    const int rank = __popc(free_mask & lt_mask);
+                    if (!has && rank < take) {
+                        s = (int)q_res[(h_res + rank) & (GD_W_SLOTS - 1)];
+                        gd_slot_load(sl, s, L, seed, first);
+                        if (L.pending) {
+                            const float *p = pair + s * 8;
+                            L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
+                        }
+                        // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the
+                        // to-side id as "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
+                        hit.t = GD_SF(22);
+                        hit.orig = __float_as_int(GD_SF(23));
+                        hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
+                        hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
+                        has = true;
+                    }
+                    h_res = (h_res + take) & (GD_W_SLOTS - 1); n_res -= take;
                 }
-                if (refill) { w_cur = new_base + (w_cur + n_need - w_end); w_end = new_base + my_chunk; }
-                else w_cur += n_need;
+                GD_PROF_ADD(2, 1); GD_PROF_ADD(3, __popc(__ballot_sync(0xFFFFFFFFu, has)));
+                // ---- one event per lane
+                GdLocalCounters cnt = {};
+                GdHistory r;
+                r.edep = 0.0f; r.flags = 0u; r.line = 0;
+                bool fin = false;
+                if (has && L.mode != GD_MODE_NEED) {
+                    const int was_pending = L.pending;
+                    fin = gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt);
+                    if (fin) {
+                        n_done++;
+                        const unsigned long long hrel = L.history - first;
+                        if (edep_out) edep_out[hrel] = r.edep;
+                        if (flags_out) flags_out[hrel] = r.flags;
+                    } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
+                        float *p = pair + s * 8;
+                        p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
+                        p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
+                    }
+                }
+                gd_tally_warp(fin, r, s_src, tally, s_spec, s_emitted, s_peak, lane);
+                {   // event counters, one shared-memory atomic per kind and pass (crossing / PE / Compton / coherent /
+                    // pair; escapes, re-localisations and cut-offs can accompany any of them)
+                    const unsigned v[8] = {cnt.n_crossings, cnt.n_pe, cnt.n_compton, cnt.n_coherent, cnt.n_pair, cnt.n_escaped,
+                                           cnt.n_leak, cnt.n_cutoff};
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const unsigned mk = __ballot_sync(0xFFFFFFFFu, v[k] != 0u);
+                        if (mk && lane == 0) atomicAdd(&s_cnt[4 + k], (unsigned)__popc(mk));
+                    }
+                }
+                // ---- refill finished slots from the history counter (warp-level chunks)
+                const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, has && L.mode == GD_MODE_NEED);
+                if (need_mask) {
+                    const unsigned n_need = __popc(need_mask);
+                    unsigned long long new_base = 0;
+                    const bool refill = w_cur + n_need > w_end;
+                    unsigned my_chunk = chunk;
+                    if (refill) {
+                        // guided: towards the end of the launch the chunks shrink with what is left, so that the last
+                        // histories spread over all warps instead of going to the few that ask last
+                        if (lane == 0) {
+                            const unsigned long long cur = *(volatile unsigned long long *)next_history;
+                            const unsigned long long rem = cur < n_hist ? n_hist - cur : 0ull;
+                            const unsigned long long g = rem / ((unsigned long long)gridDim.x * GD_W_WARPS * 2ull);
+                            if (g < my_chunk) my_chunk = g < 32ull ? 32u : (unsigned)g;
+                            new_base = atomicAdd(next_history, (unsigned long long)my_chunk);
+                        }
+                        new_base = __shfl_sync(0xFFFFFFFFu, new_base, 0);
+                        my_chunk = __shfl_sync(0xFFFFFFFFu, my_chunk, 0);
+                    }
+                    if (has && L.mode == GD_MODE_NEED) {
+                        unsigned long long h = w_cur + __popc(need_mask & lt_mask);
+                        if (h >= w_end) h = new_base + (h - w_end);
+                        if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
+                        else L.mode = GD_MODE_DONE;
+                    }
+                    if (refill) { w_cur = new_base + (w_cur + n_need - w_end); w_end = new_base + my_chunk; }
+                    else w_cur += n_need;
+                }
+                // ---- the next query: answered by the clearance grid, or handed to READY
+                const bool live = has && L.mode != GD_MODE_DONE;
+                bool skip = false;
+                if (live) {
+                    float t_min, t_max;
+                    int filter;
+                    gd_lane_query(L, M, s_tab, t_min, t_max, filter);
+                    if (L.mode == GD_MODE_FLIGHT && L.sdist < GD_INF)
+                        skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
+                }
+                const unsigned ready_mask = __ballot_sync(0xFFFFFFFFu, live && !skip);
+                if (live && !skip) {
+                    gd_slot_store(sl, s, L, first);
+                    q_ready[(h_ready + n_ready + __popc(ready_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
+                }
+                n_ready += __popc(ready_mask);
+                has = skip;
+                if (skip) { n_skip++; hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.mats = 0; }
+                __syncwarp();
             }
-            // ---- prepare the next query and hand the slot to READY
-            const bool live = act && L.mode != GD_MODE_DONE;
-            if (live) {
-                float t_min, t_max;
-                int filter;
-                gd_lane_query(L, M, s_tab, t_min, t_max, filter);
-            }
-            const unsigned ready_mask = __ballot_sync(0xFFFFFFFFu, live);
-            if (live) {
-                gd_slot_store(sl, s, L, first);
-                q_ready[(h_ready + n_ready + __popc(ready_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
-            }
-            n_ready += __popc(ready_mask);
-            __syncwarp();
         }
+#ifdef GD_PROF
+        { const long long t1 = clock64(); GD_PROF_ADD(0, t1 - p_t0); p_t0 = t1; }
+#endif
         const unsigned busy_mask = __ballot_sync(0xFFFFFFFFu, T.slot >= 0);
         if (n_ready == 0 && busy_mask == 0u) {
             if (n_res == 0) break;                           // every slot is dead
@@ -276,6 +326,8 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                     break;
                 }
             }
+            GD_PROF_ADD(4, 1); GD_PROF_ADD(5, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0 && T.node >= 0)));
+            GD_PROF_ADD(6, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0)));
             gd_trav_step<WIDTH>(T, bvh, stack, tune.n_steps, n_box, n_tri);
             const bool fin = T.slot >= 0 && T.node == GD_TRAV_DONE;
             const unsigned fin_mask = __ballot_sync(0xFFFFFFFFu, fin);
@@ -290,16 +342,23 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                 __syncwarp();
             }
         }
+#ifdef GD_PROF
+        { const long long t1 = clock64(); GD_PROF_ADD(1, t1 - p_t0); p_t0 = t1; }
+#endif
     }
+#ifdef GD_PROF
+    if (lane == 0) for (int k = 0; k < 16; ++k) if (pacc[k]) atomicAdd(&gd_prof[k], pacc[k]);
+#endif
     // ---- flush: per-lane 32-bit work counters straight to the 64-bit global totals
     {
-        unsigned v[4] = {n_done, n_query, n_box, n_tri};
+        const unsigned v[5] = {n_done, n_query, n_box, n_tri, n_skip};
+        const int where[5] = {0, 1, 2, 3, 13};           // GdCounters: n_histories, n_queries, n_box_tests, n_tri_tests, n_skipped
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
+        for (int k = 0; k < 5; ++k) {
             unsigned long long x = v[k];
 #pragma unroll
             for (int o = 16; o >= 1; o >>= 1) x += __shfl_down_sync(0xFFFFFFFFu, x, o);
-            if (lane == 0 && x) atomicAdd(&((unsigned long long *)tally.counters)[k], x);
+            if (lane == 0 && x) atomicAdd(&((unsigned long long *)tally.counters)[where[k]], x);
         }
     }
     __syncthreads();
