@@ -63,7 +63,7 @@ struct gadep_ctx {
     int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
-    GdWaveTune tune = {8, 4, 4, 16};
+    GdWaveTune tune = {8, 16, 4, 16, 2};
     float rho[GADEP_MAX_MATERIALS] = {};      // g/cm^3, electron-range mode
     bool have_rho = false;
     // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
@@ -144,10 +144,10 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (getenv("GADEP_NO_SURFACE_CLUSTERS")) c->cluster_surfaces = false;
     if (const char *t = getenv("GADEP_GRID_CELLS")) { long long v = atoll(t); if (v >= 0 && v <= (1ll << 28)) c->grid_cells = v; }
     if (const char *t = getenv("GADEP_SPLIT_BUDGET")) { double b = atof(t); if (b >= 0 && b <= 15) c->split_budget = b; }
-    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,k_exit,n_steps,p_min" (measurement sweeps)
-        int a, b, d, p = c->tune.p_min;
-        if (sscanf(t, "%d,%d,%d,%d", &a, &b, &d, &p) >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && p >= 1 && p <= 32)
-            c->tune = {a, b, d, p};
+    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,t_keep,n_steps,p_min,t_smsp" (measurement sweeps)
+        int a, b, d, p = c->tune.p_min, ts = c->tune.t_smsp;
+        if (sscanf(t, "%d,%d,%d,%d,%d", &a, &b, &d, &p, &ts) >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && p >= 1 && p <= 32 && ts >= 0 && ts <= 4)
+            c->tune = {a, b, d, p, ts};
     }
     *out = c;
     return GADEP_OK;
@@ -554,7 +554,7 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     const int variant = c->kernel_variant;
     const int threads = variant == 2 ? GD_W_THREADS : GD_RUN_THREADS;
     const bool wide8 = c->run_width == 8;
-    if (variant == 2) smem += sizeof(float) * (size_t)GD_W_WARPS * GD_W_NF * GD_W_SLOTS;
+    if (variant == 2) smem += sizeof(float) * (size_t)GD_W_NF * GD_W_NSLOT;
     if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
     const void *kern = variant == 2 ? (wide8 ? (const void *)gd_k_transport_wave<8> : (const void *)gd_k_transport_wave<4>)
                                     : (variant == 1 ? (const void *)gd_k_transport_refill
@@ -565,11 +565,11 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     int per_sm = 1;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return gd_fail(c, GADEP_E_CUDA, "transport kernel does not fit on an SM (%zu B shared memory)", smem);
-    const unsigned long long per_block = variant == 2 ? (unsigned long long)GD_W_WARPS * GD_W_SLOTS : GD_RUN_THREADS;
+    const unsigned long long per_block = variant == 2 ? (unsigned long long)GD_W_NSLOT : GD_RUN_THREADS;
     unsigned long long want = (n + per_block - 1) / per_block;
     int grid = (int)std::min<unsigned long long>((unsigned long long)c->n_sm * per_sm, std::max<unsigned long long>(want, 1));
     if (variant == 2) {
-        size_t need = (size_t)grid * GD_W_WARPS * GD_W_SLOTS * 8;
+        size_t need = (size_t)grid * GD_W_NSLOT * 8;
         if (need > c->pair_floats) {
             cudaFree(c->d_pair); c->d_pair = nullptr; c->pair_floats = 0;
             GD_CUDA(c, cudaMalloc(&c->d_pair, need * sizeof(float)));
@@ -581,6 +581,8 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0) {
         unsigned long long warps = (unsigned long long)grid * (threads / 32);
         unsigned chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / (warps * 16)));
+        if (variant == 2)     // the wavefront kernel hands out history indices per block
+            chunk = (unsigned)std::min<unsigned long long>(8192, std::max<unsigned long long>(256, n / ((unsigned long long)grid * 32)));
         if (variant == 1 || variant == 2) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
         if (variant == 2 && wide8) {
             gd_k_transport_wave<8><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,

@@ -1,17 +1,19 @@
-// gadep_wave_kernels.cuh -- warp-resident wavefront transport and the ray-cast hook.
+// gadep_wave_kernels.cuh -- block-resident wavefront transport and the ray-cast hook.
 //
-// Every warp owns GD_W_SLOTS photon slots in shared memory (SoA, GD_W_NF words per slot).  A slot is in one of
-// three places: the READY queue (its next nearest-hit query is prepared), in flight on a lane (GdTrav registers),
-// or the RESULT queue (hit known, physics pending).  The warp alternates
-//   T-burst: lanes traverse in rounds of `n_steps` 4-wide node visits + one leaf step; a lane whose ray ends writes
-//            the hit to its slot, pushes it to RESULT and -- as soon as `k_fetch` lanes are idle -- takes a READY slot
-//            (dynamic fetch).  The burst ends when READY is empty and 32 results wait (or `k_exit` times as many
-//            results as rays still in flight: sparse warps batch their few chains); unfinished rays stay in their
-//            lanes' registers across the physics burst.
+// A block owns GD_W_NSLOT photon slots in shared memory (SoA, GD_W_NF words per slot) and two block-wide queues of
+// slot numbers: READY (the slot's next nearest-hit query is prepared) and RESULT (hit known, physics pending).  A slot
+// is in one queue, or on a lane of some warp.  Every warp of the block does whichever kind of work there is:
+//   T-burst: lanes traverse in rounds of `n_steps` node visits + one leaf step; a lane whose ray ends writes the hit
+//            to its slot, pushes it to RESULT and -- as soon as `k_fetch` lanes are idle -- takes a READY slot
+//            (dynamic fetch).  Unfinished rays stay in their lanes' registers while the warp does physics.
 //   P-burst: lanes take RESULT slots and process one event each (boundary crossing / interaction / tally / refill
 //            from the history counter / attenuation lookup); a slot whose next flight ends before the clearance of
 //            its grid cell (GdGrid) stays on its lane and goes round again without a query, the others are pushed to
-//            READY and their lanes take the next waiting result.  Both queues are rings (first in, first out).
+//            READY and their lanes take the next waiting result.
+// Because the queues are shared, a warp finds 32 slots for either kind of work as long as the block has them --
+// the long scattering chains that are left when the history counter runs dry end up on the lanes of one warp instead
+// of idling in all sixteen.  The queues are rings with a ticket counter on each side; an entry carries a valid bit
+// that its producer sets last and its consumer clears, so no lock is held while a slot is read or written.
 // There is no block-level barrier inside the loop and no particle state in global memory (only the two pending
 // annihilation photons of a pair event, which are rare, sit in a global side buffer).  Results do not depend on any
 // of this scheduling: random streams are keyed by the history index and the tallies are integers.
@@ -22,7 +24,7 @@
 
 #define GD_W_THREADS 512
 #define GD_W_WARPS (GD_W_THREADS / 32)
-#define GD_W_SLOTS 64
+#define GD_W_NSLOT 1024           // photon slots per block (64 per warp)
 // fields per slot.  25 words keep the block's shared memory under the 164 KB carve-out for up to 9 materials, which
 // leaves the SM a 64 KB L1 instead of 32 KB.
 #define GD_W_NF 25
@@ -39,13 +41,141 @@ __device__ unsigned long long gd_prof[16];
 // sweeps).  None of them can change a result.
 struct GdWaveTune {
     int k_fetch;        // idle lanes needed before READY slots are fetched
-    int k_exit;         // T-burst ends when n_results >= k_exit * rays in flight (or 32 results) and READY is empty
+    int t_keep;         // a warp stays in its T-burst while at least this many of its lanes hold a ray (or READY has more)
     int n_steps;        // node visits per traversal round
     int p_min;          // a physics pass runs while this many lanes have work (or the warp has nothing else to do)
+    int t_smsp;         // SM sub-partitions (0..4) whose warps prefer traversal work
 };
 
+// ---- block-wide queue of slot numbers (multi-producer, multi-consumer, warp-granular).  Tickets count up for ever;
+// ticket k lives in entry k mod GD_W_NSLOT and carries the lap number (k / GD_W_NSLOT) mod 32 beside the valid bit, so
+// a consumer can tell the entry it waits for from the previous lap's entry that its owner has not emptied yet.
+struct GdQueue {
+    unsigned head, tail;                      // consumers have claimed tickets < head, producers hold tickets < tail
+    unsigned short ent[GD_W_NSLOT];           // 0 = empty, else 0x8000 | lap << 10 | slot
+};
+GD_D unsigned gd_q_tag(unsigned ticket) { return 0x8000u | (((ticket / GD_W_NSLOT) & 31u) << 10); }
+GD_D int gd_q_count(const GdQueue *q) {
+    const unsigned h = *(volatile const unsigned *)&q->head, t = *(volatile const unsigned *)&q->tail;
+    return (int)(t - h);
+}
+// lanes with `push` set append their slot; the slot's words must have been written by the same lane before the call
+GD_D void gd_q_push(GdQueue *q, bool push, int slot, unsigned lane) {
+    const unsigned mask = __ballot_sync(0xFFFFFFFFu, push);
+    if (mask == 0u) return;
+    unsigned base = 0;
+    const int leader = __ffs(mask) - 1;
+    if ((int)lane == leader) base = atomicAdd(&q->tail, (unsigned)__popc(mask));
+    base = __shfl_sync(0xFFFFFFFFu, base, leader);
+    if (push) {
+        const unsigned ticket = base + __popc(mask & ((1u << lane) - 1u));
+        volatile unsigned short *e = &q->ent[ticket & (GD_W_NSLOT - 1)];
+        while (*e != 0) {}                   // the consumer of the previous lap has claimed this entry but not yet emptied it
+        __threadfence_block();               // slot words before the valid bit
+        *e = (unsigned short)(gd_q_tag(ticket) | (unsigned)slot);
+    }
+}
+// up to `want` entries for the lanes with `free` set (lowest lanes first); returns how many were claimed (warp-uniform)
+// and sets slot for the lanes that got one (got = true)
+GD_D int gd_q_claim(GdQueue *q, bool free, int want, unsigned lane, int &slot, bool &got) {
+    const unsigned mask = __ballot_sync(0xFFFFFFFFu, free);
+    got = false;
+    if (mask == 0u || want <= 0) return 0;
+    unsigned base = 0;
+    int n = 0;
+    if (lane == 0) {
+        for (;;) {
+            const unsigned h = *(volatile unsigned *)&q->head, t = *(volatile unsigned *)&q->tail;
+            const int avail = (int)(t - h);
+            n = avail < want ? avail : want;
+            if (n <= 0) { n = 0; break; }
+            if (atomicCAS(&q->head, h, h + (unsigned)n) == h) { base = h; break; }
+        }
+    }
+    n = __shfl_sync(0xFFFFFFFFu, n, 0);
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    const int rank = __popc(mask & ((1u << lane) - 1u));
+    if (free && rank < n) {
+        const unsigned ticket = base + (unsigned)rank, tag = gd_q_tag(ticket);
+        volatile unsigned short *e = &q->ent[ticket & (GD_W_NSLOT - 1)];
+        unsigned v;
+        while (((v = *e) & 0xFC00u) != tag) {}   // the producer holds the ticket but has not written the entry yet
+        *e = 0;
+        __threadfence_block();               // valid bit before the slot words
+        slot = (int)(v & 0x3FFu);
+        got = true;
+    }
+    return n;
+}
+
+// ---- history indices for the block: one chunk [cur, end) of the launch's global counter, packed in a 64-bit shared
+// word (indices relative to the launch's first history, < 2^32).  Requests are served by compare-and-swap on that word;
+// the warp that finds the chunk too short takes the lock, fetches the next chunk and hands out the old chunk's rest
+// together with the head of the new one, so no index is ever dropped.
+struct GdHistPool {
+    unsigned long long state;                 // cur | end << 32
+    unsigned lock, dry;                       // dry: the global counter has passed n_hist
+};
+// n <= 32 indices for the calling warp (lane 0 works, the result is broadcast): lane of rank r gets a0 + r for r < n0,
+// else a1 + (r - n0); an index >= n_hist means "no history left"
+GD_D void gd_hist_take(GdHistPool *hp, unsigned n, unsigned long long *next_history, unsigned long long n_hist,
+                       unsigned chunk, unsigned n_blocks, unsigned lane, unsigned &a0, unsigned &n0, unsigned &a1) {
+    unsigned r0 = 0, rn0 = 0, r1 = 0;
+    if (lane == 0) {
+        const unsigned nh = (unsigned)n_hist;
+        for (;;) {
+            const unsigned long long st = *(volatile unsigned long long *)&hp->state;
+            const unsigned cur = (unsigned)st, end = (unsigned)(st >> 32);
+            if (end - cur >= n) {                                            // enough left in the chunk
+                if (atomicCAS(&hp->state, st, (unsigned long long)(cur + n) | ((unsigned long long)end << 32)) == st) {
+                    r0 = cur; rn0 = n; r1 = nh; break;
+                }
+                continue;
+            }
+            if (*(volatile unsigned *)&hp->dry) {                            // hand out what is left, then nothing
+                if (atomicCAS(&hp->state, st, (unsigned long long)end | ((unsigned long long)end << 32)) == st) {
+                    r0 = cur; rn0 = end - cur; r1 = nh; break;
+                }
+                continue;
+            }
+            if (atomicCAS(&hp->lock, 0u, 1u) != 0u) continue;                // another warp is fetching a chunk
+            const unsigned long long s1 = *(volatile unsigned long long *)&hp->state;
+            if ((unsigned)(s1 >> 32) - (unsigned)s1 >= n || *(volatile unsigned *)&hp->dry) {   // refilled meanwhile
+                atomicExch(&hp->lock, 0u);
+                continue;
+            }
+            // guided: towards the end of the launch the chunks shrink with what is left, so that the last histories
+            // spread over all blocks instead of going to the few that ask last
+            const unsigned long long seen = *(volatile unsigned long long *)next_history;
+            const unsigned long long rem = seen < n_hist ? n_hist - seen : 0ull;
+            const unsigned long long gsz = rem / ((unsigned long long)n_blocks * 2ull);
+            unsigned my_chunk = chunk;
+            if (gsz < my_chunk) my_chunk = gsz < 256ull ? 256u : (unsigned)gsz;
+            const unsigned long long g = atomicAdd(next_history, (unsigned long long)my_chunk);
+            const unsigned g0 = g >= n_hist ? nh : (unsigned)g;
+            const unsigned g1 = g + my_chunk >= n_hist ? nh : (unsigned)(g + my_chunk);
+            for (;;) {    // under the lock the old chunk can only shrink (it is shorter than n): its rest + the head of the new one
+                const unsigned long long s2 = *(volatile unsigned long long *)&hp->state;
+                const unsigned c2 = (unsigned)s2, e2 = (unsigned)(s2 >> 32);
+                const unsigned from_old = e2 - c2, from_new = n - from_old;
+                const unsigned nc = g0 + from_new < g1 ? g0 + from_new : g1;
+                if (atomicCAS(&hp->state, s2, (unsigned long long)nc | ((unsigned long long)g1 << 32)) == s2) {
+                    r0 = c2; rn0 = from_old; r1 = g0; break;
+                }
+            }
+            if (g1 >= nh) *(volatile unsigned *)&hp->dry = 1u;
+            __threadfence_block();
+            atomicExch(&hp->lock, 0u);
+            break;
+        }
+    }
+    a0 = __shfl_sync(0xFFFFFFFFu, r0, 0);
+    n0 = __shfl_sync(0xFFFFFFFFu, rn0, 0);
+    a1 = __shfl_sync(0xFFFFFFFFu, r1, 0);
+}
+
 // ---- slot <-> registers
-#define GD_SF(f) sl[(f) * GD_W_SLOTS + s]
+#define GD_SF(f) sl[(f) * GD_W_NSLOT + s]
 GD_D unsigned gd_pack_state(const GdLane &L) {
     return (unsigned)(L.m + 1) | ((unsigned)L.mode << 5) | ((unsigned)L.line << 7) | ((unsigned)L.pending << 13) |
            ((unsigned)L.n_stall << 15) | (L.g.stream << 21) | ((unsigned)L.need_mu << 23);
@@ -111,9 +241,9 @@ GD_D void gd_tally_warp(bool fin, const GdHistory &r, const GdSource &S, const G
     }
 }
 
-// dynamic shared memory: [table floats][spectrum u32 (n_bins+1)][slots: warps x GD_W_NF x GD_W_SLOTS floats]
-// pair_buf: global, 8 floats per slot of every warp of the grid
-// WIDTH: 8 = compressed 8-wide nodes (default), 4 = uncompressed 4-wide nodes (cross-check variant)
+// dynamic shared memory: [table floats][spectrum u32 (n_bins+1)][slots: GD_W_NF x GD_W_NSLOT floats]
+// pair_buf: global, 8 floats per slot of every block of the grid
+// WIDTH: 4 = uncompressed 4-wide nodes (default), 8 = compressed 8-wide nodes
 template <int WIDTH>
 __global__ void __launch_bounds__(GD_W_THREADS, 1)
 gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
@@ -124,96 +254,113 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     __shared__ GdSource s_src;
     __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];
     __shared__ unsigned s_cnt[12];
-    __shared__ unsigned char s_qready[GD_W_WARPS][GD_W_SLOTS], s_qres[GD_W_WARPS][GD_W_SLOTS];
+    __shared__ GdQueue s_ready, s_result;
+    __shared__ GdHistPool s_hist;
+    __shared__ unsigned s_live;                     // slots that still carry or may get a history
     const int n_tab = M.n_mat * 4 * M.n_grid;
     float *s_tab = (float *)gd_smem;
     unsigned *s_spec = (unsigned *)(s_tab + n_tab);
-    float *s_slots = (float *)(s_spec + tally.n_bins + 1);
+    float *sl = (float *)(s_spec + tally.n_bins + 1);
     for (int i = threadIdx.x; i < n_tab; i += blockDim.x) s_tab[i] = M.table[i];
     for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) s_spec[i] = 0;
     for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i];
     if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }
     if (threadIdx.x < 12) s_cnt[threadIdx.x] = 0;
+    // every slot starts in RESULT with mode NEED: the first P-bursts start the first histories
+    for (int s = threadIdx.x; s < GD_W_NSLOT; s += blockDim.x) {
+        GD_SF(14) = __uint_as_float((unsigned)GD_MODE_NEED << 5);
+        s_result.ent[s] = (unsigned short)(gd_q_tag((unsigned)s) | (unsigned)s);
+        s_ready.ent[s] = 0;
+    }
+    if (threadIdx.x == 0) {
+        s_result.head = 0; s_result.tail = GD_W_NSLOT; s_ready.head = 0; s_ready.tail = 0;
+        s_hist.state = 0ull; s_hist.lock = 0u; s_hist.dry = 0u;
+        s_live = GD_W_NSLOT;
+    }
     __syncthreads();
 
-    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const unsigned lane = threadIdx.x & 31u;
     const unsigned lt_mask = (1u << lane) - 1u;
-    float *sl = s_slots + (size_t)warp * GD_W_NF * GD_W_SLOTS;
-    unsigned char *q_ready = s_qready[warp], *q_res = s_qres[warp];
-    float *pair = pair_buf + ((size_t)blockIdx.x * GD_W_WARPS + warp) * GD_W_SLOTS * 8;
+    float *pair = pair_buf + (size_t)blockIdx.x * GD_W_NSLOT * 8;
     int stack[WIDTH == 8 ? GD_STACK8 : GD_STACK4];
     GdTrav T;
     gd_trav_idle(T);
     unsigned n_box = 0, n_tri = 0, n_query = 0, n_done = 0, n_skip = 0;
-    unsigned long long w_cur = 0, w_end = 0;     // warp-uniform chunk of history indices [w_cur, w_end)
-    // every slot starts in RESULT with mode NEED: the first P-bursts start the first histories
-    for (int s = lane; s < GD_W_SLOTS; s += 32) {
-        GD_SF(14) = __uint_as_float((unsigned)GD_MODE_NEED << 5);
-        q_res[s] = (unsigned char)s;
-    }
-    // both queues are rings (first in, first out): a slot of a long scattering chain is served every round instead of
-    // waiting at the bottom of a stack while fresh histories stream over it -- the chains are the critical path
-    int n_res = GD_W_SLOTS, n_ready = 0, h_res = 0, h_ready = 0;
-    static_assert((GD_W_SLOTS & (GD_W_SLOTS - 1)) == 0, "slot count must be a power of two");
+    static_assert(GD_W_NSLOT == 1024, "queue entries hold a 10-bit slot number");
 #ifdef GD_PROF
     unsigned long long pacc[16] = {};
     long long p_t0 = clock64();
 #endif
-    __syncwarp();
 
     for (;;) {
-        // ================================================================ P-burst
-        // Lanes take waiting results, run the physics of one event each, and either hand the slot to READY (the next
-        // flight needs the BVH) or -- when the clearance grid says that no facet lies within the next flight -- keep
-        // it and go round again: the answer of that query is known ("none").  Lanes that gave their slot away take the
-        // next waiting result.  The burst goes on while at least `p_min` lanes have work, or while the warp has
-        // nothing else to do; what is left then is parked in RESULT with its known answer.
-        {
+        // ---- what next?  (queue lengths are snapshots: a wrong guess costs a pass with fewer lanes, never a result)
+        const int my_rays = __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0));
+        int n_res = 0, n_rdy = 0;
+        unsigned live = 0;
+        if (lane == 0) { n_res = gd_q_count(&s_result); n_rdy = gd_q_count(&s_ready); live = *(volatile unsigned *)&s_live; }
+        n_res = __shfl_sync(0xFFFFFFFFu, n_res, 0);
+        n_rdy = __shfl_sync(0xFFFFFFFFu, n_rdy, 0);
+        live = __shfl_sync(0xFFFFFFFFu, live, 0);
+        const bool t_work = my_rays > 0 || n_rdy > 0;
+        // warps of the first `t_smsp` SM sub-partitions (warp & 3) prefer traversal, the others physics: the four warps
+        // that share an instruction cache then run the same loop most of the time
+        const bool pref_t = (int)((threadIdx.x >> 5) & 3u) < tune.t_smsp;
+        const bool do_p = pref_t ? n_res > 0 && ((my_rays < tune.t_keep && n_rdy == 0 && n_res >= tune.p_min) || !t_work)
+                                 : n_res > 0 && (n_res >= tune.p_min || !t_work);
+        if (!do_p && !t_work) {
+            if (live == 0u) break;               // every slot of the block is dead
+            __nanosleep(200);                    // other warps hold all the work there is
+            continue;
+        }
+        if (do_p) {
+            // ============================================================ P-burst
             bool has = false;
             int s = 0;
             GdLane L;
             L.mode = GD_MODE_DONE;
             GdHit hit;
             hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
-            const bool no_rays = __ballot_sync(0xFFFFFFFFu, T.slot >= 0) == 0u;
             for (bool first_pass = true;; first_pass = false) {
-                // ---- fetch
+                // ---- a pass needs p_min lanes with work -- or a warp with no ray to go back to and none to fetch.
+                // Decided on a snapshot of the queue before anything is claimed: what is parked below must be lanes
+                // whose answer is known (no facet within the flight), never a freshly claimed traversal result.
                 const unsigned free_mask = __ballot_sync(0xFFFFFFFFu, !has);
-                const int n_free = __popc(free_mask), n_has = 32 - n_free;
-                const int take = n_free < n_res ? n_free : n_res;
-                // the first pass takes whatever made the traversal burst end; later passes need p_min lanes with work,
-                // unless the warp has no ray in flight and none prepared
-                if (!(n_has + take > 0 && (first_pass || n_has + take >= tune.p_min || (no_rays && n_ready == 0)))) {
-                    // not worth a pass: park the lanes that still hold a slot (their query is answered: no facet)
+                const int n_has = 32 - __popc(free_mask);
+                int avail = 0, rdy = 0;
+                if (lane == 0) { avail = gd_q_count(&s_result); rdy = gd_q_count(&s_ready); }
+                avail = __shfl_sync(0xFFFFFFFFu, avail, 0);
+                rdy = __shfl_sync(0xFFFFFFFFu, rdy, 0);
+                const int expect = n_has + (avail < 32 - n_has ? avail : 32 - n_has);
+                const bool go = expect > 0 && (first_pass || expect >= tune.p_min || (my_rays == 0 && rdy == 0));
+                if (!go) {
                     if (has) {
                         gd_slot_store(sl, s, L, first);
                         GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
-                        q_res[(h_res + n_res + __popc(~free_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
                     }
-                    n_res += n_has;
-                    __syncwarp();
+                    gd_q_push(&s_result, has, s, lane);
                     break;
                 }
-                if (take > 0) {
-                    const int rank = __popc(free_mask & lt_mask);
-                    if (!has && rank < take) {
-                        s = (int)q_res[(h_res + rank) & (GD_W_SLOTS - 1)];
-                        gd_slot_load(sl, s, L, seed, first);
-                        if (L.pending) {
-                            const float *p = pair + s * 8;
-                            L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
-                        }
-                        // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the
-                        // to-side id as "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
-                        hit.t = GD_SF(22);
-                        hit.orig = __float_as_int(GD_SF(23));
-                        hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
-                        hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
-                        has = true;
+                // ---- fetch: lanes without a slot take waiting results
+                bool got = false;
+                int s_new = 0;
+                const int take = gd_q_claim(&s_result, !has, 32 - n_has, lane, s_new, got);
+                if (got) {
+                    s = s_new;
+                    gd_slot_load(sl, s, L, seed, first);
+                    if (L.pending) {
+                        const float *p = pair + s * 8;
+                        L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
                     }
-                    h_res = (h_res + take) & (GD_W_SLOTS - 1); n_res -= take;
+                    // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the
+                    // to-side id as "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
+                    hit.t = GD_SF(22);
+                    hit.orig = __float_as_int(GD_SF(23));
+                    hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
+                    hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
+                    has = true;
                 }
-                GD_PROF_ADD(2, 1); GD_PROF_ADD(3, __popc(__ballot_sync(0xFFFFFFFFu, has)));
+                if (n_has + take == 0) break;        // another warp was quicker
+                GD_PROF_ADD(2, 1); GD_PROF_ADD(3, n_has + take);
                 // ---- one event per lane
                 GdLocalCounters cnt = {};
                 GdHistory r;
@@ -244,103 +391,76 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                         if (mk && lane == 0) atomicAdd(&s_cnt[4 + k], (unsigned)__popc(mk));
                     }
                 }
-                // ---- refill finished slots from the history counter (warp-level chunks)
+                // ---- finished slots take the next histories of the block's chunk
                 const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, has && L.mode == GD_MODE_NEED);
                 if (need_mask) {
-                    const unsigned n_need = __popc(need_mask);
-                    unsigned long long new_base = 0;
-                    const bool refill = w_cur + n_need > w_end;
-                    unsigned my_chunk = chunk;
-                    if (refill) {
-                        // guided: towards the end of the launch the chunks shrink with what is left, so that the last
-                        // histories spread over all warps instead of going to the few that ask last
-                        if (lane == 0) {
-                            const unsigned long long cur = *(volatile unsigned long long *)next_history;
-                            const unsigned long long rem = cur < n_hist ? n_hist - cur : 0ull;
-                            const unsigned long long g = rem / ((unsigned long long)gridDim.x * GD_W_WARPS * 2ull);
-                            if (g < my_chunk) my_chunk = g < 32ull ? 32u : (unsigned)g;
-                            new_base = atomicAdd(next_history, (unsigned long long)my_chunk);
-                        }
-                        new_base = __shfl_sync(0xFFFFFFFFu, new_base, 0);
-                        my_chunk = __shfl_sync(0xFFFFFFFFu, my_chunk, 0);
-                    }
+                    unsigned a0, n0, a1;
+                    gd_hist_take(&s_hist, (unsigned)__popc(need_mask), next_history, n_hist, chunk, gridDim.x, lane, a0, n0, a1);
+                    bool died = false;
                     if (has && L.mode == GD_MODE_NEED) {
-                        unsigned long long h = w_cur + __popc(need_mask & lt_mask);
-                        if (h >= w_end) h = new_base + (h - w_end);
+                        const unsigned rk = __popc(need_mask & lt_mask);
+                        const unsigned long long h = rk < n0 ? a0 + rk : (unsigned long long)a1 + (rk - n0);
                         if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
-                        else L.mode = GD_MODE_DONE;
+                        else { L.mode = GD_MODE_DONE; died = true; }
                     }
-                    if (refill) { w_cur = new_base + (w_cur + n_need - w_end); w_end = new_base + my_chunk; }
-                    else w_cur += n_need;
+                    const unsigned died_mask = __ballot_sync(0xFFFFFFFFu, died);
+                    if (died_mask && lane == 0) atomicSub(&s_live, (unsigned)__popc(died_mask));
                 }
                 // ---- the next query: answered by the clearance grid, or handed to READY
-                const bool live = has && L.mode != GD_MODE_DONE;
+                const bool live_lane = has && L.mode != GD_MODE_DONE;
                 bool skip = false;
-                if (live) {
+                if (live_lane) {
                     float t_min, t_max;
                     int filter;
                     gd_lane_query(L, M, s_tab, t_min, t_max, filter);
                     if (L.mode == GD_MODE_FLIGHT && L.sdist < GD_INF)
                         skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
                 }
-                const unsigned ready_mask = __ballot_sync(0xFFFFFFFFu, live && !skip);
-                if (live && !skip) {
-                    gd_slot_store(sl, s, L, first);
-                    q_ready[(h_ready + n_ready + __popc(ready_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
-                }
-                n_ready += __popc(ready_mask);
+                const bool to_ready = live_lane && !skip;
+                if (to_ready) gd_slot_store(sl, s, L, first);
+                gd_q_push(&s_ready, to_ready, s, lane);
                 has = skip;
                 if (skip) { n_skip++; hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.mats = 0; }
-                __syncwarp();
             }
-        }
 #ifdef GD_PROF
-        { const long long t1 = clock64(); GD_PROF_ADD(0, t1 - p_t0); p_t0 = t1; }
+            { const long long t1 = clock64(); GD_PROF_ADD(0, t1 - p_t0); p_t0 = t1; }
 #endif
-        const unsigned busy_mask = __ballot_sync(0xFFFFFFFFu, T.slot >= 0);
-        if (n_ready == 0 && busy_mask == 0u) {
-            if (n_res == 0) break;                           // every slot is dead
             continue;
         }
         // ================================================================ T-burst
         for (;;) {
             const unsigned idle_mask = __ballot_sync(0xFFFFFFFFu, T.slot < 0);
             const int n_idle = __popc(idle_mask);
-            if (n_idle) {
-                if (n_ready > 0) {
-                    if (n_idle >= tune.k_fetch || n_idle == 32) {
-                        const int rank = __popc(idle_mask & lt_mask);
-                        if (T.slot < 0 && rank < n_ready) {
-                            const int s = (int)q_ready[(h_ready + rank) & (GD_W_SLOTS - 1)];
-                            const unsigned st = __float_as_uint(GD_SF(14));
-                            const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
-                            gd_trav_begin(T, bvh, stack, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
-                                          loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
-                                          __float_as_int(GD_SF(19)), __float_as_int(GD_SF(20)), __float_as_int(GD_SF(21)), s);
-                            n_query++;
-                        }
-                        const int tk = n_idle < n_ready ? n_idle : n_ready;
-                        h_ready = (h_ready + tk) & (GD_W_SLOTS - 1); n_ready -= tk;
-                    }
-                } else if ((n_res > 0 && (n_res >= 32 || n_res >= tune.k_exit * (32 - n_idle))) || n_idle == 32) {
-                    break;
+            if (n_idle >= tune.k_fetch || n_idle == 32) {
+                bool got = false;
+                int s = 0;
+                const int tk = gd_q_claim(&s_ready, T.slot < 0, n_idle, lane, s, got);
+                if (got) {
+                    const unsigned st = __float_as_uint(GD_SF(14));
+                    const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
+                    gd_trav_begin(T, bvh, stack, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
+                                  loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
+                                  __float_as_int(GD_SF(19)), __float_as_int(GD_SF(20)), __float_as_int(GD_SF(21)), s);
+                    n_query++;
+                }
+                // nothing to fetch and few rays left: see whether physics has piled up (the rays stay in registers)
+                if (tk == 0 && 32 - n_idle < tune.t_keep) {
+                    if (n_idle == 32) break;
+                    int r = 0;
+                    if (lane == 0) r = gd_q_count(&s_result);
+                    if (__shfl_sync(0xFFFFFFFFu, r, 0) >= tune.p_min) break;
                 }
             }
             GD_PROF_ADD(4, 1); GD_PROF_ADD(5, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0 && T.node >= 0)));
             GD_PROF_ADD(6, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0)));
             gd_trav_step<WIDTH>(T, bvh, stack, tune.n_steps, n_box, n_tri);
             const bool fin = T.slot >= 0 && T.node == GD_TRAV_DONE;
-            const unsigned fin_mask = __ballot_sync(0xFFFFFFFFu, fin);
-            if (fin_mask) {
-                if (fin) {
-                    const int s = T.slot;
-                    GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
-                    q_res[(h_res + n_res + __popc(fin_mask & lt_mask)) & (GD_W_SLOTS - 1)] = (unsigned char)s;
-                    T.slot = -1;
-                }
-                n_res += __popc(fin_mask);
-                __syncwarp();
+            if (fin) {
+                const int s = T.slot;
+                GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
             }
+            gd_q_push(&s_result, fin, T.slot, lane);
+            if (fin) T.slot = -1;
         }
 #ifdef GD_PROF
         { const long long t1 = clock64(); GD_PROF_ADD(1, t1 - p_t0); p_t0 = t1; }
