@@ -1,14 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- photon histories/s of the Gadep hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--histories 1e7] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--histories 1e8] [--impl reference]
 
-A step = one pass of the whole hot path over one batch: gadep_build_bvh + gadep_run of
-`histories` photon histories (a1-a13) on the workload of BASELINE.json configs[config] (default configs[1], the
-coaxial HPGe with 5 lines and 1e7 histories).  Inputs (mesh, tables) are resident in HBM for `value`; `e2e` repeats
-the step through the C ABI from HOST buffers (tables + mesh uploaded, spectrum read back) with wall-clock timing.
-For N > 1 (torchrun) every rank transports its own range of the global history index and the integer tallies are
-summed with one NCCL all-reduce inside the timed region (weak scaling).
+A step = one pass of the whole hot path over one batch: gadep_build_bvh (hierarchy + clearance
+grid) + gadep_run of `histories` photon histories (a1-a13).  The headline workload is BASELINE.json configs[2] (coaxial
+HPGe + water volume source, 8 lines) at its own 1e8 histories -- the paper's headline particle count.
+Inputs (mesh, tables) are resident in HBM for `value`; `e2e` repeats the step through the C ABI from HOST buffers
+(tables + mesh uploaded, validated, BVH built, spectrum read back) with wall-clock timing.  After the headline the same
+line carries, under config.per_config, one full-size timed step of each of the other four configs and the config-4 ray
+benchmark (rank 0, N = 1 only).  For N > 1 (torchrun) every rank transports its own range of the global history index
+and the whole integer tally block (spectrum + per-line counters) is summed with one NCCL all-reduce inside the timed
+region (weak scaling).
 """
 import argparse
 import json
@@ -26,8 +29,17 @@ if ROOT not in sys.path:
 
 METRIC = "photon histories/s"
 UNIT = "histories/s"
-# SURVEY.md 8(d) per-unit algorithmic work, FP32 lane-instructions (DESIGN.md "rooflines")
-INSTR_BOX, INSTR_TRI, INSTR_EVENT, INSTR_QUERY = 15, 36, 250, 60
+# SURVEY.md 8(d) per-unit algorithmic work, FP32 lane-instructions (DESIGN.md section 7)
+INSTR_BOX, INSTR_TRI, INSTR_EVENT = 15, 36, 250
+INSTR_QUERY = 60          # query set-up: not a unit of SURVEY.md 8(d); reported beside `frac`, not inside it
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of gd_k_transport_wave at the size bench.py times, from the
+# `ncu --set full` captures summarised under profiles/ (per config; None = not captured)
+NCU_TRAFFIC = {}
+try:
+    NCU_TRAFFIC = {int(k): v for k, v in json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).items()
+                   if k.isdigit()}
+except Exception:
+    pass
 
 
 def load_peaks():
@@ -76,11 +88,15 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def make_workload(dm, cfg, coh=None):
+    return dm.make_config(cfg) if coh is None else dm.make_config(cfg, coh_coeff=coh)
+
+
 def oracle_rate(w, n_sample, first=0):
     """The oracle as it stands on the host cores: histories/s on a bounded sample of the same workload."""
     from oracle import gadep_oracle as orc
     s = orc.OracleScene(w)
-    s.run(min(2000, n_sample), w.seed, w.n_bins, w.spectrum_e_max_mev)      # page in
+    s.run(min(200, n_sample), w.seed, w.n_bins, w.spectrum_e_max_mev)      # page in
     t0 = time.perf_counter()
     s.run(n_sample, w.seed, w.n_bins, w.spectrum_e_max_mev, first=first)
     dt = time.perf_counter() - t0
@@ -92,13 +108,14 @@ def run_reference(args, w, rank):
     if rank != 0:
         return
     n_sample = int(args.ref_sample)
-    rates = []
+    if n_sample <= 0:                 # sized from a pilot so that one step is a few seconds of CPU work
+        r0, _, _ = oracle_rate(w, 300)
+        n_sample = int(min(max(4.0 * r0, 300), 2e6))
     for _ in range(args.warmup):
-        oracle_rate(w, max(n_sample // 10, 1000))
-    t_all = 0.0
+        oracle_rate(w, max(n_sample // 10, 100))
+    t_all, cores = 0.0, 1
     for k in range(args.steps):
-        r, dt, cores = oracle_rate(w, n_sample, first=k * n_sample)
-        rates.append(r)
+        _, dt, cores = oracle_rate(w, n_sample, first=k * n_sample)
         t_all += dt
     value = n_sample * args.steps / t_all
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
@@ -112,19 +129,51 @@ def run_reference(args, w, rank):
     print(json.dumps(line), flush=True)
 
 
-def run_ray_bench(args, dm):
-    """BASELINE.json configs[4]: seeded isotropic rays from random points inside the endcap's bounding cylinder through
-    the 2 M-facet BVH (device arrays, CUDA events), the check of a sample against brute force is tests/test_gpu_parity.py::test_cfg4_full_size_rays."""
-    import torch
-    import paper_2605_25963_b200 as pkg
-    w = dm.make_config(4)
-    g = pkg.Gadep(0, torch.cuda.current_stream().cuda_stream)
+def counters_of(c):
+    keys = ("n_queries", "n_skipped_queries", "n_box_tests", "n_tri_tests", "n_pe", "n_compton", "n_coherent", "n_pair",
+            "n_crossings")
+    return {k: c[k] for k in keys}
+
+
+def useful_work(agg):
+    """SURVEY.md 8(d) units x the kernel's own counters = algorithmic FP32 lane-instructions."""
+    events = agg["n_pe"] + agg["n_compton"] + agg["n_coherent"] + agg["n_pair"]
+    return agg["n_box_tests"] * INSTR_BOX + agg["n_tri_tests"] * INSTR_TRI + events * INSTR_EVENT, events
+
+
+def one_step_summary(pkg, torch, w, alu_peak, n_hist=None):
+    """One warm-up (reduced) + one full-size timed step (build + run) of a workload; for the per-config table."""
+    g = pkg.Gadep(torch.cuda.current_device(), torch.cuda.current_stream().cuda_stream)
     g.load_workload(w)
-    n, chunk = int(args.ray_bench), 20_000_000
-    t_ms, boxes, tris, done = 0.0, 0, 0, 0
-    while done < n:
-        m = min(chunk, n - done)
-        org, d = dm.configs.make_rays(m, 1 + done // chunk, 41.9, -101.9, 6.0)
+    n = int(n_hist or w.n_histories)
+    g.run(min(n, 500_000), w.seed, w.n_bins, w.spectrum_e_max_mev)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    g.build_bvh()
+    g.run(n, w.seed, w.n_bins, w.spectrum_e_max_mev)
+    e1.record()
+    torch.cuda.synchronize()
+    c = g.get_counters()
+    k_s = c["last_run_ms"] * 1e-3
+    work, events = useful_work(c)
+    out = {"workload": w.name, "n_triangles": w.mesh.n_tri, "histories": n, "ms_per_step": e0.elapsed_time(e1),
+           "bvh_build_ms": c["last_build_ms"], "transport_ms": c["last_run_ms"], "histories_per_s": n / (e0.elapsed_time(e1) * 1e-3),
+           "events_per_s": events / k_s, "bvh_queries_per_s": c["n_queries"] / k_s,
+           "flights_without_query_per_s": c["n_skipped_queries"] / k_s, "box_tests_per_s": c["n_box_tests"] / k_s,
+           "tri_tests_per_s": c["n_tri_tests"] / k_s, "useful_alu_frac": work / k_s / 1e12 / alu_peak,
+           "fepe": [g.fepe(l)[0] for l in range(len(w.source["line_mev"]))]}
+    return out, g
+
+
+def ray_bench(pkg, torch, dm, g, w, n_rays):
+    """BASELINE.json configs[4]: seeded isotropic rays from random points inside the endcap's bounding cylinder through
+    the 2 M-facet BVH (device arrays, CUDA events); the 1e6-ray brute-force check is tests/test_gpu_acceptance.py."""
+    R, z0, z1 = w.notes["ray_box"]
+    chunk, done, t_ms, boxes, tris = 20_000_000, 0, 0.0, 0, 0
+    while done < n_rays:
+        m = min(chunk, n_rays - done)
+        org, d = dm.configs.make_rays(m, w.notes["ray_seed"] + done // chunk, R, z0, z1)
         to, td = torch.from_numpy(org).cuda(), torch.from_numpy(d).cuda()
         tri = torch.empty(m, dtype=torch.int32, device="cuda")
         t = torch.empty(m, dtype=torch.float32, device="cuda")
@@ -134,10 +183,9 @@ def run_ray_bench(args, dm):
         c = g.get_counters()
         t_ms += c["last_run_ms"]; boxes += c["n_box_tests"]; tris += c["n_tri_tests"]
         done += m
-    line = {"metric": "BVH nearest-hit rays/s", "value": n / (t_ms * 1e-3), "unit": "rays/s", "n_rays": n,
-            "workload": w.name, "n_triangles": w.mesh.n_tri, "kernel_ms": t_ms, "box_tests_per_s": boxes / (t_ms * 1e-3),
-            "tri_tests_per_s": tris / (t_ms * 1e-3), "bvh_build_ms": g.get_counters()["last_build_ms"]}
-    print(json.dumps(line), flush=True)
+    return {"workload": w.name, "n_triangles": w.mesh.n_tri, "n_rays": n_rays, "kernel_ms": t_ms,
+            "rays_per_s": n_rays / (t_ms * 1e-3), "box_tests_per_s": boxes / (t_ms * 1e-3),
+            "tri_tests_per_s": tris / (t_ms * 1e-3)}
 
 
 def run_calibration(args, dm):
@@ -198,15 +246,17 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--config", type=int, default=2, help="headline workload (BASELINE.json configs index)")
+    ap.add_argument("--coh-coeff", type=float, default=None, help="coherent coefficient override (SURVEY.md Q1: 7.0e-30 = calibrated variant)")
     ap.add_argument("--histories", type=float, default=0, help="per GPU per step; 0 = the config's own count")
     ap.add_argument("--impl", default="gadep")
-    ap.add_argument("--ref-sample", type=float, default=60000)
+    ap.add_argument("--ref-sample", type=float, default=0, help="--impl reference: oracle histories per step; 0 = a few seconds' worth")
     ap.add_argument("--cpu-sample", type=float, default=0, help="oracle histories; 0 = sized for ~15 s from a pilot run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the table of the other configs and the ray benchmark")
+    ap.add_argument("--rays", type=float, default=2e7, help="config-4 ray benchmark: seeded rays through gadep_trace_rays (BASELINE: 1e8)")
     ap.add_argument("--calibration", action="store_true", help="FEPE curves: 13 Table-3 energies x 3 parametric detectors")
     ap.add_argument("--locate-bench", type=float, default=0, help="localisation benchmark: side-id vs parity rule (PAPER.md:191-193)")
-    ap.add_argument("--ray-bench", type=float, default=0, help="config-4 ray benchmark: this many seeded rays through gadep_trace_rays")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -214,7 +264,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
 
     import detmesh as dm
-    w = dm.make_config(args.config)
+    w = make_workload(dm, args.config, args.coh_coeff)
     if args.impl == "reference":
         run_reference(args, w, rank)
         return
@@ -228,9 +278,6 @@ def main():
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    if args.ray_bench:
-        run_ray_bench(args, dm)
-        return
     if args.locate_bench:
         run_locate_bench(args, dm)
         return
@@ -241,17 +288,20 @@ def main():
     stream = torch.cuda.current_stream()
     g = pkg.Gadep(local_rank, stream.cuda_stream)
     g.load_workload(w)                                           # inputs resident in HBM from here on
-    n_tally = w.n_bins + 1
-    d_spec = torch.zeros(n_tally, dtype=torch.int64, device="cuda")
+    g.run(1000, w.seed, w.n_bins, w.spectrum_e_max_mev)          # fixes the tally shape
+    n_tally = g.tally_size()
+    d_tally = torch.zeros(n_tally, dtype=torch.int64, device="cuda")
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     first = rank * n_hist                                        # weak scaling: every rank its own histories
 
     def step(k):
         g.build_bvh()                                            # a0
         g.run(n_hist, w.seed, w.n_bins, w.spectrum_e_max_mev, first_history=first + k * world * n_hist,
-              spectrum=d_spec)                                   # a1-a13, spectrum stays on the device
-        if world > 1:
-            allreduce_tallies(d_spec)
+              flags=pkg.binding.RUN_ASYNC)                       # a1-a13, tallies stay on the device
+        if world > 1:                                            # the one exchange: the whole tally block
+            g.get_tallies(d_tally)
+            allreduce_tallies(d_tally)
+            g.set_tallies(d_tally)
 
     for k in range(args.warmup):
         step(k)
@@ -269,11 +319,11 @@ def main():
         ev[k][0].record(stream)
         step(args.warmup + k)
         ev[k][1].record(stream)
-        c = g.get_counters()
+        c = g.get_counters()                                     # synchronises; per-launch counters and kernel times
         kern_ms.append(c["last_run_ms"]); build_ms.append(c["last_build_ms"])
         launches += c["last_run_launches"] + c["last_build_launches"]
-        for key in ("n_queries", "n_box_tests", "n_tri_tests", "n_pe", "n_compton", "n_coherent", "n_pair", "n_crossings"):
-            agg[key] = agg.get(key, 0) + c[key]
+        for key, v in counters_of(c).items():
+            agg[key] = agg.get(key, 0) + v
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -284,12 +334,13 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     t_ms = float(t.item())
     value = world * n_hist * args.steps / (t_ms * 1e-3)
+    fepe_dev = [g.fepe(l)[0] for l in range(len(w.source["line_mev"]))]       # from the (reduced) counters of the last step
 
     # ---- e2e: same step through the C ABI from HOST buffers (tables + mesh up, spectrum down), wall clock
     m = w.mesh
     h2d = int(w.mu.nbytes + w.is_scoring.nbytes + m.vertices.nbytes + m.triangles.nbytes + m.tri_surface.nbytes
               + m.surf_inside.nbytes + m.surf_outside.nbytes + w.source["line_mev"].nbytes * 2)
-    d2h = int(8 * n_tally)
+    d2h = int(8 * (w.n_bins + 1))
     g2 = pkg.Gadep(local_rank, stream.cuda_stream)
     e2e_steps = 3                                                # median of three: one wall-clock hiccup does not count
     g2.load_workload(w); g2.run(min(n_hist, 100000), w.seed)
@@ -300,7 +351,7 @@ def main():
     for k in range(e2e_steps):
         t0 = time.perf_counter()
         g2.load_workload(w)                                      # host arrays -> device, validation, BVH build
-        h_spec = g2.run(n_hist, w.seed, w.n_bins, w.spectrum_e_max_mev, first_history=first)   # host spectrum out
+        g2.run(n_hist, w.seed, w.n_bins, w.spectrum_e_max_mev, first_history=first)   # host spectrum out
         fepe = [g2.fepe(l)[0] for l in range(len(w.source["line_mev"]))]
         torch.cuda.synchronize()
         e2e_times.append(time.perf_counter() - t0)
@@ -314,39 +365,63 @@ def main():
         peaks, peak_src = load_peaks()
         n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
         alu_peak = n_sm * 128 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12         # T lane-instr/s
-        events = agg["n_pe"] + agg["n_compton"] + agg["n_coherent"] + agg["n_pair"]
-        work = (agg["n_box_tests"] * INSTR_BOX + agg["n_tri_tests"] * INSTR_TRI + events * INSTR_EVENT
-                + agg["n_queries"] * INSTR_QUERY)
+        work, events = useful_work(agg)
         k_s = sum(kern_ms) * 1e-3
         achieved = work / k_s / 1e12
+        traffic = NCU_TRAFFIC.get(args.config) if (n_hist == w.n_histories and args.coh_coeff is None) else None
+        hbm_peak = peaks.get("hbm_gbs", 6650.0)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": w.name, "histories_per_step_per_gpu": n_hist, "n_triangles": m.n_tri,
-                           "seed": w.seed, "l2": "flushed between timed steps (256 MiB write)",
-                           "step": "gadep_build_bvh + gadep_run", "parallelism": f"history-sharded x{world}"},
+                           "seed": w.seed, "coh_coeff": args.coh_coeff if args.coh_coeff is not None else "7.0e-27 (BASELINE.json, literal)",
+                           "l2": "flushed between timed steps (256 MiB write)",
+                           "step": "gadep_build_bvh + gadep_run", "parallelism": f"history-sharded x{world}",
+                           "fepe": fepe_dev},
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "steps": e2e_steps, "fepe": fepe},
                 "gpu_launches": launches,
                 "clocks": clocks,
                 "roofline": {"bound": "alu", "kernel": "gd_k_transport_wave", "achieved": achieved, "peak": alu_peak,
                              "unit": "Tinstr/s (FP32 lane-instructions)", "frac": achieved / alu_peak,
-                             "traffic": 14633984 if args.config == 1 and n_hist == 10_000_000 else None,
-                             "traffic_source": "profiles/r01k_wave_kernel.md (ncu dram bytes of one launch)",
-                             "limiter": "L1 data pipe: l1tex__throughput 84 % of peak in the stand-alone traversal kernel, "
-                                        "51 % over a whole 1e7-history launch (ncu, profiles/r01f_trace_kernel.md, r01h)",
+                             "frac_with_query_setup": (work + agg["n_queries"] * INSTR_QUERY) / k_s / 1e12 / alu_peak,
+                             "units": {"box_test": INSTR_BOX, "triangle_test": INSTR_TRI, "event": INSTR_EVENT},
+                             "traffic": traffic,
+                             "traffic_source": "profiles/ncu_traffic.json (ncu --set full, dram bytes of one launch)",
+                             "hbm": {"achieved_gbs": (traffic / (k_s / args.steps) / 1e9) if traffic else None, "peak_gbs": hbm_peak},
+                             "limiter": "instruction issue: instruction-fetch and dependency stalls at 16 warps/SM, 14-16 of 32 "
+                                        "lanes per instruction (ncu, profiles/r02_wave_kernel.md)",
                              "peak_source": f"{n_sm} SMs x 128 lanes x sm_max_mhz ({peak_src})",
                              "kernel_ms_per_step": sum(kern_ms) / args.steps,
                              "bvh_build_ms_per_step": sum(build_ms) / args.steps,
                              "kernel_share_of_step": sum(kern_ms) / t_ms,
                              "box_tests_per_s": agg["n_box_tests"] / k_s, "tri_tests_per_s": agg["n_tri_tests"] / k_s,
-                             "queries_per_s": agg["n_queries"] / k_s, "events_per_s": events / k_s},
+                             "bvh_queries_per_s": agg["n_queries"] / k_s,
+                             "flights_without_query_per_s": agg["n_skipped_queries"] / k_s, "events_per_s": events / k_s},
                 "paper_context": "RTX 4090: 1e8 particles in 66.08 s = 1.51e6 /s (PAPER.md:270), other physics"}
+        if world == 1 and not args.no_per_config:
+            per = {}
+            g4 = w4 = None
+            for cfg in range(5):
+                if cfg == args.config and args.coh_coeff is None and n_hist == w.n_histories:
+                    continue
+                wk = dm.make_config(cfg)
+                per[str(cfg)], gk = one_step_summary(pkg, torch, wk, alu_peak)
+                if cfg == 4:
+                    g4, w4 = gk, wk
+            # config 1 with the calibrated coherent coefficient (7.0e-30), reported beside the literal one
+            per["1_calibrated_coh7e-30"], _ = one_step_summary(pkg, torch, dm.make_config(1, coh_coeff=7.0e-30), alu_peak)
+            line["config"]["per_config"] = per
+            if g4 is None:
+                w4 = dm.make_config(4)
+                g4 = pkg.Gadep(local_rank, stream.cuda_stream)
+                g4.load_workload(w4)
+            line["config"]["ray_bench"] = ray_bench(pkg, torch, dm, g4, w4, int(args.rays))
         if not args.no_cpu_baseline and world == 1:
             n_s = int(args.cpu_sample)
             if n_s <= 0:                                         # pilot -> about 15 s of CPU work
-                r0, dt0, _ = oracle_rate(w, 20000)
-                n_s = int(min(max(15.0 * r0, 20000), 5e7))
+                r0, dt0, _ = oracle_rate(w, 500)
+                n_s = int(min(max(15.0 * r0, 500), 5e7))
             r, dt, cores = oracle_rate(w, n_s)
             line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"first {n_s} histories of {w.name} ({dt:.1f} s)"}

@@ -207,8 +207,9 @@ class Gadep:
         opts = GadepRunOpts(int(n_bins), float(e_max_mev), int(first_history), int(flags))
         self._last_bins = int(n_bins)
         out = spectrum
-        if out is None:
+        if out is None and not (int(flags) & RUN_ASYNC):
             out = np.zeros(n_bins + 1, dtype=np.uint64)
+        # RUN_ASYNC without a device spectrum: nothing is copied out, the tallies stay in the context
         self._check(self.L.gadep_run(self.h, int(n_histories), int(seed), C.byref(opts), _ptr(out)))
         return out
 

@@ -63,7 +63,7 @@ struct gadep_ctx {
     int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
-    GdWaveTune tune = {8, 16, 4, 16, 2};
+    GdWaveTune tune = {16, 16, 4, 16, 2};
     float rho[GADEP_MAX_MATERIALS] = {};      // g/cm^3, electron-range mode
     bool have_rho = false;
     // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
@@ -73,7 +73,7 @@ struct gadep_ctx {
     // facet-clearance grid: box of all surfaces but the world boundary (host, from gadep_load_mesh), cell budget
     float roi_lo[3] = {0, 0, 0}, roi_hi[3] = {0, 0, 0};
     bool have_roi = false;
-    long long grid_cells = 1ll << 23;         // GADEP_GRID_CELLS overrides; 0 = no grid
+    long long grid_cells = 1ll << 22;         // GADEP_GRID_CELLS overrides; 0 = no grid
     GdGrid grid = {};
     bool cluster_surfaces = true;             // GADEP_NO_SURFACE_CLUSTERS=1 switches it off (measurement)
     double split_budget = 8.0;                // extra BVH references per facet handed out by the splitting budget
@@ -412,7 +412,8 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
             if ((e = gd_pool_get(c, 16, nc, (void **)&cells)) != cudaSuccess) break;
             g.cells = cells;
             cudaMemsetAsync(occ, 0, nc, st);
-            gd_k_grid_mark<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, g, occ);
+            if (n >= (1 << 16)) gd_k_grid_mark<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, g, occ, 1);
+            else gd_k_grid_mark<<<(unsigned)(((size_t)n * 32 + tb - 1) / tb), tb, 0, st>>>(ref_lo, ref_hi, n, g, occ, 0);
             gd_k_grid_dt_x<<<(g.ny * g.nz + 127) / 128, 128, 0, st>>>(g, occ);
             gd_k_grid_dt_y<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, occ, d2);
             gd_k_grid_dt_z<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, d2, cells);

@@ -526,25 +526,43 @@ __global__ void gd_k_collapse8(int n_inner, const int *__restrict__ child_l, con
 // separable (x by two sweeps per row, then y and z as windowed lower envelopes), capped at GD_GRID_WINDOW + 1 cells;
 // 3. clearance of a cell = (centre-to-centre distance - sqrt(3)) h: two points of the two cells are at least that far
 // apart.  Everything is rounded towards "nearer", so the stored value never exceeds the true clearance.
-#define GD_GRID_WINDOW 24
+#define GD_GRID_WINDOW 16
+// per_lane != 0: one reference box per lane, a box of more than 16 cells is marked by the whole warp (many small facets);
+// per_lane == 0: one reference box per warp (few, large facets)
 __global__ void gd_k_grid_mark(const float4 *__restrict__ ref_lo, const float4 *__restrict__ ref_hi, int n_ref, GdGrid g,
-                               unsigned char *__restrict__ occ) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_ref) return;
-    const float4 lo = ref_lo[i], hi = ref_hi[i];
-    const float pad = 2.0e-4f;          // float32 slack of the boxes and of the cell index computed in the transport kernel
-    const float ex = pad + 1.0e-6f * fmaxf(fabsf(lo.x), fabsf(hi.x)), ey = pad + 1.0e-6f * fmaxf(fabsf(lo.y), fabsf(hi.y)),
-                ez = pad + 1.0e-6f * fmaxf(fabsf(lo.z), fabsf(hi.z));
-    int x0 = (int)floorf((lo.x - ex - g.lox) * g.inv_h), x1 = (int)floorf((hi.x + ex - g.lox) * g.inv_h);
-    int y0 = (int)floorf((lo.y - ey - g.loy) * g.inv_h), y1 = (int)floorf((hi.y + ey - g.loy) * g.inv_h);
-    int z0 = (int)floorf((lo.z - ez - g.loz) * g.inv_h), z1 = (int)floorf((hi.z + ez - g.loz) * g.inv_h);
-    x0 = max(x0, 0); y0 = max(y0, 0); z0 = max(z0, 0);
-    x1 = min(x1, g.nx - 1); y1 = min(y1, g.ny - 1); z1 = min(z1, g.nz - 1);
-    for (int z = z0; z <= z1; ++z)
-        for (int y = y0; y <= y1; ++y) {
-            unsigned char *row = occ + ((size_t)z * g.ny + y) * g.nx;
-            for (int x = x0; x <= x1; ++x) row[x] = 1;
+                               unsigned char *__restrict__ occ, int per_lane) {
+    const int lane = threadIdx.x & 31;
+    const int i = per_lane ? blockIdx.x * blockDim.x + threadIdx.x : (lane == 0 ? (int)(((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) : n_ref);
+    int x0 = 0, x1 = -1, y0 = 0, y1 = -1, z0 = 0, z1 = -1;
+    if (i < n_ref) {
+        const float4 lo = ref_lo[i], hi = ref_hi[i];
+        const float pad = 2.0e-4f;      // float32 slack of the boxes and of the cell index computed in the transport kernel
+        const float ex = pad + 1.0e-6f * fmaxf(fabsf(lo.x), fabsf(hi.x)), ey = pad + 1.0e-6f * fmaxf(fabsf(lo.y), fabsf(hi.y)),
+                    ez = pad + 1.0e-6f * fmaxf(fabsf(lo.z), fabsf(hi.z));
+        x0 = max((int)floorf((lo.x - ex - g.lox) * g.inv_h), 0); x1 = min((int)floorf((hi.x + ex - g.lox) * g.inv_h), g.nx - 1);
+        y0 = max((int)floorf((lo.y - ey - g.loy) * g.inv_h), 0); y1 = min((int)floorf((hi.y + ey - g.loy) * g.inv_h), g.ny - 1);
+        z0 = max((int)floorf((lo.z - ez - g.loz) * g.inv_h), 0); z1 = min((int)floorf((hi.z + ez - g.loz) * g.inv_h), g.nz - 1);
+    }
+    const bool any = x1 >= x0 && y1 >= y0 && z1 >= z0;
+    const long long n = any ? (long long)(x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1) : 0;
+    if (any && n <= 16)
+        for (int z = z0; z <= z1; ++z)
+            for (int y = y0; y <= y1; ++y)
+                for (int x = x0; x <= x1; ++x) occ[((size_t)z * g.ny + y) * g.nx + x] = 1;
+    unsigned big = __ballot_sync(0xFFFFFFFFu, n > 16);
+    while (big) {
+        const int src = __ffs(big) - 1;
+        big &= big - 1;
+        const int bx0 = __shfl_sync(0xFFFFFFFFu, x0, src), bx1 = __shfl_sync(0xFFFFFFFFu, x1, src);
+        const int by0 = __shfl_sync(0xFFFFFFFFu, y0, src), by1 = __shfl_sync(0xFFFFFFFFu, y1, src);
+        const int bz0 = __shfl_sync(0xFFFFFFFFu, z0, src), bz1 = __shfl_sync(0xFFFFFFFFu, z1, src);
+        const int wx = bx1 - bx0 + 1, wy = by1 - by0 + 1;
+        const long long nb = (long long)wx * wy * (bz1 - bz0 + 1);
+        for (long long k = lane; k < nb; k += 32) {
+            const int x = bx0 + (int)(k % wx), y = by0 + (int)((k / wx) % wy), z = bz0 + (int)(k / ((long long)wx * wy));
+            occ[((size_t)z * g.ny + y) * g.nx + x] = 1;
         }
+    }
 }
 // rows along x: occ (1 = marked) -> distance in cells to the nearest marked cell of the row, capped, in place
 __global__ void gd_k_grid_dt_x(GdGrid g, unsigned char *__restrict__ occ) {

@@ -373,6 +373,43 @@ GD_HD bool gd_lane_post_t(GdLane &L, const GdMaterials &M, const float *tab, con
     if (!ELECTRON) gd_lane_finish(L, S, out);
     return true;
 }
+// The two event kinds that make up almost all events of a scattering chain, with the arithmetic of gd_lane_post_t
+// (same expressions, same order: results are bit-identical): a boundary crossing into another medium, and a coherent
+// scattering.  Returns 0 when the event is neither (or is a crossing into KILL, a stalled crossing, a photon below the
+// cut-off): the lane is then untouched and the event belongs to gd_lane_post.  1 = crossing done, 2 = coherent done.
+// Only for mode FLIGHT and a hit that is a crossing, or no hit with a finite flight length.
+GD_D int gd_lane_fast_event(GdLane &L, const GdMaterials &M, const GdHit &hit) {
+    if (hit.leaf >= 0) {                                                                    // O7.6 boundary first
+        const int to = hit.leaving ? gd_mat_outside(hit.mats) : gd_mat_inside(hit.mats);
+        const float t = fmaxf(hit.t, 0.0f);
+        const int stall = t > GD_TBACK ? 1 : L.n_stall + 1;
+        if (to == GD_MAT_KILL || stall > 32) return 0;
+        L.pos.x += t * L.dir.x; L.pos.y += t * L.dir.y; L.pos.z += t * L.dir.z;
+        L.tau -= L.mu_tot * t;
+        L.m = to;
+        L.need_mu = 1;
+        L.n_stall = stall;
+        L.ex.c = L.ex.b; L.ex.b = L.ex.a; L.ex.a = hit.orig;
+        return 1;
+    }
+    if (L.e < M.e_cut) return 0;
+    const GdF4u u4 = gd_rng_peek4(L.g);                   // selection draw + the three draws of a coherent event
+    const float us = u4.a * L.mu_tot;
+    float acc = 0.0f;
+    int ch = -1;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) { acc += L.mu[c]; if (ch < 0 && us < acc) ch = c; }
+    if (ch != 2) return 0;
+    L.pos.x += L.sdist * L.dir.x; L.pos.y += L.sdist * L.dir.y; L.pos.z += L.sdist * L.dir.z;     // O7.4
+    L.n_events++;
+    L.ex = gd_no_exclude(); L.n_stall = 0;
+    const float cost = gd_thomson_from(u4.b);                                               // O11
+    L.dir = gd_rotate(L.dir, cost, u4.c);
+    L.tau = -logf(u4.d);                                                                    // O7.1
+    L.g.draw += 4;
+    return 2;
+}
+
 GD_HD bool gd_lane_post(GdLane &L, const GdMaterials &M, const float *tab, const GdSource &S, unsigned long long seed,
                         const GdHit &hit, GdHistory &out, GdLocalCounters &cnt) {
     return gd_lane_post_t<false>(L, M, tab, S, seed, hit, out, cnt);

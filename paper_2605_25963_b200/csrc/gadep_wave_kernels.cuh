@@ -254,7 +254,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     __shared__ GdSource s_src;
     __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];
     __shared__ unsigned s_cnt[12];
-    __shared__ GdQueue s_ready, s_result;
+    __shared__ GdQueue s_ready, s_result, s_slow;
     __shared__ GdHistPool s_hist;
     __shared__ unsigned s_live;                     // slots that still carry or may get a history
     const int n_tab = M.n_mat * 4 * M.n_grid;
@@ -266,14 +266,14 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i];
     if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }
     if (threadIdx.x < 12) s_cnt[threadIdx.x] = 0;
-    // every slot starts in RESULT with mode NEED: the first P-bursts start the first histories
+    // every slot starts in the general queue with mode NEED: the first passes start the first histories
     for (int s = threadIdx.x; s < GD_W_NSLOT; s += blockDim.x) {
         GD_SF(14) = __uint_as_float((unsigned)GD_MODE_NEED << 5);
-        s_result.ent[s] = (unsigned short)(gd_q_tag((unsigned)s) | (unsigned)s);
-        s_ready.ent[s] = 0;
+        s_slow.ent[s] = (unsigned short)(gd_q_tag((unsigned)s) | (unsigned)s);
+        s_ready.ent[s] = 0; s_result.ent[s] = 0;
     }
     if (threadIdx.x == 0) {
-        s_result.head = 0; s_result.tail = GD_W_NSLOT; s_ready.head = 0; s_ready.tail = 0;
+        s_slow.head = 0; s_slow.tail = GD_W_NSLOT; s_result.head = 0; s_result.tail = 0; s_ready.head = 0; s_ready.tail = 0;
         s_hist.state = 0ull; s_hist.lock = 0u; s_hist.dry = 0u;
         s_live = GD_W_NSLOT;
     }
@@ -285,8 +285,12 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     int stack[WIDTH == 8 ? GD_STACK8 : GD_STACK4];
     GdTrav T;
     gd_trav_idle(T);
-    unsigned n_box = 0, n_tri = 0, n_query = 0, n_done = 0, n_skip = 0;
+    unsigned n_box = 0, n_tri = 0, n_query = 0, n_done = 0, n_skip = 0, n_fast_cross = 0, n_fast_coh = 0;
     static_assert(GD_W_NSLOT == 1024, "queue entries hold a 10-bit slot number");
+    // warps of the last SM sub-partition take the general (slow) passes first, so that the other three keep the two
+    // compact loops in their instruction caches
+    const bool slow_first = ((threadIdx.x >> 5) & 3u) == 3u;
+    unsigned idle_ns = 250u;
 #ifdef GD_PROF
     unsigned long long pacc[16] = {};
     long long p_t0 = clock64();
@@ -295,26 +299,122 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     for (;;) {
         // ---- what next?  (queue lengths are snapshots: a wrong guess costs a pass with fewer lanes, never a result)
         const int my_rays = __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0));
-        int n_res = 0, n_rdy = 0;
+        int n_res = 0, n_rdy = 0, n_slow = 0;
         unsigned live = 0;
-        if (lane == 0) { n_res = gd_q_count(&s_result); n_rdy = gd_q_count(&s_ready); live = *(volatile unsigned *)&s_live; }
+        if (lane == 0) {
+            n_res = gd_q_count(&s_result); n_rdy = gd_q_count(&s_ready); n_slow = gd_q_count(&s_slow);
+            live = *(volatile unsigned *)&s_live;
+        }
         n_res = __shfl_sync(0xFFFFFFFFu, n_res, 0);
         n_rdy = __shfl_sync(0xFFFFFFFFu, n_rdy, 0);
+        n_slow = __shfl_sync(0xFFFFFFFFu, n_slow, 0);
         live = __shfl_sync(0xFFFFFFFFu, live, 0);
         const bool t_work = my_rays > 0 || n_rdy > 0;
-        // warps of the first `t_smsp` SM sub-partitions (warp & 3) prefer traversal, the others physics: the four warps
-        // that share an instruction cache then run the same loop most of the time
-        const bool pref_t = (int)((threadIdx.x >> 5) & 3u) < tune.t_smsp;
-        const bool do_p = pref_t ? n_res > 0 && ((my_rays < tune.t_keep && n_rdy == 0 && n_res >= tune.p_min) || !t_work)
-                                 : n_res > 0 && (n_res >= tune.p_min || !t_work);
-        if (!do_p && !t_work) {
+        const bool few_rays = my_rays < tune.t_keep || n_rdy == 0;
+        const bool other_work = t_work || n_res > 0;
+        const bool do_slow = n_slow > 0 && (n_slow >= (slow_first ? tune.p_min : 8 * tune.p_min) || !other_work) && (few_rays || !t_work);
+        const bool do_fast = !do_slow && n_res > 0 && few_rays && (n_res >= tune.p_min || !t_work);
+        if (!do_slow && !do_fast && !t_work) {
             if (live == 0u) break;               // every slot of the block is dead
-            __nanosleep(200);                    // other warps hold all the work there is
+            __nanosleep(idle_ns);                // other warps hold all the work there is: back off
+            if (idle_ns < 4000u) idle_ns *= 2u;
             continue;
         }
-        if (do_p) {
-            // ============================================================ P-burst
+        idle_ns = 250u;
+        if (do_slow) {
+            // ============================================================ general pass: any event, one per slot
+            int s = 0;
             bool has = false;
+            gd_q_claim(&s_slow, true, 32, lane, s, has);
+            GdLane L;
+            L.mode = GD_MODE_DONE;
+            GdHit hit;
+            hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
+            if (has) {
+                gd_slot_load(sl, s, L, seed, first);
+                if (L.pending) {
+                    const float *p = pair + s * 8;
+                    L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
+                }
+                // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the
+                // to-side id as "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
+                hit.t = GD_SF(22);
+                hit.orig = __float_as_int(GD_SF(23));
+                hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
+                hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
+            }
+            GD_PROF_ADD(7, 1); GD_PROF_ADD(8, __popc(__ballot_sync(0xFFFFFFFFu, has)));
+            GdLocalCounters cnt = {};
+            GdHistory r;
+            r.edep = 0.0f; r.flags = 0u; r.line = 0;
+            bool fin = false;
+            if (has && L.mode != GD_MODE_NEED) {
+                const int was_pending = L.pending;
+                fin = gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt);
+                if (fin) {
+                    n_done++;
+                    const unsigned long long hrel = L.history - first;
+                    if (edep_out) edep_out[hrel] = r.edep;
+                    if (flags_out) flags_out[hrel] = r.flags;
+                } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
+                    float *p = pair + s * 8;
+                    p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
+                    p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
+                }
+            }
+            gd_tally_warp(fin, r, s_src, tally, s_spec, s_emitted, s_peak, lane);
+            {   // event counters, one shared-memory atomic per kind and pass (crossing / PE / Compton / coherent /
+                // pair; escapes, re-localisations and cut-offs can accompany any of them)
+                const unsigned v[8] = {cnt.n_crossings, cnt.n_pe, cnt.n_compton, cnt.n_coherent, cnt.n_pair, cnt.n_escaped,
+                                       cnt.n_leak, cnt.n_cutoff};
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const unsigned mk = __ballot_sync(0xFFFFFFFFu, v[k] != 0u);
+                    if (mk && lane == 0) atomicAdd(&s_cnt[4 + k], (unsigned)__popc(mk));
+                }
+            }
+            // ---- finished slots take the next histories of the block's chunk
+            const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, has && L.mode == GD_MODE_NEED);
+            if (need_mask) {
+                unsigned a0, n0, a1;
+                gd_hist_take(&s_hist, (unsigned)__popc(need_mask), next_history, n_hist, chunk, gridDim.x, lane, a0, n0, a1);
+                bool died = false;
+                if (has && L.mode == GD_MODE_NEED) {
+                    const unsigned rk = __popc(need_mask & lt_mask);
+                    const unsigned long long h = rk < n0 ? a0 + rk : (unsigned long long)a1 + (rk - n0);
+                    if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
+                    else { L.mode = GD_MODE_DONE; died = true; }
+                }
+                const unsigned died_mask = __ballot_sync(0xFFFFFFFFu, died);
+                if (died_mask && lane == 0) atomicSub(&s_live, (unsigned)__popc(died_mask));
+            }
+            // ---- the next query: answered by the clearance grid (the slot then waits in RESULT with its answer), or
+            // handed to READY
+            const bool live_lane = has && L.mode != GD_MODE_DONE;
+            bool skip = false;
+            if (live_lane) {
+                float t_min, t_max;
+                int filter;
+                gd_lane_query(L, M, s_tab, t_min, t_max, filter);
+                if (L.mode == GD_MODE_FLIGHT && L.sdist < GD_INF)
+                    skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
+                gd_slot_store(sl, s, L, first);
+                if (skip) { n_skip++; GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
+            }
+            gd_q_push(&s_ready, live_lane && !skip, s, lane);
+            gd_q_push(&s_result, live_lane && skip, s, lane);
+#ifdef GD_PROF
+            { const long long t1 = clock64(); GD_PROF_ADD(9, t1 - p_t0); p_t0 = t1; }
+#endif
+            continue;
+        }
+        if (do_fast) {
+            // ============================================================ chain burst: crossings and coherent events
+            // Lanes take RESULT slots (flights that met a facet or ended in an interaction) and handle the two event
+            // kinds of a scattering chain; anything else goes to the general queue untouched.  A slot whose next flight
+            // ends before the clearance of its grid cell stays on its lane and goes round again: the answer of that
+            // query is known ("none").  Lanes that gave their slot away take the next waiting result.
+            bool has = false, dirty = false;        // dirty: the lane's registers are newer than its slot
             int s = 0;
             GdLane L;
             L.mode = GD_MODE_DONE;
@@ -322,8 +422,8 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
             hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
             for (bool first_pass = true;; first_pass = false) {
                 // ---- a pass needs p_min lanes with work -- or a warp with no ray to go back to and none to fetch.
-                // Decided on a snapshot of the queue before anything is claimed: what is parked below must be lanes
-                // whose answer is known (no facet within the flight), never a freshly claimed traversal result.
+                // Decided on a snapshot of the queue before anything is claimed: what is parked below are lanes whose
+                // answer is known (no facet within the flight), never a freshly claimed traversal result.
                 const unsigned free_mask = __ballot_sync(0xFFFFFFFFu, !has);
                 const int n_has = 32 - __popc(free_mask);
                 int avail = 0, rdy = 0;
@@ -347,80 +447,38 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                 if (got) {
                     s = s_new;
                     gd_slot_load(sl, s, L, seed, first);
-                    if (L.pending) {
-                        const float *p = pair + s * 8;
-                        L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
-                    }
-                    // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the
-                    // to-side id as "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
                     hit.t = GD_SF(22);
                     hit.orig = __float_as_int(GD_SF(23));
                     hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
                     hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
-                    has = true;
+                    has = true; dirty = false;
                 }
                 if (n_has + take == 0) break;        // another warp was quicker
                 GD_PROF_ADD(2, 1); GD_PROF_ADD(3, n_has + take);
                 // ---- one event per lane
-                GdLocalCounters cnt = {};
-                GdHistory r;
-                r.edep = 0.0f; r.flags = 0u; r.line = 0;
-                bool fin = false;
-                if (has && L.mode != GD_MODE_NEED) {
-                    const int was_pending = L.pending;
-                    fin = gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt);
-                    if (fin) {
-                        n_done++;
-                        const unsigned long long hrel = L.history - first;
-                        if (edep_out) edep_out[hrel] = r.edep;
-                        if (flags_out) flags_out[hrel] = r.flags;
-                    } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
-                        float *p = pair + s * 8;
-                        p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
-                        p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
-                    }
+                int kind = 0;
+                if (has) kind = gd_lane_fast_event(L, M, hit);
+                const bool to_slow = has && kind == 0;
+                if (to_slow && dirty) {              // registers newer than the slot: write them back with the known answer
+                    gd_slot_store(sl, s, L, first);
+                    GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
                 }
-                gd_tally_warp(fin, r, s_src, tally, s_spec, s_emitted, s_peak, lane);
-                {   // event counters, one shared-memory atomic per kind and pass (crossing / PE / Compton / coherent /
-                    // pair; escapes, re-localisations and cut-offs can accompany any of them)
-                    const unsigned v[8] = {cnt.n_crossings, cnt.n_pe, cnt.n_compton, cnt.n_coherent, cnt.n_pair, cnt.n_escaped,
-                                           cnt.n_leak, cnt.n_cutoff};
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) {
-                        const unsigned mk = __ballot_sync(0xFFFFFFFFu, v[k] != 0u);
-                        if (mk && lane == 0) atomicAdd(&s_cnt[4 + k], (unsigned)__popc(mk));
-                    }
-                }
-                // ---- finished slots take the next histories of the block's chunk
-                const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, has && L.mode == GD_MODE_NEED);
-                if (need_mask) {
-                    unsigned a0, n0, a1;
-                    gd_hist_take(&s_hist, (unsigned)__popc(need_mask), next_history, n_hist, chunk, gridDim.x, lane, a0, n0, a1);
-                    bool died = false;
-                    if (has && L.mode == GD_MODE_NEED) {
-                        const unsigned rk = __popc(need_mask & lt_mask);
-                        const unsigned long long h = rk < n0 ? a0 + rk : (unsigned long long)a1 + (rk - n0);
-                        if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
-                        else { L.mode = GD_MODE_DONE; died = true; }
-                    }
-                    const unsigned died_mask = __ballot_sync(0xFFFFFFFFu, died);
-                    if (died_mask && lane == 0) atomicSub(&s_live, (unsigned)__popc(died_mask));
-                }
+                gd_q_push(&s_slow, to_slow, s, lane);
+                if (to_slow) has = false;
+                n_fast_cross += kind == 1; n_fast_coh += kind == 2;
                 // ---- the next query: answered by the clearance grid, or handed to READY
-                const bool live_lane = has && L.mode != GD_MODE_DONE;
                 bool skip = false;
-                if (live_lane) {
+                if (has) {
                     float t_min, t_max;
                     int filter;
                     gd_lane_query(L, M, s_tab, t_min, t_max, filter);
-                    if (L.mode == GD_MODE_FLIGHT && L.sdist < GD_INF)
-                        skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
+                    if (L.sdist < GD_INF) skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
                 }
-                const bool to_ready = live_lane && !skip;
+                const bool to_ready = has && !skip;
                 if (to_ready) gd_slot_store(sl, s, L, first);
                 gd_q_push(&s_ready, to_ready, s, lane);
                 has = skip;
-                if (skip) { n_skip++; hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.mats = 0; }
+                if (skip) { n_skip++; dirty = true; hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.mats = 0; }
             }
 #ifdef GD_PROF
             { const long long t1 = clock64(); GD_PROF_ADD(0, t1 - p_t0); p_t0 = t1; }
@@ -428,13 +486,27 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
             continue;
         }
         // ================================================================ T-burst
+        // Finished rays are retired and READY slots fetched in one go, once `k_fetch` lanes are free (finished or
+        // idle): the queue operations are paid every few rounds instead of every round.
         for (;;) {
-            const unsigned idle_mask = __ballot_sync(0xFFFFFFFFu, T.slot < 0);
-            const int n_idle = __popc(idle_mask);
-            if (n_idle >= tune.k_fetch || n_idle == 32) {
+            const bool done_l = T.slot >= 0 && T.node == GD_TRAV_DONE;
+            const unsigned free_mask = __ballot_sync(0xFFFFFFFFu, T.slot < 0 || done_l);
+            const int n_free = __popc(free_mask);
+            if (n_free >= tune.k_fetch || n_free == 32) {
+                // a start localisation, an escape (no facet, no interaction) and a crossing into KILL are general events;
+                // a crossing into another medium or an interaction goes to the chain burst
+                bool slow = false;
+                if (done_l) {
+                    const int s = T.slot;
+                    GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
+                    slow = T.filter == -2 || (T.orig == GD_NO_FACET ? !(T.t < GD_INF) : (T.fromto >> 16) == GD_MAT_KILL);
+                }
+                gd_q_push(&s_result, done_l && !slow, T.slot, lane);
+                gd_q_push(&s_slow, done_l && slow, T.slot, lane);
+                if (done_l) T.slot = -1;
                 bool got = false;
                 int s = 0;
-                const int tk = gd_q_claim(&s_ready, T.slot < 0, n_idle, lane, s, got);
+                const int tk = gd_q_claim(&s_ready, T.slot < 0, n_free, lane, s, got);
                 if (got) {
                     const unsigned st = __float_as_uint(GD_SF(14));
                     const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
@@ -444,23 +516,16 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
                     n_query++;
                 }
                 // nothing to fetch and few rays left: see whether physics has piled up (the rays stay in registers)
-                if (tk == 0 && 32 - n_idle < tune.t_keep) {
-                    if (n_idle == 32) break;
+                if (tk == 0 && 32 - n_free < tune.t_keep) {
+                    if (n_free == 32) break;
                     int r = 0;
-                    if (lane == 0) r = gd_q_count(&s_result);
+                    if (lane == 0) r = max(gd_q_count(&s_result), gd_q_count(&s_slow));
                     if (__shfl_sync(0xFFFFFFFFu, r, 0) >= tune.p_min) break;
                 }
             }
             GD_PROF_ADD(4, 1); GD_PROF_ADD(5, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0 && T.node >= 0)));
-            GD_PROF_ADD(6, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0)));
+            GD_PROF_ADD(6, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0 && T.node != GD_TRAV_DONE)));
             gd_trav_step<WIDTH>(T, bvh, stack, tune.n_steps, n_box, n_tri);
-            const bool fin = T.slot >= 0 && T.node == GD_TRAV_DONE;
-            if (fin) {
-                const int s = T.slot;
-                GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
-            }
-            gd_q_push(&s_result, fin, T.slot, lane);
-            if (fin) T.slot = -1;
         }
 #ifdef GD_PROF
         { const long long t1 = clock64(); GD_PROF_ADD(1, t1 - p_t0); p_t0 = t1; }
@@ -471,10 +536,10 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #endif
     // ---- flush: per-lane 32-bit work counters straight to the 64-bit global totals
     {
-        const unsigned v[5] = {n_done, n_query, n_box, n_tri, n_skip};
-        const int where[5] = {0, 1, 2, 3, 13};           // GdCounters: n_histories, n_queries, n_box_tests, n_tri_tests, n_skipped
+        const unsigned v[7] = {n_done, n_query, n_box, n_tri, n_skip, n_fast_cross, n_fast_coh};
+        const int where[7] = {0, 1, 2, 3, 13, 4, 7};     // GdCounters: n_histories, n_queries, n_box_tests, n_tri_tests, n_skipped, n_crossings, n_coherent
 #pragma unroll
-        for (int k = 0; k < 5; ++k) {
+        for (int k = 0; k < 7; ++k) {
             unsigned long long x = v[k];
 #pragma unroll
             for (int o = 16; o >= 1; o >>= 1) x += __shfl_down_sync(0xFFFFFFFFu, x, o);
