@@ -22,7 +22,7 @@
 #include "gadep_trav.cuh"
 #include "gadep_transport_kernels.cuh"
 
-#define GD_W_THREADS 512
+#define GD_W_THREADS 384
 #define GD_W_WARPS (GD_W_THREADS / 32)
 #define GD_W_NSLOT 1024           // photon slots per block (64 per warp)
 // fields per slot.  25 words keep the block's shared memory under the 164 KB carve-out for up to 9 materials, which
@@ -310,11 +310,13 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
         n_slow = __shfl_sync(0xFFFFFFFFu, n_slow, 0);
         live = __shfl_sync(0xFFFFFFFFu, live, 0);
         const bool t_work = my_rays > 0 || n_rdy > 0;
-        const bool few_rays = my_rays < tune.t_keep || n_rdy == 0;
+        const bool few_rays = my_rays < tune.t_keep;      // a warp with many rays in flight finishes them first: their slots are what the others wait for
         const bool other_work = t_work || n_res > 0;
         const bool do_slow = n_slow > 0 && (n_slow >= (slow_first ? tune.p_min : 8 * tune.p_min) || !other_work) && (few_rays || !t_work);
         const bool do_fast = !do_slow && n_res > 0 && few_rays && (n_res >= tune.p_min || !t_work);
+        GD_PROF_ADD(10, 1);
         if (!do_slow && !do_fast && !t_work) {
+            GD_PROF_ADD(11, 1);
             if (live == 0u) break;               // every slot of the block is dead
             __nanosleep(idle_ns);                // other warps hold all the work there is: back off
             if (idle_ns < 4000u) idle_ns *= 2u;
@@ -409,6 +411,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
             continue;
         }
         if (do_fast) {
+            GD_PROF_ADD(12, 1);
             // ============================================================ chain burst: crossings and coherent events
             // Lanes take RESULT slots (flights that met a facet or ended in an interaction) and handle the two event
             // kinds of a scattering chain; anything else goes to the general queue untouched.  A slot whose next flight
@@ -485,6 +488,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #endif
             continue;
         }
+        GD_PROF_ADD(13, 1);
         // ================================================================ T-burst
         // Finished rays are retired and READY slots fetched in one go, once `k_fetch` lanes are free (finished or
         // idle): the queue operations are paid every few rounds instead of every round.
