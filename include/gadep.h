@@ -121,6 +121,8 @@ int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
 #define GADEP_RUN_PARTIAL_XS 32     /* the paper's "partial cross-section method": one remaining    */
                                    /* optical depth per process instead of total-mu sampling + a selection draw  */
                                    /* (history-per-thread kernel; same distribution, different random streams)   */
+#define GADEP_RUN_WARP_SPECIALISED 64 /* measurement: traversal and physics on separate warps of a block, registers moved */
+                                   /* between them with setmaxnreg (same results, bit for bit)                     */
 #define GADEP_RUN_BVH8 256          /* measurement / cross-check: the wavefront kernel traverses the compressed      */
                                    /* 8-wide nodes instead of the uncompressed 4-wide ones (same results, bit for bit) */
 #define GADEP_RUN_ELECTRON_RANGE 128 /* SURVEY.md 8(f) NEXT-4 (coupled photon-electron physics): every   */

@@ -18,6 +18,7 @@ MAT_KILL = -1
 MAX_LINES = 64
 RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES, RUN_PARITY_LOCALISATION = 1, 2, 4, 8, 16
 RUN_PARTIAL_XS = 32
+RUN_WARP_SPECIALISED = 64
 RUN_BVH8 = 256
 RUN_ELECTRON_RANGE = 128
 

@@ -60,10 +60,11 @@ struct gadep_ctx {
     unsigned long long *d_next = nullptr;     // history counter of the refill kernel
     int run_width = 4;                        // width used by the current launch (bvh_width, or 8 with GADEP_RUN_BVH8)
     unsigned long long n_stack_overflow = 0;  // rays that ran out of traversal stack since the context was made (must stay 0)
+    bool prefer_ws = false;                   // GADEP_WS=1: the warp-specialised kernel instead of the default one (measurement)
     int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
-    GdWaveTune tune = {16, 16, 4, 16, 2};
+    GdWaveTune tune = {16, 16, 4, 16, 1};
     float rho[GADEP_MAX_MATERIALS] = {};      // g/cm^3, electron-range mode
     bool have_rho = false;
     // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
@@ -142,11 +143,12 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e == cudaSuccess) e = cudaEventCreate(&c->evb1);
     if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
     if (getenv("GADEP_NO_SURFACE_CLUSTERS")) c->cluster_surfaces = false;
+    if (const char *t = getenv("GADEP_WS")) c->prefer_ws = atoi(t) != 0;
     if (const char *t = getenv("GADEP_GRID_CELLS")) { long long v = atoll(t); if (v >= 0 && v <= (1ll << 28)) c->grid_cells = v; }
     if (const char *t = getenv("GADEP_SPLIT_BUDGET")) { double b = atof(t); if (b >= 0 && b <= 15) c->split_budget = b; }
-    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,t_keep,n_steps,p_min,t_smsp" (measurement sweeps)
-        int a, b, d, p = c->tune.p_min, ts = c->tune.t_smsp;
-        if (sscanf(t, "%d,%d,%d,%d,%d", &a, &b, &d, &p, &ts) >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && p >= 1 && p <= 32 && ts >= 0 && ts <= 4)
+    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,t_keep,n_steps,p_min,t_help" (measurement sweeps)
+        int a, b, d, p = c->tune.p_min, ts = c->tune.t_help;
+        if (sscanf(t, "%d,%d,%d,%d,%d", &a, &b, &d, &p, &ts) >= 3 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && p >= 1 && p <= 32 && ts >= 1 && ts <= 1024)
             c->tune = {a, b, d, p, ts};
     }
     *out = c;
@@ -553,11 +555,12 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0xFFFFFFFFull) return gd_fail(c, GADEP_E_ARG, "more than 2^32-1 histories in one launch");
     size_t smem = sizeof(float) * (size_t)c->n_mat * 4 * c->n_grid + sizeof(unsigned) * ((size_t)n_bins + 1);
     const int variant = c->kernel_variant;
-    const int threads = variant == 2 ? GD_W_THREADS : GD_RUN_THREADS;
+    const int threads = variant == 2 ? GD_W_THREADS : (variant == 5 ? GD_WS_THREADS : GD_RUN_THREADS);
     const bool wide8 = c->run_width == 8;
-    if (variant == 2) smem += sizeof(float) * (size_t)GD_W_NF * GD_W_NSLOT;
+    if (variant == 2 || variant == 5) smem += sizeof(float) * (size_t)GD_W_NF * GD_W_NSLOT;
     if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
-    const void *kern = variant == 2 ? (wide8 ? (const void *)gd_k_transport_wave<8> : (const void *)gd_k_transport_wave<4>)
+    const void *kern = variant == 5 ? (wide8 ? (const void *)gd_k_transport_ws<8> : (const void *)gd_k_transport_ws<4>)
+                     : variant == 2 ? (wide8 ? (const void *)gd_k_transport_wave<8> : (const void *)gd_k_transport_wave<4>)
                                     : (variant == 1 ? (const void *)gd_k_transport_refill
                                                   : (variant == 3 ? (const void *)gd_k_transport<true, false>
                                                      : (variant == 4 ? (const void *)gd_k_transport<false, true>
@@ -566,10 +569,10 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     int per_sm = 1;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return gd_fail(c, GADEP_E_CUDA, "transport kernel does not fit on an SM (%zu B shared memory)", smem);
-    const unsigned long long per_block = variant == 2 ? (unsigned long long)GD_W_NSLOT : GD_RUN_THREADS;
+    const unsigned long long per_block = (variant == 2 || variant == 5) ? (unsigned long long)GD_W_NSLOT : GD_RUN_THREADS;
     unsigned long long want = (n + per_block - 1) / per_block;
     int grid = (int)std::min<unsigned long long>((unsigned long long)c->n_sm * per_sm, std::max<unsigned long long>(want, 1));
-    if (variant == 2) {
+    if (variant == 2 || variant == 5) {
         size_t need = (size_t)grid * GD_W_NSLOT * 8;
         if (need > c->pair_floats) {
             cudaFree(c->d_pair); c->d_pair = nullptr; c->pair_floats = 0;
@@ -582,10 +585,16 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0) {
         unsigned long long warps = (unsigned long long)grid * (threads / 32);
         unsigned chunk = (unsigned)std::min<unsigned long long>(1024, std::max<unsigned long long>(32, n / (warps * 16)));
-        if (variant == 2)     // the wavefront kernel hands out history indices per block
+        if (variant == 2 || variant == 5)     // the wavefront kernels hand out history indices per block
             chunk = (unsigned)std::min<unsigned long long>(8192, std::max<unsigned long long>(256, n / ((unsigned long long)grid * 32)));
-        if (variant == 1 || variant == 2) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
-        if (variant == 2 && wide8) {
+        if (variant == 1 || variant == 2 || variant == 5) GD_CUDA(c, cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st));
+        if (variant == 5 && wide8) {
+            gd_k_transport_ws<8><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
+                                                              c->d_next, chunk, c->d_pair, c->tune);
+        } else if (variant == 5) {
+            gd_k_transport_ws<4><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
+                                                              c->d_next, chunk, c->d_pair, c->tune);
+        } else if (variant == 2 && wide8) {
             gd_k_transport_wave<8><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
                                                                 c->d_next, chunk, c->d_pair, c->tune);
         } else if (variant == 2) {
@@ -639,7 +648,7 @@ static int gd_fetch_results(gadep_ctx *c) {
 }
 
 static int gd_variant_of(int flags) {
-    return (flags & GADEP_RUN_ELECTRON_RANGE) ? 6 : (flags & GADEP_RUN_PARTIAL_XS) ? 4
+    return (flags & GADEP_RUN_ELECTRON_RANGE) ? 6 : (flags & GADEP_RUN_WARP_SPECIALISED) ? 5 : (flags & GADEP_RUN_PARTIAL_XS) ? 4
            : (flags & GADEP_RUN_PARITY_LOCALISATION) ? 3 : ((flags & GADEP_RUN_HISTORY_PER_THREAD) ? 0 : ((flags & GADEP_RUN_PERSISTENT_LANES) ? 1 : 2));
 }
 
@@ -666,10 +675,11 @@ extern "C" int gadep_run(gadep_ctx *c, unsigned long long n_histories, unsigned 
         return gd_fail(c, GADEP_E_ORDER, "GADEP_RUN_ELECTRON_RANGE needs gadep_set_densities");
     {   // GADEP_RUN_* kernel selectors exclude one another
         const int sel = opts->flags & (GADEP_RUN_HISTORY_PER_THREAD | GADEP_RUN_PERSISTENT_LANES | GADEP_RUN_PARITY_LOCALISATION |
-                                       GADEP_RUN_PARTIAL_XS | GADEP_RUN_ELECTRON_RANGE);
+                                       GADEP_RUN_PARTIAL_XS | GADEP_RUN_ELECTRON_RANGE | GADEP_RUN_WARP_SPECIALISED);
         if (sel & (sel - 1)) return gd_fail(c, GADEP_E_ARG, "run flags 0x%x select more than one kernel", opts->flags);
     }
     c->kernel_variant = gd_variant_of(opts->flags);
+    if (c->kernel_variant == 2 && c->prefer_ws) c->kernel_variant = 5;
     c->run_width = (opts->flags & GADEP_RUN_BVH8) ? 8 : c->bvh_width;
     int rc = gd_launch_transport(c, opts->first_history, n_histories, seed, opts->n_bins, opts->e_max_mev,
                                  (opts->flags & GADEP_RUN_ACCUMULATE) != 0, nullptr, nullptr);
@@ -862,7 +872,7 @@ extern "C" int gadep_run_histories_ex(gadep_ctx *c, unsigned long long first, lo
     float e_max = c->spec_e_max > 0 ? c->spec_e_max : 2.0f;
     {
         const int sel = run_flags & (GADEP_RUN_HISTORY_PER_THREAD | GADEP_RUN_PERSISTENT_LANES | GADEP_RUN_PARITY_LOCALISATION |
-                                     GADEP_RUN_PARTIAL_XS | GADEP_RUN_ELECTRON_RANGE);
+                                     GADEP_RUN_PARTIAL_XS | GADEP_RUN_ELECTRON_RANGE | GADEP_RUN_WARP_SPECIALISED);
         if (sel & (sel - 1)) { cudaFree(stage_e); cudaFree(stage_f); return gd_fail(c, GADEP_E_ARG, "run flags 0x%x select more than one kernel", run_flags); }
     }
     c->kernel_variant = gd_variant_of(run_flags & ~(GADEP_RUN_ASYNC | GADEP_RUN_ACCUMULATE));   // 0: the default kernel

@@ -44,8 +44,21 @@ struct GdWaveTune {
     int t_keep;         // a warp stays in its T-burst while at least this many of its lanes hold a ray (or READY has more)
     int n_steps;        // node visits per traversal round
     int p_min;          // a physics pass runs while this many lanes have work (or the warp has nothing else to do)
-    int t_smsp;         // SM sub-partitions (0..4) whose warps prefer traversal work
+    int t_help;         // READY slots that must wait before the warps that do not prefer traversal fetch any
 };
+
+// Ordering between a slot's words and the queue entry that publishes it: an acquire-release fence at block scope
+// (lighter than the sequentially consistent __threadfence_block()).
+#ifndef GD_FENCE_MODE
+#define GD_FENCE_MODE 1
+#endif
+#if GD_FENCE_MODE == 0
+#define GD_FENCE_BLOCK() __threadfence_block()
+#elif GD_FENCE_MODE == 1
+#define GD_FENCE_BLOCK() asm volatile("fence.acq_rel.cta;" ::: "memory")
+#else
+#define GD_FENCE_BLOCK() asm volatile("" ::: "memory")
+#endif
 
 // ---- block-wide queue of slot numbers (multi-producer, multi-consumer, warp-granular).  Tickets count up for ever;
 // ticket k lives in entry k mod GD_W_NSLOT and carries the lap number (k / GD_W_NSLOT) mod 32 beside the valid bit, so
@@ -71,7 +84,7 @@ GD_D void gd_q_push(GdQueue *q, bool push, int slot, unsigned lane) {
         const unsigned ticket = base + __popc(mask & ((1u << lane) - 1u));
         volatile unsigned short *e = &q->ent[ticket & (GD_W_NSLOT - 1)];
         while (*e != 0) {}                   // the consumer of the previous lap has claimed this entry but not yet emptied it
-        __threadfence_block();               // slot words before the valid bit
+        GD_FENCE_BLOCK();                    // slot words before the valid bit
         *e = (unsigned short)(gd_q_tag(ticket) | (unsigned)slot);
     }
 }
@@ -101,7 +114,7 @@ GD_D int gd_q_claim(GdQueue *q, bool free, int want, unsigned lane, int &slot, b
         unsigned v;
         while (((v = *e) & 0xFC00u) != tag) {}   // the producer holds the ticket but has not written the entry yet
         *e = 0;
-        __threadfence_block();               // valid bit before the slot words
+        GD_FENCE_BLOCK();                    // valid bit before the slot words
         slot = (int)(v & 0x3FFu);
         got = true;
     }
@@ -164,7 +177,7 @@ GD_D void gd_hist_take(GdHistPool *hp, unsigned n, unsigned long long *next_hist
                 }
             }
             if (g1 >= nh) *(volatile unsigned *)&hp->dry = 1u;
-            __threadfence_block();
+            GD_FENCE_BLOCK();
             atomicExch(&hp->lock, 0u);
             break;
         }
@@ -241,61 +254,338 @@ GD_D void gd_tally_warp(bool fin, const GdHistory &r, const GdSource &S, const G
     }
 }
 
+// The two physics routines are inlined.  Compiled out of line (GD_PASS_INLINE 0: the caller's traversal state is saved
+// around the call instead of competing with the photon state for registers) they measured 25 % slower on configs 2 / 3:
+// the block context and the launch constants then travel through local memory.
+#ifndef GD_PASS_INLINE
+#define GD_PASS_INLINE 1
+#endif
+#if GD_PASS_INLINE
+#define GD_PASS __device__ __forceinline__
+#else
+#define GD_PASS __device__ __noinline__
+#endif
+
+// ---- what the warps of a block share
+struct GdBlk {
+    float *sl;                                 // photon slots, SoA
+    const float *tab;                          // attenuation tables
+    const GdSource *src;
+    unsigned *spec, *emitted, *peak, *cnt;     // per-block tallies and event counters
+    GdQueue *ready, *result, *slow;
+    GdHistPool *hist;
+    unsigned *live;                            // slots that still carry or may get a history
+    float *pair;                               // global: parked annihilation photons of the block's slots
+};
+struct GdRunArgs {                             // launch constants of a transport kernel
+    unsigned long long first, n_hist, seed;
+    float *edep_out;
+    unsigned *flags_out;
+    unsigned long long *next_history;
+    unsigned chunk;
+};
+struct GdLaneCounters { unsigned n_done, n_skip, n_fast_cross, n_fast_coh; };
+
+// ============================================================ general pass: any event, one per claimed slot
+// (start of a history, start localisation, escape, crossing into KILL, photoelectric / Compton / pair event, cut-off,
+// the next annihilation photon, tally + the next history of the block's chunk)
+GD_PASS void gd_general_pass(const GdBlk &B, const GdBvh &bvh, const GdMaterials &M, const GdTally &tally, const GdRunArgs &A,
+                          unsigned lane, GdLaneCounters &C) {
+    float *sl = B.sl;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    int s = 0;
+    bool has = false;
+    gd_q_claim(B.slow, true, 32, lane, s, has);
+    GdLane L;
+    L.mode = GD_MODE_DONE;
+    GdHit hit;
+    hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
+    if (has) {
+        gd_slot_load(sl, s, L, A.seed, A.first);
+        if (L.pending) {
+            const float *p = B.pair + s * 8;
+            L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
+        }
+        // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the to-side id as
+        // "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
+        hit.t = GD_SF(22);
+        hit.orig = __float_as_int(GD_SF(23));
+        hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
+        hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
+    }
+    GdLocalCounters cnt = {};
+    GdHistory r;
+    r.edep = 0.0f; r.flags = 0u; r.line = 0;
+    bool fin = false;
+    if (has && L.mode != GD_MODE_NEED) {
+        const int was_pending = L.pending;
+        fin = gd_lane_post(L, M, B.tab, *B.src, A.seed, hit, r, cnt);
+        if (fin) {
+            C.n_done++;
+            const unsigned long long hrel = L.history - A.first;
+            if (A.edep_out) A.edep_out[hrel] = r.edep;
+            if (A.flags_out) A.flags_out[hrel] = r.flags;
+        } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
+            float *p = B.pair + s * 8;
+            p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
+            p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
+        }
+    }
+    gd_tally_warp(fin, r, *B.src, tally, B.spec, B.emitted, B.peak, lane);
+    {   // event counters, one shared-memory atomic per kind and pass (crossing / PE / Compton / coherent / pair; escapes,
+        // re-localisations and cut-offs can accompany any of them)
+        const unsigned v[8] = {cnt.n_crossings, cnt.n_pe, cnt.n_compton, cnt.n_coherent, cnt.n_pair, cnt.n_escaped,
+                               cnt.n_leak, cnt.n_cutoff};
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const unsigned mk = __ballot_sync(0xFFFFFFFFu, v[k] != 0u);
+            if (mk && lane == 0) atomicAdd(&B.cnt[4 + k], (unsigned)__popc(mk));
+        }
+    }
+    // ---- finished slots take the next histories of the block's chunk
+    const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, has && L.mode == GD_MODE_NEED);
+    if (need_mask) {
+        unsigned a0, n0, a1;
+        gd_hist_take(B.hist, (unsigned)__popc(need_mask), A.next_history, A.n_hist, A.chunk, gridDim.x, lane, a0, n0, a1);
+        bool died = false;
+        if (has && L.mode == GD_MODE_NEED) {
+            const unsigned rk = __popc(need_mask & lt_mask);
+            const unsigned long long h = rk < n0 ? a0 + rk : (unsigned long long)a1 + (rk - n0);
+            if (h < A.n_hist) gd_lane_start(L, *B.src, A.seed, A.first + h);
+            else { L.mode = GD_MODE_DONE; died = true; }
+        }
+        const unsigned died_mask = __ballot_sync(0xFFFFFFFFu, died);
+        if (died_mask && lane == 0) atomicSub(B.live, (unsigned)__popc(died_mask));
+    }
+    // ---- the next query: answered by the clearance grid (the slot then waits in RESULT with its answer), or handed
+    // to READY
+    const bool live_lane = has && L.mode != GD_MODE_DONE;
+    bool skip = false;
+    if (live_lane) {
+        float t_min, t_max;
+        int filter;
+        gd_lane_query(L, M, B.tab, t_min, t_max, filter);
+        if (L.mode == GD_MODE_FLIGHT && L.sdist < GD_INF)
+            skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
+        gd_slot_store(sl, s, L, A.first);
+        if (skip) { C.n_skip++; GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
+    }
+    gd_q_push(B.ready, live_lane && !skip, s, lane);
+    gd_q_push(B.result, live_lane && skip, s, lane);
+}
+
+// ============================================================ chain burst: crossings and coherent events
+// Lanes take RESULT slots (flights that met a facet or ended in an interaction) and handle the two event kinds of a
+// scattering chain; anything else goes to the general queue untouched.  A slot whose next flight ends before the
+// clearance of its grid cell stays on its lane and goes round again: the answer of that query is known ("none").  Lanes
+// that gave their slot away take the next waiting result.  `can_leave`: the warp has other work to go to (rays in
+// flight, or READY slots to fetch) once fewer than p_min lanes are busy.
+template <bool CAN_TRAVERSE>
+GD_PASS void gd_chain_burst(const GdBlk &B, const GdBvh &bvh, const GdMaterials &M, const GdRunArgs &A, const GdWaveTune &tune,
+                         int my_rays, unsigned lane, GdLaneCounters &C, unsigned long long *pacc) {
+    float *sl = B.sl;
+    bool has = false, dirty = false;        // dirty: the lane's registers are newer than its slot
+    int s = 0;
+    GdLane L;
+    L.mode = GD_MODE_DONE;
+    GdHit hit;
+    hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
+    for (bool first_pass = true;; first_pass = false) {
+        // ---- a pass needs p_min lanes with work -- or a warp with nothing else to do.  Decided on a snapshot of the
+        // queues before anything is claimed: what is parked below are lanes whose answer is known (no facet within the
+        // flight), never a freshly claimed traversal result.
+        const unsigned free_mask = __ballot_sync(0xFFFFFFFFu, !has);
+        const int n_has = 32 - __popc(free_mask);
+        int avail = 0, other = 0;
+        if (lane == 0) { avail = gd_q_count(B.result); other = CAN_TRAVERSE ? gd_q_count(B.ready) : gd_q_count(B.slow); }
+        avail = __shfl_sync(0xFFFFFFFFu, avail, 0);
+        other = __shfl_sync(0xFFFFFFFFu, other, 0);
+        const int expect = n_has + (avail < 32 - n_has ? avail : 32 - n_has);
+        const bool nothing_else = CAN_TRAVERSE ? (my_rays == 0 && other == 0) : other < tune.p_min;
+        const bool go = expect > 0 && (first_pass || expect >= tune.p_min || nothing_else);
+        if (!go) {
+            if (has) {
+                gd_slot_store(sl, s, L, A.first);
+                GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
+            }
+            gd_q_push(B.result, has, s, lane);
+            break;
+        }
+        // ---- fetch: lanes without a slot take waiting results
+        bool got = false;
+        int s_new = 0;
+        const int take = gd_q_claim(B.result, !has, 32 - n_has, lane, s_new, got);
+        if (got) {
+            s = s_new;
+            gd_slot_load(sl, s, L, A.seed, A.first);
+            hit.t = GD_SF(22);
+            hit.orig = __float_as_int(GD_SF(23));
+            hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
+            hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
+            has = true; dirty = false;
+        }
+        if (n_has + take == 0) break;        // another warp was quicker
+#ifdef GD_PROF
+        pacc[2] += 1; pacc[3] += n_has + take;
+#endif
+        // ---- one event per lane
+        int kind = 0;
+        if (has) kind = gd_lane_fast_event(L, M, hit);
+        const bool to_slow = has && kind == 0;
+        if (to_slow && dirty) {              // registers newer than the slot: write them back with the known answer
+            gd_slot_store(sl, s, L, A.first);
+            GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
+        }
+        gd_q_push(B.slow, to_slow, s, lane);
+        if (to_slow) has = false;
+        C.n_fast_cross += kind == 1; C.n_fast_coh += kind == 2;
+        // ---- the next query: answered by the clearance grid, or handed to READY
+        bool skip = false;
+        if (has) {
+            float t_min, t_max;
+            int filter;
+            gd_lane_query(L, M, B.tab, t_min, t_max, filter);
+            if (L.sdist < GD_INF) skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
+        }
+        const bool to_ready = has && !skip;
+        if (to_ready) gd_slot_store(sl, s, L, A.first);
+        gd_q_push(B.ready, to_ready, s, lane);
+        has = skip;
+        if (skip) { C.n_skip++; dirty = true; hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.mats = 0; }
+    }
+}
+
+// ============================================================ traversal service: retire finished rays, fetch READY slots
+// Returns the number of slots fetched.  A start localisation, an escape (no facet, no interaction) and a crossing into
+// KILL are general events; a crossing into another medium or an interaction goes to the chain burst.
+GD_D int gd_trav_service(GdTrav &T, const GdBlk &B, const GdBvh &bvh, int *stack, int n_free, int rdy_min, unsigned lane, unsigned &n_query) {
+    float *sl = B.sl;
+    const bool done_l = T.slot >= 0 && T.node == GD_TRAV_DONE;
+    bool slow = false;
+    if (done_l) {
+        const int s = T.slot;
+        GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
+        slow = T.filter == -2 || (T.orig == GD_NO_FACET ? !(T.t < GD_INF) : (T.fromto >> 16) == GD_MAT_KILL);
+    }
+    gd_q_push(B.result, done_l && !slow, T.slot, lane);
+    gd_q_push(B.slow, done_l && slow, T.slot, lane);
+    if (done_l) T.slot = -1;
+    bool got = false;
+    int s = 0;
+    if (rdy_min > 1) {                       // a helper warp fetches only from a READY queue that has piled up
+        int r = 0;
+        if (lane == 0) r = gd_q_count(B.ready);
+        if (__shfl_sync(0xFFFFFFFFu, r, 0) < rdy_min) return 0;
+    }
+    const int tk = gd_q_claim(B.ready, T.slot < 0, n_free, lane, s, got);
+    if (got) {
+        const unsigned st = __float_as_uint(GD_SF(14));
+        const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
+        gd_trav_begin(T, bvh, stack, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
+                      loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
+                      __float_as_int(GD_SF(19)), __float_as_int(GD_SF(20)), __float_as_int(GD_SF(21)), s);
+        n_query++;
+    }
+    return tk;
+}
+
+// ---- block set-up and tear-down shared by the two transport kernels
+#define GD_W_SHARED                                                                                              \
+    extern __shared__ __align__(16) unsigned char gd_smem[];                                                     \
+    __shared__ GdSource s_src;                                                                                   \
+    __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];                                           \
+    __shared__ unsigned s_cnt[12];                                                                               \
+    __shared__ GdQueue s_ready, s_result, s_slow;                                                                \
+    __shared__ GdHistPool s_hist;                                                                                \
+    __shared__ unsigned s_live;                                                                                  \
+    const int n_tab = M.n_mat * 4 * M.n_grid;                                                                    \
+    float *s_tab = (float *)gd_smem;                                                                             \
+    unsigned *s_spec = (unsigned *)(s_tab + n_tab);                                                              \
+    float *sl = (float *)(s_spec + tally.n_bins + 1);                                                            \
+    for (int i = threadIdx.x; i < n_tab; i += blockDim.x) s_tab[i] = M.table[i];                                 \
+    for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) s_spec[i] = 0;                                 \
+    for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i]; \
+    if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }                     \
+    if (threadIdx.x < 12) s_cnt[threadIdx.x] = 0;                                                                \
+    /* every slot starts in the general queue with mode NEED: the first passes start the first histories */     \
+    for (int s = threadIdx.x; s < GD_W_NSLOT; s += blockDim.x) {                                                 \
+        GD_SF(14) = __uint_as_float((unsigned)GD_MODE_NEED << 5);                                                \
+        s_slow.ent[s] = (unsigned short)(gd_q_tag((unsigned)s) | (unsigned)s);                                   \
+        s_ready.ent[s] = 0; s_result.ent[s] = 0;                                                                 \
+    }                                                                                                            \
+    if (threadIdx.x == 0) {                                                                                      \
+        s_slow.head = 0; s_slow.tail = GD_W_NSLOT; s_result.head = 0; s_result.tail = 0; s_ready.head = 0; s_ready.tail = 0; \
+        s_hist.state = 0ull; s_hist.lock = 0u; s_hist.dry = 0u;                                                  \
+        s_live = GD_W_NSLOT;                                                                                     \
+    }                                                                                                            \
+    __syncthreads();                                                                                             \
+    GdBlk B;                                                                                                     \
+    B.sl = sl; B.tab = s_tab; B.src = &s_src; B.spec = s_spec; B.emitted = s_emitted; B.peak = s_peak; B.cnt = s_cnt; \
+    B.ready = &s_ready; B.result = &s_result; B.slow = &s_slow; B.hist = &s_hist; B.live = &s_live;              \
+    B.pair = pair_buf + (size_t)blockIdx.x * GD_W_NSLOT * 8;                                                     \
+    GdRunArgs A;                                                                                                 \
+    A.first = first; A.n_hist = n_hist; A.seed = seed; A.edep_out = edep_out; A.flags_out = flags_out;          \
+    A.next_history = next_history; A.chunk = chunk;
+
+// per-lane 32-bit work counters straight to the 64-bit global totals
+GD_D void gd_flush_lane_counters(const GdTally &tally, unsigned lane, unsigned n_done, unsigned n_query, unsigned n_box,
+                                 unsigned n_tri, unsigned n_skip, unsigned n_fast_cross, unsigned n_fast_coh) {
+    const unsigned v[7] = {n_done, n_query, n_box, n_tri, n_skip, n_fast_cross, n_fast_coh};
+    const int where[7] = {0, 1, 2, 3, 13, 4, 7};     // GdCounters: n_histories, n_queries, n_box_tests, n_tri_tests, n_skipped, n_crossings, n_coherent
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        unsigned long long x = v[k];
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) x += __shfl_down_sync(0xFFFFFFFFu, x, o);
+        if (lane == 0 && x) atomicAdd(&((unsigned long long *)tally.counters)[where[k]], x);
+    }
+}
+GD_D void gd_flush_block_tallies(const GdTally &tally, const unsigned *s_spec, const unsigned *s_emitted, const unsigned *s_peak,
+                                 const unsigned *s_cnt) {
+    for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) {
+        unsigned v = s_spec[i];
+        if (v) atomicAdd(&tally.spectrum[i], (unsigned long long)v);
+    }
+    if (threadIdx.x < GD_MAX_LINES) {
+        if (s_emitted[threadIdx.x]) atomicAdd(&tally.emitted[threadIdx.x], (unsigned long long)s_emitted[threadIdx.x]);
+        if (s_peak[threadIdx.x]) atomicAdd(&tally.peak[threadIdx.x], (unsigned long long)s_peak[threadIdx.x]);
+    }
+    if (threadIdx.x >= 4 && threadIdx.x < 12 && s_cnt[threadIdx.x])
+        atomicAdd(&((unsigned long long *)tally.counters)[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
+}
+
 // dynamic shared memory: [table floats][spectrum u32 (n_bins+1)][slots: GD_W_NF x GD_W_NSLOT floats]
 // pair_buf: global, 8 floats per slot of every block of the grid
 // WIDTH: 4 = uncompressed 4-wide nodes (default), 8 = compressed 8-wide nodes
+// Every warp does whichever kind of work there is (the default kernel).
 template <int WIDTH>
 __global__ void __launch_bounds__(GD_W_THREADS, 1)
 gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
                     unsigned long long n_hist, unsigned long long seed, GdTally tally, float *__restrict__ edep_out,
                     unsigned *__restrict__ flags_out, unsigned long long *next_history, unsigned chunk,
                     float *__restrict__ pair_buf, GdWaveTune tune) {
-    extern __shared__ __align__(16) unsigned char gd_smem[];
-    __shared__ GdSource s_src;
-    __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];
-    __shared__ unsigned s_cnt[12];
-    __shared__ GdQueue s_ready, s_result, s_slow;
-    __shared__ GdHistPool s_hist;
-    __shared__ unsigned s_live;                     // slots that still carry or may get a history
-    const int n_tab = M.n_mat * 4 * M.n_grid;
-    float *s_tab = (float *)gd_smem;
-    unsigned *s_spec = (unsigned *)(s_tab + n_tab);
-    float *sl = (float *)(s_spec + tally.n_bins + 1);
-    for (int i = threadIdx.x; i < n_tab; i += blockDim.x) s_tab[i] = M.table[i];
-    for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) s_spec[i] = 0;
-    for (int i = threadIdx.x; i < (int)(sizeof(GdSource) / 4); i += blockDim.x) ((int *)&s_src)[i] = ((const int *)src)[i];
-    if (threadIdx.x < GD_MAX_LINES) { s_emitted[threadIdx.x] = 0; s_peak[threadIdx.x] = 0; }
-    if (threadIdx.x < 12) s_cnt[threadIdx.x] = 0;
-    // every slot starts in the general queue with mode NEED: the first passes start the first histories
-    for (int s = threadIdx.x; s < GD_W_NSLOT; s += blockDim.x) {
-        GD_SF(14) = __uint_as_float((unsigned)GD_MODE_NEED << 5);
-        s_slow.ent[s] = (unsigned short)(gd_q_tag((unsigned)s) | (unsigned)s);
-        s_ready.ent[s] = 0; s_result.ent[s] = 0;
-    }
-    if (threadIdx.x == 0) {
-        s_slow.head = 0; s_slow.tail = GD_W_NSLOT; s_result.head = 0; s_result.tail = 0; s_ready.head = 0; s_ready.tail = 0;
-        s_hist.state = 0ull; s_hist.lock = 0u; s_hist.dry = 0u;
-        s_live = GD_W_NSLOT;
-    }
-    __syncthreads();
-
+    GD_W_SHARED
     const unsigned lane = threadIdx.x & 31u;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    float *pair = pair_buf + (size_t)blockIdx.x * GD_W_NSLOT * 8;
     int stack[WIDTH == 8 ? GD_STACK8 : GD_STACK4];
     GdTrav T;
     gd_trav_idle(T);
-    unsigned n_box = 0, n_tri = 0, n_query = 0, n_done = 0, n_skip = 0, n_fast_cross = 0, n_fast_coh = 0;
+    unsigned n_box = 0, n_tri = 0, n_query = 0;
+    GdLaneCounters C = {0, 0, 0, 0};
     static_assert(GD_W_NSLOT == 1024, "queue entries hold a 10-bit slot number");
-    // warps of the last SM sub-partition take the general (slow) passes first, so that the other three keep the two
-    // compact loops in their instruction caches
+    // warps of the last SM sub-partition take the general passes first, so that the other three keep the two compact
+    // loops in their instruction caches
     const bool slow_first = ((threadIdx.x >> 5) & 3u) == 3u;
+    // every third warp takes READY slots whenever it has free lanes; the others only help when READY has piled up, so that
+    // a trickle of rays fills the lanes of a few warps instead of a quarter of the lanes of all
+    const bool t_pref = ((threadIdx.x >> 5) % 3u) == 0u;
+    const int rdy_min = t_pref ? 1 : tune.t_help;
     unsigned idle_ns = 250u;
+    unsigned long long *pacc = nullptr;
 #ifdef GD_PROF
-    unsigned long long pacc[16] = {};
+    unsigned long long pacc_[16] = {};
+    pacc = pacc_;
     long long p_t0 = clock64();
 #endif
-
     for (;;) {
         // ---- what next?  (queue lengths are snapshots: a wrong guess costs a pass with fewer lanes, never a result)
         const int my_rays = __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0));
@@ -309,7 +599,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
         n_rdy = __shfl_sync(0xFFFFFFFFu, n_rdy, 0);
         n_slow = __shfl_sync(0xFFFFFFFFu, n_slow, 0);
         live = __shfl_sync(0xFFFFFFFFu, live, 0);
-        const bool t_work = my_rays > 0 || n_rdy > 0;
+        const bool t_work = my_rays > 0 || n_rdy >= rdy_min;
         const bool few_rays = my_rays < tune.t_keep;      // a warp with many rays in flight finishes them first: their slots are what the others wait for
         const bool other_work = t_work || n_res > 0;
         const bool do_slow = n_slow > 0 && (n_slow >= (slow_first ? tune.p_min : 8 * tune.p_min) || !other_work) && (few_rays || !t_work);
@@ -324,87 +614,8 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
         }
         idle_ns = 250u;
         if (do_slow) {
-            // ============================================================ general pass: any event, one per slot
-            int s = 0;
-            bool has = false;
-            gd_q_claim(&s_slow, true, 32, lane, s, has);
-            GdLane L;
-            L.mode = GD_MODE_DONE;
-            GdHit hit;
-            hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
-            if (has) {
-                gd_slot_load(sl, s, L, seed, first);
-                if (L.pending) {
-                    const float *p = pair + s * 8;
-                    L.p_pos = gd_make(p[0], p[1], p[2]); L.p_axis = gd_make(p[3], p[4], p[5]); L.p_m = __float_as_int(p[6]);
-                }
-                // gd_lane_post reads the from-side id as "inside if leaving else outside" in LOCATE mode and the
-                // to-side id as "outside if leaving else inside" in FLIGHT mode: present (from, to) that way
-                hit.t = GD_SF(22);
-                hit.orig = __float_as_int(GD_SF(23));
-                hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
-                hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
-            }
-            GD_PROF_ADD(7, 1); GD_PROF_ADD(8, __popc(__ballot_sync(0xFFFFFFFFu, has)));
-            GdLocalCounters cnt = {};
-            GdHistory r;
-            r.edep = 0.0f; r.flags = 0u; r.line = 0;
-            bool fin = false;
-            if (has && L.mode != GD_MODE_NEED) {
-                const int was_pending = L.pending;
-                fin = gd_lane_post(L, M, s_tab, s_src, seed, hit, r, cnt);
-                if (fin) {
-                    n_done++;
-                    const unsigned long long hrel = L.history - first;
-                    if (edep_out) edep_out[hrel] = r.edep;
-                    if (flags_out) flags_out[hrel] = r.flags;
-                } else if (L.pending && !was_pending) {  // a pair event: park the two annihilation photons
-                    float *p = pair + s * 8;
-                    p[0] = L.p_pos.x; p[1] = L.p_pos.y; p[2] = L.p_pos.z;
-                    p[3] = L.p_axis.x; p[4] = L.p_axis.y; p[5] = L.p_axis.z; p[6] = __int_as_float(L.p_m);
-                }
-            }
-            gd_tally_warp(fin, r, s_src, tally, s_spec, s_emitted, s_peak, lane);
-            {   // event counters, one shared-memory atomic per kind and pass (crossing / PE / Compton / coherent /
-                // pair; escapes, re-localisations and cut-offs can accompany any of them)
-                const unsigned v[8] = {cnt.n_crossings, cnt.n_pe, cnt.n_compton, cnt.n_coherent, cnt.n_pair, cnt.n_escaped,
-                                       cnt.n_leak, cnt.n_cutoff};
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    const unsigned mk = __ballot_sync(0xFFFFFFFFu, v[k] != 0u);
-                    if (mk && lane == 0) atomicAdd(&s_cnt[4 + k], (unsigned)__popc(mk));
-                }
-            }
-            // ---- finished slots take the next histories of the block's chunk
-            const unsigned need_mask = __ballot_sync(0xFFFFFFFFu, has && L.mode == GD_MODE_NEED);
-            if (need_mask) {
-                unsigned a0, n0, a1;
-                gd_hist_take(&s_hist, (unsigned)__popc(need_mask), next_history, n_hist, chunk, gridDim.x, lane, a0, n0, a1);
-                bool died = false;
-                if (has && L.mode == GD_MODE_NEED) {
-                    const unsigned rk = __popc(need_mask & lt_mask);
-                    const unsigned long long h = rk < n0 ? a0 + rk : (unsigned long long)a1 + (rk - n0);
-                    if (h < n_hist) gd_lane_start(L, s_src, seed, first + h);
-                    else { L.mode = GD_MODE_DONE; died = true; }
-                }
-                const unsigned died_mask = __ballot_sync(0xFFFFFFFFu, died);
-                if (died_mask && lane == 0) atomicSub(&s_live, (unsigned)__popc(died_mask));
-            }
-            // ---- the next query: answered by the clearance grid (the slot then waits in RESULT with its answer), or
-            // handed to READY
-            const bool live_lane = has && L.mode != GD_MODE_DONE;
-            bool skip = false;
-            if (live_lane) {
-                float t_min, t_max;
-                int filter;
-                gd_lane_query(L, M, s_tab, t_min, t_max, filter);
-                if (L.mode == GD_MODE_FLIGHT && L.sdist < GD_INF)
-                    skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
-                gd_slot_store(sl, s, L, first);
-                if (skip) { n_skip++; GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
-            }
-            gd_q_push(&s_ready, live_lane && !skip, s, lane);
-            gd_q_push(&s_result, live_lane && skip, s, lane);
+            GD_PROF_ADD(7, 1);
+            gd_general_pass(B, bvh, M, tally, A, lane, C);
 #ifdef GD_PROF
             { const long long t1 = clock64(); GD_PROF_ADD(9, t1 - p_t0); p_t0 = t1; }
 #endif
@@ -412,77 +623,7 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
         }
         if (do_fast) {
             GD_PROF_ADD(12, 1);
-            // ============================================================ chain burst: crossings and coherent events
-            // Lanes take RESULT slots (flights that met a facet or ended in an interaction) and handle the two event
-            // kinds of a scattering chain; anything else goes to the general queue untouched.  A slot whose next flight
-            // ends before the clearance of its grid cell stays on its lane and goes round again: the answer of that
-            // query is known ("none").  Lanes that gave their slot away take the next waiting result.
-            bool has = false, dirty = false;        // dirty: the lane's registers are newer than its slot
-            int s = 0;
-            GdLane L;
-            L.mode = GD_MODE_DONE;
-            GdHit hit;
-            hit.t = 0.0f; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.leaving = 1; hit.mats = 0;
-            for (bool first_pass = true;; first_pass = false) {
-                // ---- a pass needs p_min lanes with work -- or a warp with no ray to go back to and none to fetch.
-                // Decided on a snapshot of the queue before anything is claimed: what is parked below are lanes whose
-                // answer is known (no facet within the flight), never a freshly claimed traversal result.
-                const unsigned free_mask = __ballot_sync(0xFFFFFFFFu, !has);
-                const int n_has = 32 - __popc(free_mask);
-                int avail = 0, rdy = 0;
-                if (lane == 0) { avail = gd_q_count(&s_result); rdy = gd_q_count(&s_ready); }
-                avail = __shfl_sync(0xFFFFFFFFu, avail, 0);
-                rdy = __shfl_sync(0xFFFFFFFFu, rdy, 0);
-                const int expect = n_has + (avail < 32 - n_has ? avail : 32 - n_has);
-                const bool go = expect > 0 && (first_pass || expect >= tune.p_min || (my_rays == 0 && rdy == 0));
-                if (!go) {
-                    if (has) {
-                        gd_slot_store(sl, s, L, first);
-                        GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
-                    }
-                    gd_q_push(&s_result, has, s, lane);
-                    break;
-                }
-                // ---- fetch: lanes without a slot take waiting results
-                bool got = false;
-                int s_new = 0;
-                const int take = gd_q_claim(&s_result, !has, 32 - n_has, lane, s_new, got);
-                if (got) {
-                    s = s_new;
-                    gd_slot_load(sl, s, L, seed, first);
-                    hit.t = GD_SF(22);
-                    hit.orig = __float_as_int(GD_SF(23));
-                    hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
-                    hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
-                    has = true; dirty = false;
-                }
-                if (n_has + take == 0) break;        // another warp was quicker
-                GD_PROF_ADD(2, 1); GD_PROF_ADD(3, n_has + take);
-                // ---- one event per lane
-                int kind = 0;
-                if (has) kind = gd_lane_fast_event(L, M, hit);
-                const bool to_slow = has && kind == 0;
-                if (to_slow && dirty) {              // registers newer than the slot: write them back with the known answer
-                    gd_slot_store(sl, s, L, first);
-                    GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
-                }
-                gd_q_push(&s_slow, to_slow, s, lane);
-                if (to_slow) has = false;
-                n_fast_cross += kind == 1; n_fast_coh += kind == 2;
-                // ---- the next query: answered by the clearance grid, or handed to READY
-                bool skip = false;
-                if (has) {
-                    float t_min, t_max;
-                    int filter;
-                    gd_lane_query(L, M, s_tab, t_min, t_max, filter);
-                    if (L.sdist < GD_INF) skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
-                }
-                const bool to_ready = has && !skip;
-                if (to_ready) gd_slot_store(sl, s, L, first);
-                gd_q_push(&s_ready, to_ready, s, lane);
-                has = skip;
-                if (skip) { n_skip++; dirty = true; hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.mats = 0; }
-            }
+            gd_chain_burst<true>(B, bvh, M, A, tune, my_rays, lane, C, pacc);
 #ifdef GD_PROF
             { const long long t1 = clock64(); GD_PROF_ADD(0, t1 - p_t0); p_t0 = t1; }
 #endif
@@ -491,35 +632,14 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
         GD_PROF_ADD(13, 1);
         // ================================================================ T-burst
         // Finished rays are retired and READY slots fetched in one go, once `k_fetch` lanes are free (finished or
-        // idle): the queue operations are paid every few rounds instead of every round.
+        // idle): the queue operations are paid every few rounds instead of every round.  Unfinished rays stay in their
+        // lanes' registers while the warp does physics.
         for (;;) {
             const bool done_l = T.slot >= 0 && T.node == GD_TRAV_DONE;
-            const unsigned free_mask = __ballot_sync(0xFFFFFFFFu, T.slot < 0 || done_l);
-            const int n_free = __popc(free_mask);
+            const int n_free = __popc(__ballot_sync(0xFFFFFFFFu, T.slot < 0 || done_l));
             if (n_free >= tune.k_fetch || n_free == 32) {
-                // a start localisation, an escape (no facet, no interaction) and a crossing into KILL are general events;
-                // a crossing into another medium or an interaction goes to the chain burst
-                bool slow = false;
-                if (done_l) {
-                    const int s = T.slot;
-                    GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
-                    slow = T.filter == -2 || (T.orig == GD_NO_FACET ? !(T.t < GD_INF) : (T.fromto >> 16) == GD_MAT_KILL);
-                }
-                gd_q_push(&s_result, done_l && !slow, T.slot, lane);
-                gd_q_push(&s_slow, done_l && slow, T.slot, lane);
-                if (done_l) T.slot = -1;
-                bool got = false;
-                int s = 0;
-                const int tk = gd_q_claim(&s_ready, T.slot < 0, n_free, lane, s, got);
-                if (got) {
-                    const unsigned st = __float_as_uint(GD_SF(14));
-                    const bool loc = (int)((st >> 5) & 3u) == GD_MODE_LOCATE;
-                    gd_trav_begin(T, bvh, stack, GD_SF(0), GD_SF(1), GD_SF(2), GD_SF(3), GD_SF(4), GD_SF(5),
-                                  loc ? 0.0f : -GD_TBACK, loc ? GD_INF : GD_SF(13), loc ? -2 : (int)(st & 31u) - 1,
-                                  __float_as_int(GD_SF(19)), __float_as_int(GD_SF(20)), __float_as_int(GD_SF(21)), s);
-                    n_query++;
-                }
-                // nothing to fetch and few rays left: see whether physics has piled up (the rays stay in registers)
+                const int tk = gd_trav_service(T, B, bvh, stack, n_free, rdy_min, lane, n_query);
+                // nothing to fetch and few rays left: see whether physics has piled up
                 if (tk == 0 && 32 - n_free < tune.t_keep) {
                     if (n_free == 32) break;
                     int r = 0;
@@ -538,29 +658,79 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 #ifdef GD_PROF
     if (lane == 0) for (int k = 0; k < 16; ++k) if (pacc[k]) atomicAdd(&gd_prof[k], pacc[k]);
 #endif
-    // ---- flush: per-lane 32-bit work counters straight to the 64-bit global totals
-    {
-        const unsigned v[7] = {n_done, n_query, n_box, n_tri, n_skip, n_fast_cross, n_fast_coh};
-        const int where[7] = {0, 1, 2, 3, 13, 4, 7};     // GdCounters: n_histories, n_queries, n_box_tests, n_tri_tests, n_skipped, n_crossings, n_coherent
-#pragma unroll
-        for (int k = 0; k < 7; ++k) {
-            unsigned long long x = v[k];
-#pragma unroll
-            for (int o = 16; o >= 1; o >>= 1) x += __shfl_down_sync(0xFFFFFFFFu, x, o);
-            if (lane == 0 && x) atomicAdd(&((unsigned long long *)tally.counters)[where[k]], x);
+    gd_flush_lane_counters(tally, lane, C.n_done, n_query, n_box, n_tri, C.n_skip, C.n_fast_cross, C.n_fast_coh);
+    __syncthreads();
+    gd_flush_block_tallies(tally, s_spec, s_emitted, s_peak, s_cnt);
+}
+
+// Warp-specialised variant (GADEP_RUN_WARP_SPECIALISED): GD_WS_TWARPS lean traversal warps that only run the BVH loop
+// and GD_WS_PWARPS physics warps that only run the chain bursts and general passes, on the same block-wide queues.
+// setmaxnreg moves registers from the former to the latter.  Same results, bit for bit.
+#define GD_WS_TWARPS 16
+#define GD_WS_PWARPS 8
+#define GD_WS_THREADS (32 * (GD_WS_TWARPS + GD_WS_PWARPS))
+#define GD_WS_REGS_T 56
+#define GD_WS_REGS_P 128
+// what the traversal warps give up must cover what the physics warps take, or the physics warps wait for ever
+static_assert((65536 / GD_WS_THREADS / 8 * 8 - GD_WS_REGS_T) * GD_WS_TWARPS >= (GD_WS_REGS_P - 65536 / GD_WS_THREADS / 8 * 8) * GD_WS_PWARPS,
+              "register budget of the warp-specialised kernel does not balance");
+static_assert(GD_WS_TWARPS % 4 == 0 && GD_WS_PWARPS % 4 == 0, "setmaxnreg works on warpgroups");
+template <int WIDTH>
+__global__ void __launch_bounds__(GD_WS_THREADS, 1)
+gd_k_transport_ws(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
+                  unsigned long long n_hist, unsigned long long seed, GdTally tally, float *__restrict__ edep_out,
+                  unsigned *__restrict__ flags_out, unsigned long long *next_history, unsigned chunk,
+                  float *__restrict__ pair_buf, GdWaveTune tune) {
+    GD_W_SHARED
+    const unsigned lane = threadIdx.x & 31u;
+    const int warp = threadIdx.x >> 5;
+    unsigned idle_ns = 250u;
+    if (warp < GD_WS_TWARPS) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(GD_WS_REGS_T));
+        int stack[WIDTH == 8 ? GD_STACK8 : GD_STACK4];
+        GdTrav T;
+        gd_trav_idle(T);
+        unsigned n_box = 0, n_tri = 0, n_query = 0;
+        for (;;) {
+            const bool done_l = T.slot >= 0 && T.node == GD_TRAV_DONE;
+            const int n_free = __popc(__ballot_sync(0xFFFFFFFFu, T.slot < 0 || done_l));
+            if (n_free >= tune.k_fetch || n_free == 32) {
+                const int tk = gd_trav_service(T, B, bvh, stack, n_free, 1, lane, n_query);
+                if (tk == 0 && n_free == 32) {               // no ray in flight, none to fetch
+                    unsigned live = 0;
+                    if (lane == 0) live = *(volatile unsigned *)&s_live;
+                    if (__shfl_sync(0xFFFFFFFFu, live, 0) == 0u) break;
+                    __nanosleep(idle_ns);
+                    if (idle_ns < 2000u) idle_ns *= 2u;
+                    continue;
+                }
+                idle_ns = 250u;
+            }
+            gd_trav_step<WIDTH>(T, bvh, stack, tune.n_steps, n_box, n_tri);
         }
+        gd_flush_lane_counters(tally, lane, 0, n_query, n_box, n_tri, 0, 0, 0);
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(GD_WS_REGS_P));
+        GdLaneCounters C = {0, 0, 0, 0};
+        const bool slow_first = (warp & 3) == 3;
+        for (;;) {
+            int n_res = 0, n_slow = 0;
+            unsigned live = 0;
+            if (lane == 0) { n_res = gd_q_count(&s_result); n_slow = gd_q_count(&s_slow); live = *(volatile unsigned *)&s_live; }
+            n_res = __shfl_sync(0xFFFFFFFFu, n_res, 0);
+            n_slow = __shfl_sync(0xFFFFFFFFu, n_slow, 0);
+            live = __shfl_sync(0xFFFFFFFFu, live, 0);
+            const bool do_slow = n_slow > 0 && (n_slow >= (slow_first ? tune.p_min : 8 * tune.p_min) || n_res < tune.p_min);
+            if (do_slow) { gd_general_pass(B, bvh, M, tally, A, lane, C); idle_ns = 250u; continue; }
+            if (n_res > 0) { gd_chain_burst<false>(B, bvh, M, A, tune, 0, lane, C, nullptr); idle_ns = 250u; continue; }
+            if (live == 0u) break;
+            __nanosleep(idle_ns);
+            if (idle_ns < 2000u) idle_ns *= 2u;
+        }
+        gd_flush_lane_counters(tally, lane, C.n_done, 0, 0, 0, C.n_skip, C.n_fast_cross, C.n_fast_coh);
     }
     __syncthreads();
-    for (int i = threadIdx.x; i <= tally.n_bins; i += blockDim.x) {
-        unsigned v = s_spec[i];
-        if (v) atomicAdd(&tally.spectrum[i], (unsigned long long)v);
-    }
-    if (threadIdx.x < GD_MAX_LINES) {
-        if (s_emitted[threadIdx.x]) atomicAdd(&tally.emitted[threadIdx.x], (unsigned long long)s_emitted[threadIdx.x]);
-        if (s_peak[threadIdx.x]) atomicAdd(&tally.peak[threadIdx.x], (unsigned long long)s_peak[threadIdx.x]);
-    }
-    if (threadIdx.x >= 4 && threadIdx.x < 12 && s_cnt[threadIdx.x])
-        atomicAdd(&((unsigned long long *)tally.counters)[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
+    gd_flush_block_tallies(tally, s_spec, s_emitted, s_peak, s_cnt);
 }
 
 // ---------------------------------------------------------------- ray-cast hook with dynamic fetch
