@@ -42,7 +42,8 @@ __device__ unsigned long long gd_prof[16];
 struct GdWaveTune {
     int k_fetch;        // idle lanes needed before READY slots are fetched
     int t_keep;         // a warp stays in its T-burst while at least this many of its lanes hold a ray (or READY has more)
-    int n_steps;        // node visits per traversal round
+    int n_steps;        // node visits per traversal round (lower bound of the adaptive length)
+    int n_steps_max;    // ... and its upper bound; equal to n_steps = fixed length
     int p_min;          // a physics pass runs while this many lanes have work (or the warp has nothing else to do)
     int t_help;         // READY slots that must wait before the warps that do not prefer traversal fetch any
 };
@@ -580,6 +581,8 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
     const bool t_pref = ((threadIdx.x >> 5) % 3u) == 0u;
     const int rdy_min = t_pref ? 1 : tune.t_help;
     unsigned idle_ns = 250u;
+    int n_steps = tune.n_steps;
+    unsigned round_no = 0, box_mark = 0, tri_mark = 0;
     unsigned long long *pacc = nullptr;
 #ifdef GD_PROF
     unsigned long long pacc_[16] = {};
@@ -638,7 +641,13 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
             const bool done_l = T.slot >= 0 && T.node == GD_TRAV_DONE;
             const int n_free = __popc(__ballot_sync(0xFFFFFFFFu, T.slot < 0 || done_l));
             if (n_free >= tune.k_fetch || n_free == 32) {
+#ifdef GD_PROF
+                const long long ts0 = clock64();
+#endif
                 const int tk = gd_trav_service(T, B, bvh, stack, n_free, rdy_min, lane, n_query);
+#ifdef GD_PROF
+                GD_PROF_ADD(14, clock64() - ts0); GD_PROF_ADD(15, 1);
+#endif
                 // nothing to fetch and few rays left: see whether physics has piled up
                 if (tk == 0 && 32 - n_free < tune.t_keep) {
                     if (n_free == 32) break;
@@ -649,7 +658,15 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
             }
             GD_PROF_ADD(4, 1); GD_PROF_ADD(5, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0 && T.node >= 0)));
             GD_PROF_ADD(6, __popc(__ballot_sync(0xFFFFFFFFu, T.slot >= 0 && T.node != GD_TRAV_DONE)));
-            gd_trav_step<WIDTH>(T, bvh, stack, tune.n_steps, n_box, n_tri);
+            gd_trav_step<WIDTH>(T, bvh, stack, n_steps, n_box, n_tri);
+            // node visits per round follow the warp's own ratio of node visits to triangle tests (deep walks between
+            // leaves: long rounds; a leaf every other visit: short rounds), re-evaluated every 32 rounds
+            if ((++round_no & 31u) == 0u && tune.n_steps_max > tune.n_steps) {
+                const unsigned dv = __reduce_add_sync(0xFFFFFFFFu, n_box - box_mark), dt = __reduce_add_sync(0xFFFFFFFFu, n_tri - tri_mark);
+                box_mark = n_box; tri_mark = n_tri;
+                const int want = (int)((dv / (WIDTH == 8 ? 6u : 4u) + dt / 2u) / (dt > 0u ? dt : 1u));
+                n_steps = want < tune.n_steps ? tune.n_steps : (want > tune.n_steps_max ? tune.n_steps_max : want);
+            }
         }
 #ifdef GD_PROF
         { const long long t1 = clock64(); GD_PROF_ADD(1, t1 - p_t0); p_t0 = t1; }
