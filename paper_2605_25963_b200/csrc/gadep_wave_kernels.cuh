@@ -404,52 +404,49 @@ GD_PASS void gd_chain_burst(const GdBlk &B, const GdBvh &bvh, const GdMaterials 
         const int expect = n_has + (avail < 32 - n_has ? avail : 32 - n_has);
         const bool nothing_else = CAN_TRAVERSE ? (my_rays == 0 && other == 0) : other < tune.p_min;
         const bool go = expect > 0 && (first_pass || expect >= tune.p_min || nothing_else);
-        if (!go) {
-            if (has) {
-                gd_slot_store(sl, s, L, A.first);
-                GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
+        bool to_slow = false, to_ready = false, skip = false;
+        if (go) {
+            // ---- fetch: lanes without a slot take waiting results
+            bool got = false;
+            int s_new = 0;
+            const int take = gd_q_claim(B.result, !has, 32 - n_has, lane, s_new, got);
+            if (got) {
+                s = s_new;
+                gd_slot_load(sl, s, L, A.seed, A.first);
+                hit.t = GD_SF(22);
+                hit.orig = __float_as_int(GD_SF(23));
+                hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
+                hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
+                has = true; dirty = false;
             }
-            gd_q_push(B.result, has, s, lane);
-            break;
-        }
-        // ---- fetch: lanes without a slot take waiting results
-        bool got = false;
-        int s_new = 0;
-        const int take = gd_q_claim(B.result, !has, 32 - n_has, lane, s_new, got);
-        if (got) {
-            s = s_new;
-            gd_slot_load(sl, s, L, A.seed, A.first);
-            hit.t = GD_SF(22);
-            hit.orig = __float_as_int(GD_SF(23));
-            hit.leaf = hit.orig == GD_NO_FACET ? -1 : 0;
-            hit.mats = __float_as_int(GD_SF(24));          // inside := from, outside := to
-            has = true; dirty = false;
-        }
-        if (n_has + take == 0) break;        // another warp was quicker
+            if (n_has + take == 0) break;        // another warp was quicker
 #ifdef GD_PROF
-        pacc[2] += 1; pacc[3] += n_has + take;
+            pacc[2] += 1; pacc[3] += n_has + take;
 #endif
-        // ---- one event per lane
-        int kind = 0;
-        if (has) kind = gd_lane_fast_event(L, M, hit);
-        const bool to_slow = has && kind == 0;
-        if (to_slow && dirty) {              // registers newer than the slot: write them back with the known answer
+            // ---- one event per lane
+            int kind = 0;
+            if (has) kind = gd_lane_fast_event(L, M, hit);
+            to_slow = has && kind == 0;
+            C.n_fast_cross += kind == 1; C.n_fast_coh += kind == 2;
+            // ---- the next query: answered by the clearance grid, or handed to READY
+            if (has && !to_slow) {
+                float t_min, t_max;
+                int filter;
+                gd_lane_query(L, M, B.tab, t_min, t_max, filter);
+                if (L.sdist < GD_INF) skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
+                to_ready = !skip;
+            }
+        }
+        // ---- one place where registers go back to the slot: a lane that hands its slot to READY, a lane that is parked
+        // (!go) or whose next event is a general one while its registers are newer than the slot (both with the known
+        // answer "no facet within the flight")
+        const bool known = (!go && has) || (to_slow && dirty);
+        if (to_ready || known) {
             gd_slot_store(sl, s, L, A.first);
-            GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f;
+            if (known) { GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
         }
+        if (!go) { gd_q_push(B.result, has, s, lane); break; }
         gd_q_push(B.slow, to_slow, s, lane);
-        if (to_slow) has = false;
-        C.n_fast_cross += kind == 1; C.n_fast_coh += kind == 2;
-        // ---- the next query: answered by the clearance grid, or handed to READY
-        bool skip = false;
-        if (has) {
-            float t_min, t_max;
-            int filter;
-            gd_lane_query(L, M, B.tab, t_min, t_max, filter);
-            if (L.sdist < GD_INF) skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
-        }
-        const bool to_ready = has && !skip;
-        if (to_ready) gd_slot_store(sl, s, L, A.first);
         gd_q_push(B.ready, to_ready, s, lane);
         has = skip;
         if (skip) { C.n_skip++; dirty = true; hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.mats = 0; }
