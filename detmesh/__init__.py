@@ -9,12 +9,12 @@ from .geometry import (Line, Arc, discretise, revolve, Mesh, merge_surfaces,
                        mesh_signed_volume, mesh_area, check_closed_oriented)
 from .materials import (ELEMENTS, MATERIALS, MAT, DENSITY_G_CM3, energy_grid, sigma_kn_total,
                         make_tables, N_GRID, E_MIN_MEV, E_MAX_MEV)
-from .configs import make_config, make_calibration, make_pellet_stack, Workload, philox_u01_host, TABLE3_KEV, CALIBRATION_DETECTORS
+from .configs import make_config, make_calibration, make_calibration_batch, make_pellet_stack, Workload, philox_u01_host, TABLE3_KEV, CALIBRATION_DETECTORS
 
 __all__ = [
     "Line", "Arc", "discretise", "revolve", "Mesh", "merge_surfaces",
     "mesh_signed_volume", "mesh_area", "check_closed_oriented",
     "ELEMENTS", "MATERIALS", "MAT", "DENSITY_G_CM3", "energy_grid", "sigma_kn_total", "make_tables",
-    "N_GRID", "E_MIN_MEV", "E_MAX_MEV", "make_config", "make_calibration", "make_pellet_stack", "Workload", "philox_u01_host",
+    "N_GRID", "E_MIN_MEV", "E_MAX_MEV", "make_config", "make_calibration", "make_calibration_batch", "make_pellet_stack", "Workload", "philox_u01_host",
     "TABLE3_KEV", "CALIBRATION_DETECTORS",
 ]

@@ -257,3 +257,30 @@ def make_calibration(detector: int, n_histories: int = 10_000_000, n_theta: int 
     src = _source(SRC_POINT, pos=(0, 0, p["gap"] + 1.0 + 250.0), lines_kev=TABLE3_KEV)
     return Workload(p["name"] + "_point250_13lines", mesh, mu, sc, E_MIN_MEV, E_MAX_MEV, src, n_histories, 1,
                     notes={"detector": dict(p)})
+
+
+def make_calibration_batch(detectors=(0, 1, 2), n_histories: int = 30_000_000, n_theta: int = 256, pitch_mm: float = 768.0) -> Workload:
+    """Several detector parameter sets in ONE scene and one launch (the paper's calibration
+    use-case: six detectors x 13 energies).  Detector k of `detectors` is the CALIBRATION_DETECTORS
+    geometry translated by k * pitch_mm along x inside its own world cylinder (air inside, KILL outside; the cylinders
+    are disjoint), the point source 250 mm above each endcap is one source replicated at the matching translations
+    (`notes["source_copies"]`): history h belongs to detector h mod K, and its line is counted under k * 13 + l, so one
+    run returns K FEPE curves.  Materials and tables are shared."""
+    surfs, offs = [], []
+    z0 = None
+    for k, d in enumerate(detectors):
+        p = CALIBRATION_DETECTORS[d]
+        zs = p["gap"] + 1.0 + 250.0
+        if z0 is None:
+            z0 = zs
+        shift = np.array([k * pitch_mm, 0.0, 0.0])
+        for (name, segs, mi, mo) in _param_detector_segment_lists(p, 8, 4):
+            v, t = revolve(discretise(segs), n_theta)
+            surfs.append((f"{p['name']}_{name}", v + shift, t, mi, mo))
+        offs.append([k * pitch_mm, 0.0, zs - z0])
+    mesh = merge_surfaces(surfs, MAT["air"])
+    mu, sc, _ = make_tables(coh_coeff=7.0e-27)
+    src = _source(SRC_POINT, pos=(0, 0, z0), lines_kev=TABLE3_KEV)
+    return Workload("calibration_batch_" + "_".join(CALIBRATION_DETECTORS[d]["name"] for d in detectors), mesh, mu, sc,
+                    E_MIN_MEV, E_MAX_MEV, src, n_histories, 1,
+                    notes={"source_copies": np.asarray(offs, dtype=np.float32), "detectors": [dict(CALIBRATION_DETECTORS[d]) for d in detectors]})

@@ -110,6 +110,17 @@ typedef struct {
 } gadep_source;
 int gadep_set_source(gadep_ctx *ctx, const gadep_source *src);
 
+/*
+ * Batched geometries (the paper's calibration use-case: several detectors x 13
+ * energies): the source set by gadep_set_source is replicated at n_copies translations, offsets HOST float[n_copies][3]
+ * -- one per detector of a scene that holds the detectors side by side, each in its own closed world surface.  History
+ * h is emitted from copy h mod n_copies; its line is counted under copy * n_lines + l in emitted[] / peak[] /
+ * gadep_fepe / the per-history flags, so one gadep_run returns one FEPE curve per detector (the spectrum is their sum).
+ * n_copies in 1..8 with n_copies * n_lines <= GADEP_MAX_LINES; n_copies = 1 restores the plain source (offsets may be
+ * NULL).  gadep_set_source resets it.
+ */
+int gadep_set_source_copies(gadep_ctx *ctx, int n_copies, const float *offsets);
+
 #define GADEP_RUN_ASYNC 1          /* do not synchronise the stream; spectrum must then be a DEVICE pointer     */
 #define GADEP_RUN_ACCUMULATE 2     /* add to the context's tallies instead of starting from zero                */
 #define GADEP_RUN_HISTORY_PER_THREAD 4  /* measurement: the plain one-history-per-thread kernel instead of the   */

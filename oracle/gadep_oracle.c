@@ -60,6 +60,10 @@ typedef struct {
     double src_pos[3], src_dir[3], cyl_r, cyl_z0, cyl_z1, ex_r, ex_z0, ex_z1;
     int n_lines;
     double *line_mev, *line_int, line_int_sum;
+    /* NEXT-3: the source replicated at n_copies translations, one per detector of a
+     * batched scene; history h is emitted from copy h mod n_copies and counted under line copy * n_lines + l */
+    int n_copies;
+    double copy_off[8][3];
     /* NEXT-4 ("coupled photon-electron"): straight CSDA electron segments, see deposit() */
     int electron_mode;
     double rho[16];          /* g/cm^3 per material */
@@ -196,6 +200,7 @@ int orc_set_source(orc_scene *s, int kind, const double *pos, const double *dir,
                    const float *line_intensity) {
     if (!s || n_lines <= 0 || kind < 0 || kind > 2) return -1;
     s->src_kind = kind;
+    if (s->n_copies < 1) s->n_copies = 1;
     memcpy(s->src_pos, pos, sizeof(double) * 3);
     memcpy(s->src_dir, dir, sizeof(double) * 3);
     s->cyl_r = cyl_r; s->cyl_z0 = cyl_z0; s->cyl_z1 = cyl_z1;
@@ -565,7 +570,18 @@ static void transport_photon(const orc_scene *s, orc_photon ph, uint64_t seed, u
     }
 }
 
-/* O4: line by cumulative intensity (draw 0, always consumed), emission point, direction.  Returns the line. */
+/* Batched scenes: n_copies translations of the source (NULL / 1 = the plain source).  n_copies * n_lines <= 64. */
+int orc_set_source_copies(orc_scene *s, int n_copies, const double *offsets) {
+    if (!s || n_copies < 1 || n_copies > 8 || (n_copies > 1 && !offsets)) return -1;
+    s->n_copies = n_copies;
+    memset(s->copy_off, 0, sizeof(s->copy_off));
+    for (int c = 0; c < n_copies && offsets; ++c)
+        for (int a = 0; a < 3; ++a) s->copy_off[c][a] = offsets[3 * c + a];
+    return 0;
+}
+
+/* O4: line by cumulative intensity (draw 0, always consumed), emission point, direction.  Returns the line
+ * (copy * n_lines + l for a replicated source). */
 static int sample_source(const orc_scene *s, orc_rng *g, orc_photon *ph) {
     double ul = rng_next(g) * s->line_int_sum;
     int line = s->n_lines - 1; double acc = 0.0;
@@ -585,6 +601,11 @@ static int sample_source(const orc_scene *s, orc_rng *g, orc_photon *ph) {
     }
     if (s->src_kind == 2) memcpy(ph->dir, s->src_dir, sizeof(ph->dir));
     else sample_isotropic(g, ph->dir);
+    if (s->n_copies > 1) {
+        const int copy = (int)(g->history % (uint64_t)s->n_copies);
+        for (int a = 0; a < 3; ++a) ph->pos[a] += s->copy_off[copy][a];
+        line += copy * s->n_lines;
+    }
     return line;
 }
 
@@ -659,7 +680,7 @@ int orc_run_histories(const orc_scene *s, uint64_t first, long long n, uint64_t 
         for (long long i = 0; i < n; ++i) {
             orc_hist h;
             int line = run_history(s, seed, first + (uint64_t)i, &h, &local);
-            double e = (h.flags & ORC_F_PEAK) ? s->line_mev[line] : h.dep_scoring;
+            double e = (h.flags & ORC_F_PEAK) ? s->line_mev[line % s->n_lines] : h.dep_scoring;
             if (edep_out) edep_out[i] = e;
             if (flags_out) flags_out[i] = h.flags;
             if (dep_other_out) dep_other_out[i] = h.dep_other;
@@ -677,15 +698,16 @@ int orc_run(const orc_scene *s, uint64_t first, long long n, uint64_t seed, int 
             uint64_t *spectrum, uint64_t *emitted, uint64_t *peak, orc_counters *cnt_out) {
     if (!s || !s->mu || !s->v0 || !s->line_mev || n_bins <= 0) return -1;
     memset(spectrum, 0, sizeof(uint64_t) * (n_bins + 1));
-    memset(emitted, 0, sizeof(uint64_t) * s->n_lines);
-    memset(peak, 0, sizeof(uint64_t) * s->n_lines);
+    const int n_ctr = s->n_lines * (s->n_copies > 1 ? s->n_copies : 1);
+    memset(emitted, 0, sizeof(uint64_t) * n_ctr);
+    memset(peak, 0, sizeof(uint64_t) * n_ctr);
     double de = e_max_mev / (double)n_bins;
     orc_counters total; memset(&total, 0, sizeof(total));
 #pragma omp parallel
     {
         uint64_t *sp = (uint64_t *)calloc(n_bins + 1, sizeof(uint64_t));
-        uint64_t *em = (uint64_t *)calloc(s->n_lines, sizeof(uint64_t));
-        uint64_t *pk = (uint64_t *)calloc(s->n_lines, sizeof(uint64_t));
+        uint64_t *em = (uint64_t *)calloc(n_ctr, sizeof(uint64_t));
+        uint64_t *pk = (uint64_t *)calloc(n_ctr, sizeof(uint64_t));
         orc_counters local; memset(&local, 0, sizeof(local));
 #pragma omp for schedule(dynamic, 256)
         for (long long i = 0; i < n; ++i) {
@@ -693,7 +715,7 @@ int orc_run(const orc_scene *s, uint64_t first, long long n, uint64_t seed, int 
             int line = run_history(s, seed, first + (uint64_t)i, &h, &local);
             em[line]++;
             double e = h.dep_scoring;
-            if (h.flags & ORC_F_PEAK) { pk[line]++; e = s->line_mev[line]; }
+            if (h.flags & ORC_F_PEAK) { pk[line]++; e = s->line_mev[line % s->n_lines]; }
             if (e > 0.0) {
                 double b = floor(e / de);
                 int bin = b >= (double)n_bins ? n_bins : (int)b;
@@ -703,7 +725,7 @@ int orc_run(const orc_scene *s, uint64_t first, long long n, uint64_t seed, int 
 #pragma omp critical
         {
             for (int b = 0; b <= n_bins; ++b) spectrum[b] += sp[b];
-            for (int l = 0; l < s->n_lines; ++l) { emitted[l] += em[l]; peak[l] += pk[l]; }
+            for (int l = 0; l < n_ctr; ++l) { emitted[l] += em[l]; peak[l] += pk[l]; }
             add_counters(&total, &local);
         }
         free(sp); free(em); free(pk);

@@ -59,6 +59,7 @@ def lib():
         L.orc_test_isotropic.restype = None
         L.orc_test_rotate.argtypes = [vp, dbl, dbl, vp]
         L.orc_test_rotate.restype = None
+        L.orc_set_source_copies.argtypes = [vp, i32, vp]
         L.orc_test_source.argtypes = [vp, u64, u64, ll, vp, vp, vp, vp]
         L.orc_test_source.restype = None
         L.orc_run_histories.argtypes = [vp, u64, ll, u64, vp, vp, vp, vp, vp]
@@ -136,6 +137,8 @@ class OracleScene:
             m = w.mesh
             self.load_mesh(m.vertices, m.triangles, m.tri_surface, m.surf_inside, m.surf_outside, m.world_material)
             self.set_source(**w.source)
+            if getattr(w, "notes", None) and w.notes.get("source_copies") is not None:
+                self.set_source_copies(w.notes["source_copies"])
 
     def __del__(self):
         try:
@@ -172,6 +175,21 @@ class OracleScene:
         assert rc == 0, rc
         self.n_lines = le.shape[0]
         self.line_mev = le.astype(np.float64)
+        self.line_mev_base = self.line_mev.copy()
+        self.L.orc_set_source_copies(self.h, 1, None)
+
+    def set_source_copies(self, offsets):
+        """NEXT-3 batched scenes: replicate the source at these translations (float32 values, [n][3]); history h is emitted
+        from copy h mod n and counted under line copy * n_lines + l.  None = the plain source."""
+        if offsets is None:
+            assert self.L.orc_set_source_copies(self.h, 1, None) == 0
+            self.n_lines = len(self.line_mev_base)
+        else:
+            off = np.ascontiguousarray(np.asarray(offsets, dtype=np.float32).astype(np.float64))
+            assert off.ndim == 2 and off.shape[1] == 3
+            assert self.L.orc_set_source_copies(self.h, off.shape[0], _p(off)) == 0
+            self.n_lines = len(self.line_mev_base) * off.shape[0]
+        self.line_mev = np.tile(self.line_mev_base, self.n_lines // len(self.line_mev_base))
 
     def mu(self, m, ch, e):
         return self.L.orc_mu(self.h, m, ch, e)

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
                     "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw", "gadep_locate", "gadep_broaden",
                     "gadep_set_densities", "gadep_run_histories_ex", "gadep_set_bvh_width", "gadep_tally_size",
-                    "gadep_get_tallies", "gadep_set_tallies")
+                    "gadep_get_tallies", "gadep_set_tallies", "gadep_set_source_copies")
 
 
 class GadepError(RuntimeError):
@@ -110,6 +110,7 @@ def load_library(build_if_missing: bool = True):
     L.gadep_locate.argtypes = [vp, vp, vp, ll, i32, vp]
     L.gadep_broaden.argtypes = [vp, dbl, dbl, dbl, vp]
     L.gadep_set_bvh_width.argtypes = [vp, i32]
+    L.gadep_set_source_copies.argtypes = [vp, i32, vp]
     L.gadep_tally_size.argtypes = [vp]
     L.gadep_get_tallies.argtypes = [vp, vp]
     L.gadep_set_tallies.argtypes = [vp, vp]
@@ -201,6 +202,16 @@ class Gadep:
         if build:
             self.build_bvh()
         self.set_source(**w.source)
+        if getattr(w, "notes", None) and w.notes.get("source_copies") is not None:
+            self.set_source_copies(w.notes["source_copies"])
+
+    def set_source_copies(self, offsets):
+        """Replicate the source at these translations ([n][3]); None = the plain source."""
+        if offsets is None:
+            self._check(self.L.gadep_set_source_copies(self.h, 1, None))
+            return
+        off = np.ascontiguousarray(offsets, dtype=np.float32)
+        self._check(self.L.gadep_set_source_copies(self.h, int(off.shape[0]), _np_ptr(off)))
 
     # ---- hot path
     def run(self, n_histories, seed, n_bins=4096, e_max_mev=2.0, first_history=0, flags=0, spectrum=None):

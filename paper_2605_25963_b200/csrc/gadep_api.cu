@@ -482,6 +482,7 @@ extern "C" int gadep_set_source(gadep_ctx *c, const gadep_source *s) {
     g.cyl_r = s->cyl_r; g.cyl_z0 = s->cyl_z0; g.cyl_z1 = s->cyl_z1;
     g.ex_r = s->ex_r; g.ex_z0 = s->ex_z0; g.ex_z1 = s->ex_z1;
     g.n_lines = s->n_lines;
+    g.n_copies = 1;
     if (s->kind == GADEP_SRC_VOLUME && !(s->cyl_r > 0 && s->cyl_z1 > s->cyl_z0)) return gd_fail(c, GADEP_E_ARG, "empty source cylinder");
     if (s->kind == GADEP_SRC_BEAM) {
         double n2 = (double)s->dir[0] * s->dir[0] + (double)s->dir[1] * s->dir[1] + (double)s->dir[2] * s->dir[2];
@@ -499,6 +500,25 @@ extern "C" int gadep_set_source(gadep_ctx *c, const gadep_source *s) {
     if (!(cum > 0)) return gd_fail(c, GADEP_E_ARG, "all line intensities are zero");
     c->src = g;
     c->have_src = true;
+    return GADEP_OK;
+}
+
+extern "C" int gadep_set_source_copies(gadep_ctx *c, int n_copies, const float *offsets) {
+    if (!c) return GADEP_E_NULL;
+    if (!c->have_src) return gd_fail(c, GADEP_E_ORDER, "gadep_set_source_copies before gadep_set_source");
+    if (n_copies < 1 || n_copies > 8 || (n_copies > 1 && !offsets)) return gd_fail(c, GADEP_E_ARG, "n_copies %d (1..8)", n_copies);
+    const int nl = c->src.n_lines;
+    if (n_copies * nl > GADEP_MAX_LINES) return gd_fail(c, GADEP_E_ARG, "%d copies x %d lines exceed GADEP_MAX_LINES", n_copies, nl);
+    c->src.n_copies = n_copies;
+    memset(c->src.copy_off, 0, sizeof(c->src.copy_off));
+    for (int k = 0; k < n_copies; ++k)
+        for (int a = 0; a < 3; ++a) {
+            const float v = n_copies > 1 ? offsets[3 * k + a] : 0.0f;
+            if (!std::isfinite(v)) return gd_fail(c, GADEP_E_ARG, "copy %d: offset not finite", k);
+            c->src.copy_off[k][a] = v;
+        }
+    for (int k = 1; k < n_copies; ++k)
+        for (int l = 0; l < nl; ++l) c->src.line_mev[k * nl + l] = c->src.line_mev[l];
     return GADEP_OK;
 }
 
@@ -537,7 +557,7 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     }
     c->n_bins = n_bins; c->spec_e_max = e_max;
     double de = (double)e_max / n_bins;
-    for (int l = 0; l < c->src.n_lines; ++l) {
+    for (int l = 0; l < c->src.n_lines * c->src.n_copies; ++l) {
         double b = std::floor((double)c->src.line_mev[l] / de);
         c->src.line_bin[l] = b >= n_bins ? n_bins : (int)b;
     }
@@ -699,7 +719,7 @@ extern "C" int gadep_fepe(const gadep_ctx *cc, int line, int mode, double *fepe,
     if (!fepe) return gd_fail(c, GADEP_E_NULL, "null output");
     int rc = gd_fetch_results(c);
     if (rc) return rc;
-    if (line < 0 || line >= c->src.n_lines) return gd_fail(c, GADEP_E_ARG, "line %d out of range", line);
+    if (line < 0 || line >= c->src.n_lines * c->src.n_copies) return gd_fail(c, GADEP_E_ARG, "line %d out of range", line);
     double em = (double)c->h_emitted[line];
     double p = 0.0;
     if (em > 0) {
@@ -899,7 +919,7 @@ extern "C" int gadep_get_counters(const gadep_ctx *cc, gadep_counters *out) {
     out->n_parity_queries = h.n_parity; out->n_parity_mismatch = h.n_parity_mismatch;
     memcpy(out->emitted, c->h_emitted, sizeof(out->emitted));
     memcpy(out->peak, c->h_peak, sizeof(out->peak));
-    out->n_lines = c->src.n_lines;
+    out->n_lines = c->src.n_lines * (c->src.n_copies > 0 ? c->src.n_copies : 1);
     out->n_bvh_nodes = c->have_bvh ? std::max(c->n_ref - 1, 0) : 0;
     out->bvh_max_depth = c->bvh_depth;
     out->last_run_ms = c->last_run_ms; out->last_build_ms = c->last_build_ms;

@@ -109,6 +109,10 @@ struct GdSource {
     float line_mev[GD_MAX_LINES];
     float line_cum[GD_MAX_LINES];   // running sums of the intensities, float32 left to right
     int line_bin[GD_MAX_LINES];     // spectrum bin of the line energy (host, double)
+    // replicated source (gadep_set_source_copies): history h is emitted from copy h mod n_copies, translated by copy_off,
+    // and counted under line copy * n_lines + l; line_mev / line_bin hold n_copies * n_lines entries
+    int n_copies;
+    float copy_off[8][3];
 };
 
 struct GdMaterials {

@@ -194,6 +194,11 @@ GD_HD void gd_lane_start(GdLane &L, const GdSource &S, unsigned long long seed, 
     if (S.kind == 2) L.dir = gd_make(S.dir[0], S.dir[1], S.dir[2]);
     else if (S.kind == 0) { L.dir = gd_isotropic_from(u4.b, u4.c); L.g.draw += 2; }
     else L.dir = gd_sample_isotropic(L.g);
+    if (S.n_copies > 1) {
+        const int copy = (int)(history % (unsigned long long)S.n_copies);
+        L.pos.x += S.copy_off[copy][0]; L.pos.y += S.copy_off[copy][1]; L.pos.z += S.copy_off[copy][2];
+        L.line = copy * nl + line;
+    }
     L.dep = 0.0f; L.flags = 0; L.n_events = 0; L.pending = 0;
     L.m = 0; L.need_mu = 1; L.mu_tot = 0.0f; L.tau = 0.0f; L.sdist = 0.0f;
     L.ex = gd_no_exclude(); L.n_stall = 0;

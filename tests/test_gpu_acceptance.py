@@ -294,12 +294,16 @@ def test_cfg4_full_mesh_1e6_rays_vs_stored_brute_force(pkg, orc):
         cosang = np.maximum(np.abs(np.einsum("ij,ij->i", nrm, d.astype(np.float64))), 1e-7)
         floor = 8 * ulp / cosang                     # DESIGN.md R12: float32 inputs bound the hit point, 1/cos amplifies
         err = np.abs(t.astype(np.float64) - ot)
-        assert (err <= 1e-5 * np.abs(ot) + floor).all(), float((err / (1e-5 * np.abs(ot) + floor)).max())
+        same_idx = tri == otri
+        assert (err[same_idx] <= 1e-5 * np.abs(ot[same_idx]) + floor[same_idx]).all(), \
+            float((err[same_idx] / (1e-5 * np.abs(ot[same_idx]) + floor[same_idx])).max())
         n_rel_only = int((err <= 1e-5 * np.abs(ot)).sum())
-        diff = np.nonzero(tri != otri)[0]
-        # index mismatches: ties only -- the GPU's facet, in the oracle's double arithmetic, lies at the same distance
+        diff = np.nonzero(~same_idx)[0]
+        # index mismatches: ties only -- the GPU's facet, in the oracle's double arithmetic, lies at the same distance as
+        # the oracle's facet; or the ray starts on a facet (the oracle sees it a few nm behind the origin, float32 a few nm
+        # ahead: a tie at the edge of the window t > 0)
         s = None
-        n_edge = 0
+        n_edge = n_origin = 0
         for i in diff:
             if s is None:
                 s = orc.OracleScene(w)
@@ -312,10 +316,58 @@ def test_cfg4_full_mesh_1e6_rays_vs_stored_brute_force(pkg, orc):
                 n_edge += 1
                 tt = float(nn @ (p[0] - o64)) / float(nn @ d64)
                 q = o64 + tt * d64
-                bary = [float(np.cross(p[(k + 1) % 3] - p[k], q - p[k]) @ nn) / float(nn @ nn) for k in range(3)]
-                assert min(bary) >= -1e-5, (i, bary)
+                # signed in-plane distance of the hit point to each edge line (positive inside): the GPU's facet must hold
+                # the point within the float32 resolution of the hit point (a relative barycentric bound would be
+                # meaningless on the 0.05 mm slivers of this mesh)
+                nl = float(np.linalg.norm(nn))
+                dist = [float(np.cross(p[(k + 1) % 3] - p[k], q - p[k]) @ nn) / (nl * float(np.linalg.norm(p[(k + 1) % 3] - p[k]))) for k in range(3)]
+                assert min(dist) >= -8 * ulp / cs, (i, dist)
+            if tt <= 0.0 and abs(tt) <= 8 * ulp / cs and abs(float(t[i]) - tt) <= 8 * ulp / cs:
+                n_origin += 1                        # origin on the facet within float32 resolution
+                continue
             assert abs(tt - ot[i]) <= 1e-6 * abs(ot[i]) + 8 * ulp / cs, (i, tri[i], otri[i], tt, ot[i])
+            assert abs(float(t[i]) - ot[i]) <= 1e-5 * abs(ot[i]) + 8 * ulp / cs
+        assert n_origin <= 5
         assert len(diff) <= 1e-4 * n + 2
-        report[f"width{width}"] = {"index_identical": n - len(diff), "ties": len(diff), "of_which_through_an_edge": n_edge,
+        report[f"width{width}"] = {"index_identical": n - len(diff), "ties": len(diff), "of_which_through_an_edge": n_edge, "origin_on_a_facet": n_origin,
                                    "t_within_1e-5_relative_alone": n_rel_only}
     print("\nconfig-4 rays", json.dumps(report))
+
+
+# ------------------------------------------------------------------ NEXT-3: several detectors in one scene, one launch
+def test_batched_detectors_one_launch_vs_oracle_and_vs_separate_launches(pkg, orc):
+    dets = (0, 1, 2)
+    wb = dm.make_calibration_batch(dets, n_histories=3_000_000)
+    g = pkg.Gadep(0)
+    g.load_workload(wb)                         # applies notes["source_copies"] through gadep_set_source_copies
+    # per-history parity with the oracle on the batched scene (same streams)
+    n = 30_000
+    s = orc.OracleScene(wb)
+    edep, flags = g.run_histories(0, n, wb.seed)
+    oe, of, oc = s.run_histories(0, n, wb.seed)
+    same = (flags == of) & (np.abs(edep.astype(np.float64) - oe) <= 2e-6 + 1e-5 * oe)
+    assert same.mean() >= 0.999, same.mean()
+    assert np.array_equal((flags >> 8) & 0xFF, (of >> 8) & 0xFF)          # copy * 13 + line on both sides
+    # one launch = three FEPE curves; each equals the curve of that detector run on its own (same histories: history h
+    # of the batch is history h of the single-detector run for h = k mod 3 -- the other two thirds of the single run are
+    # different histories, so the comparison is statistical, 4 sigma)
+    nb = wb.n_histories
+    g.run(nb, wb.seed, wb.n_bins, wb.spectrum_e_max_mev)
+    cb = g.get_counters()
+    assert cb["n_lines"] == 39 and cb["n_leak"] == 0
+    em = np.array(cb["emitted"]).reshape(3, 13)
+    assert em.sum(axis=1).tolist() == [nb // 3] * 3                      # round robin
+    for k, d in enumerate(dets):
+        w1 = dm.make_calibration(d, n_histories=nb // 3)
+        g1 = pkg.Gadep(0)
+        g1.load_workload(w1)
+        g1.run(nb // 3, w1.seed + 1, w1.n_bins, w1.spectrum_e_max_mev)       # an independent sample of the same detector
+        for l in range(13):
+            fb, sb_ = g.fepe(13 * k + l, 0)
+            f1, s1_ = g1.fepe(l, 0)
+            assert abs(fb - f1) <= 4 * math.sqrt(sb_ * sb_ + s1_ * s1_) + 1e-9, (k, l, fb, f1)
+    # the replicated source is reset by a new gadep_set_source and refuses too many lines
+    with pytest.raises(pkg.GadepError):
+        g.set_source_copies(np.zeros((5, 3), dtype=np.float32))           # 5 x 13 > 64 lines
+    g.set_source_copies(None)
+    assert g.get_counters()["n_lines"] == 13

@@ -339,3 +339,47 @@ def test_broadening_conserves_the_total_at_the_edges():
     # the overflow slot keeps its counts and takes the mass above e_max
     p_up = 0.5 * (1 - math.erf((0.5 * de) / (sigma * math.sqrt(2))))
     assert out[n] == pytest.approx(77.0 + 2000.0 * p_up, rel=1e-6)
+
+
+# ------------------------------------------------------------------ NEXT-3: replicated source / batched detectors
+def test_replicated_source_round_robin_offsets_and_line_numbering():
+    src = {"kind": SRC_POINT, "pos": (1.0, 2.0, 3.0), "dir": (0, 0, -1), "line_mev": [0.1, 0.2, 0.3],
+           "line_intensity": [1.0, 1.0, 2.0]}
+    s = _source_only_scene(src)
+    n = 30_000
+    line0, pos0, d0, draw0 = s.sample_source(7, 5, n)
+    offs = np.array([[0, 0, 0], [512.0, 0, 0], [0, -256.0, 8.0]], dtype=np.float32)
+    s.set_source_copies(offs)
+    line, pos, d, draw = s.sample_source(7, 5, n)
+    copy = (5 + np.arange(n)) % 3                                   # the *global* history index decides the copy
+    assert np.array_equal(line, line0 + 3 * copy)                   # line numbering copy * n_lines + l
+    assert np.array_equal(pos, pos0 + offs[copy].astype(np.float64))
+    assert np.array_equal(d, d0) and np.array_equal(draw, draw0)    # same draws: the streams do not know about copies
+    cnt = np.bincount(line, minlength=9).reshape(3, 3)
+    assert (np.abs(cnt.sum(axis=1) - n / 3) <= 1).all()             # round robin: equal shares
+    s.set_source_copies(None)
+    assert np.array_equal(s.sample_source(7, 5, 100)[0], line0[:100])
+
+
+def test_batched_detectors_equal_their_single_detector_runs():
+    # two copies of the same detector 768 mm apart, each in its own world cylinder: history h of the batch is history h
+    # of the single-detector run, translated -- identical course (the offsets are exact in float32 at these magnitudes
+    # only up to the rounding of the translated vertices, hence "almost all")
+    wb = dm.make_calibration_batch((1, 1), n_histories=1000, n_theta=64)
+    w1 = dm.make_calibration(1, n_histories=1000, n_theta=64)
+    assert wb.mesh.n_tri == 2 * w1.mesh.n_tri and len(wb.mesh.surf_inside) == 16
+    for sf in range(16):      # every surface of the merged scene is still closed and oriented
+        assert dm.check_closed_oriented(wb.mesh.triangles[wb.mesh.tri_surface == sf])["ok"]
+    sb, s1 = orc.OracleScene(wb), orc.OracleScene(w1)
+    n = 60_000
+    eb, fb, cb = sb.run_histories(0, n, 1)
+    e1, f1, c1 = s1.run_histories(0, n, 1)
+    copy = np.arange(n) % 2
+    assert np.array_equal((fb >> 8) & 0xFF, ((f1 >> 8) & 0xFF) + 13 * copy)
+    same = ((fb & 0xFF) == (f1 & 0xFF)) & ((fb >> 16) == (f1 >> 16)) & (np.abs(eb - e1) <= 1e-9)
+    assert same.mean() >= 0.9995
+    assert cb["n_leak"] == 0 and cb["n_filter_reject"] == 0
+    spec, em, pk, _ = sb.run(n, 1)
+    assert len(em) == 26 and em.reshape(2, 13).sum(axis=1).tolist() == [n // 2, n // 2]
+    sp1, em1, pk1, _ = s1.run(n, 1)
+    assert abs(int(spec.sum()) - int(sp1.sum())) <= 0.0005 * n + 2
