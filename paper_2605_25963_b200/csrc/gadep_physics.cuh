@@ -205,7 +205,7 @@ GD_HD void gd_lane_start(GdLane &L, const GdSource &S, unsigned long long seed, 
     L.mode = GD_MODE_LOCATE;
 }
 
-// ---- "partial cross-section method" (R2 / section 13): every process c keeps its own remaining
+// ---- "partial cross-section method" (R2 / section 12): every process c keeps its own remaining
 // optical depth tau_c; the flight ends where the first budget runs out (s = min_c tau_c / mu_c), that process fires, and
 // only its budget is sampled again.  Same distribution as total-mu sampling + a selection draw, one draw fewer per event.
 GD_HD void gd_partial_birth(GdLane &L) {
