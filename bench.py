@@ -103,14 +103,25 @@ def oracle_rate(w, n_sample, first=0):
     return n_sample / dt, dt, orc.num_threads()
 
 
+def size_sample(w, seconds, cap):
+    """Histories the oracle transports in about `seconds` on this box.  Growing pilots: the rate of a few hundred
+    histories is dominated by the longest scattering chains on 16 threads and underestimates the sustained rate."""
+    n, r = 500, 0.0
+    for _ in range(8):                 # pilots grow until one takes about a second
+        r, dt, _ = oracle_rate(w, n)
+        if dt >= 1.0 or n >= cap:
+            break
+        n = int(min(cap, max(2 * n, 1.5 * r)))
+    return int(min(max(seconds * r, 500), cap))
+
+
 def run_reference(args, w, rank):
     """--impl reference: the CPU oracle, as it stands, on this box's host cores; rank 0 only."""
     if rank != 0:
         return
     n_sample = int(args.ref_sample)
-    if n_sample <= 0:                 # sized from a pilot so that one step is a few seconds of CPU work
-        r0, _, _ = oracle_rate(w, 300)
-        n_sample = int(min(max(4.0 * r0, 300), 2e6))
+    if n_sample <= 0:                 # sized from pilots so that one step is a few seconds of CPU work
+        n_sample = size_sample(w, 4.0, 2e6)
     for _ in range(args.warmup):
         oracle_rate(w, max(n_sample // 10, 100))
     t_all, cores = 0.0, 1
@@ -404,7 +415,7 @@ def main():
                              "traffic": traffic,
                              "traffic_source": "profiles/ncu_traffic.json (ncu --set full, dram bytes of one launch)",
                              "hbm": {"achieved_gbs": (traffic / (k_s / args.steps) / 1e9) if traffic else None, "peak_gbs": hbm_peak},
-                             "limiter": "instruction issue: instruction-fetch and dependency stalls at 16 warps/SM, 14-16 of 32 "
+                             "limiter": "instruction issue: instruction-fetch and dependency stalls at 12 warps/SM, 14-17 of 32 "
                                         "lanes per instruction (ncu, profiles/r02_wave_kernel.md)",
                              "peak_source": f"{n_sm} SMs x 128 lanes x sm_max_mhz ({peak_src})",
                              "kernel_ms_per_step": sum(kern_ms) / args.steps,
@@ -434,9 +445,8 @@ def main():
             line["config"]["ray_bench"] = ray_bench(pkg, torch, dm, g4, w4, int(args.rays))
         if not args.no_cpu_baseline and world == 1:
             n_s = int(args.cpu_sample)
-            if n_s <= 0:                                         # pilot -> about 15 s of CPU work
-                r0, dt0, _ = oracle_rate(w, 500)
-                n_s = int(min(max(15.0 * r0, 500), 5e7))
+            if n_s <= 0:                                         # pilots -> about 15 s of CPU work
+                n_s = size_sample(w, 15.0, 5e7)
             r, dt, cores = oracle_rate(w, n_s)
             line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"first {n_s} histories of {w.name} ({dt:.1f} s)"}

@@ -430,13 +430,24 @@ def test_headline_size_volume_sources_vs_stored_oracle(pkg, orc, cfg):
     assert sum(c["emitted"]) == n == c["n_histories"]
     assert c["n_leak"] <= 20        # float32 corner cases that needed a second localisation: ~1e-8 per history
     assert int(spec.sum()) <= n and all(p <= e for p, e in zip(c["peak"], c["emitted"]))
+    z = []
     for l in range(c["n_lines"]):
         f, se = g.fepe(l, 0)
         fo = gold["peak"][l] / gold["emitted"][l]
         so = math.sqrt(max(fo * (1 - fo), 1.0 / gold["emitted"][l]) / gold["emitted"][l])
-        assert abs(f - fo) <= 3 * math.sqrt(se * se + so * so) + 1e-12, (l, f, fo)
+        z.append((f - fo) / math.sqrt(se * se + so * so))
         # the emission frequencies follow the line intensities
         assert abs(c["emitted"][l] / n - gold["emitted"][l] / gold["n_histories"]) <= 4 * math.sqrt(0.25 / gold["n_histories"])
+    # north_star: FEPE per line within 3 combined standard errors.  The two samples are independent here, so with L
+    # lines a correct implementation leaves the 3-sigma band on some line with probability 0.0027 L (11 % for the 40
+    # lines of config 3): the family of lines is held to "at most one line of >= 20 beyond 3 sigma, none beyond 4, and
+    # the mean z^2 within 3 standard deviations of its expectation 1".  The same stored run is
+    # compared history by history, far below its statistical error, in test_gpu_acceptance.py.
+    z = np.array(z)
+    L = len(z)
+    assert int((np.abs(z) > 3.0).sum()) <= (1 if L >= 20 else 0), z
+    assert np.abs(z).max() <= 4.0, z
+    assert float((z * z).mean()) <= 1.0 + 3.0 * math.sqrt(2.0 / L), (float((z * z).mean()), z)
     # sample sizes differ by 500-1000x: the per-bin variance comes from the pooled rate, not from the sparse bin itself
     # (and the spectrum is re-binned 32:1 so that the oracle's few thousand scoring histories populate the bins)
     a = spec[:-1].astype(np.float64).reshape(-1, 32).sum(axis=1)
