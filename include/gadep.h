@@ -195,6 +195,25 @@ int gadep_trace_rays(gadep_ctx *ctx, const float *org, const float *dir, long lo
                      float t_min, int *tri_out, float *t_out);
 
 /*
+ * gadep_trace_rays for callers that must not allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same nearest-facet query through the same traversal kernel, with every byte of
+ * scratch -- the kernel's ray-fetch counter, its work counters and, for HOST arrays, the staging copies of org / dir /
+ * tri_out / t_out (32 B per ray) -- in ONE file-scope `static __device__` array of the library
+ * (256 + 256 + 32 * GADEP_STATIC_MAX_RAYS bytes = 8 MiB + 512 B, held by every GPU that loads the library until the
+ * process exits).  Calls no cudaMalloc / cudaFree and no allocating library routine.
+ *   org, dir, tri_out, t_out   as gadep_trace_rays (HOST or DEVICE, all in one memory space); the caller owns them
+ *   n_rays                     0 .. GADEP_STATIC_MAX_RAYS; more -> GADEP_E_ARG ("... exceeds GADEP_STATIC_MAX_RAYS")
+ * The array is shared by every context and every call on a device and keeps the previous call's contents: the entry
+ * point clears the counters it needs at zero on the context's stream before the launch, and returns after the stream
+ * has drained.  Two calls that overlap on the GPU (two contexts / streams / host threads on the same device) RACE on it;
+ * serialise them.  The first call on a device resolves the array's device address (cudaGetSymbolAddress, which may load
+ * the module); make that call outside a capture.  Work counters of the call: gadep_get_counters, as for gadep_trace_rays.
+ */
+#define GADEP_STATIC_MAX_RAYS (1 << 18)
+int gadep_trace_rays_static(gadep_ctx *ctx, const float *org, const float *dir, long long n_rays, int filter_material,
+                            float t_min, int *tri_out, float *t_out);
+
+/*
  * Material in which each point lies (sec 2.4.2), found from a ray cast along dir.
  *   mode GADEP_LOCATE_SIDE_ID  the paper's original rule: nearest facet ahead; its normal tells entering from leaving and
  *                              the facet's side ids give the material (what gadep_run uses).

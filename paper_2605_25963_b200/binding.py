@@ -14,6 +14,7 @@ from .build import LIB, build_library
 
 F_ESCAPED, F_PEAK, F_LEAK, F_NONSCORING = 1, 2, 4, 8
 FILTER_NONE = -2
+STATIC_MAX_RAYS = 1 << 18      # GADEP_STATIC_MAX_RAYS of include/gadep.h
 MAT_KILL = -1
 MAX_LINES = 64
 RUN_ASYNC, RUN_ACCUMULATE, RUN_HISTORY_PER_THREAD, RUN_PERSISTENT_LANES, RUN_PARITY_LOCALISATION = 1, 2, 4, 8, 16
@@ -26,7 +27,7 @@ EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
                     "gadep_run_histories", "gadep_get_counters", "gadep_philox_raw", "gadep_locate", "gadep_broaden",
                     "gadep_set_densities", "gadep_run_histories_ex", "gadep_set_bvh_width", "gadep_tally_size",
-                    "gadep_get_tallies", "gadep_set_tallies", "gadep_set_source_copies")
+                    "gadep_get_tallies", "gadep_set_tallies", "gadep_set_source_copies", "gadep_trace_rays_static")
 
 
 class GadepError(RuntimeError):
@@ -102,6 +103,7 @@ def load_library(build_if_missing: bool = True):
     L.gadep_run.argtypes = [vp, ull, ull, C.POINTER(GadepRunOpts), vp]
     L.gadep_fepe.argtypes = [vp, i32, i32, C.POINTER(dbl), C.POINTER(dbl)]
     L.gadep_trace_rays.argtypes = [vp, vp, vp, ll, i32, f32, vp, vp]
+    L.gadep_trace_rays_static.argtypes = [vp, vp, vp, ll, i32, f32, vp, vp]
     L.gadep_run_histories.argtypes = [vp, ull, ll, ull, vp, vp]
     L.gadep_run_histories_ex.argtypes = [vp, ull, ll, ull, C.c_int, vp, vp]
     L.gadep_set_densities.argtypes = [vp, C.c_int, vp]
@@ -243,6 +245,24 @@ class Gadep:
                 raise ValueError("device inputs need device outputs")
         self._check(self.L.gadep_trace_rays(self.h, _ptr(org), _ptr(dir), n, int(filter_material), float(t_min),
                                             _ptr(tri_out), _ptr(t_out)))
+        return tri_out, t_out
+
+    def trace_rays_static(self, org, dir, filter_material=FILTER_NONE, t_min=0.0, tri_out=None, t_out=None):
+        """gadep_trace_rays_static: the same query without any device allocation (scratch in a static device array of
+        the library, at most STATIC_MAX_RAYS rays per call; calls on one device must not overlap).  With numpy inputs
+        and no outputs given, the two HOST result arrays are made here, by the caller's side."""
+        if isinstance(org, np.ndarray):
+            org = np.ascontiguousarray(org, dtype=np.float32)
+            dir = np.ascontiguousarray(dir, dtype=np.float32)
+            n = org.shape[0]
+            tri_out = np.empty(n, dtype=np.int32) if tri_out is None else tri_out
+            t_out = np.empty(n, dtype=np.float32) if t_out is None else t_out
+        else:
+            n = org.shape[0]
+            if tri_out is None or t_out is None:
+                raise ValueError("device inputs need device outputs")
+        self._check(self.L.gadep_trace_rays_static(self.h, _ptr(org), _ptr(dir), n, int(filter_material), float(t_min),
+                                                   _ptr(tri_out), _ptr(t_out)))
         return tri_out, t_out
 
     def broaden(self, fwhm_a, fwhm_b=0.0, fwhm_c=0.0, out=None):

@@ -988,6 +988,90 @@ extern "C" int gadep_set_tallies(gadep_ctx *c, const unsigned long long *in) {
     return GADEP_OK;
 }
 
+// ---------------------------------------------------------------- ray cast without any allocation
+// gadep_trace_rays_static (include/gadep.h): gd_k_trace_wave with all of its scratch in one file-scope device array.
+//   [0, 256)     ray-fetch counter of the kernel (unsigned long long), must start at zero
+//   [256, 512)   GdCounters of the launch, must start at zero
+//   [512, ...)   staging for HOST arrays: org float[n][3], dir float[n][3], tri int[n], t float[n] (32 B per ray)
+// In host code `gd_static_scratch` names a host-side stand-in, not device memory: the device address comes from
+// cudaGetSymbolAddress, once per device with that device current, and that pointer is what the kernel is given.
+#define GD_STATIC_HDR 512
+static_assert(sizeof(GdCounters) <= 256, "GdCounters must fit its 256-byte cell");
+static __device__ __align__(256) unsigned char gd_static_scratch[GD_STATIC_HDR + 32ull * GADEP_STATIC_MAX_RAYS];
+#define GD_STATIC_MAX_DEVICES 64
+static unsigned char *gd_static_addr[GD_STATIC_MAX_DEVICES] = {};
+
+// device address of the array on `device` (which the caller has made current); resolved on the first call per device
+static cudaError_t gd_static_scratch_on(int device, unsigned char **out) {
+    if (device < 0 || device >= GD_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    unsigned char *p = __atomic_load_n(&gd_static_addr[device], __ATOMIC_ACQUIRE);
+    if (!p) {
+        void *sym = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&sym, gd_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!sym) return cudaErrorInvalidSymbol;
+        p = (unsigned char *)sym;
+        __atomic_store_n(&gd_static_addr[device], p, __ATOMIC_RELEASE);    // every thread resolves the same address
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+extern "C" int gadep_trace_rays_static(gadep_ctx *c, const float *org, const float *dir, long long n_rays,
+                                       int filter_material, float t_min, int *tri_out, float *t_out) {
+    if (!c) return GADEP_E_NULL;
+    if (!org || !dir || !tri_out || !t_out) return gd_fail(c, GADEP_E_NULL, "null ray array");
+    if (!c->have_bvh) return gd_fail(c, GADEP_E_ORDER, "gadep_trace_rays_static before gadep_build_bvh");
+    if (n_rays < 0) return gd_fail(c, GADEP_E_ARG, "negative ray count");
+    if (n_rays > (long long)GADEP_STATIC_MAX_RAYS)
+        return gd_fail(c, GADEP_E_ARG, "n_rays %lld exceeds GADEP_STATIC_MAX_RAYS (%d): the static scratch array holds no more; "
+                       "split the batch or use gadep_trace_rays", n_rays, (int)GADEP_STATIC_MAX_RAYS);
+    if (n_rays == 0) return GADEP_OK;
+    GD_CUDA(c, cudaSetDevice(c->device));
+    const bool dev = gd_is_device_ptr(org);
+    if (dev != gd_is_device_ptr(dir) || dev != gd_is_device_ptr(tri_out) || dev != gd_is_device_ptr(t_out))
+        return gd_fail(c, GADEP_E_ARG, "ray arrays must live in one memory space");
+    unsigned char *scratch = nullptr;
+    GD_CUDA(c, gd_static_scratch_on(c->device, &scratch));
+    unsigned long long *d_next = (unsigned long long *)scratch;
+    GdCounters *d_cnt = (GdCounters *)(scratch + 256);
+    float *stage = (float *)(scratch + GD_STATIC_HDR);
+    cudaStream_t st = c->stream;
+    const float *d_org = org, *d_dir = dir;
+    int *d_tri = tri_out;
+    float *d_t = t_out;
+    const size_t nb3 = sizeof(float) * 3 * (size_t)n_rays, nb1 = sizeof(float) * (size_t)n_rays;
+    if (!dev) {
+        d_org = stage; d_dir = stage + 3 * n_rays; d_tri = (int *)(stage + 6 * n_rays); d_t = stage + 7 * n_rays;
+        GD_CUDA(c, cudaMemcpyAsync(stage, org, nb3, cudaMemcpyHostToDevice, st));
+        GD_CUDA(c, cudaMemcpyAsync(stage + 3 * n_rays, dir, nb3, cudaMemcpyHostToDevice, st));
+    }
+    GD_CUDA(c, cudaMemsetAsync(scratch, 0, GD_STATIC_HDR, st));       // the last call's counter and totals are still there
+    int per_sm = 1;
+    const bool wide8 = c->bvh_width == 8;
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, wide8 ? gd_k_trace_wave<8> : gd_k_trace_wave<4>, 256, 0));
+    const int grid = (int)std::min<long long>((n_rays + 255) / 256, (long long)c->n_sm * std::max(per_sm, 1));
+    const unsigned chunk = (unsigned)std::min<long long>(2048, std::max<long long>(32, n_rays / ((long long)grid * 8 * 8)));
+    cudaEventRecord(c->ev0, st);
+    if (wide8) gd_k_trace_wave<8><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
+                                                         d_cnt, d_next, chunk, c->tune);
+    else gd_k_trace_wave<4><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
+                                                   d_cnt, d_next, chunk, c->tune);
+    cudaEventRecord(c->ev1, st);
+    c->last_run_launches = 1;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && !dev) {
+        e = cudaMemcpyAsync(tri_out, d_tri, nb1, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(t_out, d_t, nb1, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaMemcpy(&c->h_counters, d_cnt, sizeof(GdCounters), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return gd_fail(c, GADEP_E_CUDA, "static trace failed: %s", cudaGetErrorString(e));
+    cudaEventElapsedTime(&c->last_run_ms, c->ev0, c->ev1);
+    c->run_timed = false;
+    return GADEP_OK;
+}
+
 #ifdef GD_PROF
 extern "C" int gadep_prof_read(unsigned long long *out16, int reset) {
     cudaDeviceSynchronize();
