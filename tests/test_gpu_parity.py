@@ -421,7 +421,7 @@ def test_headline_size_volume_sources_vs_stored_oracle(pkg, orc, cfg):
     files = sorted(glob.glob(os.path.join(GOLDEN, f"cfg{cfg}_oracle_n*.json")))
     if not files:
         pytest.skip("stored oracle result not generated")
-    gold = json.load(open(files[-1]))
+    gold = max((json.load(open(f)) for f in files), key=lambda d: d["n_histories"])
     w, g, s = _setup(pkg, orc, cfg)
     n = w.n_histories
     assert n == 100_000_000
@@ -467,7 +467,7 @@ def test_headline_size_config4_vs_coarser_tessellation_oracle(pkg, orc):
     files = sorted(glob.glob(os.path.join(GOLDEN, "cfg4_oracle_n*_nt512_b128.json")))
     if not files:
         pytest.skip("stored oracle result not generated")
-    gold = json.load(open(files[-1]))
+    gold = max((json.load(open(f)) for f in files), key=lambda d: d["n_histories"])
     w, g, s = _setup(pkg, orc, 4)
     n = w.n_histories
     assert n == 100_000_000 and w.mesh.n_tri > 2_000_000
