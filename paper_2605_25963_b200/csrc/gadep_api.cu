@@ -47,8 +47,8 @@ struct gadep_ctx {
     // [6..9] the mesh copies (vertices, triangles, side materials, surface ids)
     // [10..12] mesh validation: edge table keys, edge table surfaces, error record + surface sides
     // [14] clearance grid: marks / x distances [15] squared distances after the y pass [16] the grid itself
-    void *pool[17] = {};
-    size_t pool_cap[17] = {};
+    void *pool[20] = {};
+    size_t pool_cap[20] = {};
     // source
     bool have_src = false;
     GdSource src;
@@ -75,6 +75,8 @@ struct gadep_ctx {
     float roi_lo[3] = {0, 0, 0}, roi_hi[3] = {0, 0, 0};
     bool have_roi = false;
     long long grid_cells = 1ll << 22;         // GADEP_GRID_CELLS overrides; 0 = no grid
+    double list_reach_cells = 1.0;            // reach of the cells' plane lists in cells; GADEP_GRID_REACH overrides, 0 = no lists
+    unsigned n_list_cells = 0, n_listed = 0;  // cells below the reach / cells that got a list (last build)
     GdGrid grid = {};
     bool cluster_surfaces = true;             // GADEP_NO_SURFACE_CLUSTERS=1 switches it off (measurement)
     double split_budget = 8.0;                // extra BVH references per facet handed out by the splitting budget
@@ -145,7 +147,7 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (getenv("GADEP_NO_SURFACE_CLUSTERS")) c->cluster_surfaces = false;
     if (const char *t = getenv("GADEP_WS")) c->prefer_ws = atoi(t) != 0;
     if (const char *t = getenv("GADEP_GRID_CELLS")) { long long v = atoll(t); if (v >= 0 && v <= (1ll << 28)) c->grid_cells = v; }
-    if (const char *t = getenv("GADEP_SPLIT_BUDGET")) { double b = atof(t); if (b >= 0 && b <= 15) c->split_budget = b; }
+    if (const char *t = getenv("GADEP_GRID_REACH")) { double v = atof(t); if (v >= 0.0 && v <= 8.0) c->list_reach_cells = v; }
     if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,t_keep,n_steps,n_steps_max,p_min,t_help" (measurement sweeps)
         int a, b, d, dm = 0, p = c->tune.p_min, ts = c->tune.t_help;
         if (sscanf(t, "%d,%d,%d,%d,%d,%d", &a, &b, &d, &dm, &p, &ts) >= 4 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && dm >= d && dm <= 32 && p >= 1 && p <= 32 && ts >= 1 && ts <= 1024)
@@ -179,7 +181,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    for (int k = 0; k < 17; ++k) cudaFree(c->pool[k]);
+    for (int k = 0; k < 20; ++k) cudaFree(c->pool[k]);
     cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair); cudaFree(c->d_mat_entry);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -406,6 +408,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
             g.nx = dim[0]; g.ny = dim[1]; g.nz = dim[2];
             g.lox = (float)(c->roi_lo[0] - h); g.loy = (float)(c->roi_lo[1] - h); g.loz = (float)(c->roi_lo[2] - h);
             g.inv_h = (float)(1.0 / h); g.quarter_h = (float)(0.25 * h * (1.0 - 1e-6));
+            g.h = (float)h; g.reach = 0.0f; g.cell_ref = nullptr; g.planes = nullptr;
             const size_t nc = (size_t)g.nx * g.ny * g.nz;
             unsigned char *occ = nullptr, *cells = nullptr;
             unsigned short *d2 = nullptr;
@@ -420,6 +423,30 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
             gd_k_grid_dt_y<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, occ, d2);
             gd_k_grid_dt_z<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, d2, cells);
             launches += 4;
+            // plane lists for the cells whose scalar clearance is below the reach
+            c->n_list_cells = 0; c->n_listed = 0;
+            if (c->list_reach_cells > 0.0 && n > 1) {
+                const float reach = (float)(c->list_reach_cells * h);
+                const unsigned thr = (unsigned)std::min(255.0, std::ceil((double)reach / (double)g.quarter_h));
+                unsigned *lc = nullptr, *cell_ref = nullptr;
+                float4 *planes = nullptr;
+                if ((e = gd_pool_get(c, 17, 16, (void **)&lc)) != cudaSuccess) break;
+                cudaMemsetAsync(lc, 0, 16, st);
+                gd_k_grid_list_count<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(cells, nc, thr, lc);
+                unsigned n_list = 0;
+                if ((e = cudaMemcpyAsync(&n_list, lc, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
+                if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
+                launches += 1;
+                if (n_list > 0 && n_list < (1u << 28)) {
+                    if ((e = gd_pool_get(c, 18, 4 * nc, (void **)&cell_ref)) != cudaSuccess) break;
+                    if ((e = gd_pool_get(c, 19, sizeof(float4) * GD_CELL_PLANES * (size_t)n_list, (void **)&planes)) != cudaSuccess) break;
+                    g.reach = reach; g.cell_ref = cell_ref; g.planes = planes;
+                    gd_k_grid_planes<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(g, cells, thr, c->d_nodes4, c->d_leaf_tris, cell_ref, planes, lc + 1, n_list);
+                    launches += 1;
+                    c->n_list_cells = n_list;
+                    if ((e = cudaMemcpyAsync(&c->n_listed, lc + 1, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
+                }
+            }
             c->grid = g;
         }
         cudaEventRecord(c->evb1, st);
@@ -427,6 +454,9 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
         if (n > 1 && (e = cudaMemcpy(&depth, scene + 6, sizeof(int), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
         cudaEventElapsedTime(&c->last_build_ms, c->evb0, c->evb1);
+        if (getenv("GADEP_GRID_DEBUG"))
+            fprintf(stderr, "[gadep] grid %d x %d x %d, h %.4f mm, reach %.4f mm: %u cells below the reach, %u with a plane list\n",
+                    c->grid.nx, c->grid.ny, c->grid.nz, c->grid.h, c->grid.reach, c->n_list_cells, c->n_listed);
         // per-material entry table: the surfaces that have the material on one side.  A surface without an entry node
         // (never for a closed surface of >= 2 references) or too many surfaces around one material -> root for it.
         c->have_entries = false;

@@ -612,3 +612,80 @@ __global__ void gd_k_grid_dt_z(GdGrid g, const unsigned short *__restrict__ d2, 
     const float cl = sqrtf((float)best) * 0.999999f - 1.7320509f;
     out[i] = (unsigned char)fminf(fmaxf(floorf(cl * 4.0f), 0.0f), 255.0f);
 }
+
+// ---- plane lists of the cells near facets (GdGrid::cell_ref / planes).  One thread per cell whose scalar clearance is
+// below `thr` (= the reach in units of h / 4): a box query of the 4-wide hierarchy with the cell dilated by the reach
+// collects the facets that can come within reach of a point of the cell (every reference box that overlaps the dilated
+// cell; a facet whose plane passes farther than reach + half a cell diagonal from the centre is dropped), their planes
+// are computed in double from the float32 vertices, referred to the cell centre and merged when they agree to 2e-5 mm
+// over the cell.  More than GD_CELL_PLANES distinct planes, or a query that runs out of stack: no list (the BVH answers).
+__global__ void gd_k_grid_list_count(const unsigned char *__restrict__ cells, size_t n, unsigned thr, unsigned *count) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool want = i < n && cells[i] < thr;
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, want);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(count, (unsigned)__popc(m));
+}
+__global__ void __launch_bounds__(128)
+gd_k_grid_planes(GdGrid g, const unsigned char *__restrict__ cells, unsigned thr, const GdNode4 *__restrict__ nodes4,
+                 const GdTri *__restrict__ tris, unsigned *__restrict__ cell_ref, float4 *__restrict__ planes,
+                 unsigned *counter, unsigned capacity) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t n = (size_t)g.nx * g.ny * g.nz;
+    if (i >= n) return;
+    if (cells[i] >= thr) { cell_ref[i] = 0u; return; }
+    const int ix = (int)(i % g.nx), iy = (int)((i / g.nx) % g.ny), iz = (int)(i / ((size_t)g.nx * g.ny));
+    // the centre exactly as gd_flight_clear computes it
+    const float cx = fmaf((float)ix + 0.5f, g.h, g.lox), cy = fmaf((float)iy + 0.5f, g.h, g.loy), cz = fmaf((float)iz + 0.5f, g.h, g.loz);
+    const float half = 0.5f * g.h * 1.0001f, pad = 1.0e-3f;
+    const float r = half + g.reach + pad + 1.0e-6f * fmaxf(fmaxf(fabsf(cx), fabsf(cy)), fabsf(cz));
+    const float qlx = cx - r, qhx = cx + r, qly = cy - r, qhy = cy + r, qlz = cz - r, qhz = cz + r;
+    const double far_plane = (double)g.reach + 0.8661 * (double)g.h + (double)pad;
+    float4 pl[GD_CELL_PLANES];
+    int cnt = 0;
+    bool overflow = false;
+    int stack[96];
+    int sp = 0, node = 0;
+    for (;;) {
+        const GdNode4 nd = nodes4[node];
+        const float lo_x[4] = {nd.lox.x, nd.lox.y, nd.lox.z, nd.lox.w}, hi_x[4] = {nd.hix.x, nd.hix.y, nd.hix.z, nd.hix.w};
+        const float lo_y[4] = {nd.loy.x, nd.loy.y, nd.loy.z, nd.loy.w}, hi_y[4] = {nd.hiy.x, nd.hiy.y, nd.hiy.z, nd.hiy.w};
+        const float lo_z[4] = {nd.loz.x, nd.loz.y, nd.loz.z, nd.loz.w}, hi_z[4] = {nd.hiz.x, nd.hiz.y, nd.hiz.z, nd.hiz.w};
+        const int ch[4] = {nd.child.x, nd.child.y, nd.child.z, nd.child.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (ch[k] == GD_NO_CHILD) continue;
+            if (lo_x[k] > qhx || hi_x[k] < qlx || lo_y[k] > qhy || hi_y[k] < qly || lo_z[k] > qhz || hi_z[k] < qlz) continue;
+            if (ch[k] >= 0) {
+                if (sp == 96) overflow = true; else stack[sp++] = ch[k];
+                continue;
+            }
+            const GdTri tr = tris[~ch[k]];
+            const double e1x = (double)tr.v1.x - tr.v0.x, e1y = (double)tr.v1.y - tr.v0.y, e1z = (double)tr.v1.z - tr.v0.z;
+            const double e2x = (double)tr.v2.x - tr.v0.x, e2y = (double)tr.v2.y - tr.v0.y, e2z = (double)tr.v2.z - tr.v0.z;
+            double nx = e1y * e2z - e1z * e2y, ny = e1z * e2x - e1x * e2z, nz = e1x * e2y - e1y * e2x;
+            const double len = sqrt(nx * nx + ny * ny + nz * nz);
+            if (!(len > 0.0)) { overflow = true; continue; }
+            nx /= len; ny /= len; nz /= len;
+            const double d = nx * ((double)cx - tr.v0.x) + ny * ((double)cy - tr.v0.y) + nz * ((double)cz - tr.v0.z);
+            if (fabs(d) > far_plane) continue;
+            const float4 q = make_float4((float)nx, (float)ny, (float)nz, (float)d);
+            bool seen = false;
+            for (int j = 0; j < cnt; ++j) {
+                const float sgn = (q.x * pl[j].x + q.y * pl[j].y + q.z * pl[j].z) < 0.0f ? -1.0f : 1.0f;
+                const float dn = fabsf(q.x - sgn * pl[j].x) + fabsf(q.y - sgn * pl[j].y) + fabsf(q.z - sgn * pl[j].z);
+                seen = seen || dn * r + fabsf(q.w - sgn * pl[j].w) < 2.0e-5f;
+            }
+            if (seen) continue;
+            if (cnt == GD_CELL_PLANES) overflow = true; else pl[cnt++] = q;
+        }
+        if (overflow || sp == 0) break;
+        node = stack[--sp];
+    }
+    if (overflow) { cell_ref[i] = 0u; return; }
+    if (cnt == 0) { cell_ref[i] = 15u; return; }
+    const unsigned slot = atomicAdd(counter, 1u);
+    if (slot >= capacity) { cell_ref[i] = 0u; return; }
+    for (int k = 0; k < cnt; ++k) planes[(size_t)slot * GD_CELL_PLANES + k] = pl[k];
+    cell_ref[i] = (slot << 4) | (unsigned)cnt;
+}
+

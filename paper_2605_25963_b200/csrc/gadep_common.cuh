@@ -70,10 +70,20 @@ struct __align__(32) GdNode8 {
 // surfaces but the world boundary; a cell holds a lower bound of the distance from any of its points to any facet, in
 // units of h / 4 (0 = unknown / a facet may be near).  A flight that ends before that distance cannot meet a facet, so
 // its nearest-hit query is answered ("none") without touching the BVH -- the answer the traversal would give.
+#define GD_CELL_PLANES 8           // plane slots per listed cell
 struct GdGrid {
     const unsigned char *cells;     // [nz][ny][nx], nullptr = no grid
     float lox, loy, loz, inv_h, quarter_h;
     int nx, ny, nz;
+    // Plane lists of the cells near facets (gd_k_grid_planes): every facet that comes within `reach` of the cell lies in
+    // one of the listed planes, so for a point p of the cell min(reach, min_k |n_k . (p - centre) + d_k|) is a lower bound
+    // of the distance to any facet (a triangle is never nearer than its plane) -- it resolves the tiny steps of a
+    // scattering chain inside a thin layer or beside a wall, where the cell's scalar clearance is zero.
+    // cell_ref[cell] = list index << 4 | number of planes (15 = no facet within reach; 0 = no list: too many planes, or
+    // the scalar is good enough); planes[list index * GD_CELL_PLANES + k] = (n, d_k) with the cell centre as origin.
+    const unsigned *cell_ref;       // nullptr = no lists
+    const float4 *planes;
+    float h, reach;
 };
 
 struct GdBvh {

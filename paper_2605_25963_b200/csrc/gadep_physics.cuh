@@ -103,19 +103,40 @@ GD_HD float gd_sample_compton(GdRng &g, float e, float &cos_t) {
 }
 
 // O11: Thomson (1 + cos^2) law by exact inversion of the CDF (3c + c^3 + 4)/8
+// (the two cube roots of Cardano's formula multiply to -1: one cube root and one reciprocal, taken on the side without
+// cancellation)
 GD_HD float gd_thomson_from(float u) {
-    float c = 8.0f * u - 4.0f;
-    float r = sqrtf(0.25f * c * c + 1.0f);
-    return cbrtf(0.5f * c + r) + cbrtf(0.5f * c - r);
+    const float q = 4.0f * u - 2.0f;
+    const float a = cbrtf(sqrtf(q * q + 1.0f) + fabsf(q));
+    return copysignf(a - 1.0f / a, q);
 }
 
-// lower bound of the distance from p to the nearest facet, from the clearance grid (0 = unknown)
-GD_D float gd_clearance(const GdGrid &g, const GdVec3 &p) {
-    if (!g.cells) return 0.0f;
-    const int ix = (int)floorf((p.x - g.lox) * g.inv_h), iy = (int)floorf((p.y - g.loy) * g.inv_h),
-              iz = (int)floorf((p.z - g.loz) * g.inv_h);
-    if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) return 0.0f;
-    return (float)__ldg(g.cells + ((size_t)iz * g.ny + iy) * g.nx + ix) * g.quarter_h;
+// "No facet within the flight of length s from p" decided on the clearance grid alone (true = certain, false = ask the
+// BVH): s (+ the float32 slack of s, of the cell lookup and of the plane distances) is shorter than the clearance of
+// p's cell, or -- where that scalar is too small -- than the distance from p to every plane of the cell's list and
+// than the list's reach.
+GD_D bool gd_flight_clear(const GdGrid &g, const GdVec3 &p, float s) {
+    if (!g.cells) return false;
+    const float need = fmaf(s, 1.0001f, 4.0f * GD_TBACK);
+    const float fx = floorf((p.x - g.lox) * g.inv_h), fy = floorf((p.y - g.loy) * g.inv_h), fz = floorf((p.z - g.loz) * g.inv_h);
+    const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
+    if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) return false;
+    const size_t cell = ((size_t)iz * g.ny + iy) * g.nx + ix;
+    if (need < (float)__ldg(g.cells + cell) * g.quarter_h) return true;
+    if (!g.cell_ref || !(need < g.reach)) return false;
+    const unsigned ref = __ldg(g.cell_ref + cell);
+    const unsigned cnt = ref & 15u;
+    if (cnt == 0u) return false;
+    if (cnt == 15u) return true;
+    const float rx = p.x - fmaf(fx + 0.5f, g.h, g.lox), ry = p.y - fmaf(fy + 0.5f, g.h, g.loy), rz = p.z - fmaf(fz + 0.5f, g.h, g.loz);
+    const float4 *pl = g.planes + (size_t)(ref >> 4) * GD_CELL_PLANES;
+    float lb = g.reach;
+#pragma unroll 1
+    for (unsigned k = 0; k < cnt; ++k) {
+        const float4 q = __ldg(pl + k);
+        lb = fminf(lb, fabsf(fmaf(q.x, rx, fmaf(q.y, ry, fmaf(q.z, rz, q.w)))));
+    }
+    return need < lb;
 }
 
 struct GdHistory {

@@ -22,7 +22,9 @@
 #include "gadep_trav.cuh"
 #include "gadep_transport_kernels.cuh"
 
+#ifndef GD_W_THREADS
 #define GD_W_THREADS 384
+#endif
 #define GD_W_WARPS (GD_W_THREADS / 32)
 #define GD_W_NSLOT 1024           // photon slots per block (64 per warp)
 // fields per slot.  25 words keep the block's shared memory under the 164 KB carve-out for up to 9 materials, which
@@ -64,6 +66,9 @@ struct GdWaveTune {
 // ---- block-wide queue of slot numbers (multi-producer, multi-consumer, warp-granular).  Tickets count up for ever;
 // ticket k lives in entry k mod GD_W_NSLOT and carries the lap number (k / GD_W_NSLOT) mod 32 beside the valid bit, so
 // a consumer can tell the entry it waits for from the previous lap's entry that its owner has not emptied yet.
+#define GD_Q_READY 0
+#define GD_Q_RESULT 1
+#define GD_Q_SLOW 2
 struct GdQueue {
     unsigned head, tail;                      // consumers have claimed tickets < head, producers hold tickets < tail
     unsigned short ent[GD_W_NSLOT];           // 0 = empty, else 0x8000 | lap << 10 | slot
@@ -88,6 +93,12 @@ GD_D void gd_q_push(GdQueue *q, bool push, int slot, unsigned lane) {
         GD_FENCE_BLOCK();                    // slot words before the valid bit
         *e = (unsigned short)(gd_q_tag(ticket) | (unsigned)slot);
     }
+}
+// every lane with dest >= 0 appends its slot to queue q0[dest]: one copy of the push code for all destinations (the
+// kernel is bound by instruction fetch)
+GD_D void gd_q_push_to(GdQueue *q0, int n_queues, int dest, int slot, unsigned lane) {
+#pragma unroll 1
+    for (int k = 0; k < n_queues; ++k) gd_q_push(q0 + k, dest == k, slot, lane);
 }
 // up to `want` entries for the lanes with `free` set (lowest lanes first); returns how many were claimed (warp-uniform)
 // and sets slot for the lanes that got one (got = true)
@@ -273,6 +284,7 @@ struct GdBlk {
     const float *tab;                          // attenuation tables
     const GdSource *src;
     unsigned *spec, *emitted, *peak, *cnt;     // per-block tallies and event counters
+    GdQueue *q;                                // q[GD_Q_READY], q[GD_Q_RESULT], q[GD_Q_SLOW]
     GdQueue *ready, *result, *slow;
     GdHistPool *hist;
     unsigned *live;                            // slots that still carry or may get a history
@@ -367,12 +379,11 @@ GD_PASS void gd_general_pass(const GdBlk &B, const GdBvh &bvh, const GdMaterials
         int filter;
         gd_lane_query(L, M, B.tab, t_min, t_max, filter);
         if (L.mode == GD_MODE_FLIGHT && L.sdist < GD_INF)
-            skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
+            skip = gd_flight_clear(bvh.grid, L.pos, L.sdist);
         gd_slot_store(sl, s, L, A.first);
         if (skip) { C.n_skip++; GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
     }
-    gd_q_push(B.ready, live_lane && !skip, s, lane);
-    gd_q_push(B.result, live_lane && skip, s, lane);
+    gd_q_push_to(B.q, 2, live_lane ? (skip ? GD_Q_RESULT : GD_Q_READY) : -1, s, lane);
 }
 
 // ============================================================ chain burst: crossings and coherent events
@@ -433,7 +444,7 @@ GD_PASS void gd_chain_burst(const GdBlk &B, const GdBvh &bvh, const GdMaterials 
                 float t_min, t_max;
                 int filter;
                 gd_lane_query(L, M, B.tab, t_min, t_max, filter);
-                if (L.sdist < GD_INF) skip = fmaf(L.sdist, 1.0001f, 4.0f * GD_TBACK) < gd_clearance(bvh.grid, L.pos);
+                if (L.sdist < GD_INF) skip = gd_flight_clear(bvh.grid, L.pos, L.sdist);
                 to_ready = !skip;
             }
         }
@@ -445,9 +456,8 @@ GD_PASS void gd_chain_burst(const GdBlk &B, const GdBvh &bvh, const GdMaterials 
             gd_slot_store(sl, s, L, A.first);
             if (known) { GD_SF(22) = L.sdist; GD_SF(23) = __int_as_float(GD_NO_FACET); GD_SF(24) = 0.0f; }
         }
-        if (!go) { gd_q_push(B.result, has, s, lane); break; }
-        gd_q_push(B.slow, to_slow, s, lane);
-        gd_q_push(B.ready, to_ready, s, lane);
+        gd_q_push_to(B.q, 3, !go ? (has ? GD_Q_RESULT : -1) : (to_slow ? GD_Q_SLOW : (to_ready ? GD_Q_READY : -1)), s, lane);
+        if (!go) break;
         has = skip;
         if (skip) { C.n_skip++; dirty = true; hit.t = L.sdist; hit.leaf = -1; hit.orig = GD_NO_FACET; hit.mats = 0; }
     }
@@ -465,8 +475,7 @@ GD_D int gd_trav_service(GdTrav &T, const GdBlk &B, const GdBvh &bvh, int *stack
         GD_SF(22) = T.t; GD_SF(23) = __int_as_float(T.orig); GD_SF(24) = __int_as_float(T.fromto);
         slow = T.filter == -2 || (T.orig == GD_NO_FACET ? !(T.t < GD_INF) : (T.fromto >> 16) == GD_MAT_KILL);
     }
-    gd_q_push(B.result, done_l && !slow, T.slot, lane);
-    gd_q_push(B.slow, done_l && slow, T.slot, lane);
+    gd_q_push_to(B.q + GD_Q_RESULT, 2, done_l ? (slow ? 1 : 0) : -1, T.slot, lane);
     if (done_l) T.slot = -1;
     bool got = false;
     int s = 0;
@@ -493,7 +502,8 @@ GD_D int gd_trav_service(GdTrav &T, const GdBlk &B, const GdBvh &bvh, int *stack
     __shared__ GdSource s_src;                                                                                   \
     __shared__ unsigned s_emitted[GD_MAX_LINES], s_peak[GD_MAX_LINES];                                           \
     __shared__ unsigned s_cnt[12];                                                                               \
-    __shared__ GdQueue s_ready, s_result, s_slow;                                                                \
+    __shared__ GdQueue s_q[3];                                                                                   \
+    GdQueue &s_ready = s_q[GD_Q_READY], &s_result = s_q[GD_Q_RESULT], &s_slow = s_q[GD_Q_SLOW];                    \
     __shared__ GdHistPool s_hist;                                                                                \
     __shared__ unsigned s_live;                                                                                  \
     const int n_tab = M.n_mat * 4 * M.n_grid;                                                                    \
@@ -519,7 +529,7 @@ GD_D int gd_trav_service(GdTrav &T, const GdBlk &B, const GdBvh &bvh, int *stack
     __syncthreads();                                                                                             \
     GdBlk B;                                                                                                     \
     B.sl = sl; B.tab = s_tab; B.src = &s_src; B.spec = s_spec; B.emitted = s_emitted; B.peak = s_peak; B.cnt = s_cnt; \
-    B.ready = &s_ready; B.result = &s_result; B.slow = &s_slow; B.hist = &s_hist; B.live = &s_live;              \
+    B.q = s_q; B.ready = &s_ready; B.result = &s_result; B.slow = &s_slow; B.hist = &s_hist; B.live = &s_live;              \
     B.pair = pair_buf + (size_t)blockIdx.x * GD_W_NSLOT * 8;                                                     \
     GdRunArgs A;                                                                                                 \
     A.first = first; A.n_hist = n_hist; A.seed = seed; A.edep_out = edep_out; A.flags_out = flags_out;          \
@@ -610,6 +620,9 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
             if (live == 0u) break;               // every slot of the block is dead
             __nanosleep(idle_ns);                // other warps hold all the work there is: back off
             if (idle_ns < 4000u) idle_ns *= 2u;
+#ifdef GD_PROF
+            { const long long t1 = clock64(); GD_PROF_ADD(8, t1 - p_t0); p_t0 = t1; }
+#endif
             continue;
         }
         idle_ns = 250u;
@@ -680,11 +693,13 @@ gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, 
 // Warp-specialised variant (GADEP_RUN_WARP_SPECIALISED): GD_WS_TWARPS lean traversal warps that only run the BVH loop
 // and GD_WS_PWARPS physics warps that only run the chain bursts and general passes, on the same block-wide queues.
 // setmaxnreg moves registers from the former to the latter.  Same results, bit for bit.
+#ifndef GD_WS_TWARPS
 #define GD_WS_TWARPS 16
 #define GD_WS_PWARPS 8
-#define GD_WS_THREADS (32 * (GD_WS_TWARPS + GD_WS_PWARPS))
 #define GD_WS_REGS_T 56
 #define GD_WS_REGS_P 128
+#endif
+#define GD_WS_THREADS (32 * (GD_WS_TWARPS + GD_WS_PWARPS))
 // what the traversal warps give up must cover what the physics warps take, or the physics warps wait for ever
 static_assert((65536 / GD_WS_THREADS / 8 * 8 - GD_WS_REGS_T) * GD_WS_TWARPS >= (GD_WS_REGS_P - 65536 / GD_WS_THREADS / 8 * 8) * GD_WS_PWARPS,
               "register budget of the warp-specialised kernel does not balance");
