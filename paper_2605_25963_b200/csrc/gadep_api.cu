@@ -408,45 +408,45 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
             g.nx = dim[0]; g.ny = dim[1]; g.nz = dim[2];
             g.lox = (float)(c->roi_lo[0] - h); g.loy = (float)(c->roi_lo[1] - h); g.loz = (float)(c->roi_lo[2] - h);
             g.inv_h = (float)(1.0 / h); g.quarter_h = (float)(0.25 * h * (1.0 - 1e-6));
-            g.h = (float)h; g.reach = 0.0f; g.cell_ref = nullptr; g.planes = nullptr;
+            g.h = (float)h; g.reach = 0.0f; g.info = nullptr; g.planes = nullptr;
             const size_t nc = (size_t)g.nx * g.ny * g.nz;
             unsigned char *occ = nullptr, *cells = nullptr;
             unsigned short *d2 = nullptr;
+            unsigned *lc = nullptr, *info = nullptr;
+            float4 *planes = nullptr;
             if ((e = gd_pool_get(c, 14, nc, (void **)&occ)) != cudaSuccess) break;
             if ((e = gd_pool_get(c, 15, 2 * nc, (void **)&d2)) != cudaSuccess) break;
             if ((e = gd_pool_get(c, 16, nc, (void **)&cells)) != cudaSuccess) break;
-            g.cells = cells;
+            if ((e = gd_pool_get(c, 17, 16, (void **)&lc)) != cudaSuccess) break;
+            if ((e = gd_pool_get(c, 18, 4 * nc, (void **)&info)) != cudaSuccess) break;
             cudaMemsetAsync(occ, 0, nc, st);
+            cudaMemsetAsync(lc, 0, 16, st);
             if (n >= (1 << 16)) gd_k_grid_mark<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, g, occ, 1);
             else gd_k_grid_mark<<<(unsigned)(((size_t)n * 32 + tb - 1) / tb), tb, 0, st>>>(ref_lo, ref_hi, n, g, occ, 0);
             gd_k_grid_dt_x<<<(g.ny * g.nz + 127) / 128, 128, 0, st>>>(g, occ);
             gd_k_grid_dt_y<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, occ, d2);
             gd_k_grid_dt_z<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, d2, cells);
             launches += 4;
-            // plane lists for the cells whose scalar clearance is below the reach
+            // plane lists for the cells whose scalar clearance is below the reach; sized by a count of those cells
             c->n_list_cells = 0; c->n_listed = 0;
+            unsigned thr = 0, n_list = 0;
             if (c->list_reach_cells > 0.0 && n > 1) {
-                const float reach = (float)(c->list_reach_cells * h);
-                const unsigned thr = (unsigned)std::min(255.0, std::ceil((double)reach / (double)g.quarter_h));
-                unsigned *lc = nullptr, *cell_ref = nullptr;
-                float4 *planes = nullptr;
-                if ((e = gd_pool_get(c, 17, 16, (void **)&lc)) != cudaSuccess) break;
-                cudaMemsetAsync(lc, 0, 16, st);
+                g.reach = (float)(c->list_reach_cells * h);
+                thr = (unsigned)std::min(255.0, std::ceil((double)g.reach / (double)g.quarter_h));
                 gd_k_grid_list_count<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(cells, nc, thr, lc);
-                unsigned n_list = 0;
                 if ((e = cudaMemcpyAsync(&n_list, lc, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
                 if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
                 launches += 1;
-                if (n_list > 0 && n_list < (1u << 28)) {
-                    if ((e = gd_pool_get(c, 18, 4 * nc, (void **)&cell_ref)) != cudaSuccess) break;
-                    if ((e = gd_pool_get(c, 19, sizeof(float4) * GD_CELL_PLANES * (size_t)n_list, (void **)&planes)) != cudaSuccess) break;
-                    g.reach = reach; g.cell_ref = cell_ref; g.planes = planes;
-                    gd_k_grid_planes<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(g, cells, thr, c->d_nodes4, c->d_leaf_tris, cell_ref, planes, lc + 1, n_list);
-                    launches += 1;
-                    c->n_list_cells = n_list;
-                    if ((e = cudaMemcpyAsync(&c->n_listed, lc + 1, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
-                }
+                n_list = std::min(n_list, 1u << 24);
+                if (n_list == 0) { thr = 0; g.reach = 0.0f; }
+                else if ((e = gd_pool_get(c, 19, sizeof(float4) * GD_CELL_PLANES * (size_t)n_list, (void **)&planes)) != cudaSuccess) break;
             }
+            g.planes = planes;
+            gd_k_grid_planes<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(g, cells, thr, c->d_nodes4, c->d_leaf_tris, info, planes, lc + 1, n_list);
+            launches += 1;
+            g.info = info;
+            c->n_list_cells = n_list;
+            if ((e = cudaMemcpyAsync(&c->n_listed, lc + 1, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
             c->grid = g;
         }
         cudaEventRecord(c->evb1, st);

@@ -613,12 +613,13 @@ __global__ void gd_k_grid_dt_z(GdGrid g, const unsigned short *__restrict__ d2, 
     out[i] = (unsigned char)fminf(fmaxf(floorf(cl * 4.0f), 0.0f), 255.0f);
 }
 
-// ---- plane lists of the cells near facets (GdGrid::cell_ref / planes).  One thread per cell whose scalar clearance is
-// below `thr` (= the reach in units of h / 4): a box query of the 4-wide hierarchy with the cell dilated by the reach
-// collects the facets that can come within reach of a point of the cell (every reference box that overlaps the dilated
-// cell; a facet whose plane passes farther than reach + half a cell diagonal from the centre is dropped), their planes
-// are computed in double from the float32 vertices, referred to the cell centre and merged when they agree to 2e-5 mm
-// over the cell.  More than GD_CELL_PLANES distinct planes, or a query that runs out of stack: no list (the BVH answers).
+// ---- the cells' 32-bit words (GdGrid::info) and the plane lists of the cells near facets.  One thread per cell.  A cell
+// whose scalar clearance is below `thr` (= the reach in units of h / 4; 0 = no lists) gets a list: a box query of the
+// 4-wide hierarchy with the cell dilated by the reach collects the facets that can come within reach of a point of the
+// cell (every reference box that overlaps the dilated cell; a facet whose plane passes farther than reach + half a cell
+// diagonal from the centre is dropped), their planes are computed in double from the float32 vertices, referred to the
+// cell centre and merged when they agree to 2e-5 mm over the cell.  More than GD_CELL_PLANES distinct planes, or a query
+// that runs out of stack: no list (the BVH answers).
 __global__ void gd_k_grid_list_count(const unsigned char *__restrict__ cells, size_t n, unsigned thr, unsigned *count) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool want = i < n && cells[i] < thr;
@@ -627,12 +628,14 @@ __global__ void gd_k_grid_list_count(const unsigned char *__restrict__ cells, si
 }
 __global__ void __launch_bounds__(128)
 gd_k_grid_planes(GdGrid g, const unsigned char *__restrict__ cells, unsigned thr, const GdNode4 *__restrict__ nodes4,
-                 const GdTri *__restrict__ tris, unsigned *__restrict__ cell_ref, float4 *__restrict__ planes,
+                 const GdTri *__restrict__ tris, unsigned *__restrict__ info, float4 *__restrict__ planes,
                  unsigned *counter, unsigned capacity) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t n = (size_t)g.nx * g.ny * g.nz;
     if (i >= n) return;
-    if (cells[i] >= thr) { cell_ref[i] = 0u; return; }
+    const unsigned scalar = cells[i];
+    info[i] = scalar;
+    if (scalar >= thr) return;
     const int ix = (int)(i % g.nx), iy = (int)((i / g.nx) % g.ny), iz = (int)(i / ((size_t)g.nx * g.ny));
     // the centre exactly as gd_flight_clear computes it
     const float cx = fmaf((float)ix + 0.5f, g.h, g.lox), cy = fmaf((float)iy + 0.5f, g.h, g.loy), cz = fmaf((float)iz + 0.5f, g.h, g.loz);
@@ -681,11 +684,11 @@ gd_k_grid_planes(GdGrid g, const unsigned char *__restrict__ cells, unsigned thr
         if (overflow || sp == 0) break;
         node = stack[--sp];
     }
-    if (overflow) { cell_ref[i] = 0u; return; }
-    if (cnt == 0) { cell_ref[i] = 15u; return; }
+    if (overflow) return;
+    const unsigned low = scalar < 7u ? scalar : 7u;          // the scalar bound stays valid rounded down
+    if (cnt == 0) { info[i] = GD_CELL_LIST | (15u << 3) | low; return; }
     const unsigned slot = atomicAdd(counter, 1u);
-    if (slot >= capacity) { cell_ref[i] = 0u; return; }
+    if (slot >= capacity || slot >= (1u << 24)) return;
     for (int k = 0; k < cnt; ++k) planes[(size_t)slot * GD_CELL_PLANES + k] = pl[k];
-    cell_ref[i] = (slot << 4) | (unsigned)cnt;
+    info[i] = GD_CELL_LIST | (slot << 7) | ((unsigned)cnt << 3) | low;
 }
-

@@ -66,25 +66,26 @@ struct __align__(32) GdNode8 {
 };
 #define GD_STACK8 224               // 8-wide traversal: up to 7 pushes per node visited; overflow is detected and reported
 
-// Facet-clearance grid (built by gadep_build_bvh beside the hierarchy): uniform cells of edge h over the box of all
-// surfaces but the world boundary; a cell holds a lower bound of the distance from any of its points to any facet, in
-// units of h / 4 (0 = unknown / a facet may be near).  A flight that ends before that distance cannot meet a facet, so
-// its nearest-hit query is answered ("none") without touching the BVH -- the answer the traversal would give.
 #define GD_CELL_PLANES 8           // plane slots per listed cell
+// Facet-clearance grid (built by gadep_build_bvh beside the hierarchy): uniform cells of edge h over the box of all
+// surfaces but the world boundary.  One 32-bit word per cell:
+//   bit 31 clear: bits 0-7 = lower bound of the distance from any point of the cell to any facet, in units of h / 4
+//                 (0 = unknown / a facet may be near).  A flight that ends before that distance cannot meet a facet, so
+//                 its nearest-hit query is answered ("none") without touching the BVH -- the answer the traversal gives.
+//   bit 31 set:   the cell lies near facets and has a plane list: bits 0-2 = the scalar bound as above, bits 3-6 = number
+//                 of planes (15 = no facet within reach), bits 7-30 = list index.  Every facet that comes within `reach`
+//                 of the cell lies in one of the listed planes, so for a point p of the cell
+//                 min(reach, min_k |n_k . (p - centre) + d_k|) is a lower bound of the distance to any facet (a triangle
+//                 is never nearer than its plane) -- it resolves the tiny steps of a scattering chain inside a thin layer
+//                 or beside a wall, where the scalar is zero.  planes[index * GD_CELL_PLANES + k] = (n_k, d_k), cell
+//                 centre as origin.
 struct GdGrid {
-    const unsigned char *cells;     // [nz][ny][nx], nullptr = no grid
-    float lox, loy, loz, inv_h, quarter_h;
-    int nx, ny, nz;
-    // Plane lists of the cells near facets (gd_k_grid_planes): every facet that comes within `reach` of the cell lies in
-    // one of the listed planes, so for a point p of the cell min(reach, min_k |n_k . (p - centre) + d_k|) is a lower bound
-    // of the distance to any facet (a triangle is never nearer than its plane) -- it resolves the tiny steps of a
-    // scattering chain inside a thin layer or beside a wall, where the cell's scalar clearance is zero.
-    // cell_ref[cell] = list index << 4 | number of planes (15 = no facet within reach; 0 = no list: too many planes, or
-    // the scalar is good enough); planes[list index * GD_CELL_PLANES + k] = (n, d_k) with the cell centre as origin.
-    const unsigned *cell_ref;       // nullptr = no lists
+    const unsigned *info;           // [nz][ny][nx], nullptr = no grid
     const float4 *planes;
-    float h, reach;
+    float lox, loy, loz, inv_h, quarter_h, h, reach;
+    int nx, ny, nz;
 };
+#define GD_CELL_LIST 0x80000000u
 
 struct GdBvh {
     GdGrid grid;

@@ -116,23 +116,22 @@ GD_HD float gd_thomson_from(float u) {
 // p's cell, or -- where that scalar is too small -- than the distance from p to every plane of the cell's list and
 // than the list's reach.
 GD_D bool gd_flight_clear(const GdGrid &g, const GdVec3 &p, float s) {
-    if (!g.cells) return false;
+    if (!g.info) return false;
     const float need = fmaf(s, 1.0001f, 4.0f * GD_TBACK);
     const float fx = floorf((p.x - g.lox) * g.inv_h), fy = floorf((p.y - g.loy) * g.inv_h), fz = floorf((p.z - g.loz) * g.inv_h);
     const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
     if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) return false;
-    const size_t cell = ((size_t)iz * g.ny + iy) * g.nx + ix;
-    if (need < (float)__ldg(g.cells + cell) * g.quarter_h) return true;
-    if (!g.cell_ref || !(need < g.reach)) return false;
-    const unsigned ref = __ldg(g.cell_ref + cell);
-    const unsigned cnt = ref & 15u;
-    if (cnt == 0u) return false;
+    const unsigned w = __ldg(g.info + ((size_t)iz * g.ny + iy) * g.nx + ix);
+    if (!(w & GD_CELL_LIST)) return need < (float)w * g.quarter_h;
+    if (need < (float)(w & 7u) * g.quarter_h) return true;
+    if (!(need < g.reach)) return false;
+    const unsigned cnt = (w >> 3) & 15u;
     if (cnt == 15u) return true;
     const float rx = p.x - fmaf(fx + 0.5f, g.h, g.lox), ry = p.y - fmaf(fy + 0.5f, g.h, g.loy), rz = p.z - fmaf(fz + 0.5f, g.h, g.loz);
-    const float4 *pl = g.planes + (size_t)(ref >> 4) * GD_CELL_PLANES;
+    const float4 *pl = g.planes + (size_t)((w >> 7) & 0xFFFFFFu) * GD_CELL_PLANES;
     float lb = g.reach;
 #pragma unroll 1
-    for (unsigned k = 0; k < cnt; ++k) {
+    for (unsigned k = 0; k < cnt; ++k) {                     // one 128-byte line: the first load brings the others
         const float4 q = __ldg(pl + k);
         lb = fminf(lb, fabsf(fmaf(q.x, rx, fmaf(q.y, ry, fmaf(q.z, rz, q.w)))));
     }
