@@ -87,8 +87,14 @@ int gadep_load_mesh(gadep_ctx *ctx, const float *vertices, int n_vert, const int
                     int n_tri, const int *surf_inside, const int *surf_outside, int n_surf, int world_material);
 
 /* Builds the BVH over the facets on the GPU: binary LBVH -> uncompressed 4-wide nodes (default
- * traversal) and 8-wide nodes with 8-bit quantised child boxes (measured alternative).
- * flags: 0.  Timed by bench.py. */
+ * traversal) and 8-wide nodes with 8-bit quantised child boxes (measured alternative), and the
+ * facet-clearance grid beside it (flights that provably meet no facet need no traversal; same answers).
+ * flags: 0, or one of the two below.  The grid's plane lists (cells near facets; 2 - 3 ms for 40 k facets, they pay on long
+ * runs of volume sources) are made by the first gadep_run of >= 2e7 histories after the build (flags 0), with the build
+ * (GADEP_BUILD_PLANE_LISTS) or never (GADEP_BUILD_NO_PLANE_LISTS).  No result depends on the choice.  Timed by bench.py;
+ * the time of lists made by a run is added to last_build_ms. */
+#define GADEP_BUILD_PLANE_LISTS 1
+#define GADEP_BUILD_NO_PLANE_LISTS 2
 int gadep_build_bvh(gadep_ctx *ctx, int flags);
 
 /* Node width the wavefront kernels and gadep_trace_rays traverse: 4 (default; uncompressed nodes) or 8 (compressed
@@ -256,6 +262,8 @@ typedef struct {
                                            /* run that sees one fails with GADEP_E_ARG)                              */
     unsigned long long n_parity_queries;   /* GADEP_RUN_PARITY_LOCALISATION: all-hits localisation queries       */
     unsigned long long n_parity_mismatch;  /* ... of which the parity rule and the side ids named different media */
+    unsigned n_grid_list_cells;            /* clearance grid: cells near facets (scalar bound below the lists' reach) ...  */
+    unsigned n_grid_lists;                 /* ... of which got a plane list (0 = no lists made since the last build)      */
 } gadep_counters;
 /* Counters of the last gadep_run / gadep_run_histories / gadep_trace_rays (HOST output). */
 int gadep_get_counters(const gadep_ctx *ctx, gadep_counters *out);

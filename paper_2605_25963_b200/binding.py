@@ -22,6 +22,7 @@ RUN_PARTIAL_XS = 32
 RUN_WARP_SPECIALISED = 64
 RUN_BVH8 = 256
 RUN_ELECTRON_RANGE = 128
+BUILD_PLANE_LISTS, BUILD_NO_PLANE_LISTS = 1, 2
 
 EXPORTED_SYMBOLS = ("gadep_create", "gadep_destroy", "gadep_last_error", "gadep_set_materials", "gadep_load_mesh",
                     "gadep_build_bvh", "gadep_set_source", "gadep_run", "gadep_fepe", "gadep_trace_rays",
@@ -55,7 +56,8 @@ class GadepCounters(C.Structure):
                 ("n_bvh_nodes", C.c_int), ("bvh_max_depth", C.c_int), ("last_run_ms", C.c_float),
                 ("last_build_ms", C.c_float), ("last_run_launches", C.c_int), ("last_build_launches", C.c_int),
                 ("n_skipped_queries", C.c_ulonglong), ("n_stack_overflow", C.c_ulonglong),
-                ("n_parity_queries", C.c_ulonglong), ("n_parity_mismatch", C.c_ulonglong)]
+                ("n_parity_queries", C.c_ulonglong), ("n_parity_mismatch", C.c_ulonglong),
+                ("n_grid_list_cells", C.c_uint), ("n_grid_lists", C.c_uint)]
 
     def as_dict(self):
         d = {n: int(getattr(self, n)) for n, _ in self._fields_[:12]}
@@ -65,7 +67,8 @@ class GadepCounters(C.Structure):
                  last_run_ms=float(self.last_run_ms), last_build_ms=float(self.last_build_ms),
                  last_run_launches=int(self.last_run_launches), last_build_launches=int(self.last_build_launches),
                  n_skipped_queries=int(self.n_skipped_queries), n_stack_overflow=int(self.n_stack_overflow),
-                 n_parity_queries=int(self.n_parity_queries), n_parity_mismatch=int(self.n_parity_mismatch))
+                 n_parity_queries=int(self.n_parity_queries), n_parity_mismatch=int(self.n_parity_mismatch),
+                 n_grid_list_cells=int(self.n_grid_list_cells), n_grid_lists=int(self.n_grid_lists))
         return d
 
 
@@ -196,13 +199,13 @@ class Gadep:
         self._check(self.L.gadep_set_source(self.h, C.byref(s)))
         self.n_lines = le.shape[0]
 
-    def load_workload(self, w, build=True):
+    def load_workload(self, w, build=True, build_flags=0):
         """Convenience: all set-up calls for a detmesh.Workload-like object."""
         self.set_materials(w.mu, w.is_scoring, w.e_min_mev, w.e_max_mev)
         m = w.mesh
         self.load_mesh(m.vertices, m.triangles, m.tri_surface, m.surf_inside, m.surf_outside, m.world_material)
         if build:
-            self.build_bvh()
+            self.build_bvh(build_flags)
         self.set_source(**w.source)
         if getattr(w, "notes", None) and w.notes.get("source_copies") is not None:
             self.set_source_copies(w.notes["source_copies"])

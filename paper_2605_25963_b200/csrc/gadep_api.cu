@@ -47,8 +47,8 @@ struct gadep_ctx {
     // [6..9] the mesh copies (vertices, triangles, side materials, surface ids)
     // [10..12] mesh validation: edge table keys, edge table surfaces, error record + surface sides
     // [14] clearance grid: marks / x distances [15] squared distances after the y pass [16] the grid itself
-    void *pool[20] = {};
-    size_t pool_cap[20] = {};
+    void *pool[21] = {};
+    size_t pool_cap[21] = {};
     // source
     bool have_src = false;
     GdSource src;
@@ -76,6 +76,11 @@ struct gadep_ctx {
     bool have_roi = false;
     long long grid_cells = 1ll << 22;         // GADEP_GRID_CELLS overrides; 0 = no grid
     double list_reach_cells = 1.0;            // reach of the cells' plane lists in cells; GADEP_GRID_REACH overrides, 0 = no lists
+    unsigned long long list_min_hist = 20000000ull;   // GADEP_BUILD default: lists are made by the first run of at least this many
+                                              // histories after a build (GADEP_LIST_MIN_HISTORIES overrides)
+    int list_policy = 0;                      // build flags of the last gadep_build_bvh: 0 by run size, 1 built with the BVH, 2 never
+    bool lists_built = false;
+    unsigned char *grid_scalar = nullptr;     // u8 scalar clearance of the last build (input of the list kernel)
     unsigned n_list_cells = 0, n_listed = 0;  // cells below the reach / cells that got a list (last build)
     GdGrid grid = {};
     bool cluster_surfaces = true;             // GADEP_NO_SURFACE_CLUSTERS=1 switches it off (measurement)
@@ -148,6 +153,7 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (const char *t = getenv("GADEP_WS")) c->prefer_ws = atoi(t) != 0;
     if (const char *t = getenv("GADEP_GRID_CELLS")) { long long v = atoll(t); if (v >= 0 && v <= (1ll << 28)) c->grid_cells = v; }
     if (const char *t = getenv("GADEP_GRID_REACH")) { double v = atof(t); if (v >= 0.0 && v <= 8.0) c->list_reach_cells = v; }
+    if (const char *t = getenv("GADEP_LIST_MIN_HISTORIES")) { long long v = atoll(t); if (v >= 0) c->list_min_hist = (unsigned long long)v; }
     if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,t_keep,n_steps,n_steps_max,p_min,t_help" (measurement sweeps)
         int a, b, d, dm = 0, p = c->tune.p_min, ts = c->tune.t_help;
         if (sscanf(t, "%d,%d,%d,%d,%d,%d", &a, &b, &d, &dm, &p, &ts) >= 4 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && dm >= d && dm <= 32 && p >= 1 && p <= 32 && ts >= 1 && ts <= 1024)
@@ -181,7 +187,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    for (int k = 0; k < 20; ++k) cudaFree(c->pool[k]);
+    for (int k = 0; k < 21; ++k) cudaFree(c->pool[k]);
     cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair); cudaFree(c->d_mat_entry);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -301,10 +307,60 @@ extern "C" int gadep_load_mesh(gadep_ctx *c, const float *vertices, int n_vert, 
     return GADEP_OK;
 }
 
+// ---------------------------------------------------------------- plane lists of the clearance grid
+// For the cells whose scalar clearance is below the reach (GdGrid, gd_k_grid_planes).  Costs 2 - 3 ms on the 40 k-facet
+// set-ups and pays on runs whose photons scatter in tiny steps beside walls (volume sources; 10 % of a 1e8-history run),
+// not on short point-source runs: so it runs with the build only when asked (GADEP_BUILD_PLANE_LISTS), otherwise before
+// the first run of at least list_min_hist histories.  Its time and launches are added to the build's.
+static int gd_build_plane_lists(gadep_ctx *c) {
+    if (c->lists_built || !c->have_bvh || !c->grid.info || !c->grid_scalar || c->n_ref < 2 || !(c->list_reach_cells > 0.0)) return GADEP_OK;
+    GD_CUDA(c, cudaSetDevice(c->device));
+    cudaStream_t st = c->stream;
+    GdGrid g = c->grid;
+    const size_t nc = (size_t)g.nx * g.ny * g.nz;
+    g.reach = (float)(c->list_reach_cells * (double)g.h);
+    const unsigned thr = (unsigned)std::min(255.0, std::ceil((double)g.reach / (double)g.quarter_h));
+    unsigned *lc = nullptr;
+    float4 *planes = nullptr, *nrm = nullptr;
+    GD_CUDA(c, gd_pool_get(c, 17, 16, (void **)&lc));
+    GD_CUDA(c, cudaEventRecord(c->evb0, st));
+    GD_CUDA(c, cudaMemsetAsync(lc, 0, 16, st));
+    gd_k_grid_list_count<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(c->grid_scalar, nc, thr, lc);
+    unsigned n_list = 0;
+    GD_CUDA(c, cudaMemcpyAsync(&n_list, lc, 4, cudaMemcpyDeviceToHost, st));
+    GD_CUDA(c, cudaStreamSynchronize(st));
+    c->lists_built = true;
+    n_list = std::min(n_list, 1u << 24);
+    // a mesh with more references than cells near facets (config 4: 4096 angular segments) has tens of facets around
+    // every such cell, hardly any cell gets by with GD_CELL_PLANES planes: no lists
+    if (n_list == 0 || (unsigned)c->n_ref > n_list) return GADEP_OK;
+    GD_CUDA(c, gd_pool_get(c, 19, sizeof(float4) * GD_CELL_PLANES * (size_t)n_list, (void **)&planes));
+    GD_CUDA(c, gd_pool_get(c, 20, sizeof(float4) * (size_t)c->n_ref, (void **)&nrm));
+    g.planes = planes;
+    gd_k_tri_normals<<<(c->n_ref + 255) / 256, 256, 0, st>>>(c->d_leaf_tris, c->n_ref, nrm);
+    gd_k_grid_planes<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(g, c->grid_scalar, thr, c->d_nodes4, c->d_leaf_tris, nrm,
+                                                                   (unsigned *)g.info, planes, lc + 1, n_list);
+    GD_CUDA(c, cudaEventRecord(c->evb1, st));
+    GD_CUDA(c, cudaGetLastError());
+    GD_CUDA(c, cudaMemcpyAsync(&c->n_listed, lc + 1, 4, cudaMemcpyDeviceToHost, st));
+    GD_CUDA(c, cudaStreamSynchronize(st));
+    float ms = 0.0f;
+    cudaEventElapsedTime(&ms, c->evb0, c->evb1);
+    c->last_build_ms += ms;
+    c->last_build_launches += 3;
+    c->n_list_cells = n_list;
+    c->grid = g;
+    if (getenv("GADEP_GRID_DEBUG"))
+        fprintf(stderr, "[gadep] grid %d x %d x %d, h %.4f mm, reach %.4f mm: %u cells below the reach, %u with a plane list, %.2f ms\n",
+                g.nx, g.ny, g.nz, g.h, g.reach, c->n_list_cells, c->n_listed, ms);
+    return GADEP_OK;
+}
+
 // ---------------------------------------------------------------- BVH build
 extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     if (!c) return GADEP_E_NULL;
-    if (flags != 0) return gd_fail(c, GADEP_E_ARG, "unknown build flags %d", flags);
+    if (flags != 0 && flags != GADEP_BUILD_PLANE_LISTS && flags != GADEP_BUILD_NO_PLANE_LISTS)
+        return gd_fail(c, GADEP_E_ARG, "unknown build flags %d", flags);
     if (!c->have_mesh) return gd_fail(c, GADEP_E_ORDER, "gadep_build_bvh before gadep_load_mesh");
     GD_CUDA(c, cudaSetDevice(c->device));
     const int n_tri = c->n_tri;
@@ -393,6 +449,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         }
         // ---- facet-clearance grid over the box of the inner surfaces
         c->grid = GdGrid{};
+        c->lists_built = false; c->n_list_cells = 0; c->n_listed = 0; c->grid_scalar = nullptr; c->list_policy = flags;
         if (c->grid_cells > 0 && c->have_roi) {
             double ext[3], vol = 1.0;
             for (int a = 0; a < 3; ++a) { ext[a] = std::max((double)c->roi_hi[a] - (double)c->roi_lo[a], 1e-3); vol *= ext[a]; }
@@ -412,41 +469,22 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
             const size_t nc = (size_t)g.nx * g.ny * g.nz;
             unsigned char *occ = nullptr, *cells = nullptr;
             unsigned short *d2 = nullptr;
-            unsigned *lc = nullptr, *info = nullptr;
-            float4 *planes = nullptr;
+            unsigned *info = nullptr;
             if ((e = gd_pool_get(c, 14, nc, (void **)&occ)) != cudaSuccess) break;
             if ((e = gd_pool_get(c, 15, 2 * nc, (void **)&d2)) != cudaSuccess) break;
             if ((e = gd_pool_get(c, 16, nc, (void **)&cells)) != cudaSuccess) break;
-            if ((e = gd_pool_get(c, 17, 16, (void **)&lc)) != cudaSuccess) break;
             if ((e = gd_pool_get(c, 18, 4 * nc, (void **)&info)) != cudaSuccess) break;
             cudaMemsetAsync(occ, 0, nc, st);
-            cudaMemsetAsync(lc, 0, 16, st);
             if (n >= (1 << 16)) gd_k_grid_mark<<<nb, tb, 0, st>>>(ref_lo, ref_hi, n, g, occ, 1);
             else gd_k_grid_mark<<<(unsigned)(((size_t)n * 32 + tb - 1) / tb), tb, 0, st>>>(ref_lo, ref_hi, n, g, occ, 0);
             gd_k_grid_dt_x<<<(g.ny * g.nz + 127) / 128, 128, 0, st>>>(g, occ);
             gd_k_grid_dt_y<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, occ, d2);
-            gd_k_grid_dt_z<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, d2, cells);
+            gd_k_grid_dt_z<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(g, d2, cells, info);
             launches += 4;
-            // plane lists for the cells whose scalar clearance is below the reach; sized by a count of those cells
-            c->n_list_cells = 0; c->n_listed = 0;
-            unsigned thr = 0, n_list = 0;
-            if (c->list_reach_cells > 0.0 && n > 1) {
-                g.reach = (float)(c->list_reach_cells * h);
-                thr = (unsigned)std::min(255.0, std::ceil((double)g.reach / (double)g.quarter_h));
-                gd_k_grid_list_count<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(cells, nc, thr, lc);
-                if ((e = cudaMemcpyAsync(&n_list, lc, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
-                if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
-                launches += 1;
-                n_list = std::min(n_list, 1u << 24);
-                if (n_list == 0) { thr = 0; g.reach = 0.0f; }
-                else if ((e = gd_pool_get(c, 19, sizeof(float4) * GD_CELL_PLANES * (size_t)n_list, (void **)&planes)) != cudaSuccess) break;
-            }
-            g.planes = planes;
-            gd_k_grid_planes<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(g, cells, thr, c->d_nodes4, c->d_leaf_tris, info, planes, lc + 1, n_list);
-            launches += 1;
+            // so far the cells' words hold scalar bounds only; the plane lists come with the build (GADEP_BUILD_PLANE_LISTS)
+            // or with the first large run (gd_build_plane_lists)
             g.info = info;
-            c->n_list_cells = n_list;
-            if ((e = cudaMemcpyAsync(&c->n_listed, lc + 1, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
+            c->grid_scalar = cells;
             c->grid = g;
         }
         cudaEventRecord(c->evb1, st);
@@ -454,9 +492,6 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) break;
         if (n > 1 && (e = cudaMemcpy(&depth, scene + 6, sizeof(int), cudaMemcpyDeviceToHost)) != cudaSuccess) break;
         cudaEventElapsedTime(&c->last_build_ms, c->evb0, c->evb1);
-        if (getenv("GADEP_GRID_DEBUG"))
-            fprintf(stderr, "[gadep] grid %d x %d x %d, h %.4f mm, reach %.4f mm: %u cells below the reach, %u with a plane list\n",
-                    c->grid.nx, c->grid.ny, c->grid.nz, c->grid.h, c->grid.reach, c->n_list_cells, c->n_listed);
         // per-material entry table: the surfaces that have the material on one side.  A surface without an entry node
         // (never for a closed surface of >= 2 references) or too many surfaces around one material -> root for it.
         c->have_entries = false;
@@ -487,6 +522,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     c->n_ref = n;
     c->last_build_launches = launches;
     c->have_bvh = true;
+    if (flags == GADEP_BUILD_PLANE_LISTS) return gd_build_plane_lists(c);
     return GADEP_OK;
 }
 
@@ -629,6 +665,10 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
             GD_CUDA(c, cudaMalloc(&c->d_pair, need * sizeof(float)));
             c->pair_floats = need;
         }
+    }
+    if ((variant == 2 || variant == 5) && c->list_policy == 0 && !c->lists_built && n >= c->list_min_hist) {
+        rc = gd_build_plane_lists(c);
+        if (rc) return rc;
     }
     GD_CUDA(c, cudaEventRecord(c->ev0, st));
     c->last_run_launches = 0;
@@ -947,6 +987,7 @@ extern "C" int gadep_get_counters(const gadep_ctx *cc, gadep_counters *out) {
     out->n_coherent = h.n_coherent; out->n_pair = h.n_pair; out->n_escaped = h.n_escaped; out->n_leak = h.n_leak;
     out->n_cutoff = h.n_cutoff; out->n_stack_overflow = c->n_stack_overflow; out->n_skipped_queries = h.n_skipped;
     out->n_parity_queries = h.n_parity; out->n_parity_mismatch = h.n_parity_mismatch;
+    out->n_grid_list_cells = c->n_list_cells; out->n_grid_lists = c->n_listed;
     memcpy(out->emitted, c->h_emitted, sizeof(out->emitted));
     memcpy(out->peak, c->h_peak, sizeof(out->peak));
     out->n_lines = c->src.n_lines * (c->src.n_copies > 0 ? c->src.n_copies : 1);

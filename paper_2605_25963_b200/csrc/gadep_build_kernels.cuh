@@ -595,7 +595,8 @@ __global__ void gd_k_grid_dt_y(GdGrid g, const unsigned char *__restrict__ gx, u
     (void)x;
     d2[i] = (unsigned short)best;
 }
-__global__ void gd_k_grid_dt_z(GdGrid g, const unsigned short *__restrict__ d2, unsigned char *__restrict__ out) {
+__global__ void gd_k_grid_dt_z(GdGrid g, const unsigned short *__restrict__ d2, unsigned char *__restrict__ out,
+                               unsigned *__restrict__ info) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t plane = (size_t)g.nx * g.ny, n = plane * g.nz;
     if (i >= n) return;
@@ -610,26 +611,42 @@ __global__ void gd_k_grid_dt_z(GdGrid g, const unsigned short *__restrict__ d2, 
     }
     // centre distance sqrt(best) cells; any two points of the two cells: at least sqrt(best) - sqrt(3) cells apart
     const float cl = sqrtf((float)best) * 0.999999f - 1.7320509f;
-    out[i] = (unsigned char)fminf(fmaxf(floorf(cl * 4.0f), 0.0f), 255.0f);
+    const unsigned char v = (unsigned char)fminf(fmaxf(floorf(cl * 4.0f), 0.0f), 255.0f);
+    out[i] = v;
+    info[i] = v;          // GdGrid::info: bit 31 clear = scalar bound only
 }
 
 // ---- the cells' 32-bit words (GdGrid::info) and the plane lists of the cells near facets.  One thread per cell.  A cell
 // whose scalar clearance is below `thr` (= the reach in units of h / 4; 0 = no lists) gets a list: a box query of the
 // 4-wide hierarchy with the cell dilated by the reach collects the facets that can come within reach of a point of the
 // cell (every reference box that overlaps the dilated cell; a facet whose plane passes farther than reach + half a cell
-// diagonal from the centre is dropped), their planes are computed in double from the float32 vertices, referred to the
-// cell centre and merged when they agree to 2e-5 mm over the cell.  More than GD_CELL_PLANES distinct planes, or a query
-// that runs out of stack: no list (the BVH answers).
+// diagonal from the centre is dropped), their planes (gd_k_tri_normals) are referred to the cell centre and merged when
+// they agree to 2e-5 mm over the cell.  More than GD_CELL_PLANES distinct planes, more than GD_LIST_MAX_CANDIDATES
+// reference boxes, or a query that runs out of stack: no list (the BVH answers).
 __global__ void gd_k_grid_list_count(const unsigned char *__restrict__ cells, size_t n, unsigned thr, unsigned *count) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool want = i < n && cells[i] < thr;
     const unsigned m = __ballot_sync(0xFFFFFFFFu, want);
     if ((threadIdx.x & 31) == 0 && m) atomicAdd(count, (unsigned)__popc(m));
 }
+// unit normal of every leaf-ordered triangle, from the float32 vertices in double, rounded to float32; w = 0 marks a
+// triangle without a normal.  (The plane through v0 with the rounded normal leaves the triangle's own plane by at most
+// 6e-8 x the triangle's extent: < 1e-5 mm.)
+__global__ void gd_k_tri_normals(const GdTri *__restrict__ tris, int n, float4 *__restrict__ nrm) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const GdTri tr = tris[i];
+    const double e1x = (double)tr.v1.x - tr.v0.x, e1y = (double)tr.v1.y - tr.v0.y, e1z = (double)tr.v1.z - tr.v0.z;
+    const double e2x = (double)tr.v2.x - tr.v0.x, e2y = (double)tr.v2.y - tr.v0.y, e2z = (double)tr.v2.z - tr.v0.z;
+    const double nx = e1y * e2z - e1z * e2y, ny = e1z * e2x - e1x * e2z, nz = e1x * e2y - e1y * e2x;
+    const double len = sqrt(nx * nx + ny * ny + nz * nz);
+    nrm[i] = len > 0.0 ? make_float4((float)(nx / len), (float)(ny / len), (float)(nz / len), 1.0f) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+}
+#define GD_LIST_MAX_CANDIDATES 96   // reference boxes looked at per cell before the cell is given up (dense meshes)
 __global__ void __launch_bounds__(128)
 gd_k_grid_planes(GdGrid g, const unsigned char *__restrict__ cells, unsigned thr, const GdNode4 *__restrict__ nodes4,
-                 const GdTri *__restrict__ tris, unsigned *__restrict__ info, float4 *__restrict__ planes,
-                 unsigned *counter, unsigned capacity) {
+                 const GdTri *__restrict__ tris, const float4 *__restrict__ nrm, unsigned *__restrict__ info,
+                 float4 *__restrict__ planes, unsigned *counter, unsigned capacity) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t n = (size_t)g.nx * g.ny * g.nz;
     if (i >= n) return;
@@ -642,9 +659,9 @@ gd_k_grid_planes(GdGrid g, const unsigned char *__restrict__ cells, unsigned thr
     const float half = 0.5f * g.h * 1.0001f, pad = 1.0e-3f;
     const float r = half + g.reach + pad + 1.0e-6f * fmaxf(fmaxf(fabsf(cx), fabsf(cy)), fabsf(cz));
     const float qlx = cx - r, qhx = cx + r, qly = cy - r, qhy = cy + r, qlz = cz - r, qhz = cz + r;
-    const double far_plane = (double)g.reach + 0.8661 * (double)g.h + (double)pad;
+    const float far_plane = g.reach + 0.8661f * g.h + pad;
     float4 pl[GD_CELL_PLANES];
-    int cnt = 0;
+    int cnt = 0, n_cand = 0;
     bool overflow = false;
     int stack[96];
     int sp = 0, node = 0;
@@ -662,16 +679,16 @@ gd_k_grid_planes(GdGrid g, const unsigned char *__restrict__ cells, unsigned thr
                 if (sp == 96) overflow = true; else stack[sp++] = ch[k];
                 continue;
             }
-            const GdTri tr = tris[~ch[k]];
-            const double e1x = (double)tr.v1.x - tr.v0.x, e1y = (double)tr.v1.y - tr.v0.y, e1z = (double)tr.v1.z - tr.v0.z;
-            const double e2x = (double)tr.v2.x - tr.v0.x, e2y = (double)tr.v2.y - tr.v0.y, e2z = (double)tr.v2.z - tr.v0.z;
-            double nx = e1y * e2z - e1z * e2y, ny = e1z * e2x - e1x * e2z, nz = e1x * e2y - e1y * e2x;
-            const double len = sqrt(nx * nx + ny * ny + nz * nz);
-            if (!(len > 0.0)) { overflow = true; continue; }
-            nx /= len; ny /= len; nz /= len;
-            const double d = nx * ((double)cx - tr.v0.x) + ny * ((double)cy - tr.v0.y) + nz * ((double)cz - tr.v0.z);
-            if (fabs(d) > far_plane) continue;
-            const float4 q = make_float4((float)nx, (float)ny, (float)nz, (float)d);
+            if (++n_cand > GD_LIST_MAX_CANDIDATES) { overflow = true; continue; }
+            const float4 nf = nrm[~ch[k]];
+            if (nf.w == 0.0f) { overflow = true; continue; }
+            const float4 v0 = tris[~ch[k]].v0;
+            // signed distance of the cell centre from the plane through v0, in double (the centre and v0 are ~100 mm, the
+            // distance ~1 mm and wanted to 1e-5)
+            const double d = (double)nf.x * ((double)cx - v0.x) + (double)nf.y * ((double)cy - v0.y) + (double)nf.z * ((double)cz - v0.z);
+            const float df = (float)d;
+            if (fabsf(df) > far_plane) continue;
+            const float4 q = make_float4(nf.x, nf.y, nf.z, df);
             bool seen = false;
             for (int j = 0; j < cnt; ++j) {
                 const float sgn = (q.x * pl[j].x + q.y * pl[j].y + q.z * pl[j].z) < 0.0f ? -1.0f : 1.0f;

@@ -121,7 +121,7 @@ GD_D bool gd_flight_clear(const GdGrid &g, const GdVec3 &p, float s) {
     const float fx = floorf((p.x - g.lox) * g.inv_h), fy = floorf((p.y - g.loy) * g.inv_h), fz = floorf((p.z - g.loz) * g.inv_h);
     const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
     if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) return false;
-    const unsigned w = __ldg(g.info + ((size_t)iz * g.ny + iy) * g.nx + ix);
+    const unsigned w = __ldg(g.info + ((unsigned)iz * (unsigned)g.ny + (unsigned)iy) * (unsigned)g.nx + (unsigned)ix);   // <= 2^28 cells
     if (!(w & GD_CELL_LIST)) return need < (float)w * g.quarter_h;
     if (need < (float)(w & 7u) * g.quarter_h) return true;
     if (!(need < g.reach)) return false;

@@ -2,6 +2,7 @@
 profiler (the ncu captures under profiles/ name it).
 
     python -m paper_2605_25963_b200.run_config <config 0..4> <n_histories> [--coh COEFF] [--bvh-width 4|8] [--flags N]
+                                               [--build-flags 0|1|2]     (1 = plane lists with the build, 2 = never)
     python -m paper_2605_25963_b200.run_config <config> --rays <n_rays> [--bvh-width 4|8]
 
 Histories: gadep_load_mesh / gadep_build_bvh / gadep_set_source, then ONE gadep_run of n_histories (no warm-up launch, so
@@ -26,13 +27,14 @@ def main():
     ap.add_argument("--bvh-width", type=int, default=0)
     ap.add_argument("--flags", type=int, default=0)
     ap.add_argument("--rays", type=float, default=0)
+    ap.add_argument("--build-flags", type=int, default=0)
     a = ap.parse_args()
     import torch
     import detmesh as dm
     import paper_2605_25963_b200 as pkg
     w = dm.make_config(a.config) if a.coh is None else dm.make_config(a.config, coh_coeff=a.coh)
     g = pkg.Gadep(0, torch.cuda.current_stream().cuda_stream)
-    g.load_workload(w)
+    g.load_workload(w, build_flags=a.build_flags)
     if a.bvh_width:
         g.set_bvh_width(a.bvh_width)
     if a.rays:
@@ -50,7 +52,7 @@ def main():
     g.run(n, w.seed, w.n_bins, w.spectrum_e_max_mev, flags=a.flags)
     c = g.get_counters()
     keep = ("n_histories", "n_queries", "n_skipped_queries", "n_box_tests", "n_tri_tests", "n_crossings", "n_pe", "n_compton",
-            "n_coherent", "n_pair", "n_escaped", "n_leak", "last_run_ms", "last_build_ms")
+            "n_coherent", "n_pair", "n_escaped", "n_leak", "last_run_ms", "last_build_ms", "n_grid_lists")
     print(json.dumps({"workload": w.name, **{k: c[k] for k in keep}, "fepe": [g.fepe(l)[0] for l in range(c["n_lines"])]}))
 
 

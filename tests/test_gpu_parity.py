@@ -530,6 +530,42 @@ def test_all_kernel_variants_give_identical_tallies(pkg, orc):
         assert ca["n_histories"] == n
 
 
+def test_clearance_grid_plane_lists_change_no_result(pkg, orc, monkeypatch):
+    # The plane lists of the clearance grid only decide *which* flights are answered without a BVH query: tallies, event
+    # counts and the number of flights are those of a run without lists (and of the grid-free kernels, test above).
+    # Build flags: lists with the build, never, or (0) by the size of the first run.
+    from paper_2605_25963_b200.binding import BUILD_NO_PLANE_LISTS, BUILD_PLANE_LISTS
+    for cfg, n in ((2, 60_000), (3, 30_000)):
+        w = dm.make_config(cfg)
+        res = {}
+        for name, flags in (("lists", BUILD_PLANE_LISTS), ("none", BUILD_NO_PLANE_LISTS)):
+            g = pkg.Gadep(0)
+            g.load_workload(w, build_flags=flags)
+            c0 = g.get_counters()
+            assert (c0["n_grid_lists"] > 0) == (name == "lists")
+            spec = g.run(n, 11, w.n_bins, w.spectrum_e_max_mev).copy()
+            res[name] = (spec, g.get_counters())
+        (sa, ca), (sb, cb) = res["lists"], res["none"]
+        assert cb["n_grid_lists"] == 0 and ca["n_grid_lists"] <= ca["n_grid_list_cells"]
+        assert np.array_equal(sa, sb)
+        for k in ("n_histories", "n_crossings", "n_pe", "n_compton", "n_coherent", "n_pair", "n_escaped", "n_leak",
+                  "n_cutoff", "emitted", "peak"):
+            assert ca[k] == cb[k], k
+        assert ca["n_queries"] + ca["n_skipped_queries"] == cb["n_queries"] + cb["n_skipped_queries"]
+        assert ca["n_queries"] < 0.8 * cb["n_queries"]            # the lists answer the tiny steps beside walls
+    # flags 0: a small run makes no lists, a run of at least the threshold does (threshold lowered for the test)
+    w = dm.make_config(2)
+    monkeypatch.setenv("GADEP_LIST_MIN_HISTORIES", "50000")
+    g = pkg.Gadep(0)
+    g.load_workload(w)
+    g.run(20_000, 11, w.n_bins, w.spectrum_e_max_mev)
+    assert g.get_counters()["n_grid_lists"] == 0
+    g.run(50_000, 11, w.n_bins, w.spectrum_e_max_mev)
+    assert g.get_counters()["n_grid_lists"] > 0
+    g.build_bvh()                                                 # a new build starts without lists again
+    assert g.get_counters()["n_grid_lists"] == 0
+
+
 def test_slab_transmission_on_gpu(pkg, orc):
     # closed form directly on the CUDA path: P(no event) = exp(-mu_tot x) through 10 mm Ge at 661.7 keV = 0.693573
     from detmesh.geometry import Line, discretise, merge_surfaces, revolve
