@@ -64,7 +64,7 @@ struct gadep_ctx {
     int kernel_variant = 2;                   // 2 = warp-resident wavefront, 1 = persistent lanes, 0 = history per thread
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
-    GdWaveTune tune = {16, 16, 2, 6, 16, 1};
+    GdWaveTune tune = {16, 16, 2, 6, 16, 1, 6};
     float rho[GADEP_MAX_MATERIALS] = {};      // g/cm^3, electron-range mode
     bool have_rho = false;
     // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
@@ -154,10 +154,10 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (const char *t = getenv("GADEP_GRID_CELLS")) { long long v = atoll(t); if (v >= 0 && v <= (1ll << 28)) c->grid_cells = v; }
     if (const char *t = getenv("GADEP_GRID_REACH")) { double v = atof(t); if (v >= 0.0 && v <= 8.0) c->list_reach_cells = v; }
     if (const char *t = getenv("GADEP_LIST_MIN_HISTORIES")) { long long v = atoll(t); if (v >= 0) c->list_min_hist = (unsigned long long)v; }
-    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,t_keep,n_steps,n_steps_max,p_min,t_help" (measurement sweeps)
-        int a, b, d, dm = 0, p = c->tune.p_min, ts = c->tune.t_help;
-        if (sscanf(t, "%d,%d,%d,%d,%d,%d", &a, &b, &d, &dm, &p, &ts) >= 4 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && dm >= d && dm <= 32 && p >= 1 && p <= 32 && ts >= 1 && ts <= 1024)
-            c->tune = {a, b, d, dm, p, ts};
+    if (const char *t = getenv("GADEP_TUNE")) {      // "k_fetch,t_keep,n_steps,n_steps_max,p_min,t_help,k_claim" (measurement sweeps)
+        int a, b, d, dm = 0, p = c->tune.p_min, ts = c->tune.t_help, kc = c->tune.k_claim;
+        if (sscanf(t, "%d,%d,%d,%d,%d,%d,%d", &a, &b, &d, &dm, &p, &ts, &kc) >= 4 && a >= 1 && a <= 32 && b >= 1 && b <= 32 && d >= 1 && d <= 32 && dm >= d && dm <= 32 && p >= 1 && p <= 32 && ts >= 1 && ts <= 1024 && kc >= 1 && kc <= 32)
+            c->tune = {a, b, d, dm, p, ts, kc};
     }
     *out = c;
     return GADEP_OK;

@@ -48,6 +48,7 @@ struct GdWaveTune {
     int n_steps_max;    // ... and its upper bound; equal to n_steps = fixed length
     int p_min;          // a physics pass runs while this many lanes have work (or the warp has nothing else to do)
     int t_help;         // READY slots that must wait before the warps that do not prefer traversal fetch any
+    int k_claim;        // chain burst: free lanes needed before the queues are consulted and waiting results claimed
 };
 
 // Ordering between a slot's words and the queue entry that publishes it: an acquire-release fence at block scope
@@ -408,10 +409,15 @@ GD_PASS void gd_chain_burst(const GdBlk &B, const GdBvh &bvh, const GdMaterials 
         // flight), never a freshly claimed traversal result.
         const unsigned free_mask = __ballot_sync(0xFFFFFFFFu, !has);
         const int n_has = 32 - __popc(free_mask);
-        int avail = 0, other = 0;
-        if (lane == 0) { avail = gd_q_count(B.result); other = CAN_TRAVERSE ? gd_q_count(B.ready) : gd_q_count(B.slow); }
-        avail = __shfl_sync(0xFFFFFFFFu, avail, 0);
-        other = __shfl_sync(0xFFFFFFFFu, other, 0);
+        // the queues are consulted (and waiting results claimed) only once k_claim lanes are free: the claim and the
+        // slot loads of one or two lanes are otherwise paid in every pass
+        const bool refill = first_pass || 32 - n_has >= tune.k_claim || n_has < tune.p_min;
+        int avail = 0, other = 1;
+        if (refill) {
+            if (lane == 0) { avail = gd_q_count(B.result); other = CAN_TRAVERSE ? gd_q_count(B.ready) : gd_q_count(B.slow); }
+            avail = __shfl_sync(0xFFFFFFFFu, avail, 0);
+            other = __shfl_sync(0xFFFFFFFFu, other, 0);
+        }
         const int expect = n_has + (avail < 32 - n_has ? avail : 32 - n_has);
         const bool nothing_else = CAN_TRAVERSE ? (my_rays == 0 && other == 0) : other < tune.p_min;
         const bool go = expect > 0 && (first_pass || expect >= tune.p_min || nothing_else);
@@ -420,7 +426,8 @@ GD_PASS void gd_chain_burst(const GdBlk &B, const GdBvh &bvh, const GdMaterials 
             // ---- fetch: lanes without a slot take waiting results
             bool got = false;
             int s_new = 0;
-            const int take = gd_q_claim(B.result, !has, 32 - n_has, lane, s_new, got);
+            int take = 0;
+            if (refill) take = gd_q_claim(B.result, !has, 32 - n_has, lane, s_new, got);
             if (got) {
                 s = s_new;
                 gd_slot_load(sl, s, L, A.seed, A.first);
