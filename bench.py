@@ -415,8 +415,9 @@ def main():
                              "traffic": traffic,
                              "traffic_source": "profiles/ncu_traffic.json (ncu --set full, dram bytes of one launch)",
                              "hbm": {"achieved_gbs": (traffic / (k_s / args.steps) / 1e9) if traffic else None, "peak_gbs": hbm_peak},
-                             "limiter": "instruction issue: instruction-fetch and dependency stalls at 12 warps/SM, 14-17 of 32 "
-                                        "lanes per instruction (ncu, profiles/r02_wave_kernel.md)",
+                             "limiter": "instruction issue: dependency, node-fetch latency and branch stalls at 12 warps/SM, 15-17 of 32 "
+                                        "lanes per instruction; instruction-cache hit rate 94 %, its GPC-level backing cache at "
+                                        "80 % of its request peak (ncu, profiles/r02b_wave_kernel.md)",
                              "peak_source": f"{n_sm} SMs x 128 lanes x sm_max_mhz ({peak_src})",
                              "kernel_ms_per_step": sum(kern_ms) / args.steps,
                              "bvh_build_ms_per_step": sum(build_ms) / args.steps,
