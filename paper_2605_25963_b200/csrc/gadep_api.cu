@@ -65,6 +65,7 @@ struct gadep_ctx {
     float *d_pair = nullptr;                  // wavefront kernel: parked annihilation photons, 8 floats per slot
     size_t pair_floats = 0;
     GdWaveTune tune = {16, 16, 2, 6, 16, 1, 6};
+    int wave_threads = 0;                     // 0 = by the size of the hierarchy; GADEP_WAVE_THREADS=384|896 forces an instance (measurement)
     float rho[GADEP_MAX_MATERIALS] = {};      // g/cm^3, electron-range mode
     bool have_rho = false;
     // surface-clustered hierarchy: side materials of every surface (host copy), per-material entry table (device)
@@ -151,6 +152,7 @@ extern "C" int gadep_create(gadep_ctx **out, int device, void *cuda_stream) {
     if (e != cudaSuccess) { delete c; return GADEP_E_CUDA; }
     if (getenv("GADEP_NO_SURFACE_CLUSTERS")) c->cluster_surfaces = false;
     if (const char *t = getenv("GADEP_WS")) c->prefer_ws = atoi(t) != 0;
+    if (const char *t = getenv("GADEP_WAVE_THREADS")) { int v = atoi(t); if (v == GD_W_THREADS || v == GD_W_THREADS_LAT) c->wave_threads = v; }
     if (const char *t = getenv("GADEP_GRID_CELLS")) { long long v = atoll(t); if (v >= 0 && v <= (1ll << 28)) c->grid_cells = v; }
     if (const char *t = getenv("GADEP_GRID_REACH")) { double v = atof(t); if (v >= 0.0 && v <= 8.0) c->list_reach_cells = v; }
     if (const char *t = getenv("GADEP_LIST_MIN_HISTORIES")) { long long v = atoll(t); if (v >= 0) c->list_min_hist = (unsigned long long)v; }
@@ -641,12 +643,15 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     if (n > 0xFFFFFFFFull) return gd_fail(c, GADEP_E_ARG, "more than 2^32-1 histories in one launch");
     size_t smem = sizeof(float) * (size_t)c->n_mat * 4 * c->n_grid + sizeof(unsigned) * ((size_t)n_bins + 1);
     const int variant = c->kernel_variant;
-    const int threads = variant == 2 ? GD_W_THREADS : (variant == 5 ? GD_WS_THREADS : GD_RUN_THREADS);
     const bool wide8 = c->run_width == 8;
+    // a hierarchy far larger than the L2 (126 MB): the 28-warp instance of the wavefront kernel (more rays in flight)
+    const bool lat16 = variant == 2 && !wide8 && c->wave_threads != GD_W_THREADS &&
+                       (c->wave_threads == GD_W_THREADS_LAT || (size_t)c->n_ref * (sizeof(GdNode4) + sizeof(GdTri)) > ((size_t)256 << 20));
+    const int threads = variant == 2 ? (lat16 ? GD_W_THREADS_LAT : GD_W_THREADS) : (variant == 5 ? GD_WS_THREADS : GD_RUN_THREADS);
     if (variant == 2 || variant == 5) smem += sizeof(float) * (size_t)GD_W_NF * GD_W_NSLOT;
     if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
     const void *kern = variant == 5 ? (wide8 ? (const void *)gd_k_transport_ws<8> : (const void *)gd_k_transport_ws<4>)
-                     : variant == 2 ? (wide8 ? (const void *)gd_k_transport_wave<8> : (const void *)gd_k_transport_wave<4>)
+                     : variant == 2 ? (wide8 ? (const void *)gd_k_transport_wave<8> : (lat16 ? (const void *)gd_k_transport_wave<4, GD_W_THREADS_LAT> : (const void *)gd_k_transport_wave<4>))
                                     : (variant == 1 ? (const void *)gd_k_transport_refill
                                                   : (variant == 3 ? (const void *)gd_k_transport<true, false>
                                                      : (variant == 4 ? (const void *)gd_k_transport<false, true>
@@ -687,6 +692,9 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
         } else if (variant == 2 && wide8) {
             gd_k_transport_wave<8><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
                                                                 c->d_next, chunk, c->d_pair, c->tune);
+        } else if (variant == 2 && lat16) {
+            gd_k_transport_wave<4, GD_W_THREADS_LAT><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
+                                                                                  d_flags, c->d_next, chunk, c->d_pair, c->tune);
         } else if (variant == 2) {
             gd_k_transport_wave<4><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
                                                                 c->d_next, chunk, c->d_pair, c->tune);

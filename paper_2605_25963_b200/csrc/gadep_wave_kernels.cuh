@@ -22,10 +22,11 @@
 #include "gadep_trav.cuh"
 #include "gadep_transport_kernels.cuh"
 
-#ifndef GD_W_THREADS
-#define GD_W_THREADS 384
-#endif
-#define GD_W_WARPS (GD_W_THREADS / 32)
+#define GD_W_THREADS 384           // 12 warps x 160 registers: the default
+#define GD_W_THREADS_LAT 896       // 28 warps x 72 registers (540 bytes of spills): for hierarchies far larger than the L2,
+                                   // where the kernel waits for node fetches from HBM and rays in flight are what pays.
+                                   // Config 4, 1e8 histories: 1727 ms at 12 warps, 1515 at 16, 1408 at 20, 1318 at 24,
+                                   // 1262 at 28, 1430 at 32; the cache-resident configs lose 2 - 4 % already at 16.
 #define GD_W_NSLOT 1024           // photon slots per block (64 per warp)
 // fields per slot.  25 words keep the block's shared memory under the 164 KB carve-out for up to 9 materials, which
 // leaves the SM a 64 KB L1 instead of 32 KB.
@@ -573,8 +574,8 @@ GD_D void gd_flush_block_tallies(const GdTally &tally, const unsigned *s_spec, c
 // pair_buf: global, 8 floats per slot of every block of the grid
 // WIDTH: 4 = uncompressed 4-wide nodes (default), 8 = compressed 8-wide nodes
 // Every warp does whichever kind of work there is (the default kernel).
-template <int WIDTH>
-__global__ void __launch_bounds__(GD_W_THREADS, 1)
+template <int WIDTH, int THREADS = GD_W_THREADS>
+__global__ void __launch_bounds__(THREADS, 1)
 gd_k_transport_wave(GdBvh bvh, GdMaterials M, const GdSource *__restrict__ src, unsigned long long first,
                     unsigned long long n_hist, unsigned long long seed, GdTally tally, float *__restrict__ edep_out,
                     unsigned *__restrict__ flags_out, unsigned long long *next_history, unsigned chunk,

@@ -566,6 +566,23 @@ def test_clearance_grid_plane_lists_change_no_result(pkg, orc, monkeypatch):
     assert g.get_counters()["n_grid_lists"] == 0
 
 
+def test_many_warp_instance_gives_identical_tallies(pkg, orc, monkeypatch):
+    # the 28-warp x 72-register instance of the wavefront kernel (chosen for hierarchies far larger than the L2; forced
+    # here on a small one) against the 12-warp default: same streams, integer tallies
+    w = dm.make_config(3)
+    res = []
+    for threads in ("384", "896"):
+        monkeypatch.setenv("GADEP_WAVE_THREADS", threads)
+        g = pkg.Gadep(0)
+        g.load_workload(w)
+        res.append((g.run(40_000, 9, w.n_bins, w.spectrum_e_max_mev).copy(), g.get_counters()))
+    (sa, ca), (sb, cb) = res
+    assert np.array_equal(sa, sb)
+    for k in ("n_histories", "n_queries", "n_skipped_queries", "n_crossings", "n_pe", "n_compton", "n_coherent", "n_pair",
+              "n_escaped", "n_leak", "n_cutoff", "emitted", "peak", "n_box_tests", "n_tri_tests"):
+        assert ca[k] == cb[k], k
+
+
 def test_slab_transmission_on_gpu(pkg, orc):
     # closed form directly on the CUDA path: P(no event) = exp(-mu_tot x) through 10 mm Ge at 661.7 keV = 0.693573
     from detmesh.geometry import Line, discretise, merge_surfaces, revolve
