@@ -1,22 +1,28 @@
 // gadep_wave_kernels.cuh -- block-resident wavefront transport and the ray-cast hook.
 //
-// A block owns GD_W_NSLOT photon slots in shared memory (SoA, GD_W_NF words per slot) and two block-wide queues of
-// slot numbers: READY (the slot's next nearest-hit query is prepared) and RESULT (hit known, physics pending).  A slot
-// is in one queue, or on a lane of some warp.  Every warp of the block does whichever kind of work there is:
-//   T-burst: lanes traverse in rounds of `n_steps` node visits + one leaf step; a lane whose ray ends writes the hit
-//            to its slot, pushes it to RESULT and -- as soon as `k_fetch` lanes are idle -- takes a READY slot
-//            (dynamic fetch).  Unfinished rays stay in their lanes' registers while the warp does physics.
-//   P-burst: lanes take RESULT slots and process one event each (boundary crossing / interaction / tally / refill
-//            from the history counter / attenuation lookup); a slot whose next flight ends before the clearance of
-//            its grid cell (GdGrid) stays on its lane and goes round again without a query, the others are pushed to
-//            READY and their lanes take the next waiting result.
-// Because the queues are shared, a warp finds 32 slots for either kind of work as long as the block has them --
-// the long scattering chains that are left when the history counter runs dry end up on the lanes of one warp instead
-// of idling in all sixteen.  The queues are rings with a ticket counter on each side; an entry carries a valid bit
-// that its producer sets last and its consumer clears, so no lock is held while a slot is read or written.
+// A block owns GD_W_NSLOT photon slots in shared memory (SoA, GD_W_NF words per slot) and three block-wide queues of
+// slot numbers: READY (the slot's next nearest-hit query is prepared), RESULT (hit known; the event is a boundary
+// crossing into another medium or an interaction) and SLOW (any other event: start of a history, start localisation,
+// escape, crossing into KILL).  A slot is in one queue, or on a lane of some warp.  Every warp of the block does
+// whichever kind of work there is:
+//   T-burst:      lanes traverse in rounds of `n_steps` node visits + one leaf step; a lane whose ray ends writes the hit
+//                 to its slot, pushes it to RESULT or SLOW and -- as soon as `k_fetch` lanes are idle -- takes a READY
+//                 slot (dynamic fetch).  Unfinished rays stay in their lanes' registers while the warp does physics.
+//   chain burst:  lanes take RESULT slots and handle crossings and coherent scattering in place; a slot whose next
+//                 flight provably meets no facet (clearance grid: scalar bound of its cell, or the distances to the
+//                 planes of the cell's list) stays on its lane and goes round again without a query; photoelectric,
+//                 Compton and pair events go to SLOW, flights that need the BVH to READY.
+//   general pass: lanes take SLOW slots and process one event each (any kind), tally finished histories, start the next
+//                 histories of the block's chunk and prepare their first query.
+// Because the queues are shared, a warp finds 32 slots for either kind of work as long as the block has them -- the
+// long scattering chains that are left when the history counter runs dry end up on the lanes of one warp instead of
+// idling in all of them.  The queues are rings with a ticket counter on each side; an entry carries a valid bit that its
+// producer sets last and its consumer clears, so no lock is held while a slot is read or written.
 // There is no block-level barrier inside the loop and no particle state in global memory (only the two pending
 // annihilation photons of a pair event, which are rare, sit in a global side buffer).  Results do not depend on any
 // of this scheduling: random streams are keyed by the history index and the tallies are integers.
+// The kernel is bound by instruction fetch as much as by anything else: code that several call
+// sites share is written once (one push routine for all queues, out-of-line Philox / rotation / attenuation lookup).
 #pragma once
 #include "gadep_physics.cuh"
 #include "gadep_trav.cuh"
@@ -27,7 +33,7 @@
                                    // where the kernel waits for node fetches from HBM and rays in flight are what pays.
                                    // Config 4, 1e8 histories: 1727 ms at 12 warps, 1515 at 16, 1408 at 20, 1318 at 24,
                                    // 1262 at 28, 1430 at 32; the cache-resident configs lose 2 - 4 % already at 16.
-#define GD_W_NSLOT 1024           // photon slots per block (64 per warp)
+#define GD_W_NSLOT 1024           // photon slots per block
 // fields per slot.  25 words keep the block's shared memory under the 164 KB carve-out for up to 9 materials, which
 // leaves the SM a 64 KB L1 instead of 32 KB.
 #define GD_W_NF 25
