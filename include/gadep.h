@@ -97,8 +97,11 @@ int gadep_load_mesh(gadep_ctx *ctx, const float *vertices, int n_vert, const int
 #define GADEP_BUILD_NO_PLANE_LISTS 2
 int gadep_build_bvh(gadep_ctx *ctx, int flags);
 
-/* Node width the wavefront kernels and gadep_trace_rays traverse: 4 (default; uncompressed nodes) or 8 (compressed
- * nodes).  Both hierarchies hold the same facets, so every result is identical. */
+/* Nodes the wavefront kernels and gadep_trace_rays traverse: 4 = uncompressed 4-wide nodes (128 bytes; the default),
+ * 5 = the same four children with 8-bit quantised boxes (64 bytes), 8 = compressed 8-wide nodes (96 bytes).  All hold the
+ * same facets in conservative boxes: the ray cast returns identical hits (tests: 1e6 rays against brute force, 6e7 rays
+ * between the three).  Without a call the ray cast takes the 64-byte nodes on hierarchies of more than 256 MB (a node
+ * visit is a fetch from HBM there: 14 % faster) and everything else the uncompressed ones. */
 int gadep_set_bvh_width(gadep_ctx *ctx, int width);
 
 #define GADEP_SRC_POINT 0

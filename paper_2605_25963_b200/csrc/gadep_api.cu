@@ -37,7 +37,11 @@ struct gadep_ctx {
     GdNode *d_nodes = nullptr;
     GdNode4 *d_nodes4 = nullptr;
     GdNode8 *d_nodes8 = nullptr;
-    int bvh_width = 4;             // traversal of the wavefront kernels: 4 = uncompressed 4-wide nodes, 8 = compressed 8-wide
+    GdNode4q *d_nodes4q = nullptr;
+    int bvh_width = 4;             // traversal of the wavefront kernels: 4 = uncompressed 4-wide nodes, 5 = compressed 4-wide
+                                   // (64 bytes), 8 = compressed 8-wide
+    bool width_set = false;        // gadep_set_bvh_width was called; otherwise the ray cast takes the 64-byte nodes on
+                                   // hierarchies far larger than the L2 (14 % faster there), everything else the 4-wide ones
     GdTri *d_leaf_tris = nullptr;
     int bvh_depth = 0;
     int n_ref = 0;                 // leaves of the BVH: facet references after splitting
@@ -47,8 +51,8 @@ struct gadep_ctx {
     // [6..9] the mesh copies (vertices, triangles, side materials, surface ids)
     // [10..12] mesh validation: edge table keys, edge table surfaces, error record + surface sides
     // [14] clearance grid: marks / x distances [15] squared distances after the y pass [16] the grid itself
-    void *pool[21] = {};
-    size_t pool_cap[21] = {};
+    void *pool[22] = {};
+    size_t pool_cap[22] = {};
     // source
     bool have_src = false;
     GdSource src;
@@ -178,7 +182,7 @@ static cudaError_t gd_pool_get(gadep_ctx *c, int k, size_t bytes, void **out) {
 }
 
 static void gd_free_mesh(gadep_ctx *c) {
-    c->d_nodes4 = nullptr; c->d_nodes8 = nullptr;
+    c->d_nodes4 = nullptr; c->d_nodes8 = nullptr; c->d_nodes4q = nullptr;
     c->d_verts = nullptr; c->d_tris = c->d_tri_mats = c->d_tri_surf = nullptr;
     c->d_nodes = nullptr; c->d_leaf_tris = nullptr;
     c->have_mesh = c->have_bvh = false;
@@ -189,7 +193,7 @@ extern "C" void gadep_destroy(gadep_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     gd_free_mesh(c);
-    for (int k = 0; k < 21; ++k) cudaFree(c->pool[k]);
+    for (int k = 0; k < 22; ++k) cudaFree(c->pool[k]);
     cudaFree(c->d_table); cudaFree(c->d_src); cudaFree(c->d_tally); cudaFree(c->d_counters); cudaFree(c->d_next); cudaFree(c->d_pair); cudaFree(c->d_mat_entry);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -367,7 +371,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     GD_CUDA(c, cudaSetDevice(c->device));
     const int n_tri = c->n_tri;
     cudaStream_t st = c->stream;
-    c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->d_nodes4 = nullptr; c->d_nodes8 = nullptr; c->have_bvh = false;
+    c->d_nodes = nullptr; c->d_leaf_tris = nullptr; c->d_nodes4 = nullptr; c->d_nodes8 = nullptr; c->d_nodes4q = nullptr; c->have_bvh = false;
     const int tb = 256, nbt = (n_tri + tb - 1) / tb;
     int launches = 0;
     // ---- phase A: how many references (reference splitting) -> one 4-byte read-back sizes the arena
@@ -414,6 +418,7 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
         if ((e = gd_pool_get(c, 4, sizeof(GdTri) * (size_t)n, (void **)&c->d_leaf_tris)) != cudaSuccess) break;
         if ((e = gd_pool_get(c, 5, sizeof(GdNode4) * (size_t)std::max(n - 1, 1), (void **)&c->d_nodes4)) != cudaSuccess) break;
         if ((e = gd_pool_get(c, 13, sizeof(GdNode8) * (size_t)std::max(n - 1, 1), (void **)&c->d_nodes8)) != cudaSuccess) break;
+        if ((e = gd_pool_get(c, 21, sizeof(GdNode4q) * (size_t)std::max(n - 1, 1), (void **)&c->d_nodes4q)) != cudaSuccess) break;
         float4 *ref_lo = (float4 *)(arena + o_tlo), *ref_hi = (float4 *)(arena + o_thi);
         float4 *node_lo = (float4 *)(arena + o_nlo), *node_hi = (float4 *)(arena + o_nhi);
         unsigned long long *keys[2] = {(unsigned long long *)(arena + o_k0), (unsigned long long *)(arena + o_k1)};
@@ -447,7 +452,8 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
                                           node_hi, visits, c->d_nodes, scene + 6);
             gd_k_collapse4<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes4);
             gd_k_collapse8<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes8);
-            launches += 4;
+            gd_k_collapse4q<<<nb, tb, 0, st>>>(n - 1, child_l, child_r, ref_lo, ref_hi, vals[cur], node_lo, node_hi, c->d_nodes4q);
+            launches += 5;
         }
         // ---- facet-clearance grid over the box of the inner surfaces
         c->grid = GdGrid{};
@@ -528,10 +534,13 @@ extern "C" int gadep_build_bvh(gadep_ctx *c, int flags) {
     return GADEP_OK;
 }
 
+// nodes + triangle records far beyond the 126 MB L2: a node visit is then a fetch from HBM
+static bool gd_large_hierarchy(const gadep_ctx *c) { return (size_t)c->n_ref * (sizeof(GdNode4) + sizeof(GdTri)) > ((size_t)256 << 20); }
+
 static GdBvh gd_bvh_view(const gadep_ctx *c) {
     GdBvh b;
     b.grid = c->grid;
-    b.nodes = c->d_nodes; b.nodes4 = c->d_nodes4; b.nodes8 = c->d_nodes8; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
+    b.nodes = c->d_nodes; b.nodes4 = c->d_nodes4; b.nodes8 = c->d_nodes8; b.nodes4q = c->d_nodes4q; b.tris = c->d_leaf_tris; b.n_tri = c->n_ref; b.root_is_leaf = c->n_ref == 1;
     b.mat_entry = c->have_entries ? c->d_mat_entry : nullptr;
     return b;
 }
@@ -645,13 +654,16 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
     const int variant = c->kernel_variant;
     const bool wide8 = c->run_width == 8;
     // a hierarchy far larger than the L2 (126 MB): the 28-warp instance of the wavefront kernel (more rays in flight)
+    const bool q4 = c->run_width == GD_WIDTH_4Q;
     const bool lat16 = variant == 2 && !wide8 && c->wave_threads != GD_W_THREADS &&
-                       (c->wave_threads == GD_W_THREADS_LAT || (size_t)c->n_ref * (sizeof(GdNode4) + sizeof(GdTri)) > ((size_t)256 << 20));
+                       (c->wave_threads == GD_W_THREADS_LAT || gd_large_hierarchy(c));
     const int threads = variant == 2 ? (lat16 ? GD_W_THREADS_LAT : GD_W_THREADS) : (variant == 5 ? GD_WS_THREADS : GD_RUN_THREADS);
     if (variant == 2 || variant == 5) smem += sizeof(float) * (size_t)GD_W_NF * GD_W_NSLOT;
     if (smem > 220 * 1024) return gd_fail(c, GADEP_E_ARG, "tables + spectrum + photon slots (%zu B) do not fit in shared memory", smem);
     const void *kern = variant == 5 ? (wide8 ? (const void *)gd_k_transport_ws<8> : (const void *)gd_k_transport_ws<4>)
-                     : variant == 2 ? (wide8 ? (const void *)gd_k_transport_wave<8> : (lat16 ? (const void *)gd_k_transport_wave<4, GD_W_THREADS_LAT> : (const void *)gd_k_transport_wave<4>))
+                     : variant == 2 ? (wide8 ? (const void *)gd_k_transport_wave<8>
+                                      : q4 ? (lat16 ? (const void *)gd_k_transport_wave<GD_WIDTH_4Q, GD_W_THREADS_LAT> : (const void *)gd_k_transport_wave<GD_WIDTH_4Q>)
+                                           : (lat16 ? (const void *)gd_k_transport_wave<4, GD_W_THREADS_LAT> : (const void *)gd_k_transport_wave<4>))
                                     : (variant == 1 ? (const void *)gd_k_transport_refill
                                                   : (variant == 3 ? (const void *)gd_k_transport<true, false>
                                                      : (variant == 4 ? (const void *)gd_k_transport<false, true>
@@ -692,6 +704,12 @@ static int gd_launch_transport(gadep_ctx *c, unsigned long long first, unsigned 
         } else if (variant == 2 && wide8) {
             gd_k_transport_wave<8><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
                                                                 c->d_next, chunk, c->d_pair, c->tune);
+        } else if (variant == 2 && q4 && lat16) {
+            gd_k_transport_wave<GD_WIDTH_4Q, GD_W_THREADS_LAT><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
+                                                                                            d_flags, c->d_next, chunk, c->d_pair, c->tune);
+        } else if (variant == 2 && q4) {
+            gd_k_transport_wave<GD_WIDTH_4Q><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep, d_flags,
+                                                                          c->d_next, chunk, c->d_pair, c->tune);
         } else if (variant == 2 && lat16) {
             gd_k_transport_wave<4, GD_W_THREADS_LAT><<<grid, threads, smem, st>>>(gd_bvh_view(c), M, c->d_src, first, n, seed, T, d_edep,
                                                                                   d_flags, c->d_next, chunk, c->d_pair, c->tune);
@@ -839,14 +857,16 @@ extern "C" int gadep_trace_rays(gadep_ctx *c, const float *org, const float *dir
     }
     cudaMemsetAsync(c->d_counters, 0, sizeof(GdCounters), st);
     int per_sm = 1;
-    const bool wide8 = c->bvh_width == 8;
-    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, wide8 ? gd_k_trace_wave<8> : gd_k_trace_wave<4>, 256, 0));
+    const bool wide8 = c->bvh_width == 8, q4 = c->bvh_width == GD_WIDTH_4Q || (!c->width_set && gd_large_hierarchy(c));
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, wide8 ? gd_k_trace_wave<8> : (q4 ? gd_k_trace_wave<GD_WIDTH_4Q> : gd_k_trace_wave<4>), 256, 0));
     int grid = (int)std::min<long long>((n_rays + 255) / 256, (long long)c->n_sm * std::max(per_sm, 1));
     unsigned chunk = (unsigned)std::min<long long>(2048, std::max<long long>(32, n_rays / ((long long)grid * 8 * 8)));
     cudaMemsetAsync(c->d_next, 0, sizeof(unsigned long long), st);
     cudaEventRecord(c->ev0, st);
     if (wide8) gd_k_trace_wave<8><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
                                                          c->d_counters, c->d_next, chunk, c->tune);
+    else if (q4) gd_k_trace_wave<GD_WIDTH_4Q><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
+                                                                   c->d_counters, c->d_next, chunk, c->tune);
     else gd_k_trace_wave<4><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
                                                    c->d_counters, c->d_next, chunk, c->tune);
     cudaEventRecord(c->ev1, st);
@@ -1034,8 +1054,9 @@ extern "C" int gadep_philox_raw(gadep_ctx *c, const unsigned *ctr4, const unsign
 // ---------------------------------------------------------------- traversal width, whole-tally exchange
 extern "C" int gadep_set_bvh_width(gadep_ctx *c, int width) {
     if (!c) return GADEP_E_NULL;
-    if (width != 4 && width != 8) return gd_fail(c, GADEP_E_ARG, "BVH width %d (4 or 8)", width);
+    if (width != 4 && width != 8 && width != GD_WIDTH_4Q) return gd_fail(c, GADEP_E_ARG, "BVH width %d (4, 5 or 8)", width);
     c->bvh_width = width;
+    c->width_set = true;
     return GADEP_OK;
 }
 
@@ -1127,13 +1148,15 @@ extern "C" int gadep_trace_rays_static(gadep_ctx *c, const float *org, const flo
     }
     GD_CUDA(c, cudaMemsetAsync(scratch, 0, GD_STATIC_HDR, st));       // the last call's counter and totals are still there
     int per_sm = 1;
-    const bool wide8 = c->bvh_width == 8;
-    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, wide8 ? gd_k_trace_wave<8> : gd_k_trace_wave<4>, 256, 0));
+    const bool wide8 = c->bvh_width == 8, q4 = c->bvh_width == GD_WIDTH_4Q || (!c->width_set && gd_large_hierarchy(c));
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, wide8 ? gd_k_trace_wave<8> : (q4 ? gd_k_trace_wave<GD_WIDTH_4Q> : gd_k_trace_wave<4>), 256, 0));
     const int grid = (int)std::min<long long>((n_rays + 255) / 256, (long long)c->n_sm * std::max(per_sm, 1));
     const unsigned chunk = (unsigned)std::min<long long>(2048, std::max<long long>(32, n_rays / ((long long)grid * 8 * 8)));
     cudaEventRecord(c->ev0, st);
     if (wide8) gd_k_trace_wave<8><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
                                                          d_cnt, d_next, chunk, c->tune);
+    else if (q4) gd_k_trace_wave<GD_WIDTH_4Q><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
+                                                                   d_cnt, d_next, chunk, c->tune);
     else gd_k_trace_wave<4><<<grid, 256, 0, st>>>(gd_bvh_view(c), d_org, d_dir, n_rays, filter_material, t_min, d_tri, d_t,
                                                    d_cnt, d_next, chunk, c->tune);
     cudaEventRecord(c->ev1, st);

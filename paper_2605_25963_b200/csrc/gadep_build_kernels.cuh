@@ -521,6 +521,76 @@ __global__ void gd_k_collapse8(int n_inner, const int *__restrict__ child_l, con
     out[i] = nd;
 }
 
+// 4-wide compressed nodes (GdNode4q): the children of gd_k_collapse4 (same choice, same order), boxes quantised like
+// gd_k_collapse8 on the grid of the binary node's own box.
+__global__ void gd_k_collapse4q(int n_inner, const int *__restrict__ child_l, const int *__restrict__ child_r,
+                                const float4 *__restrict__ ref_lo, const float4 *__restrict__ ref_hi,
+                                const unsigned *__restrict__ order, const float4 *__restrict__ node_lo,
+                                const float4 *__restrict__ node_hi, GdNode4q *__restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_inner) return;
+    int c[4] = {child_l[i], child_r[i], GD_NO_CHILD, GD_NO_CHILD};
+    int k = 2;
+    while (k < 4) {
+        int best = -1;
+        float best_a = -1.0f;
+        for (int j = 0; j < k; ++j)
+            if (c[j] >= 0) {
+                const float a = gd_half_area(node_lo[c[j]], node_hi[c[j]]);
+                if (a > best_a) { best_a = a; best = j; }
+            }
+        if (best < 0) break;
+        const int b = c[best];
+        c[best] = child_l[b];
+        c[k++] = child_r[b];
+    }
+    const float4 nlo = node_lo[i], nhi = node_hi[i];
+    const float blo[3] = {nlo.x, nlo.y, nlo.z}, bhi[3] = {nhi.x, nhi.y, nhi.z};
+    float clo[4][3], chi[4][3];
+    for (int j = 0; j < 4; ++j) {
+        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+        if (c[j] != GD_NO_CHILD) {
+            if (c[j] < 0) { const int o = (int)order[~c[j]]; a = ref_lo[o]; b = ref_hi[o]; }
+            else { a = node_lo[c[j]]; b = node_hi[c[j]]; }
+        }
+        clo[j][0] = a.x; clo[j][1] = a.y; clo[j][2] = a.z; chi[j][0] = b.x; chi[j][1] = b.y; chi[j][2] = b.z;
+    }
+    unsigned q[3][2] = {{0, 0}, {0, 0}, {0, 0}};
+    unsigned exyz = 0;
+    float org[3];
+    for (int a = 0; a < 3; ++a) {
+        const float ext = bhi[a] - blo[a];
+        int e = -100;
+        if (ext > 0.0f) {
+            int kk;
+            const float m = frexpf(ext, &kk);               // ext = m 2^kk, m in [0.5, 1)
+            e = m * 256.0f <= 254.5f ? kk - 8 : kk - 7;     // (hi - o) / 2^e + margins stays <= 255
+            e = e < -100 ? -100 : (e > 100 ? 100 : e);
+        }
+        const float S = __int_as_float((e + 127) << 23), invS = __int_as_float((127 - e) << 23);
+        const float o = blo[a] - S * (1.0f / 32.0f);
+        org[a] = o;
+        exyz |= (unsigned)(e + 127) << (8 * a);
+        for (int j = 0; j < 4; ++j) {
+            unsigned ql = 255u, qh = 0u;
+            if (c[j] != GD_NO_CHILD) {
+                const float fl = floorf((clo[j][a] - o) * invS - (1.0f / 64.0f));
+                const float fh = ceilf((chi[j][a] - o) * invS + (1.0f / 64.0f));
+                ql = (unsigned)fminf(fmaxf(fl, 0.0f), 255.0f);
+                qh = (unsigned)fminf(fmaxf(fh, 0.0f), 255.0f);
+            }
+            q[a][0] |= ql << (8 * j);
+            q[a][1] |= qh << (8 * j);
+        }
+    }
+    GdNode4q nd;
+    nd.ox = org[0]; nd.oy = org[1]; nd.oz = org[2]; nd.exyz = exyz;
+    nd.qx_lo = q[0][0]; nd.qx_hi = q[0][1]; nd.qy_lo = q[1][0]; nd.qy_hi = q[1][1]; nd.qz_lo = q[2][0]; nd.qz_hi = q[2][1];
+    nd.pad0 = 0; nd.pad1 = 0;
+    for (int j = 0; j < 4; ++j) nd.child[j] = c[j];
+    out[i] = nd;
+}
+
 // ---------------------------------------------------------------- facet-clearance grid (GdGrid, gadep_common.cuh)
 // 1. every cell a reference box touches is marked; 2. exact Euclidean distance transform of the marks in cell units,
 // separable (x by two sweeps per row, then y and z as windowed lower envelopes), capped at GD_GRID_WINDOW + 1 cells;

@@ -256,6 +256,47 @@ GD_D void gd_trav_node8(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box
                            : ((low & 0x30u) ? ((low & 0x10u) ? c4 : c5) : ((low & 0x40u) ? c6 : c7));
 }
 
+// one 4-wide compressed node visit (GdNode4q): four 16-byte loads for four boxes; dequantisation and error bounds as in
+// gd_trav_node8, distance-sorted descent as in gd_trav_node4
+GD_D void gd_trav_node4q(GdTrav &T, const GdBvh &bvh, int *stack, unsigned &n_box_tests) {
+    const uint4 *nd = reinterpret_cast<const uint4 *>(bvh.nodes4q + T.node);
+    const uint4 hd = nd[0], qa = nd[1], qb = nd[2];
+    const int4 ch = *reinterpret_cast<const int4 *>(nd + 3);
+    n_box_tests += 4;
+    const float Bx = __uint_as_float((hd.w & 0xFFu) << 23) * T.ix;
+    const float By = __uint_as_float(((hd.w >> 8) & 0xFFu) << 23) * T.iy;
+    const float Bz = __uint_as_float(((hd.w >> 16) & 0xFFu) << 23) * T.iz;
+    const float Ax = fmaf(-32768.0f, Bx, fmaf(__uint_as_float(hd.x), T.ix, -T.bx));
+    const float Ay = fmaf(-32768.0f, By, fmaf(__uint_as_float(hd.y), T.iy, -T.by));
+    const float Az = fmaf(-32768.0f, Bz, fmaf(__uint_as_float(hd.z), T.iz, -T.bz));
+    const float ex = fmaf(fabsf(Bx), 1.0f / 256.0f, T.err), ey = fmaf(fabsf(By), 1.0f / 256.0f, T.err), ez = fmaf(fabsf(Bz), 1.0f / 256.0f, T.err);
+    const float Anx = Ax - ex, Afx = Ax + ex, Any = Ay - ey, Afy = Ay + ey, Anz = Az - ez, Afz = Az + ez;
+    const bool ngx = __float_as_int(T.ix) < 0, ngy = __float_as_int(T.iy) < 0, ngz = __float_as_int(T.iz) < 0;
+    const unsigned nx = GD_SELB(ngx, qa.y, qa.x), fx = GD_SELB(ngx, qa.x, qa.y);
+    const unsigned ny = GD_SELB(ngy, qa.w, qa.z), fy = GD_SELB(ngy, qa.z, qa.w);
+    const unsigned nz = GD_SELB(ngz, qb.y, qb.x), fz = GD_SELB(ngz, qb.x, qb.y);
+    const float pad = 4.0e-7f;
+    float key[4];
+    int cc[4] = {ch.x, ch.y, ch.z, ch.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const unsigned sel = 0x7604u | ((unsigned)k << 4);       // byte k of the word -> bits 8..15 of 0x47000000
+        const float x0 = fmaf(__uint_as_float(__byte_perm(nx, 0x47000000u, sel)), Bx, Anx);
+        const float x1 = fmaf(__uint_as_float(__byte_perm(fx, 0x47000000u, sel)), Bx, Afx);
+        const float y0 = fmaf(__uint_as_float(__byte_perm(ny, 0x47000000u, sel)), By, Any);
+        const float y1 = fmaf(__uint_as_float(__byte_perm(fy, 0x47000000u, sel)), By, Afy);
+        const float z0 = fmaf(__uint_as_float(__byte_perm(nz, 0x47000000u, sel)), Bz, Anz);
+        const float z1 = fmaf(__uint_as_float(__byte_perm(fz, 0x47000000u, sel)), Bz, Afz);
+        const float n = fmaxf(fmaxf(x0, y0), fmaxf(z0, T.tmin));
+        float f = fminf(fminf(x1, y1), fminf(z1, T.t));
+        f = fmaf(fabsf(f), pad, f);
+        const bool h = n <= f && cc[k] != GD_NO_CHILD;
+        key[k] = h ? n : GD_TINF;
+        cc[k] = h ? cc[k] : GD_NO_CHILD;
+    }
+    gd_trav_descend4(T, stack, key[0], key[1], key[2], key[3], cc[0], cc[1], cc[2], cc[3]);
+}
+
 // Advance the warp: every busy lane makes up to `n_steps` inner-node visits (no warp vote in between: a lane that
 // reaches a leaf or the end of its ray idles for the rest of the round), then the lanes waiting at a leaf run
 // their triangle test together.  One vote-free round amortises the scheduling work of the caller (fetch, retire)
@@ -267,6 +308,7 @@ GD_D void gd_trav_step(GdTrav &T, const GdBvh &bvh, int *stack, int n_steps, uns
     for (int k = 0; k < n_steps; ++k) {
         if (T.node >= 0) {
             if (WIDTH == 8) gd_trav_node8(T, bvh, stack, n_box_tests);
+            else if (WIDTH == GD_WIDTH_4Q) gd_trav_node4q(T, bvh, stack, n_box_tests);
             else gd_trav_node4(T, bvh, stack, n_box_tests);
         }
     }

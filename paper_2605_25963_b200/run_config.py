@@ -1,9 +1,9 @@
 """Runs one of the BASELINE.json set-ups once and prints time and counters -- the smallest command to put under a
 profiler (the ncu captures under profiles/ name it).
 
-    python -m paper_2605_25963_b200.run_config <config 0..4> <n_histories> [--coh COEFF] [--bvh-width 4|8] [--flags N]
+    python -m paper_2605_25963_b200.run_config <config 0..4> <n_histories> [--coh COEFF] [--bvh-width 4|5|8] [--flags N]
                                                [--build-flags 0|1|2]     (1 = plane lists with the build, 2 = never)
-    python -m paper_2605_25963_b200.run_config <config> --rays <n_rays> [--bvh-width 4|8]
+    python -m paper_2605_25963_b200.run_config <config> --rays <n_rays> [--bvh-width 4|5|8]
 
 Histories: gadep_load_mesh / gadep_build_bvh / gadep_set_source, then ONE gadep_run of n_histories (no warm-up launch, so
 the transport kernel of interest is the first `gd_k_transport_wave` launch of the process).  Rays: ONE gadep_trace_rays

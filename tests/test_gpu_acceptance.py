@@ -249,17 +249,18 @@ def test_compressed_wide_nodes_give_the_same_hits(pkg, orc, cfg, n_rays, box):
     g.load_workload(w)
     org, d = make_rays(n_rays, 2, *box)
     res = {}
-    for width in (4, 8):
+    for width in (4, 5, 8):                    # 5 = 4-wide with 8-bit quantised boxes (64-byte nodes)
         g.set_bvh_width(width)
         for filt, tmin in ((-2, 0.0), (dm.MAT["Ge_active"], -1.0e-4)):
             tri, t = g.trace_rays(org, d, filt, tmin)
             res[(width, filt)] = (tri.copy(), t.copy())
             assert g.get_counters()["n_stack_overflow"] == 0
     for filt in (-2, dm.MAT["Ge_active"]):
-        assert np.array_equal(res[(4, filt)][0], res[(8, filt)][0])
-        assert np.array_equal(res[(4, filt)][1], res[(8, filt)][1])
+        for width in (5, 8):
+            assert np.array_equal(res[(4, filt)][0], res[(width, filt)][0])
+            assert np.array_equal(res[(4, filt)][1], res[(width, filt)][1])
     with pytest.raises(pkg.GadepError):
-        g.set_bvh_width(5)
+        g.set_bvh_width(6)
 
 
 # ------------------------------------------------------------------ config 4: 1e6 seeded rays, full mesh, brute force
@@ -277,9 +278,11 @@ def test_cfg4_full_mesh_1e6_rays_vs_stored_brute_force(pkg, orc):
     R, z0, z1 = w.notes["ray_box"]
     org, d = make_rays(n, w.notes["ray_seed"], R, z0, z1)
     report = {"n_rays": n}
-    for width in (4, 8):
+    tri_auto, t_auto = g.trace_rays(org, d)          # no width set: the 64-byte nodes on a hierarchy of this size
+    for width in (4, 5, 8):
         g.set_bvh_width(width)
         tri, t = g.trace_rays(org, d)
+        assert np.array_equal(tri, tri_auto) and np.array_equal(t, t_auto)
         assert g.get_counters()["n_stack_overflow"] == 0
         hit = otri >= 0
         assert hit.all()                             # origins lie inside the world surface: every ray meets a facet

@@ -515,6 +515,14 @@ def test_all_kernel_variants_give_identical_tallies(pkg, orc):
         d = g.run(n, 5, w.n_bins, w.spectrum_e_max_mev, flags=RUN_BVH8).copy()      # compressed 8-wide nodes
         cd = g.get_counters()
         assert np.array_equal(a, d)
+        g.set_bvh_width(5)                                                          # compressed 4-wide nodes (64 bytes)
+        e = g.run(n, 5, w.n_bins, w.spectrum_e_max_mev).copy()
+        ce = g.get_counters()
+        g.set_bvh_width(4)
+        assert np.array_equal(a, e)
+        for k in ("n_histories", "n_queries", "n_skipped_queries", "n_crossings", "n_pe", "n_compton", "n_coherent",
+                  "n_pair", "n_escaped", "n_leak", "n_cutoff", "emitted", "peak"):
+            assert ca[k] == ce[k], k
         for k in ("n_histories", "n_queries", "n_crossings", "n_pe", "n_compton", "n_coherent",
                   "n_pair", "n_escaped", "n_leak", "n_cutoff", "emitted", "peak"):
             assert ca[k] == cd[k], k
